@@ -1,0 +1,208 @@
+/*
+ * kv_pool.h — C-ABI of the D-instance (consumer) KV data path for sm_100a (B200).
+ *
+ * What this library is.  DOPD (arxiv 2511.20982) models PD-disaggregated serving as a
+ * producer/consumer pair: "P-instances produce prefill-completed requests (together with
+ * KV-cache), and D-instances consume those prefill-completed requests to perform token
+ * generation" (§IV-B-1).  The consumer keeps each request's KV in "KV-cache
+ * blocks" (§V-C), re-reads all of it from HBM on every decode step
+ * (§IV-B-2: "the entire decoding inference latency ... is dedicated to
+ * reading the KV-cache and model weights") and evaluates softmax(QK^T)V (PAPER.md:146,
+ * Eq. 1) for the one new query token of every in-flight request.  The calls below are
+ * that path and nothing else:
+ *
+ *   kv_pool_create          paged KV block pool + host block allocator
+ *   kv_ingest               prefill-completed request's contiguous K/V -> paged blocks
+ *                           (a2); with n_tokens = 1 it is the decode-step append (a3)
+ *   paged_decode_attention  split-KV paged attention (a4) + log-sum-exp combine (a5)
+ *   kv_free                 completed request's blocks back to the free list (a6)
+ *
+ * Conventions.
+ *   - extern "C"; every entry point returns an int32_t status (KV_OK = 0, errors < 0)
+ *     unless stated otherwise.  No exceptions, no aborts, nothing is printed.
+ *   - "device" pointers are CUDA device pointers valid in the current context; "host"
+ *     pointers are ordinary process memory.  The CALLER owns all device memory (slab, q,
+ *     out, sources) and the stream; the library owns only its host metadata and pinned
+ *     staging buffers.  Device pointers must be 16-byte aligned.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All
+ *     GPU work of a call is enqueued on it and the call returns without synchronising;
+ *     source buffers may be released once the stream has passed the call.
+ *   - bf16 = IEEE bfloat16 bit patterns (uint16_t).  No other KV dtype in this version.
+ *   - One host thread per pool.  Pools are independent.
+ *
+ * Slab layout (caller-visible so that an independent checker can read the pool).
+ *   The caller allocates `kv_pool_required_bytes(cfg)` bytes at `device_base`.  The first
+ *   `kv_pool_kv_bytes(cfg)` bytes are the KV region, bf16, indexed as
+ *
+ *       kv[layer][block][kv_head][c][slot][j]      c = 0: K, c = 1: V
+ *         layer   in [0, num_layers)      block in [0, num_blocks)
+ *         kv_head in [0, num_kv_heads)    slot  in [0, block_size)    j in [0, head_dim)
+ *
+ *   i.e. element offset ((((layer*num_blocks + block)*num_kv_heads + kv_head)*2 + c)
+ *   *block_size + slot)*head_dim + j.  Token t of a request lives in block
+ *   block_table[t / block_size] at slot t % block_size.  Bytes after the KV region are
+ *   library-private metadata (device block_table mirror, work lists, split-KV partials).
+ *   Slots at or beyond a request's length and blocks that are not allocated are never
+ *   written by the library and never influence any output.
+ */
+#ifndef KV_POOL_H_
+#define KV_POOL_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- status codes -------------------------------------------------------------------- */
+#define KV_OK                      0
+#define KV_ERR_INVALID            -1  /* null / misaligned pointer, bad shape, bad argument  */
+#define KV_ERR_NO_BLOCKS          -2  /* pool exhausted; the call changed nothing (atomic)   */
+#define KV_ERR_UNKNOWN_REQUEST    -3  /* req_id not live                                     */
+#define KV_ERR_TOO_LONG           -4  /* request would exceed max_blocks_per_request         */
+#define KV_ERR_TOO_MANY_REQUESTS  -5  /* more than max_requests live requests                */
+#define KV_ERR_CUDA               -6  /* a CUDA runtime call failed; see kv_last_cuda_error  */
+#define KV_ERR_NO_DEVICE          -7  /* pool was created without a device slab (host-only)  */
+
+typedef struct kv_pool kv_pool_t; /* opaque, library-owned host object */
+
+/*
+ * Pool geometry.  Supported: head_dim in {64, 128}; block_size = 16;
+ * num_q_heads % num_kv_heads == 0 with group size G = num_q_heads / num_kv_heads <= 8
+ * (GQA mapping: query head h reads KV head h / G).
+ */
+typedef struct kv_pool_config {
+  int32_t  num_layers;
+  int32_t  num_q_heads;
+  int32_t  num_kv_heads;
+  int32_t  head_dim;
+  int32_t  block_size;
+  int64_t  num_blocks;              /* physical blocks per layer                            */
+  int32_t  max_requests;            /* live requests (rows of the device block_table)       */
+  int32_t  max_blocks_per_request;  /* columns of the device block_table                    */
+  uint64_t alloc_seed;              /* 0: free list hands out 0,1,2,... (LIFO on reuse);
+                                       !=0: initial free list is a Fisher-Yates permutation
+                                       driven by splitmix64(alloc_seed) — fragmented pool   */
+  void*    device_base;             /* device, >= kv_pool_required_bytes(cfg), 256-B aligned;
+                                       NULL => host-only pool: allocator and planner work,
+                                       calls that launch kernels return KV_ERR_NO_DEVICE    */
+  int64_t  device_bytes;            /* size of the slab at device_base                      */
+} kv_pool_config_t;
+
+/* Bytes of the KV region / of the whole slab (KV region + private metadata) for `cfg`
+ * (device_base / device_bytes ignored).  Return < 0 (a KV_ERR_*) on an invalid config.    */
+int64_t kv_pool_kv_bytes(const kv_pool_config_t* cfg);
+int64_t kv_pool_required_bytes(const kv_pool_config_t* cfg);
+
+/* Create / destroy.  Create validates cfg, builds the free list, allocates pinned staging
+ * (skipped for a host-only pool) and does NOT touch the KV region (prior bytes retained).
+ * Destroy synchronises nothing: the caller must have drained streams using the pool.       */
+int32_t kv_pool_create(const kv_pool_config_t* cfg, kv_pool_t** out_pool);
+int32_t kv_pool_destroy(kv_pool_t* pool);
+
+/*
+ * a1 — block allocation + block_table build, host only ("KV-cache blocks";
+ * PAPER.md:82 "block fragmentation and count").  Grows each request from len to
+ * len + n_tokens[i] tokens: takes ceil((len+n)/bs) - ceil(len/bs) block ids from the free
+ * list and appends them to the request's block list.  Unknown req_id => created with
+ * length 0.  Atomic over the batch: on any error nothing changes.  Duplicate ids in one
+ * call => KV_ERR_INVALID.  n_tokens[i] = 0 is allowed (creates an empty request).
+ * kv_ingest calls this internally; it is exported for host-side planning and tests.
+ */
+int32_t kv_reserve(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids /*host*/,
+                   const int32_t* n_tokens /*host*/);
+
+/*
+ * a2 / a3 — KV ingest ("prefill-completed requests (together with KV-cache)";
+ * PAPER.md:360 transfer into the consumer's KV-cache blocks; PAPER.md:219 decode steps).
+ * For request i, layers [layer_begin, layer_begin + layer_count):
+ *     kv[l][block_table_i[(p+t)/bs]][h][c][(p+t)%bs][:] = src_c[i][l-layer_begin][h][t][:]
+ * for t in [0, n_tokens[i]), where p is the request's length before the reservation.
+ *   k_src[i], v_src[i]: device, bf16, contiguous [layer_count][num_kv_heads][n_tokens[i]][head_dim].
+ *   layer_begin == 0 : performs kv_reserve(n_tokens) first (p = current length), then copies.
+ *   layer_begin  > 0 : layer-sliced continuation: copies into the LAST reservation of each
+ *                      request (p = length - n_tokens[i]); n_tokens[i] must equal that
+ *                      reservation's size, else KV_ERR_INVALID.  This lets a producer stream
+ *                      KV layer by layer, and a decode loop append per layer.
+ * A pure bit copy: no arithmetic, no conversion.  Bytes outside the written slots keep
+ * their previous contents.  Errors as kv_reserve, plus KV_ERR_NO_DEVICE / KV_ERR_CUDA.
+ */
+int32_t kv_ingest(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids /*host*/,
+                  const int32_t* n_tokens /*host*/,
+                  const void* const* k_src /*host array of device ptrs*/,
+                  const void* const* v_src /*host array of device ptrs*/,
+                  int32_t layer_begin, int32_t layer_count, void* cuda_stream);
+
+/*
+ * a4 + a5 — one decode step's attention for one layer (Eq. 1 restricted to
+ * the decode case of PAPER.md:200/:219: one query token per request over that request's
+ * stored KV, all n tokens visible, no mask; scale reading SURVEY §8(c) A1):
+ *     out[i][h][:] = sum_t softmax_t( sm_scale * <q[i][h], K_t> ) * V_t ,
+ *     K_t, V_t = token t of request req_ids[i], KV head h / G, layer `layer`, t < len_i.
+ *   q, out: device, bf16, [batch][num_q_heads][head_dim]; out is written RNE-rounded from
+ *   fp32 accumulation.  sm_scale <= 0 selects 1/sqrt(head_dim).
+ * Runs a split-KV main kernel (per (request, kv_head, chunk) online softmax -> partial
+ * (m, l, O)) and an LSE combine kernel; both on `cuda_stream`.
+ * Errors: KV_ERR_UNKNOWN_REQUEST; a request of length 0 or a duplicate id => KV_ERR_INVALID;
+ * batch > max_requests => KV_ERR_INVALID; KV_ERR_NO_DEVICE; KV_ERR_CUDA.
+ */
+int32_t paged_decode_attention(kv_pool_t* pool, int32_t layer, int32_t batch,
+                               const int64_t* req_ids /*host*/, const void* q /*device*/,
+                               void* out /*device*/, float sm_scale, void* cuda_stream);
+
+/*
+ * a6 — free (a completed request releases consumer capacity).  Host only
+ * and immediate: blocks return to the free list (LIFO) and the table row is dropped.  The
+ * caller must not ingest into recycled blocks on a different stream before the attention
+ * that last read them has finished.  Atomic: an unknown or duplicate id => nothing freed.
+ */
+int32_t kv_free(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids /*host*/);
+
+/* ---- introspection ------------------------------------------------------------------- */
+
+/* Block list and length of a live request (host).  Writes min(cap, n_blocks) ids.         */
+int32_t kv_block_table(const kv_pool_t* pool, int64_t req_id, int32_t* out_blocks /*host*/,
+                       int32_t cap, int32_t* out_n_blocks, int32_t* out_len);
+
+/* Occupancy — the `load_kv` signal of PAPER.md:352 / :419.  Any out pointer may be NULL.  */
+int32_t kv_pool_stats(const kv_pool_t* pool, int64_t* blocks_total, int64_t* blocks_free,
+                      int32_t* live_requests, int64_t* blocks_high_water);
+
+/* Inverse of ingest for one request, all layers: k_dst/v_dst device bf16
+ * [num_layers][num_kv_heads][len][head_dim].  Test support; also the producer-side
+ * paged->contiguous step of SURVEY §8(f) NEXT-4.                                           */
+int32_t kv_gather(kv_pool_t* pool, int64_t req_id, void* k_dst /*device*/,
+                  void* v_dst /*device*/, void* cuda_stream);
+
+/*
+ * Host-only view of the split-KV plan paged_decode_attention would use for this batch
+ * (no GPU work).  A work item is (batch index, kv_head, first block, block count,
+ * partial slot or -1 when the item is its request's only chunk and writes `out` directly).
+ * out_items: host int32[cap_items][5]; *out_n_items = total item count (may exceed cap);
+ * *out_chunk_blocks = chunk size in blocks.  Items are ordered longest-first.
+ */
+int32_t kv_plan_decode(kv_pool_t* pool, int32_t batch, const int64_t* req_ids /*host*/,
+                       int32_t* out_items /*host*/, int32_t cap_items, int32_t* out_n_items,
+                       int32_t* out_chunk_blocks);
+
+/* Number of kernels this pool has launched since creation (bench `gpu_launches`).         */
+int64_t kv_launch_count(const kv_pool_t* pool);
+
+/* Tuning knobs (all optional; defaults chosen for B200).  key: "min_chunk_blocks",
+ * "ctas_per_sm", "attn_variant" (0 = register-direct, 1 = bulk-copy smem ring).
+ * Unknown key => KV_ERR_INVALID.                                                           */
+int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value);
+
+/* Last CUDA error code seen by this pool (cudaError_t as int; 0 = none).                  */
+int32_t kv_last_cuda_error(const kv_pool_t* pool);
+
+/* Static string for a status code.                                                        */
+const char* kv_strerror(int32_t status);
+
+/* Library version, "major.minor.patch".                                                   */
+const char* kv_version(void);
+
+#ifdef __cplusplus
+} /* extern "C" */
+#endif
+#endif /* KV_POOL_H_ */

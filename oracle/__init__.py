@@ -1,0 +1,193 @@
+"""ORACLE — test infrastructure only.
+
+A plain fp64 CPU statement (plain C, ``kv_oracle.c``) of what the D-instance KV path computes,
+written from the paper before any kernel.  Only ``tests/``, ``__graft_entry__.smoke()`` and
+``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may import this package; it imports
+nothing from ``paper_2511_20982_b200`` and shares no code with the CUDA path.
+
+This module is argument marshalling (numpy <-> C) only; every number comes from kv_oracle.c.
+bf16 tensors cross this boundary as ``numpy.uint16`` bit patterns.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "kv_oracle.c")
+_LIB = os.path.join(_HERE, "libkv_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    """Compile kv_oracle.c with gcc (-O2, OpenMP).  Building the checker is not using it."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".{os.getpid()}.tmp"
+        subprocess.run(
+            ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-Wall", "-Wextra",
+             "-o", tmp, _SRC, "-lm"],
+            check=True,
+        )
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Dims(ctypes.Structure):
+    _fields_ = [
+        ("num_layers", ctypes.c_int32),
+        ("num_kv_heads", ctypes.c_int32),
+        ("head_dim", ctypes.c_int32),
+        ("block_size", ctypes.c_int32),
+        ("num_blocks", ctypes.c_int64),
+    ]
+
+
+@dataclass(frozen=True)
+class Dims:
+    """Pool geometry as the oracle sees it (see include/kv_pool.h, "Slab layout")."""
+
+    num_layers: int
+    num_kv_heads: int
+    head_dim: int
+    block_size: int
+    num_blocks: int
+
+    @property
+    def kv_elems(self) -> int:
+        return self.num_layers * self.num_blocks * self.num_kv_heads * 2 * self.block_size * self.head_dim
+
+    def shape(self):
+        return (self.num_layers, self.num_blocks, self.num_kv_heads, 2, self.block_size, self.head_dim)
+
+    def _c(self) -> _Dims:
+        return _Dims(self.num_layers, self.num_kv_heads, self.head_dim, self.block_size, self.num_blocks)
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        P = ctypes.c_void_p
+        lib.oracle_num_threads.restype = ctypes.c_int
+        lib.oracle_scatter.restype = None
+        lib.oracle_scatter.argtypes = [P, ctypes.POINTER(_Dims), P, ctypes.c_int32, ctypes.c_int32, P, P,
+                                       ctypes.c_int32, ctypes.c_int32]
+        lib.oracle_gather.restype = None
+        lib.oracle_gather.argtypes = [P, ctypes.POINTER(_Dims), P, ctypes.c_int32, P, P]
+        lib.oracle_attention.restype = ctypes.c_int
+        lib.oracle_attention.argtypes = [P, ctypes.POINTER(_Dims), ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
+                                         P, P, P, P, ctypes.c_double, P, P]
+        lib.oracle_chunk.restype = None
+        lib.oracle_chunk.argtypes = [P, ctypes.POINTER(_Dims), ctypes.c_int32, ctypes.c_int32, P, ctypes.c_int32,
+                                     ctypes.c_int32, P, ctypes.c_double, P, P, P]
+        lib.oracle_combine.restype = None
+        lib.oracle_combine.argtypes = [ctypes.c_int32, ctypes.c_int32, P, P, P, P]
+        _lib = lib
+    return _lib
+
+
+def _ptr(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _u16(a, name) -> np.ndarray:
+    a = np.asarray(a)
+    if a.dtype != np.uint16:
+        raise TypeError(f"{name}: expected uint16 bf16 bit patterns, got {a.dtype}")
+    return np.ascontiguousarray(a)
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def new_slab(dims: Dims, fill: int = 0) -> np.ndarray:
+    """A host KV region, flat uint16, pre-filled with a 16-bit sentinel pattern."""
+    return np.full(dims.kv_elems, fill, dtype=np.uint16)
+
+
+def scatter(kv: np.ndarray, dims: Dims, blocks, start_pos: int, k_src, v_src, layer_begin: int = 0) -> None:
+    """In place: kv <- request tokens.  k_src/v_src: uint16 [layer_count][Hkv][n][d]."""
+    assert kv.dtype == np.uint16 and kv.flags.c_contiguous and kv.size == dims.kv_elems
+    k_src, v_src = _u16(k_src, "k_src"), _u16(v_src, "v_src")
+    layer_count, hkv, n, d = k_src.shape
+    assert v_src.shape == k_src.shape and hkv == dims.num_kv_heads and d == dims.head_dim
+    assert 0 <= layer_begin and layer_begin + layer_count <= dims.num_layers
+    blocks = np.ascontiguousarray(blocks, dtype=np.int32)
+    assert (start_pos + n + dims.block_size - 1) // dims.block_size <= blocks.size
+    assert blocks.size == 0 or (0 <= blocks.min() and blocks.max() < dims.num_blocks)
+    c = dims._c()
+    _load().oracle_scatter(_ptr(kv), ctypes.byref(c), _ptr(blocks), start_pos, n, _ptr(k_src), _ptr(v_src),
+                           layer_begin, layer_count)
+
+
+def gather(kv: np.ndarray, dims: Dims, blocks, length: int):
+    """Returns (k, v) uint16 [L][Hkv][length][d]."""
+    assert kv.dtype == np.uint16 and kv.flags.c_contiguous and kv.size == dims.kv_elems
+    blocks = np.ascontiguousarray(blocks, dtype=np.int32)
+    assert (length + dims.block_size - 1) // dims.block_size <= blocks.size
+    shape = (dims.num_layers, dims.num_kv_heads, length, dims.head_dim)
+    k = np.empty(shape, dtype=np.uint16)
+    v = np.empty(shape, dtype=np.uint16)
+    c = dims._c()
+    _load().oracle_gather(_ptr(kv), ctypes.byref(c), _ptr(blocks), length, _ptr(k), _ptr(v))
+    return k, v
+
+
+def attention(kv: np.ndarray, dims: Dims, layer: int, num_q_heads: int, block_lists, seq_lens, q,
+              scale: float | None = None, return_wsum: bool = False):
+    """Decode attention by the definition.  q: uint16 [B][Hq][d].  Returns float64 [B][Hq][d]."""
+    assert kv.dtype == np.uint16 and kv.flags.c_contiguous and kv.size == dims.kv_elems
+    q = _u16(q, "q")
+    batch = q.shape[0]
+    assert q.shape == (batch, num_q_heads, dims.head_dim)
+    assert num_q_heads % dims.num_kv_heads == 0 and 0 <= layer < dims.num_layers
+    seq_lens = np.ascontiguousarray(seq_lens, dtype=np.int32)
+    assert seq_lens.shape == (batch,) and len(block_lists) == batch
+    lists = [np.ascontiguousarray(b, dtype=np.int32) for b in block_lists]
+    for b, n in zip(lists, seq_lens):
+        assert (int(n) + dims.block_size - 1) // dims.block_size <= b.size
+        assert b.size == 0 or (0 <= b.min() and b.max() < dims.num_blocks)
+    off = np.zeros(batch + 1, dtype=np.int64)
+    off[1:] = np.cumsum([b.size for b in lists])
+    bt = np.concatenate(lists) if lists else np.zeros(0, np.int32)
+    bt = np.ascontiguousarray(bt, dtype=np.int32)
+    if scale is None:
+        scale = 1.0 / float(np.sqrt(np.float64(dims.head_dim)))
+    out = np.empty((batch, num_q_heads, dims.head_dim), dtype=np.float64)
+    wsum = np.empty((batch, num_q_heads), dtype=np.float64)
+    c = dims._c()
+    rc = _load().oracle_attention(_ptr(kv), ctypes.byref(c), layer, num_q_heads, batch, _ptr(bt), _ptr(off),
+                                  _ptr(seq_lens), _ptr(q), float(scale), _ptr(out), _ptr(wsum))
+    if rc != 0:
+        raise ValueError(f"oracle_attention failed ({rc}): empty context or out of memory")
+    return (out, wsum) if return_wsum else out
+
+
+def chunk(kv: np.ndarray, dims: Dims, layer: int, kv_head: int, blocks, t0: int, t1: int, qv, scale: float):
+    """(m, l, O) of tokens [t0, t1) for one query vector qv (uint16 [d])."""
+    qv = _u16(qv, "qv")
+    blocks = np.ascontiguousarray(blocks, dtype=np.int32)
+    m = ctypes.c_double()
+    l = ctypes.c_double()
+    O = np.empty(dims.head_dim, dtype=np.float64)
+    c = dims._c()
+    _load().oracle_chunk(_ptr(kv), ctypes.byref(c), layer, kv_head, _ptr(blocks), t0, t1, _ptr(qv), float(scale),
+                         ctypes.byref(m), ctypes.byref(l), _ptr(O))
+    return m.value, l.value, O
+
+
+def combine(m, l, O) -> np.ndarray:
+    m = np.ascontiguousarray(m, dtype=np.float64)
+    l = np.ascontiguousarray(l, dtype=np.float64)
+    O = np.ascontiguousarray(O, dtype=np.float64)
+    n, d = O.shape
+    out = np.empty(d, dtype=np.float64)
+    _load().oracle_combine(n, d, _ptr(m), _ptr(l), _ptr(O), _ptr(out))
+    return out

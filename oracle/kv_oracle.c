@@ -1,0 +1,207 @@
+/*
+ * kv_oracle.c — the ORACLE: a plain, slow, fp64 CPU statement of what the D-instance KV
+ * path computes.  TEST INFRASTRUCTURE ONLY: nothing outside tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may call it, and it shares no code,
+ * header, table or helper with paper_2511_20982_b200/ (the CUDA path).
+ *
+ * What it states (citations are /root/reference/PAPER.md lines):
+ *   - oracle_attention: PAPER.md:146 (§IV-A, Eq. 1) Output = softmax(Q K^T) V, in the decode
+ *     form of PAPER.md:200 / :219 (one query token per in-flight request over that request's
+ *     stored KV).  Readings: A1 the omitted 1/sqrt(d) scale is an
+ *     explicit argument; A2 query head h reads KV head h / G; A3/A4 all n stored tokens are
+ *     visible, no mask.  This is the DEFINITION written out: the CUDA path's paging,
+ *     split-KV, online softmax and LSE combine reach the same value (up to rounding), so
+ *     none of that appears here.
+ *   - oracle_scatter / oracle_gather: the relocation of a prefill-completed request's
+ *     contiguous KV ("prefill-completed requests (together with KV-cache)")
+ *     into the consumer's KV-cache blocks, and its inverse.  Pure bit copies.
+ *   - oracle_chunk / oracle_combine: the per-chunk (m, l, O) triple and the log-sum-exp
+ *     merge, in fp64, so that tests can pin the merge identity.  Not used
+ *     by oracle_attention.
+ *
+ * Slab layout is the one include/kv_pool.h documents for the caller-owned slab, restated
+ * here independently (kv_index).  bf16 inputs are widened exactly: a bf16 is the top 16 bits
+ * of an IEEE float.  Sums are plain left-to-right loops in double.
+ *
+ * Parity pins (tests/test_oracle_pins.py): n = 1 returns V_0; q = 0 gives the mean of V;
+ * hand-computed weights (1/3, 2/3), (1/7, 2/7, 4/7), (1/6, 2/6, 3/6); weights sum to 1;
+ * block-permutation invariance; GQA map; shift invariance / no overflow; agreement with
+ * torch.nn.functional.scaled_dot_product_attention in fp64; an independent numpy
+ * brute-force over gathered rows; chunk+combine == unsplit; scatter o gather == identity and
+ * whole-slab equality with a numpy fancy-index scatter.  No function here is "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+#include <stdlib.h>
+#include <string.h>
+
+typedef struct {
+  int32_t num_layers, num_kv_heads, head_dim, block_size;
+  int64_t num_blocks;
+} oracle_dims_t;
+
+static double bf16_to_double(uint16_t b) {
+  uint32_t u = ((uint32_t)b) << 16;
+  float f;
+  memcpy(&f, &u, sizeof f);
+  return (double)f;
+}
+
+/* element index of kv[layer][block][kv_head][c][slot][j] (include/kv_pool.h, "Slab layout") */
+static int64_t kv_index(const oracle_dims_t* D, int64_t layer, int64_t block, int64_t head,
+                        int64_t c, int64_t slot, int64_t j) {
+  return ((((layer * D->num_blocks + block) * D->num_kv_heads + head) * 2 + c) * D->block_size +
+          slot) * D->head_dim + j;
+}
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+/*
+ * Reference scatter.  blocks[] is the request's block list (logical
+ * block i -> physical id).  Copies tokens t in [0,n) of src (layout
+ * [layer_count][num_kv_heads][n][head_dim]) to logical positions start_pos + t of layers
+ * layer_begin .. layer_begin+layer_count-1.
+ */
+void oracle_scatter(uint16_t* kv, const oracle_dims_t* D, const int32_t* blocks,
+                    int32_t start_pos, int32_t n, const uint16_t* k_src, const uint16_t* v_src,
+                    int32_t layer_begin, int32_t layer_count) {
+  for (int32_t ll = 0; ll < layer_count; ++ll)
+    for (int32_t h = 0; h < D->num_kv_heads; ++h)
+      for (int32_t t = 0; t < n; ++t) {
+        int32_t pos = start_pos + t;
+        int32_t blk = blocks[pos / D->block_size];
+        int32_t slot = pos % D->block_size;
+        int64_t s = (((int64_t)ll * D->num_kv_heads + h) * n + t) * D->head_dim;
+        for (int32_t j = 0; j < D->head_dim; ++j) {
+          kv[kv_index(D, layer_begin + ll, blk, h, 0, slot, j)] = k_src[s + j];
+          kv[kv_index(D, layer_begin + ll, blk, h, 1, slot, j)] = v_src[s + j];
+        }
+      }
+}
+
+/* Reference gather: inverse of oracle_scatter over tokens [0,len), all layers.
+ * k_dst / v_dst: [num_layers][num_kv_heads][len][head_dim]. */
+void oracle_gather(const uint16_t* kv, const oracle_dims_t* D, const int32_t* blocks, int32_t len,
+                   uint16_t* k_dst, uint16_t* v_dst) {
+  for (int32_t l = 0; l < D->num_layers; ++l)
+    for (int32_t h = 0; h < D->num_kv_heads; ++h)
+      for (int32_t t = 0; t < len; ++t) {
+        int32_t blk = blocks[t / D->block_size];
+        int32_t slot = t % D->block_size;
+        int64_t s = (((int64_t)l * D->num_kv_heads + h) * len + t) * D->head_dim;
+        for (int32_t j = 0; j < D->head_dim; ++j) {
+          k_dst[s + j] = kv[kv_index(D, l, blk, h, 0, slot, j)];
+          v_dst[s + j] = kv[kv_index(D, l, blk, h, 1, slot, j)];
+        }
+      }
+}
+
+/*
+ * Decode attention, the definition:
+ *   for request r, query head h:  g = h / G;  n = seq_lens[r]
+ *     s_t = scale * sum_j q[r][h][j] * K_t[j]        t in [0,n)
+ *     m = max_t s_t;  w_t = exp(s_t - m);  Z = sum_t w_t
+ *     out[r][h][:] = sum_t (w_t / Z) * V_t[:]         (fp64, not rounded)
+ * Block lists are ragged: request r's list is bt[bt_off[r] .. bt_off[r+1]).
+ * wsum (optional, may be NULL): wsum[r*Hq+h] = sum_t (w_t / Z), for the sum-to-1 invariant.
+ * Returns 0, or -1 if some request has n < 1 (empty context is an error).
+ */
+int oracle_attention(const uint16_t* kv, const oracle_dims_t* D, int32_t layer, int32_t num_q_heads,
+                     int32_t batch, const int32_t* bt, const int64_t* bt_off,
+                     const int32_t* seq_lens, const uint16_t* q, double scale, double* out,
+                     double* wsum) {
+  const int32_t d = D->head_dim, Hq = num_q_heads, G = num_q_heads / D->num_kv_heads;
+  for (int32_t r = 0; r < batch; ++r)
+    if (seq_lens[r] < 1) return -1;
+  int bad = 0;
+#pragma omp parallel for collapse(2) schedule(dynamic, 1)
+  for (int32_t r = 0; r < batch; ++r)
+    for (int32_t h = 0; h < Hq; ++h) {
+      const int32_t g = h / G, n = seq_lens[r];
+      const int32_t* blocks = bt + bt_off[r];
+      const uint16_t* qv = q + ((int64_t)r * Hq + h) * d;
+      double* s = (double*)malloc(sizeof(double) * (size_t)n);
+      double* o = out + ((int64_t)r * Hq + h) * d;
+      if (!s) { bad = 1; continue; }
+      for (int32_t t = 0; t < n; ++t) {
+        int64_t kb = kv_index(D, layer, blocks[t / D->block_size], g, 0, t % D->block_size, 0);
+        double acc = 0.0;
+        for (int32_t j = 0; j < d; ++j) acc += bf16_to_double(qv[j]) * bf16_to_double(kv[kb + j]);
+        s[t] = scale * acc;
+      }
+      double m = s[0];
+      for (int32_t t = 1; t < n; ++t)
+        if (s[t] > m) m = s[t];
+      double Z = 0.0;
+      for (int32_t t = 0; t < n; ++t) {
+        s[t] = exp(s[t] - m);
+        Z += s[t];
+      }
+      for (int32_t j = 0; j < d; ++j) o[j] = 0.0;
+      double ws = 0.0;
+      for (int32_t t = 0; t < n; ++t) {
+        int64_t vb = kv_index(D, layer, blocks[t / D->block_size], g, 1, t % D->block_size, 0);
+        double w = s[t] / Z;
+        ws += w;
+        for (int32_t j = 0; j < d; ++j) o[j] += w * bf16_to_double(kv[vb + j]);
+      }
+      if (wsum) wsum[(int64_t)r * Hq + h] = ws;
+      free(s);
+    }
+  return bad ? -2 : 0;
+}
+
+/*
+ * One split-KV chunk in fp64: over tokens [t0, t1) of one request and
+ * one query head,  m = max s_t,  l = sum exp(s_t - m),  O = sum exp(s_t - m) V_t.
+ */
+void oracle_chunk(const uint16_t* kv, const oracle_dims_t* D, int32_t layer, int32_t kv_head,
+                  const int32_t* blocks, int32_t t0, int32_t t1, const uint16_t* qv, double scale,
+                  double* m_out, double* l_out, double* O_out) {
+  const int32_t d = D->head_dim;
+  double m = -INFINITY;
+  for (int32_t t = t0; t < t1; ++t) {
+    int64_t kb = kv_index(D, layer, blocks[t / D->block_size], kv_head, 0, t % D->block_size, 0);
+    double acc = 0.0;
+    for (int32_t j = 0; j < d; ++j) acc += bf16_to_double(qv[j]) * bf16_to_double(kv[kb + j]);
+    if (scale * acc > m) m = scale * acc;
+  }
+  double l = 0.0;
+  for (int32_t j = 0; j < d; ++j) O_out[j] = 0.0;
+  for (int32_t t = t0; t < t1; ++t) {
+    int64_t kb = kv_index(D, layer, blocks[t / D->block_size], kv_head, 0, t % D->block_size, 0);
+    int64_t vb = kv_index(D, layer, blocks[t / D->block_size], kv_head, 1, t % D->block_size, 0);
+    double acc = 0.0;
+    for (int32_t j = 0; j < d; ++j) acc += bf16_to_double(qv[j]) * bf16_to_double(kv[kb + j]);
+    double w = exp(scale * acc - m);
+    l += w;
+    for (int32_t j = 0; j < d; ++j) O_out[j] += w * bf16_to_double(kv[vb + j]);
+  }
+  *m_out = m;
+  *l_out = l;
+}
+
+/* LSE combine:  M = max_c m_c;  out = sum_c e^{m_c-M} O_c / sum_c e^{m_c-M} l_c */
+void oracle_combine(int32_t n_chunks, int32_t d, const double* m, const double* l, const double* O,
+                    double* out) {
+  double M = m[0];
+  for (int32_t c = 1; c < n_chunks; ++c)
+    if (m[c] > M) M = m[c];
+  double den = 0.0;
+  for (int32_t j = 0; j < d; ++j) out[j] = 0.0;
+  for (int32_t c = 0; c < n_chunks; ++c) {
+    double a = exp(m[c] - M);
+    den += a * l[c];
+    for (int32_t j = 0; j < d; ++j) out[j] += a * O[(int64_t)c * d + j];
+  }
+  for (int32_t j = 0; j < d; ++j) out[j] /= den;
+}
