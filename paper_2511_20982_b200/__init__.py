@@ -19,6 +19,7 @@ _BINDING_NAMES = (
 
 def __getattr__(name):
     if name in _BINDING_NAMES or name == "binding":
-        from . import binding as _b  # raises ImportError if the .so is missing
+        import importlib
+        _b = importlib.import_module(__name__ + ".binding")  # raises ImportError if the .so is missing
         return _b if name == "binding" else getattr(_b, name)
     raise AttributeError(f"module {__name__!r} has no attribute {name!r}")

@@ -1,0 +1,310 @@
+"""Thin ctypes binding of include/kv_pool.h — argument marshalling only.
+
+Every function has the name and meaning of its C counterpart; device tensors are passed as
+their ``data_ptr()``.  ``KVPool`` bundles a pool handle with the torch slab it lives in.  There
+is no fallback of any kind: a missing ``csrc/libkvpool.so`` raises ImportError at import.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+lib_path = os.path.join(_HERE, "csrc", "libkvpool.so")
+
+if not os.path.exists(lib_path):
+    raise ImportError(
+        f"{lib_path} is missing: build it with `python -m paper_2511_20982_b200.build` "
+        "(nvcc, sm_100a).  There is no CPU or PyTorch fallback for this path.")
+
+lib = ctypes.CDLL(lib_path)
+
+KV_OK = 0
+KV_ERR_INVALID, KV_ERR_NO_BLOCKS, KV_ERR_UNKNOWN_REQUEST, KV_ERR_TOO_LONG = -1, -2, -3, -4
+KV_ERR_TOO_MANY_REQUESTS, KV_ERR_CUDA, KV_ERR_NO_DEVICE = -5, -6, -7
+
+
+class _Config(ctypes.Structure):
+    _fields_ = [
+        ("num_layers", ctypes.c_int32), ("num_q_heads", ctypes.c_int32), ("num_kv_heads", ctypes.c_int32),
+        ("head_dim", ctypes.c_int32), ("block_size", ctypes.c_int32), ("num_blocks", ctypes.c_int64),
+        ("max_requests", ctypes.c_int32), ("max_blocks_per_request", ctypes.c_int32),
+        ("alloc_seed", ctypes.c_uint64), ("device_base", ctypes.c_void_p), ("device_bytes", ctypes.c_int64),
+    ]
+
+
+_P = ctypes.c_void_p
+_i32, _i64 = ctypes.c_int32, ctypes.c_int64
+_CFG = ctypes.POINTER(_Config)
+_SIGS = {
+    "kv_pool_kv_bytes": (_i64, [_CFG]),
+    "kv_pool_required_bytes": (_i64, [_CFG]),
+    "kv_pool_create": (_i32, [_CFG, ctypes.POINTER(_P)]),
+    "kv_pool_destroy": (_i32, [_P]),
+    "kv_reserve": (_i32, [_P, _i32, _P, _P]),
+    "kv_ingest": (_i32, [_P, _i32, _P, _P, _P, _P, _i32, _i32, _P]),
+    "paged_decode_attention": (_i32, [_P, _i32, _i32, _P, _P, _P, ctypes.c_float, _P]),
+    "kv_free": (_i32, [_P, _i32, _P]),
+    "kv_block_table": (_i32, [_P, _i64, _P, _i32, ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
+    "kv_pool_stats": (_i32, [_P, ctypes.POINTER(_i64), ctypes.POINTER(_i64), ctypes.POINTER(_i32),
+                             ctypes.POINTER(_i64)]),
+    "kv_gather": (_i32, [_P, _i64, _P, _P, _P]),
+    "kv_plan_decode": (_i32, [_P, _i32, _P, _P, _i32, ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
+    "kv_launch_count": (_i64, [_P]),
+    "kv_pool_set_option": (_i32, [_P, ctypes.c_char_p, _i64]),
+    "kv_last_cuda_error": (_i32, [_P]),
+    "kv_strerror": (ctypes.c_char_p, [_i32]),
+    "kv_version": (ctypes.c_char_p, []),
+}
+EXPORTS = tuple(_SIGS)
+for _name, (_res, _args) in _SIGS.items():
+    _f = getattr(lib, _name)  # AttributeError here = the .so does not export what the header declares
+    _f.restype, _f.argtypes = _res, _args
+
+
+class KVError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {kv_strerror(status)} ({status})")
+
+
+def _check(status: int, where: str) -> None:
+    if status != KV_OK:
+        raise KVError(status, where)
+
+
+@dataclass
+class PoolConfig:
+    num_layers: int
+    num_q_heads: int
+    num_kv_heads: int
+    head_dim: int
+    num_blocks: int
+    max_requests: int
+    max_blocks_per_request: int
+    block_size: int = 16
+    alloc_seed: int = 0
+
+    def _c(self, device_base: int = 0, device_bytes: int = 0) -> _Config:
+        return _Config(self.num_layers, self.num_q_heads, self.num_kv_heads, self.head_dim, self.block_size,
+                       self.num_blocks, self.max_requests, self.max_blocks_per_request, self.alloc_seed,
+                       device_base or None, device_bytes)
+
+
+def _ids(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.int64)
+
+
+def _i32s(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _ptrs(a) -> np.ndarray:
+    """list of tensors / ints -> uint64 array of device addresses."""
+    return np.ascontiguousarray([x if isinstance(x, int) else x.data_ptr() for x in a], dtype=np.uint64)
+
+
+def _np(a: np.ndarray):
+    return a.ctypes.data_as(_P)
+
+
+def kv_strerror(status: int) -> str:
+    return lib.kv_strerror(status).decode()
+
+
+def kv_version() -> str:
+    return lib.kv_version().decode()
+
+
+def kv_pool_kv_bytes(cfg: PoolConfig) -> int:
+    c = cfg._c()
+    n = lib.kv_pool_kv_bytes(ctypes.byref(c))
+    if n < 0:
+        raise KVError(int(n), "kv_pool_kv_bytes")
+    return int(n)
+
+
+def kv_pool_required_bytes(cfg: PoolConfig) -> int:
+    c = cfg._c()
+    n = lib.kv_pool_required_bytes(ctypes.byref(c))
+    if n < 0:
+        raise KVError(int(n), "kv_pool_required_bytes")
+    return int(n)
+
+
+def kv_pool_create(cfg: PoolConfig, device_base: int = 0, device_bytes: int = 0) -> int:
+    c = cfg._c(device_base, device_bytes)
+    h = _P()
+    _check(lib.kv_pool_create(ctypes.byref(c), ctypes.byref(h)), "kv_pool_create")
+    return h.value
+
+
+def kv_pool_destroy(handle: int) -> None:
+    _check(lib.kv_pool_destroy(handle), "kv_pool_destroy")
+
+
+def kv_reserve(handle: int, req_ids, n_tokens) -> None:
+    ids, n = _ids(req_ids), _i32s(n_tokens)
+    assert ids.shape == n.shape
+    _check(lib.kv_reserve(handle, ids.size, _np(ids), _np(n)), "kv_reserve")
+
+
+def kv_ingest(handle: int, req_ids, n_tokens, k_src, v_src, layer_begin: int = 0, layer_count: int = 1,
+              stream: int = 0) -> None:
+    ids, n, kp, vp = _ids(req_ids), _i32s(n_tokens), _ptrs(k_src), _ptrs(v_src)
+    assert ids.shape == n.shape == kp.shape == vp.shape
+    _check(lib.kv_ingest(handle, ids.size, _np(ids), _np(n), _np(kp), _np(vp), layer_begin, layer_count,
+                         stream or None), "kv_ingest")
+
+
+def paged_decode_attention(handle: int, layer: int, req_ids, q_ptr: int, out_ptr: int, sm_scale: float = 0.0,
+                           stream: int = 0) -> None:
+    ids = _ids(req_ids)
+    _check(lib.paged_decode_attention(handle, layer, ids.size, _np(ids), q_ptr, out_ptr, sm_scale, stream or None),
+           "paged_decode_attention")
+
+
+def kv_free(handle: int, req_ids) -> None:
+    ids = _ids(req_ids)
+    _check(lib.kv_free(handle, ids.size, _np(ids)), "kv_free")
+
+
+def kv_block_table(handle: int, req_id: int):
+    nb, ln = _i32(), _i32()
+    _check(lib.kv_block_table(handle, req_id, None, 0, ctypes.byref(nb), ctypes.byref(ln)), "kv_block_table")
+    out = np.empty(nb.value, dtype=np.int32)
+    _check(lib.kv_block_table(handle, req_id, _np(out), out.size, ctypes.byref(nb), ctypes.byref(ln)),
+           "kv_block_table")
+    return out, ln.value
+
+
+def kv_pool_stats(handle: int) -> dict:
+    t, f, r, hw = _i64(), _i64(), _i32(), _i64()
+    _check(lib.kv_pool_stats(handle, ctypes.byref(t), ctypes.byref(f), ctypes.byref(r), ctypes.byref(hw)),
+           "kv_pool_stats")
+    return {"blocks_total": t.value, "blocks_free": f.value, "live_requests": r.value, "blocks_high_water": hw.value}
+
+
+def kv_gather(handle: int, req_id: int, k_dst_ptr: int, v_dst_ptr: int, stream: int = 0) -> None:
+    _check(lib.kv_gather(handle, req_id, k_dst_ptr, v_dst_ptr, stream or None), "kv_gather")
+
+
+def kv_plan_decode(handle: int, req_ids):
+    """Returns (items int32 [n][5] = (batch_idx, kv_head, blk_begin, n_blocks, partial_idx), chunk_blocks)."""
+    ids = _ids(req_ids)
+    n, ch = _i32(), _i32()
+    _check(lib.kv_plan_decode(handle, ids.size, _np(ids), None, 0, ctypes.byref(n), ctypes.byref(ch)),
+           "kv_plan_decode")
+    items = np.empty((n.value, 5), dtype=np.int32)
+    _check(lib.kv_plan_decode(handle, ids.size, _np(ids), _np(items), n.value, ctypes.byref(n), ctypes.byref(ch)),
+           "kv_plan_decode")
+    return items, ch.value
+
+
+def kv_launch_count(handle: int) -> int:
+    return int(lib.kv_launch_count(handle))
+
+
+def kv_pool_set_option(handle: int, key: str, value: int) -> None:
+    _check(lib.kv_pool_set_option(handle, key.encode(), value), f"kv_pool_set_option({key})")
+
+
+def kv_last_cuda_error(handle: int) -> int:
+    return int(lib.kv_last_cuda_error(handle))
+
+
+class KVPool:
+    """A pool handle plus the torch uint8 slab it lives in (PyTorch = device memory and streams only)."""
+
+    def __init__(self, cfg: PoolConfig, device=None, fill_byte: int | None = None):
+        import torch
+
+        self.cfg = cfg
+        self.kv_bytes = kv_pool_kv_bytes(cfg)
+        if device is None:  # host-only pool: allocator + planner, no kernels
+            self.slab = None
+            self.handle = kv_pool_create(cfg)
+        else:
+            nbytes = kv_pool_required_bytes(cfg)
+            self.slab = torch.empty(nbytes, dtype=torch.uint8, device=device)
+            if fill_byte is not None:
+                self.slab[: self.kv_bytes].fill_(fill_byte)
+            self.handle = kv_pool_create(cfg, self.slab.data_ptr(), nbytes)
+
+    def kv_region(self):
+        """The KV region as a bf16 tensor [L][num_blocks][Hkv][2][block_size][head_dim] (a view)."""
+        import torch
+
+        c = self.cfg
+        return self.slab[: self.kv_bytes].view(torch.bfloat16).view(
+            c.num_layers, c.num_blocks, c.num_kv_heads, 2, c.block_size, c.head_dim)
+
+    @staticmethod
+    def _stream(stream) -> int:
+        if stream is None:
+            import torch
+            return torch.cuda.current_stream().cuda_stream
+        return stream if isinstance(stream, int) else stream.cuda_stream
+
+    def reserve(self, req_ids, n_tokens):
+        kv_reserve(self.handle, req_ids, n_tokens)
+
+    def ingest(self, req_ids, k_src, v_src, layer_begin=0, layer_count=None, stream=None):
+        """k_src[i], v_src[i]: bf16 CUDA tensors [layer_count][Hkv][n_i][d], contiguous."""
+        lc = self.cfg.num_layers - layer_begin if layer_count is None else layer_count
+        n = [int(k.shape[2]) for k in k_src]
+        for k, v in zip(k_src, v_src):
+            assert k.is_contiguous() and v.is_contiguous() and k.shape == v.shape and k.shape[0] == lc
+        kv_ingest(self.handle, req_ids, n, k_src, v_src, layer_begin, lc, self._stream(stream))
+
+    def attention(self, layer, req_ids, q, out=None, sm_scale=0.0, stream=None):
+        import torch
+
+        assert q.is_contiguous() and q.dtype == torch.bfloat16
+        if out is None:
+            out = torch.empty_like(q)
+        paged_decode_attention(self.handle, layer, req_ids, q.data_ptr(), out.data_ptr(), sm_scale, self._stream(stream))
+        return out
+
+    def gather(self, req_id, stream=None):
+        import torch
+
+        _, n = kv_block_table(self.handle, req_id)
+        c = self.cfg
+        k = torch.empty((c.num_layers, c.num_kv_heads, n, c.head_dim), dtype=torch.bfloat16, device=self.slab.device)
+        v = torch.empty_like(k)
+        kv_gather(self.handle, req_id, k.data_ptr(), v.data_ptr(), self._stream(stream))
+        return k, v
+
+    def free(self, req_ids):
+        kv_free(self.handle, req_ids)
+
+    def block_table(self, req_id):
+        return kv_block_table(self.handle, req_id)
+
+    def stats(self):
+        return kv_pool_stats(self.handle)
+
+    def plan(self, req_ids):
+        return kv_plan_decode(self.handle, req_ids)
+
+    def set_option(self, key, value):
+        kv_pool_set_option(self.handle, key, value)
+
+    @property
+    def launches(self) -> int:
+        return kv_launch_count(self.handle)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            kv_pool_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,238 @@
+// kv_host.h — host-side runtime of the D-instance KV pool: block allocator, request table,
+// split-KV planner.  Pure C++17, no CUDA: everything here is integer bookkeeping (SURVEY §8(a)
+// rows a1 and a6, and the work-list half of a4).  The paper prices none of this beyond noting
+// that transfer cost depends on "block fragmentation and count" and that KV
+// occupancy is a monitored signal.
+#pragma once
+
+#include <algorithm>
+#include <cstdint>
+#include <unordered_map>
+#include <unordered_set>
+#include <vector>
+
+#include "../../include/kv_pool.h"
+
+namespace kvp {
+
+inline uint64_t splitmix64_next(uint64_t& state) {
+  uint64_t z = (state += 0x9E3779B97F4A7C15ull);
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+// Free list of physical block ids.  pop() hands out ids from the back.
+//   seed == 0 : initial order such that the first pops return 0, 1, 2, ...
+//   seed != 0 : initial order is a Fisher-Yates permutation (fragmented pool).
+// Freed blocks are pushed back and reused LIFO.
+class BlockAllocator {
+ public:
+  void init(int64_t num_blocks, uint64_t seed) {
+    total_ = num_blocks;
+    free_.resize(static_cast<size_t>(num_blocks));
+    for (int64_t i = 0; i < num_blocks; ++i) free_[static_cast<size_t>(i)] = static_cast<int32_t>(num_blocks - 1 - i);
+    if (seed != 0) {
+      uint64_t s = seed;
+      for (int64_t i = num_blocks - 1; i > 0; --i) {
+        uint64_t j = splitmix64_next(s) % static_cast<uint64_t>(i + 1);
+        std::swap(free_[static_cast<size_t>(i)], free_[static_cast<size_t>(j)]);
+      }
+    }
+    high_water_ = 0;
+  }
+  int64_t total() const { return total_; }
+  int64_t free_count() const { return static_cast<int64_t>(free_.size()); }
+  int64_t high_water() const { return high_water_; }
+  int32_t pop() {
+    int32_t b = free_.back();
+    free_.pop_back();
+    high_water_ = std::max(high_water_, total_ - free_count());
+    return b;
+  }
+  void push(int32_t b) { free_.push_back(b); }
+
+ private:
+  std::vector<int32_t> free_;
+  int64_t total_ = 0, high_water_ = 0;
+};
+
+struct Request {
+  int32_t slot = -1;    // row of the device block_table mirror
+  int32_t len = 0;      // tokens stored (reserved)
+  int32_t last_n = 0;   // size of the last reservation (for layer-sliced ingest)
+  std::vector<int32_t> blocks;
+};
+
+// One split-KV work item: a run of logical blocks of one (request, kv_head).
+struct WorkItem {
+  int32_t batch_idx;    // row of q / out
+  int32_t slot;         // row of the device block_table
+  int32_t kv_head;
+  int32_t blk_begin;    // first logical block
+  int32_t n_blocks;
+  int32_t n_tokens;     // valid tokens in this run (last block of a request may be partial)
+  int32_t partial_idx;  // slot in the partials workspace, or -1: only chunk, writes `out`
+  int32_t pad;
+};
+static_assert(sizeof(WorkItem) == 32, "WorkItem is read by the kernel as two int4");
+
+struct CombineEntry {
+  int32_t batch_idx, kv_head, partial_begin, n_chunks;
+};
+
+struct DecodePlan {
+  std::vector<WorkItem> items;
+  std::vector<CombineEntry> combines;
+  int32_t chunk_blocks = 0;
+  int32_t n_partials = 0;
+};
+
+class HostState {
+ public:
+  kv_pool_config_t cfg{};
+  BlockAllocator alloc;
+  std::unordered_map<int64_t, Request> reqs;
+  std::vector<int32_t> free_slots;
+  uint64_t epoch = 1;  // bumped whenever any request's blocks or length change
+
+  static int32_t validate(const kv_pool_config_t& c) {
+    if (c.num_layers < 1 || c.num_q_heads < 1 || c.num_kv_heads < 1) return KV_ERR_INVALID;
+    if (c.head_dim != 64 && c.head_dim != 128) return KV_ERR_INVALID;
+    if (c.block_size != 16) return KV_ERR_INVALID;
+    if (c.num_q_heads % c.num_kv_heads != 0 || c.num_q_heads / c.num_kv_heads > 8) return KV_ERR_INVALID;
+    if (c.num_blocks < 1 || c.num_blocks > 0x7fffffffLL) return KV_ERR_INVALID;
+    if (c.max_requests < 1 || c.max_blocks_per_request < 1) return KV_ERR_INVALID;
+    if (static_cast<int64_t>(c.max_requests) * c.max_blocks_per_request > (1LL << 31)) return KV_ERR_INVALID;
+    return KV_OK;
+  }
+
+  void init(const kv_pool_config_t& c) {
+    cfg = c;
+    alloc.init(c.num_blocks, c.alloc_seed);
+    free_slots.resize(static_cast<size_t>(c.max_requests));
+    for (int32_t i = 0; i < c.max_requests; ++i) free_slots[static_cast<size_t>(i)] = c.max_requests - 1 - i;
+  }
+
+  int32_t blocks_for(int64_t tokens) const {
+    return static_cast<int32_t>((tokens + cfg.block_size - 1) / cfg.block_size);
+  }
+
+  // a1.  Atomic over the batch: validate everything, then mutate.
+  int32_t reserve(int32_t n_req, const int64_t* ids, const int32_t* n_tokens) {
+    if (n_req < 0 || (n_req > 0 && (!ids || !n_tokens))) return KV_ERR_INVALID;
+    std::unordered_set<int64_t> seen;
+    int64_t need_blocks = 0;
+    int32_t need_slots = 0;
+    for (int32_t i = 0; i < n_req; ++i) {
+      if (n_tokens[i] < 0) return KV_ERR_INVALID;
+      if (!seen.insert(ids[i]).second) return KV_ERR_INVALID;
+      auto it = reqs.find(ids[i]);
+      int64_t len = it == reqs.end() ? 0 : it->second.len;
+      int64_t new_len = len + n_tokens[i];
+      if (new_len > static_cast<int64_t>(cfg.max_blocks_per_request) * cfg.block_size) return KV_ERR_TOO_LONG;
+      need_blocks += blocks_for(new_len) - blocks_for(len);
+      if (it == reqs.end()) ++need_slots;
+    }
+    if (need_slots > static_cast<int32_t>(free_slots.size())) return KV_ERR_TOO_MANY_REQUESTS;
+    if (need_blocks > alloc.free_count()) return KV_ERR_NO_BLOCKS;
+    for (int32_t i = 0; i < n_req; ++i) {
+      auto it = reqs.find(ids[i]);
+      if (it == reqs.end()) {
+        Request r;
+        r.slot = free_slots.back();
+        free_slots.pop_back();
+        it = reqs.emplace(ids[i], std::move(r)).first;
+      }
+      Request& r = it->second;
+      int32_t want = blocks_for(static_cast<int64_t>(r.len) + n_tokens[i]);
+      while (static_cast<int32_t>(r.blocks.size()) < want) r.blocks.push_back(alloc.pop());
+      r.len += n_tokens[i];
+      r.last_n = n_tokens[i];
+    }
+    ++epoch;
+    return KV_OK;
+  }
+
+  // a6.  Atomic: unknown or duplicate id => nothing freed.
+  int32_t release(int32_t n_req, const int64_t* ids) {
+    if (n_req < 0 || (n_req > 0 && !ids)) return KV_ERR_INVALID;
+    std::unordered_set<int64_t> seen;
+    for (int32_t i = 0; i < n_req; ++i) {
+      if (!seen.insert(ids[i]).second) return KV_ERR_INVALID;
+      if (reqs.find(ids[i]) == reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
+    }
+    for (int32_t i = 0; i < n_req; ++i) {
+      auto it = reqs.find(ids[i]);
+      Request& r = it->second;
+      for (auto b = r.blocks.rbegin(); b != r.blocks.rend(); ++b) alloc.push(*b);
+      free_slots.push_back(r.slot);
+      reqs.erase(it);
+    }
+    ++epoch;
+    return KV_OK;
+  }
+
+  // Work-list half of a4.  `slots` = resident warps the main kernel will run; the planner aims
+  // at `items_per_slot` near-uniform items per slot so that dynamic scheduling has a short tail,
+  // while keeping chunks >= min_chunk_blocks so split-KV partial traffic stays << KV traffic.
+  int32_t plan_decode(int32_t batch, const int64_t* ids, int32_t slots, int32_t items_per_slot,
+                      int32_t min_chunk_blocks, int32_t max_partials, DecodePlan* plan) const {
+    if (batch < 1 || !ids || batch > cfg.max_requests) return KV_ERR_INVALID;
+    std::vector<const Request*> rs(static_cast<size_t>(batch));
+    std::unordered_set<int64_t> seen;
+    int64_t total_blocks = 0;
+    for (int32_t i = 0; i < batch; ++i) {
+      if (!seen.insert(ids[i]).second) return KV_ERR_INVALID;
+      auto it = reqs.find(ids[i]);
+      if (it == reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
+      if (it->second.len < 1) return KV_ERR_INVALID;
+      rs[static_cast<size_t>(i)] = &it->second;
+      total_blocks += blocks_for(it->second.len);
+    }
+    const int64_t total_tiles = total_blocks * cfg.num_kv_heads;
+    const int64_t target_items = std::max<int64_t>(1, static_cast<int64_t>(slots) * items_per_slot);
+    int64_t chunk = std::max<int64_t>(min_chunk_blocks, (total_tiles + target_items - 1) / target_items);
+    for (;;) {  // grow the chunk until the partials fit the workspace
+      int64_t partials = 0;
+      for (const Request* r : rs) {
+        int64_t nc = (blocks_for(r->len) + chunk - 1) / chunk;
+        if (nc > 1) partials += nc * cfg.num_kv_heads;
+      }
+      if (partials <= max_partials) break;
+      chunk *= 2;
+    }
+    plan->items.clear();
+    plan->combines.clear();
+    plan->chunk_blocks = static_cast<int32_t>(chunk);
+    int32_t next_partial = 0;
+    for (int32_t i = 0; i < batch; ++i) {
+      const Request* r = rs[static_cast<size_t>(i)];
+      const int32_t nb = blocks_for(r->len);
+      const int32_t nc0 = static_cast<int32_t>((nb + chunk - 1) / chunk);
+      const int32_t per = (nb + nc0 - 1) / nc0;  // even split: ceil(nb / nc0) <= chunk blocks per chunk
+      const int32_t nc = (nb + per - 1) / per;   // <= nc0
+      for (int32_t h = 0; h < cfg.num_kv_heads; ++h) {
+        if (nc > 1) plan->combines.push_back({i, h, next_partial, nc});
+        for (int32_t c = 0; c < nc; ++c) {
+          WorkItem w;
+          w.batch_idx = i;
+          w.slot = r->slot;
+          w.kv_head = h;
+          w.blk_begin = c * per;
+          w.n_blocks = std::min(per, nb - c * per);
+          w.n_tokens = std::min(r->len - w.blk_begin * cfg.block_size, w.n_blocks * cfg.block_size);
+          w.partial_idx = nc > 1 ? next_partial++ : -1;
+          w.pad = 0;
+          plan->items.push_back(w);
+        }
+      }
+    }
+    plan->n_partials = next_partial;
+    std::stable_sort(plan->items.begin(), plan->items.end(),
+                     [](const WorkItem& a, const WorkItem& b) { return a.n_blocks > b.n_blocks; });
+    return KV_OK;
+  }
+};
+
+}  // namespace kvp

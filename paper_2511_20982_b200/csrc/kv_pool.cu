@@ -1,0 +1,482 @@
+// kv_pool.cu — the C-ABI of include/kv_pool.h: argument checking, host bookkeeping
+// (kv_host.h), staging of small descriptor blobs, and kernel launches (kv_kernels.cuh).
+// Every step of the data path runs in the kernels; nothing here touches KV bytes on the host.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/kv_pool.h"
+#include "kv_host.h"
+#include "kv_kernels.cuh"
+
+namespace {
+
+using namespace kvp;
+
+constexpr int64_t kAlign = 256;
+constexpr int kRing = 4;                       // staging slots per blob kind
+constexpr int64_t kIngestBlobBytes = 1 << 20;  // per ingest launch; larger calls are sub-batched
+constexpr int32_t kMaxPartials = 32768;        // split-KV partial slots in the workspace
+
+inline int64_t align_up(int64_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+struct Layout {  // byte offsets inside the caller's slab
+  int64_t kv_bytes, block_table, counters, ingest_blobs, plan_blobs, part_o, part_ml, total;
+  int64_t plan_blob_bytes;
+};
+
+Layout make_layout(const kv_pool_config_t& c) {
+  Layout L{};
+  const int64_t G = c.num_q_heads / c.num_kv_heads;
+  L.kv_bytes = static_cast<int64_t>(c.num_layers) * c.num_blocks * c.num_kv_heads * 2 * c.block_size * c.head_dim * 2;
+  int64_t off = align_up(L.kv_bytes);
+  L.block_table = off;
+  off = align_up(off + static_cast<int64_t>(c.max_requests) * c.max_blocks_per_request * 4);
+  L.counters = off;
+  off = align_up(off + 256);
+  L.ingest_blobs = off;
+  off = align_up(off + kRing * kIngestBlobBytes);
+  const int64_t items_cap = static_cast<int64_t>(c.max_requests) * c.num_kv_heads + kMaxPartials;
+  const int64_t comb_cap = static_cast<int64_t>(c.max_requests) * c.num_kv_heads;
+  L.plan_blob_bytes = align_up(items_cap * static_cast<int64_t>(sizeof(WorkItem)) + comb_cap * static_cast<int64_t>(sizeof(CombineEntry)));
+  L.plan_blobs = off;
+  off = align_up(off + kRing * L.plan_blob_bytes);
+  L.part_o = off;
+  off = align_up(off + static_cast<int64_t>(kMaxPartials) * G * c.head_dim * 4);
+  L.part_ml = off;
+  off = align_up(off + static_cast<int64_t>(kMaxPartials) * G * 2 * 4);
+  L.total = off;
+  return L;
+}
+
+struct StageSlot {
+  char* host = nullptr;   // pinned
+  char* dev = nullptr;    // inside the slab
+  cudaEvent_t ev = nullptr;
+  bool in_flight = false;
+};
+
+}  // namespace
+
+struct kv_pool {
+  kvp::HostState hs;
+  Layout lay{};
+  bool has_device = false;
+  char* base = nullptr;
+  int num_sms = 148;
+  int32_t last_cuda = 0;
+  int64_t launches = 0;
+  // tuning
+  int32_t min_chunk_blocks = 16;
+  int32_t ctas_per_sm = 2;
+  int32_t items_per_slot = 8;
+  // staging
+  StageSlot ingest_ring[kRing], plan_ring[kRing];
+  int ingest_next = 0, plan_next = 0;
+  // cached decode plan (reused across the layers of one step)
+  uint64_t plan_epoch = 0;
+  std::vector<int64_t> plan_ids;
+  int plan_slot = -1;
+  int32_t plan_n_items = 0, plan_n_combines = 0;
+  int64_t plan_combine_off = 0;
+  kvp::DecodePlan plan;
+
+  int32_t cuda_fail(cudaError_t e) {
+    last_cuda = static_cast<int32_t>(e);
+    return KV_ERR_CUDA;
+  }
+  int32_t slots() const { return num_sms * ctas_per_sm * kvp::kAttnWarps; }
+};
+
+namespace {
+
+#define KV_CUDA(pool, expr)                                   \
+  do {                                                        \
+    cudaError_t e_ = (expr);                                  \
+    if (e_ != cudaSuccess) return (pool)->cuda_fail(e_);      \
+  } while (0)
+
+int32_t acquire(kv_pool* pool, StageSlot* ring, int* next, StageSlot** out, int avoid = -1) {
+  int idx = *next;
+  if (idx == avoid) idx = (idx + 1) % kRing;
+  *next = (idx + 1) % kRing;
+  StageSlot& s = ring[idx];
+  if (s.in_flight) {
+    KV_CUDA(pool, cudaEventSynchronize(s.ev));
+    s.in_flight = false;
+  }
+  *out = &s;
+  return idx;
+}
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+template <bool kGather>
+int32_t launch_ingest(kv_pool* pool, const std::vector<IngestReq>& reqs, const std::vector<int32_t>& ids,
+                      int64_t total_units, int32_t layer_begin, int32_t layer_count, cudaStream_t stream) {
+  if (total_units == 0) return KV_OK;
+  StageSlot* s = nullptr;
+  int32_t rc = acquire(pool, pool->ingest_ring, &pool->ingest_next, &s);
+  if (rc < 0) return rc;
+  const size_t req_bytes = reqs.size() * sizeof(IngestReq);
+  const size_t id_bytes = ids.size() * sizeof(int32_t);
+  std::memcpy(s->host, reqs.data(), req_bytes);
+  std::memcpy(s->host + req_bytes, ids.data(), id_bytes);
+  KV_CUDA(pool, cudaMemcpyAsync(s->dev, s->host, req_bytes + id_bytes, cudaMemcpyHostToDevice, stream));
+  const kv_pool_config_t& c = pool->hs.cfg;
+  IngestParams p{};
+  p.reqs = reinterpret_cast<const IngestReq*>(s->dev);
+  p.blk_ids = reinterpret_cast<const int32_t*>(s->dev + req_bytes);
+  p.n_req = static_cast<int32_t>(reqs.size());
+  p.total_units = total_units;
+  p.kv = reinterpret_cast<uint16_t*>(pool->base);
+  p.block_table = reinterpret_cast<int32_t*>(pool->base + pool->lay.block_table);
+  p.bt_stride = c.max_blocks_per_request;
+  p.layer_begin = layer_begin;
+  p.layer_count = layer_count;
+  p.num_kv_heads = c.num_kv_heads;
+  p.num_blocks = c.num_blocks;
+  const unsigned grid = static_cast<unsigned>((total_units + kIngestWarps - 1) / kIngestWarps);
+  if (c.head_dim == 128)
+    ingest_kernel<128, kGather><<<grid, kIngestThreads, 0, stream>>>(p);
+  else
+    ingest_kernel<64, kGather><<<grid, kIngestThreads, 0, stream>>>(p);
+  KV_CUDA(pool, cudaGetLastError());
+  ++pool->launches;
+  KV_CUDA(pool, cudaEventRecord(s->ev, stream));
+  s->in_flight = true;
+  return KV_OK;
+}
+
+// Serialise requests into ingest launches, sub-batching so each blob fits its staging slot.
+template <bool kGather>
+int32_t run_ingest(kv_pool* pool, int32_t n_req, const int64_t* req_ids, const int32_t* n_tokens,
+                   const void* const* k_ptrs, const void* const* v_ptrs, const int32_t* start_pos,
+                   int32_t layer_begin, int32_t layer_count, cudaStream_t stream) {
+  const kv_pool_config_t& c = pool->hs.cfg;
+  std::vector<IngestReq> reqs;
+  std::vector<int32_t> ids;
+  int64_t units = 0;
+  auto flush = [&]() -> int32_t {
+    int32_t rc = launch_ingest<kGather>(pool, reqs, ids, units, layer_begin, layer_count, stream);
+    reqs.clear();
+    ids.clear();
+    units = 0;
+    return rc;
+  };
+  for (int32_t i = 0; i < n_req; ++i) {
+    if (n_tokens[i] == 0) continue;
+    const Request& r = pool->hs.reqs.find(req_ids[i])->second;
+    const int32_t sp = start_pos[i];
+    const int32_t b0 = sp / c.block_size;
+    const int32_t b1 = (sp + n_tokens[i] - 1) / c.block_size;
+    const int32_t touched = b1 - b0 + 1;
+    const int64_t need = static_cast<int64_t>(sizeof(IngestReq)) + 4LL * touched;
+    const int64_t used = static_cast<int64_t>(reqs.size() * sizeof(IngestReq) + ids.size() * 4);
+    if (need > kIngestBlobBytes) return KV_ERR_TOO_LONG;
+    if (used + need > kIngestBlobBytes) {
+      int32_t rc = flush();
+      if (rc != KV_OK) return rc;
+    }
+    IngestReq q{};
+    q.k_src = reinterpret_cast<uint64_t>(k_ptrs[i]);
+    q.v_src = reinterpret_cast<uint64_t>(v_ptrs[i]);
+    q.unit_begin = units;
+    q.n_tokens = n_tokens[i];
+    q.start_pos = sp;
+    q.slot = r.slot;
+    q.blk0 = b0;
+    q.n_touched = touched;
+    q.blk_off = static_cast<int32_t>(ids.size());
+    reqs.push_back(q);
+    ids.insert(ids.end(), r.blocks.begin() + b0, r.blocks.begin() + b1 + 1);
+    units += static_cast<int64_t>(touched) * layer_count * c.num_kv_heads;
+  }
+  return flush();
+}
+
+int32_t check_ids_known(const kv_pool* pool, int32_t n, const int64_t* ids) {
+  for (int32_t i = 0; i < n; ++i)
+    if (pool->hs.reqs.find(ids[i]) == pool->hs.reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
+  return KV_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int64_t kv_pool_kv_bytes(const kv_pool_config_t* cfg) {
+  if (!cfg) return KV_ERR_INVALID;
+  int32_t rc = HostState::validate(*cfg);
+  if (rc != KV_OK) return rc;
+  return make_layout(*cfg).kv_bytes;
+}
+
+int64_t kv_pool_required_bytes(const kv_pool_config_t* cfg) {
+  if (!cfg) return KV_ERR_INVALID;
+  int32_t rc = HostState::validate(*cfg);
+  if (rc != KV_OK) return rc;
+  return make_layout(*cfg).total;
+}
+
+int32_t kv_pool_create(const kv_pool_config_t* cfg, kv_pool_t** out_pool) {
+  if (!cfg || !out_pool) return KV_ERR_INVALID;
+  *out_pool = nullptr;
+  int32_t rc = HostState::validate(*cfg);
+  if (rc != KV_OK) return rc;
+  const Layout lay = make_layout(*cfg);
+  if (cfg->device_base) {
+    if ((reinterpret_cast<uintptr_t>(cfg->device_base) & (kAlign - 1)) != 0) return KV_ERR_INVALID;
+    if (cfg->device_bytes < lay.total) return KV_ERR_INVALID;
+  }
+  kv_pool* pool = new (std::nothrow) kv_pool();
+  if (!pool) return KV_ERR_INVALID;
+  pool->hs.init(*cfg);
+  pool->lay = lay;
+  if (cfg->device_base) {
+    pool->has_device = true;
+    pool->base = static_cast<char*>(cfg->device_base);
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&pool->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    for (int i = 0; e == cudaSuccess && i < kRing; ++i) {
+      e = cudaHostAlloc(reinterpret_cast<void**>(&pool->ingest_ring[i].host), kIngestBlobBytes, cudaHostAllocDefault);
+      if (e == cudaSuccess) e = cudaHostAlloc(reinterpret_cast<void**>(&pool->plan_ring[i].host), lay.plan_blob_bytes, cudaHostAllocDefault);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pool->ingest_ring[i].ev, cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pool->plan_ring[i].ev, cudaEventDisableTiming);
+      pool->ingest_ring[i].dev = pool->base + lay.ingest_blobs + i * kIngestBlobBytes;
+      pool->plan_ring[i].dev = pool->base + lay.plan_blobs + i * lay.plan_blob_bytes;
+    }
+    // work counters start at zero; the attention kernel rewinds them itself afterwards
+    if (e == cudaSuccess) e = cudaMemset(pool->base + lay.counters, 0, 256);
+    if (e != cudaSuccess) {
+      kv_pool_destroy(pool);
+      return KV_ERR_CUDA;
+    }
+  }
+  *out_pool = pool;
+  return KV_OK;
+}
+
+int32_t kv_pool_destroy(kv_pool_t* pool) {
+  if (!pool) return KV_ERR_INVALID;
+  for (int i = 0; i < kRing; ++i) {
+    if (pool->ingest_ring[i].host) cudaFreeHost(pool->ingest_ring[i].host);
+    if (pool->plan_ring[i].host) cudaFreeHost(pool->plan_ring[i].host);
+    if (pool->ingest_ring[i].ev) cudaEventDestroy(pool->ingest_ring[i].ev);
+    if (pool->plan_ring[i].ev) cudaEventDestroy(pool->plan_ring[i].ev);
+  }
+  delete pool;
+  return KV_OK;
+}
+
+int32_t kv_reserve(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const int32_t* n_tokens) {
+  if (!pool) return KV_ERR_INVALID;
+  return pool->hs.reserve(n_req, req_ids, n_tokens);
+}
+
+int32_t kv_ingest(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const int32_t* n_tokens,
+                  const void* const* k_src, const void* const* v_src, int32_t layer_begin, int32_t layer_count,
+                  void* cuda_stream) {
+  if (!pool || n_req < 0) return KV_ERR_INVALID;
+  if (n_req > 0 && (!req_ids || !n_tokens || !k_src || !v_src)) return KV_ERR_INVALID;
+  const kv_pool_config_t& c = pool->hs.cfg;
+  if (layer_begin < 0 || layer_count < 1 || layer_begin + layer_count > c.num_layers) return KV_ERR_INVALID;
+  if (!pool->has_device) return KV_ERR_NO_DEVICE;
+  for (int32_t i = 0; i < n_req; ++i) {
+    if (n_tokens[i] < 0) return KV_ERR_INVALID;
+    if (n_tokens[i] > 0 && (!k_src[i] || !v_src[i] || !aligned16(k_src[i]) || !aligned16(v_src[i]))) return KV_ERR_INVALID;
+  }
+  if (layer_begin == 0) {
+    int32_t rc = pool->hs.reserve(n_req, req_ids, n_tokens);
+    if (rc != KV_OK) return rc;
+  } else {  // continuation of the last reservation
+    std::unordered_set<int64_t> seen;
+    for (int32_t i = 0; i < n_req; ++i) {
+      if (!seen.insert(req_ids[i]).second) return KV_ERR_INVALID;
+      auto it = pool->hs.reqs.find(req_ids[i]);
+      if (it == pool->hs.reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
+      if (it->second.last_n != n_tokens[i]) return KV_ERR_INVALID;
+    }
+  }
+  std::vector<int32_t> start(static_cast<size_t>(n_req));
+  for (int32_t i = 0; i < n_req; ++i) start[static_cast<size_t>(i)] = pool->hs.reqs.find(req_ids[i])->second.len - n_tokens[i];
+  return run_ingest<false>(pool, n_req, req_ids, n_tokens, k_src, v_src, start.data(), layer_begin, layer_count,
+                           static_cast<cudaStream_t>(cuda_stream));
+}
+
+int32_t kv_gather(kv_pool_t* pool, int64_t req_id, void* k_dst, void* v_dst, void* cuda_stream) {
+  if (!pool || !k_dst || !v_dst || !aligned16(k_dst) || !aligned16(v_dst)) return KV_ERR_INVALID;
+  if (!pool->has_device) return KV_ERR_NO_DEVICE;
+  auto it = pool->hs.reqs.find(req_id);
+  if (it == pool->hs.reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
+  const int32_t n = it->second.len, zero = 0;
+  const void* kp = k_dst;
+  const void* vp = v_dst;
+  return run_ingest<true>(pool, 1, &req_id, &n, &kp, &vp, &zero, 0, pool->hs.cfg.num_layers,
+                          static_cast<cudaStream_t>(cuda_stream));
+}
+
+int32_t kv_free(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids) {
+  if (!pool) return KV_ERR_INVALID;
+  return pool->hs.release(n_req, req_ids);
+}
+
+int32_t kv_block_table(const kv_pool_t* pool, int64_t req_id, int32_t* out_blocks, int32_t cap, int32_t* out_n_blocks,
+                       int32_t* out_len) {
+  if (!pool || cap < 0 || (cap > 0 && !out_blocks)) return KV_ERR_INVALID;
+  auto it = pool->hs.reqs.find(req_id);
+  if (it == pool->hs.reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
+  const Request& r = it->second;
+  const int32_t nb = static_cast<int32_t>(r.blocks.size());
+  for (int32_t i = 0; i < std::min(nb, cap); ++i) out_blocks[i] = r.blocks[static_cast<size_t>(i)];
+  if (out_n_blocks) *out_n_blocks = nb;
+  if (out_len) *out_len = r.len;
+  return KV_OK;
+}
+
+int32_t kv_pool_stats(const kv_pool_t* pool, int64_t* blocks_total, int64_t* blocks_free, int32_t* live_requests,
+                      int64_t* blocks_high_water) {
+  if (!pool) return KV_ERR_INVALID;
+  if (blocks_total) *blocks_total = pool->hs.alloc.total();
+  if (blocks_free) *blocks_free = pool->hs.alloc.free_count();
+  if (live_requests) *live_requests = static_cast<int32_t>(pool->hs.reqs.size());
+  if (blocks_high_water) *blocks_high_water = pool->hs.alloc.high_water();
+  return KV_OK;
+}
+
+int32_t kv_plan_decode(kv_pool_t* pool, int32_t batch, const int64_t* req_ids, int32_t* out_items, int32_t cap_items,
+                       int32_t* out_n_items, int32_t* out_chunk_blocks) {
+  if (!pool || cap_items < 0 || (cap_items > 0 && !out_items)) return KV_ERR_INVALID;
+  DecodePlan plan;
+  int32_t rc = pool->hs.plan_decode(batch, req_ids, pool->slots(), pool->items_per_slot, pool->min_chunk_blocks,
+                                    kMaxPartials, &plan);
+  if (rc != KV_OK) return rc;
+  const int32_t n = static_cast<int32_t>(plan.items.size());
+  for (int32_t i = 0; i < std::min(n, cap_items); ++i) {
+    const WorkItem& w = plan.items[static_cast<size_t>(i)];
+    int32_t* o = out_items + 5 * i;
+    o[0] = w.batch_idx; o[1] = w.kv_head; o[2] = w.blk_begin; o[3] = w.n_blocks; o[4] = w.partial_idx;
+  }
+  if (out_n_items) *out_n_items = n;
+  if (out_chunk_blocks) *out_chunk_blocks = plan.chunk_blocks;
+  return KV_OK;
+}
+
+int32_t paged_decode_attention(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const void* q,
+                               void* out, float sm_scale, void* cuda_stream) {
+  if (!pool || !req_ids || !q || !out || !aligned16(q) || !aligned16(out)) return KV_ERR_INVALID;
+  const kv_pool_config_t& c = pool->hs.cfg;
+  if (layer < 0 || layer >= c.num_layers || batch < 1) return KV_ERR_INVALID;
+  if (!pool->has_device) return KV_ERR_NO_DEVICE;
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+
+  // plan: reuse across the layers of a step (same ids, no reserve/free since)
+  const bool cached = pool->plan_slot >= 0 && pool->plan_epoch == pool->hs.epoch &&
+                      static_cast<int32_t>(pool->plan_ids.size()) == batch &&
+                      std::memcmp(pool->plan_ids.data(), req_ids, sizeof(int64_t) * static_cast<size_t>(batch)) == 0;
+  if (!cached) {
+    int32_t rc = pool->hs.plan_decode(batch, req_ids, pool->slots(), pool->items_per_slot, pool->min_chunk_blocks,
+                                      kMaxPartials, &pool->plan);
+    if (rc != KV_OK) return rc;
+    StageSlot* s = nullptr;
+    int idx = acquire(pool, pool->plan_ring, &pool->plan_next, &s);
+    if (idx < 0) return idx;
+    const size_t item_bytes = pool->plan.items.size() * sizeof(WorkItem);
+    const size_t comb_bytes = pool->plan.combines.size() * sizeof(CombineEntry);
+    if (static_cast<int64_t>(item_bytes + comb_bytes) > pool->lay.plan_blob_bytes) return KV_ERR_INVALID;
+    std::memcpy(s->host, pool->plan.items.data(), item_bytes);
+    std::memcpy(s->host + item_bytes, pool->plan.combines.data(), comb_bytes);
+    pool->plan_slot = -1;
+    KV_CUDA(pool, cudaMemcpyAsync(s->dev, s->host, item_bytes + comb_bytes, cudaMemcpyHostToDevice, stream));
+    pool->plan_slot = idx;
+    pool->plan_epoch = pool->hs.epoch;
+    pool->plan_ids.assign(req_ids, req_ids + batch);
+    pool->plan_n_items = static_cast<int32_t>(pool->plan.items.size());
+    pool->plan_n_combines = static_cast<int32_t>(pool->plan.combines.size());
+    pool->plan_combine_off = static_cast<int64_t>(item_bytes);
+  }
+  StageSlot& s = pool->plan_ring[pool->plan_slot];
+  const int32_t G = c.num_q_heads / c.num_kv_heads;
+  const float scale = sm_scale > 0.f ? sm_scale : 1.0f / std::sqrt(static_cast<float>(c.head_dim));
+
+  AttnParams p{};
+  const int64_t layer_elems = c.num_blocks * c.num_kv_heads * 2LL * c.block_size * c.head_dim;
+  p.kv_layer = reinterpret_cast<const uint16_t*>(pool->base) + static_cast<int64_t>(layer) * layer_elems;
+  p.block_table = reinterpret_cast<const int32_t*>(pool->base + pool->lay.block_table);
+  p.bt_stride = c.max_blocks_per_request;
+  p.items = reinterpret_cast<const WorkItemDev*>(s.dev);
+  p.n_items = pool->plan_n_items;
+  p.q = static_cast<const uint16_t*>(q);
+  p.out = static_cast<uint16_t*>(out);
+  p.part_o = reinterpret_cast<float*>(pool->base + pool->lay.part_o);
+  p.part_ml = reinterpret_cast<float*>(pool->base + pool->lay.part_ml);
+  p.counters = reinterpret_cast<int32_t*>(pool->base + pool->lay.counters);
+  p.num_q_heads = c.num_q_heads;
+  p.num_kv_heads = c.num_kv_heads;
+  p.group = G;
+  p.scale_log2 = scale * 1.4426950408889634f;
+  const int32_t want = (p.n_items + kAttnWarps - 1) / kAttnWarps;
+  const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * pool->ctas_per_sm)));
+  if (c.head_dim == 128)
+    attn_splitkv_kernel<128><<<grid, kAttnThreads, 0, stream>>>(p);
+  else
+    attn_splitkv_kernel<64><<<grid, kAttnThreads, 0, stream>>>(p);
+  KV_CUDA(pool, cudaGetLastError());
+  ++pool->launches;
+
+  if (pool->plan_n_combines > 0) {
+    CombineParams cp{};
+    cp.entries = reinterpret_cast<const CombineEntryDev*>(s.dev + pool->plan_combine_off);
+    cp.n_entries = pool->plan_n_combines;
+    cp.part_o = p.part_o;
+    cp.part_ml = p.part_ml;
+    cp.out = p.out;
+    cp.num_q_heads = c.num_q_heads;
+    cp.group = G;
+    const unsigned cgrid = static_cast<unsigned>((static_cast<int64_t>(cp.n_entries) * G + 3) / 4);
+    if (c.head_dim == 128)
+      combine_kernel<128><<<cgrid, 128, 0, stream>>>(cp);
+    else
+      combine_kernel<64><<<cgrid, 128, 0, stream>>>(cp);
+    KV_CUDA(pool, cudaGetLastError());
+    ++pool->launches;
+  }
+  KV_CUDA(pool, cudaEventRecord(s.ev, stream));
+  s.in_flight = true;
+  return KV_OK;
+}
+
+int64_t kv_launch_count(const kv_pool_t* pool) { return pool ? pool->launches : KV_ERR_INVALID; }
+
+int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
+  if (!pool || !key) return KV_ERR_INVALID;
+  pool->plan_slot = -1;  // any option may change the plan
+  if (!std::strcmp(key, "min_chunk_blocks") && value >= 1 && value <= 65536) { pool->min_chunk_blocks = static_cast<int32_t>(value); return KV_OK; }
+  if (!std::strcmp(key, "ctas_per_sm") && value >= 1 && value <= 8) { pool->ctas_per_sm = static_cast<int32_t>(value); return KV_OK; }
+  if (!std::strcmp(key, "items_per_slot") && value >= 1 && value <= 1024) { pool->items_per_slot = static_cast<int32_t>(value); return KV_OK; }
+  return KV_ERR_INVALID;
+}
+
+int32_t kv_last_cuda_error(const kv_pool_t* pool) { return pool ? pool->last_cuda : KV_ERR_INVALID; }
+
+const char* kv_strerror(int32_t status) {
+  switch (status) {
+    case KV_OK: return "ok";
+    case KV_ERR_INVALID: return "invalid argument";
+    case KV_ERR_NO_BLOCKS: return "KV pool exhausted (nothing changed)";
+    case KV_ERR_UNKNOWN_REQUEST: return "unknown request id";
+    case KV_ERR_TOO_LONG: return "request exceeds max_blocks_per_request";
+    case KV_ERR_TOO_MANY_REQUESTS: return "more than max_requests live requests";
+    case KV_ERR_CUDA: return "CUDA runtime error (see kv_last_cuda_error)";
+    case KV_ERR_NO_DEVICE: return "pool has no device slab (host-only)";
+    default: return "unknown status";
+  }
+}
+
+const char* kv_version(void) { return "0.1.0"; }
+
+}  // extern "C"
