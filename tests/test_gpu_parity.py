@@ -240,8 +240,11 @@ def test_p3_needle_every_boundary(opts):
     q = np.broadcast_to(qf, (len(positions), 1, d)).copy()
     out, want = run_structured(1, 1, d, lens, K, V, q, options=opts)
     got = bits_to_f64(bits_of(out))
+    # the other 1039 tokens weigh e^-45 each: the exact answer is V_needle + O(1e-15), which bf16
+    # keeps as a tiny non-zero where V_needle is 0 — hence a 1e-9 band instead of equality
     for r, pos in enumerate(positions):
-        assert got[r, 0, 0] == pos % 128 and got[r, 0, 1] == pos // 128, (pos, got[r, 0, :2])
+        assert abs(got[r, 0, 0] - pos % 128) <= 1e-9 and abs(got[r, 0, 1] - pos // 128) <= 1e-9, (pos, got[r, 0, :2])
+        assert np.all(np.abs(got[r, 0] - want[r, 0]) <= 2 ** -7 * np.abs(want[r, 0]) + 1e-30)
 
 
 def test_p13_large_scores_do_not_overflow():
