@@ -1,0 +1,481 @@
+#!/usr/bin/env python
+"""bench.py — decode-attention + KV-ingest HBM throughput of the D-instance KV path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3_8b_gqa] [--impl cuda|reference]
+
+One "step" is one pass of the whole hot path over one decode batch of
+a BASELINE.json workload: retire finished requests, ingest the newly prefilled ones, and for
+every layer append the new token's K/V and run paged decode attention + LSE combine
+(paper_2511_20982_b200/engine.py).  Prints ONE JSON line (rank 0).
+
+  value     algorithmic bytes (attention + ingest + append) of the K timed steps
+            / device time, GB/s, inputs resident in HBM, max over ranks, summed over ranks
+  e2e       the same metric through the host-buffer C-ABI calls (kv_ingest_host,
+            paged_decode_attention_host): every step's q, appended K/V and arriving requests' K/V
+            come from pinned host memory and the outputs go back to it, inside the timed region
+  roofline  attn_splitkv_kernel: algorithmic bytes per launch / mean launch duration (CUDA event
+            pairs recorded by the library around every launch of the timed region)
+  cpu_baseline  the fp64 oracle timed on this box's host cores on a bounded sample
+
+Multi-GPU: the path shards by request with no exchange step: N independent
+replicas, one process per GPU, weak scaling; torch.distributed is used for the barrier and
+the max-over-ranks time only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "decode-attn + KV-ingest HBM GB/s"
+NOMINAL_HBM_GBS = 8000.0          # BASELINE.json north_star: "B200 HBM peak (~8 TB/s)"
+FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+DEFAULT_WORKLOAD = "cfg3_8b_gqa"  # first BASELINE.json config with both legs of the metric
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=32)
+    ap.add_argument("--warmup", type=int, default=4)
+    ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
+    ap.add_argument("--streams", type=int, default=2, help="2: ingest on its own stream, overlapping attention")
+    ap.add_argument("--e2e-steps", type=int, default=4, help="timed steps of the host-buffer leg (0 = skip)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-isolated", action="store_true", help="skip the attention-alone / ingest-alone legs")
+    ap.add_argument("--opt", action="append", default=[], help="pool option key=value (tuning)")
+    return ap.parse_args()
+
+
+def hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+# ---------------------------------------------------------------------------------------------
+# clocks during the timed region: a side process polls NVML every 10 ms
+# ---------------------------------------------------------------------------------------------
+_SAMPLER = r"""
+import sys, time
+import pynvml as N
+N.nvmlInit()
+h = N.nvmlDeviceGetHandleByIndex(int(sys.argv[1]))
+mx = N.nvmlDeviceGetMaxClockInfo(h, N.NVML_CLOCK_SM)
+out = open(sys.argv[2], "w")
+out.write("max %d\n" % mx); out.flush()
+while True:
+    try:
+        c = N.nvmlDeviceGetClockInfo(h, N.NVML_CLOCK_SM)
+        r = N.nvmlDeviceGetCurrentClocksEventReasons(h)
+        p = N.nvmlDeviceGetPowerUsage(h)
+        out.write("%.6f %d %d %d\n" % (time.time(), c, r, p)); out.flush()
+    except Exception as e:
+        out.write("err %r\n" % (e,)); out.flush()
+    time.sleep(0.01)
+"""
+_REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+            0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+            0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+
+class ClockSampler:
+    def __init__(self, index: int):
+        self.path = tempfile.mktemp(prefix="kvclocks_", suffix=".txt")
+        self.windows = []
+        try:
+            self.proc = subprocess.Popen([sys.executable, "-c", _SAMPLER, str(index), self.path],
+                                         stdout=subprocess.DEVNULL, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def window(self, t0: float, t1: float):
+        self.windows.append((t0, t1))
+
+    def finish(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "note": "sampler unavailable"}
+        time.sleep(0.03)
+        self.proc.kill()
+        self.proc.wait()
+        mx, clocks, reasons, power = None, [], 0, []
+        try:
+            for line in open(self.path):
+                f = line.split()
+                if f[0] == "max":
+                    mx = int(f[1])
+                elif f[0] != "err" and len(f) == 4:
+                    t = float(f[0])
+                    if any(a - 0.005 <= t <= b + 0.005 for a, b in self.windows):
+                        clocks.append(int(f[1])); reasons |= int(f[2]); power.append(int(f[3]) / 1000.0)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        clocks.sort()
+        names = [n for bit, n in _REASONS.items() if reasons & bit and n != "gpu_idle"]
+        return {"sm_mhz": clocks[len(clocks) // 2] if clocks else None, "sm_max_mhz": mx, "reasons": names,
+                "samples": len(clocks), "power_w_max": max(power) if power else None}
+
+
+# ---------------------------------------------------------------------------------------------
+# the oracle on the host cores: cpu_baseline leg and the --impl reference arm
+# ---------------------------------------------------------------------------------------------
+class OracleSample:
+    """A bounded sample of a workload for the fp64 oracle: `reqs` = [(content uid, length)], one layer.
+    Builds a private host slab with sequential block lists, times oracle.scatter (ingest) and
+    oracle.attention, and returns the algorithmic bytes moved."""
+
+    def __init__(self, w, reqs, layer: int, q_bits):
+        import numpy as np
+        import oracle
+        from paper_2511_20982_b200 import workloads as W
+        self.w, self.reqs, self.layer, self.q_bits = w, reqs, layer, q_bits
+        bs = w.block_size
+        nblk = [(n + bs - 1) // bs for _, n in reqs]
+        self.dims = oracle.Dims(1, w.num_kv_heads, w.head_dim, bs, max(1, sum(nblk)))
+        self.lists, off = [], 0
+        for b in nblk:
+            self.lists.append(np.arange(off, off + b, dtype=np.int32))
+            off += b
+        bits = lambda t: t.contiguous().view(__import__("torch").int16).numpy().view(np.uint16)
+        self.src = [(bits(W.kv_values(w.seed, W.KIND_K, cu, w.num_kv_heads, w.head_dim, layer, 1, 0, n, "cpu")),
+                     bits(W.kv_values(w.seed, W.KIND_V, cu, w.num_kv_heads, w.head_dim, layer, 1, 0, n, "cpu")))
+                    for cu, n in reqs]
+
+    def run(self):
+        """-> (seconds scatter, seconds attention, out float64 [R][Hq][d])."""
+        import oracle
+        slab = oracle.new_slab(self.dims, 0x7FC0)
+        t0 = time.perf_counter()
+        for (k, v), bl in zip(self.src, self.lists):
+            oracle.scatter(slab, self.dims, bl, 0, k, v)
+        t1 = time.perf_counter()
+        out = oracle.attention(slab, self.dims, 0, self.w.num_q_heads, self.lists, [n for _, n in self.reqs],
+                               self.q_bits)
+        t2 = time.perf_counter()
+        return t1 - t0, t2 - t1, out
+
+    def bytes(self):
+        from paper_2511_20982_b200.engine import attention_bytes
+        lens = [n for _, n in self.reqs]
+        ingest = 2 * sum(lens) * 2 * self.w.num_kv_heads * self.w.head_dim * 2
+        return attention_bytes(self.w, lens), ingest
+
+
+def run_reference(args):
+    """Reference arm = the oracle as it stands on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import numpy as np
+    import oracle
+    from paper_2511_20982_b200 import workloads as W
+    w = W.CONFIGS[args.workload]
+    oracle.build()
+    lens = [int(n) for n in w.draw_lengths()]
+    budget_tokens = 120_000                      # ~0.5 s of oracle work per step on 8-16 cores
+    reqs, tot = [], 0
+    for i, n in enumerate(lens):
+        if reqs and tot + n > budget_tokens:
+            break
+        reqs.append((i, n)); tot += n
+    q = W.q_values(w.seed, 0, 0, w.batch, w.num_q_heads, w.head_dim, "cpu")[: len(reqs)]
+    q_bits = q.contiguous().view(__import__("torch").int16).numpy().view(np.uint16).copy()
+    smp = OracleSample(w, reqs, 0, q_bits)
+    for _ in range(args.warmup):
+        smp.run()
+    t = time.perf_counter()
+    for _ in range(args.steps):
+        smp.run()
+    dt = time.perf_counter() - t
+    ab, ib = smp.bytes()
+    val = (ab + ib) * args.steps / dt / 1e9
+    sample = f"{len(reqs)} requests ({tot} tokens) of {args.workload}, 1 of {w.num_layers} layers per step: scatter + attention"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "GB/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": "GB/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def cpu_baseline_and_check(loop, last_step: int, budget_s: float = 12.0):
+    """Oracle on a bounded sample of the LAST timed step's batch (last layer), timed on the host cores,
+    and compared with what the GPU wrote for those rows in that step."""
+    import numpy as np
+    import torch
+    import oracle
+    from paper_2511_20982_b200 import workloads as W
+    w, sp = loop.w, loop.sched.steps[last_step]
+    layer = w.num_layers - 1
+    q = loop.q[last_step][layer].cpu()
+    got = loop.out[last_step][layer].cpu()
+    bits = lambda t: t.contiguous().view(torch.int16).numpy().view(np.uint16).copy()
+    t_sc = t_at = 0.0
+    ab = ib = 0
+    n_req = tokens = 0
+    max_err = mean_err_sum = 0.0
+    n_el = 0
+    chunk = 8
+    order = np.argsort(sp.lens_after, kind="stable")          # a spread of lengths: interleave short and long
+    order = np.stack([order[: len(order) // 2], order[::-1][: len(order) // 2]], 1).reshape(-1) if len(order) > 1 else order
+    for c0 in range(0, len(order), chunk):
+        rows = order[c0:c0 + chunk]
+        reqs = [(loop.sched.content_uid[int(sp.batch[r])], int(sp.lens_after[r])) for r in rows]
+        smp = OracleSample(w, reqs, layer, bits(q[rows]))
+        a, b, want = smp.run()
+        t_sc += a; t_at += b
+        x, y = smp.bytes(); ab += x; ib += y
+        g = (bits(got[rows]).astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+        err = np.abs(g - want)
+        max_err = max(max_err, float(err.max())); mean_err_sum += float(err.sum()); n_el += err.size
+        n_req += len(rows); tokens += sum(n for _, n in reqs)
+        if t_sc + t_at >= budget_s:
+            break
+    val = (ab + ib) / (t_sc + t_at) / 1e9
+    sample = (f"{n_req} of {len(sp.batch)} requests ({tokens} tokens, short and long interleaved) of the last timed "
+              f"step, layer {layer} of {w.num_layers}: oracle scatter {t_sc:.2f} s + attention {t_at:.2f} s")
+    base = {"value": val, "unit": "GB/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample,
+            "attention_gbs": ab / t_at / 1e9 if t_at else None, "scatter_gbs": ib / t_sc / 1e9 if t_sc else None}
+    check = {"rows": n_req, "max_abs_err": max_err, "mean_abs_err": mean_err_sum / max(n_el, 1),
+             "pass": bool(max_err <= 1e-2 and mean_err_sum / max(n_el, 1) <= 1e-3)}
+    return base, check
+
+
+# ---------------------------------------------------------------------------------------------
+# the CUDA arm
+# ---------------------------------------------------------------------------------------------
+def run_cuda(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import paper_2511_20982_b200 as kv              # ImportError if libkvpool.so is missing: no fallback
+    from paper_2511_20982_b200 import binding as B
+    from paper_2511_20982_b200 import workloads as W
+    from paper_2511_20982_b200.engine import DecodeLoop
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py --impl cuda needs a GPU; there is no CPU fallback"
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier(device_ids=[local])
+        torch.cuda.synchronize(dev)
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    w = W.CONFIGS[args.workload]
+    K, Wm = args.steps, args.warmup
+    e2e_w = 3 if args.e2e_steps > 0 else 0
+    opts = {k: int(v) for k, v in (o.split("=") for o in args.opt)}
+    t_setup = time.time()
+    loop = DecodeLoop(w, Wm + K, n_host_steps=e2e_w + args.e2e_steps, device=dev, streams=args.streams, salt=rank,
+                      options=opts)
+    t_setup = time.time() - t_setup
+    pool = loop.pool
+    phys = int(os.environ.get("CUDA_VISIBLE_DEVICES", "").split(",")[local]) if os.environ.get("CUDA_VISIBLE_DEVICES") else local
+    sampler = ClockSampler(phys) if rank == 0 else None
+    A = loop.sA
+
+    # ---- device-resident leg: W warm-up steps, then exactly K timed steps ----------------------
+    for _ in range(Wm):
+        loop.step()
+    loop.join()
+    barrier()
+    pool.profile_reset()
+    launches0 = pool.launches
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    wall0 = time.time()
+    ev0.record(A)
+    for _ in range(K):
+        loop.step()
+    host_s = time.time() - wall0
+    loop.join()
+    ev1.record(A)
+    barrier()
+    wall1 = time.time()
+    if sampler:
+        sampler.window(wall0, wall1)
+    ms = max_over_ranks(ev0.elapsed_time(ev1))
+    launches = pool.launches - launches0
+    prof = pool.profile()
+    by = loop.bytes_of_steps(Wm, Wm + K)
+    total_bytes = sum_over_ranks(float(by["attn"] + by["append"] + by["ingest"]))
+    total_tokens = sum_over_ranks(float(by["tokens"]))
+    value = total_bytes / (ms * 1e-3) / 1e9
+    peak, peak_src = hbm_peak()
+
+    attn_n, attn_ms = prof["attn"]
+    comb_n, comb_ms = prof["combine"]
+    ing_n, ing_ms = prof["ingest"]
+    attn_bytes_per_launch = by["attn"] / max(attn_n, 1)
+    achieved = attn_bytes_per_launch / (attn_ms / max(attn_n, 1) * 1e-3) / 1e9 if attn_ms > 0 else None
+    roofline = {"kernel": "attn_splitkv_kernel", "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak if achieved else None, "peak_source": peak_src,
+                "frac_of_nominal_8000": achieved / NOMINAL_HBM_GBS if achieved else None,
+                "launches": attn_n, "avg_launch_us": attn_ms / max(attn_n, 1) * 1e3,
+                "algorithmic_bytes_per_launch": attn_bytes_per_launch, "traffic": None}
+    kernels = {
+        "attn_splitkv_kernel": {"launches": attn_n, "ms": attn_ms},
+        "combine_kernel": {"launches": comb_n, "ms": comb_ms},
+        "ingest_kernel": {"launches": ing_n, "ms": ing_ms,
+                          "gbs": (by["ingest"] + by["append"]) / (ing_ms * 1e-3) / 1e9 if ing_ms > 0 else None},
+        "attn_plus_combine_gbs": by["attn"] / ((attn_ms + comb_ms) * 1e-3) / 1e9 if attn_ms > 0 else None,
+    }
+
+    # ---- isolated legs: attention alone and ingest alone on the final state -------------------
+    isolated = None
+    if not args.no_isolated:
+        isolated = isolated_legs(loop, Wm + K - 1, peak)
+
+    # ---- cpu baseline + sampled parity of the last timed step (rank 0, N = 1 only) -------------
+    cpu_base = check = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        torch.cuda.synchronize(dev)
+        cpu_base, check = cpu_baseline_and_check(loop, Wm + K - 1)
+
+    # ---- host-buffer leg (e2e) ------------------------------------------------------------------
+    e2e = None
+    if args.e2e_steps > 0:
+        for _ in range(e2e_w):
+            loop.step()
+        loop.join()
+        barrier()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        w0 = time.time()
+        f0.record(A)
+        lo = loop.step_idx
+        for _ in range(args.e2e_steps):
+            loop.step()
+        loop.join()
+        f1.record(A)
+        barrier()
+        w1 = time.time()
+        if sampler:
+            sampler.window(w0, w1)
+        ems = max_over_ranks(max(f0.elapsed_time(f1), (w1 - w0) * 1e3 if world == 1 else 0.0))
+        eb = loop.bytes_of_steps(lo, lo + args.e2e_steps)
+        h2d, d2h = loop.io_bytes(lo, lo + args.e2e_steps)
+        etotal = sum_over_ranks(float(eb["attn"] + eb["append"] + eb["ingest"]))
+        e2e = {"value": etotal / (ems * 1e-3) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": h2d // args.e2e_steps,
+               "d2h_bytes_per_step": d2h // args.e2e_steps, "steps": args.e2e_steps, "warmup": e2e_w,
+               "ms_per_step": ems / args.e2e_steps,
+               "decode_tokens_per_s": sum_over_ranks(float(eb["tokens"])) / (ems * 1e-3),
+               "pcie_gbs": sum_over_ranks(float(h2d + d2h)) / (ems * 1e-3) / 1e9,
+               "api": "kv_ingest_host + paged_decode_attention_host (pinned host q / K / V in, out back)"}
+    clocks = sampler.finish() if sampler else None
+    stats = pool.stats()
+    kv_gb_layer = by["attn"] / K / w.num_layers / 1e9
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16 (fp32 accumulate)", "data": "synthetic",
+            "config": {"workload": args.workload, "layers": w.num_layers, "q_heads": w.num_q_heads,
+                       "kv_heads": w.num_kv_heads, "head_dim": w.head_dim, "block_size": w.block_size,
+                       "batch": w.batch, "ingest_per_step": w.ingest_per_step, "streams": 2 if loop.two_streams else 1,
+                       "pool_blocks": loop.cfg.num_blocks, "pool_gb": pool.kv_bytes / 1e9,
+                       "blocks_high_water": stats["blocks_high_water"],
+                       "l2": f"inputs larger than L2: each layer's attention streams {kv_gb_layer:.2f} GB of KV",
+                       "parallelism": f"replicas x{world} (no collective)", "setup_s": round(t_setup, 1)},
+            "frac_of_measured_peak": value / world / peak, "frac_of_nominal_8000": value / world / NOMINAL_HBM_GBS,
+            "decode_tokens_per_s": total_tokens / (ms * 1e-3),
+            "bytes_per_step": {"attention": by["attn"] // K, "ingest": by["ingest"] // K, "append": by["append"] // K},
+            "host_enqueue_ms_per_step": host_s / K * 1e3,
+            "gpu_launches": launches, "kernels": kernels, "roofline": roofline, "isolated": isolated,
+            "cpu_baseline": cpu_base, "parity_sample": check, "e2e": e2e, "clocks": clocks,
+        }))
+    loop.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def isolated_legs(loop, last_step: int, peak: float, reps: int = 5):
+    """Attention alone (all layers, the last step's batch, no append) and ingest alone (one step's
+    arrivals into fresh requests, freed again), each timed with CUDA events on stream A."""
+    import numpy as np
+    import torch
+    from paper_2511_20982_b200 import binding as B
+    w, sp, h, A = loop.w, loop.sched.steps[last_step], loop.pool.handle, loop.sA
+    L = w.num_layers
+    torch.cuda.synchronize(loop.dev)
+    q, out = loop.q[last_step], loop.out[last_step]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    times = []
+    for r in range(reps + 1):
+        e0.record(A)
+        for l in range(L):
+            B.paged_decode_attention(h, l, sp.batch, q.data_ptr() + l * loop.q_layer_bytes,
+                                     out.data_ptr() + l * loop.q_layer_bytes, 0.0, A.cuda_stream)
+        e1.record(A)
+        A.synchronize()
+        times.append(e0.elapsed_time(e1))
+    t_attn = float(np.median(times[1:]))
+    res = {"attention_gbs": sp.attn_bytes_layer * L / (t_attn * 1e-3) / 1e9, "attention_ms": t_attn}
+    res["attention_frac"] = res["attention_gbs"] / peak
+    if w.ingest_per_step and loop.bank:
+        k = w.ingest_per_step
+        ents = list(range(k))
+        nt = loop.sched.bank_lens[ents].astype(np.int32)
+        kp = np.asarray([loop.bank[e][0].data_ptr() for e in ents], dtype=np.uint64)
+        vp = np.asarray([loop.bank[e][1].data_ptr() for e in ents], dtype=np.uint64)
+        ids = np.arange(k, dtype=np.int64) + (1 << 40)
+        nbytes = 2 * 2 * loop.tok_bytes * int(nt.sum())
+        times = []
+        try:
+            for r in range(reps + 1):
+                e0.record(A)
+                B.kv_ingest(h, ids, nt, kp, vp, 0, L, A.cuda_stream)
+                e1.record(A)
+                A.synchronize()
+                B.kv_free(h, ids)
+                times.append(e0.elapsed_time(e1))
+            t_ing = float(np.median(times[1:]))
+            res.update({"ingest_gbs": nbytes / (t_ing * 1e-3) / 1e9, "ingest_ms": t_ing,
+                        "ingest_frac": nbytes / (t_ing * 1e-3) / 1e9 / peak, "ingest_bytes": nbytes})
+        except B.KVError as e:
+            res["ingest_error"] = str(e)
+    return res
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

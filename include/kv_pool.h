@@ -185,12 +185,55 @@ int32_t kv_plan_decode(kv_pool_t* pool, int32_t batch, const int64_t* req_ids /*
                        int32_t* out_items /*host*/, int32_t cap_items, int32_t* out_n_items,
                        int32_t* out_chunk_blocks);
 
+/*
+ * Host-buffer forms of a2/a3 and a4+a5 — the producer's KV (the request
+ * "together with KV-cache" handed from P to D) and the step's queries arriving in HOST
+ * memory.  Same semantics and errors as kv_ingest / paged_decode_attention, except that
+ * k_src[i] / v_src[i] / q / out are HOST pointers (pinned memory for true asynchrony;
+ * pageable memory works but the copy is synchronous for the host).  The copies are issued
+ * on `cuda_stream` through the caller-owned device staging buffer `staging` (device,
+ * 256-byte aligned): ingest needs sum_i 2 * layer_count*Hkv*n_tokens[i]*d*2 bytes (each
+ * tensor rounded up to 256 B), attention needs 2 * batch*Hq*d*2 bytes (rounded likewise);
+ * a smaller `staging_bytes` => KV_ERR_INVALID before anything changes.  Host source ranges
+ * that are adjacent in memory (request i+1 starts where request i ends) are moved with one
+ * copy.  The staging buffer may be reused by the next call on the same stream; the host
+ * buffers may be reused once the stream has passed the call.
+ */
+int32_t kv_ingest_host(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids /*host*/,
+                       const int32_t* n_tokens /*host*/,
+                       const void* const* k_src /*host array of HOST ptrs*/,
+                       const void* const* v_src /*host array of HOST ptrs*/,
+                       int32_t layer_begin, int32_t layer_count, void* staging /*device*/,
+                       int64_t staging_bytes, void* cuda_stream);
+int32_t paged_decode_attention_host(kv_pool_t* pool, int32_t layer, int32_t batch,
+                                    const int64_t* req_ids /*host*/, const void* q /*HOST*/,
+                                    void* out /*HOST*/, float sm_scale, void* staging /*device*/,
+                                    int64_t staging_bytes, void* cuda_stream);
+
 /* Number of kernels this pool has launched since creation (bench `gpu_launches`).         */
 int64_t kv_launch_count(const kv_pool_t* pool);
 
-/* Tuning knobs (all optional; defaults chosen for B200).  key: "min_chunk_blocks",
- * "ctas_per_sm", "attn_variant" (0 = register-direct, 1 = bulk-copy smem ring).
- * Unknown key => KV_ERR_INVALID.                                                           */
+/*
+ * Per-kernel device timing (bench `roofline`).  With option "profile" = 1 every kernel
+ * launch is bracketed by a pair of CUDA events on its own stream (a ring of
+ * KV_PROFILE_RING pairs per kind; older samples are folded into the running sums when their
+ * slot is reused, which synchronises on that sample).  kv_profile_read synchronises on the
+ * outstanding samples of `kind`, returns the number of launches and their summed duration in
+ * milliseconds since the last kv_profile_reset, and leaves the sums in place.
+ */
+#define KV_KERNEL_ATTN     0   /* attn_splitkv_kernel (a4)          */
+#define KV_KERNEL_COMBINE  1   /* combine_kernel (a5)               */
+#define KV_KERNEL_INGEST   2   /* ingest_kernel, scatter (a2 / a3)  */
+#define KV_KERNEL_GATHER   3   /* ingest_kernel, gather direction   */
+#define KV_KERNEL_KINDS    4
+#define KV_PROFILE_RING    1024
+int32_t kv_profile_read(kv_pool_t* pool, int32_t kind, int64_t* out_launches, double* out_ms);
+int32_t kv_profile_reset(kv_pool_t* pool);
+
+/* Tuning knobs (all optional; defaults chosen for B200).  key: "min_chunk_blocks" (smallest
+ * split-KV chunk, in blocks), "ctas_per_sm" (resident attention CTAs per SM the planner
+ * sizes the work list for), "items_per_slot" (work items per resident warp), "profile"
+ * (0/1, see kv_profile_read).  Unknown key or out-of-range value => KV_ERR_INVALID.        */
 int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value);
 
 /* Last CUDA error code seen by this pool (cudaError_t as int; 0 = none).                  */

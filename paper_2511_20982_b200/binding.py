@@ -53,7 +53,11 @@ _SIGS = {
                              ctypes.POINTER(_i64)]),
     "kv_gather": (_i32, [_P, _i64, _P, _P, _P]),
     "kv_plan_decode": (_i32, [_P, _i32, _P, _P, _i32, ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
+    "kv_ingest_host": (_i32, [_P, _i32, _P, _P, _P, _P, _i32, _i32, _P, _i64, _P]),
+    "paged_decode_attention_host": (_i32, [_P, _i32, _i32, _P, _P, _P, ctypes.c_float, _P, _i64, _P]),
     "kv_launch_count": (_i64, [_P]),
+    "kv_profile_read": (_i32, [_P, _i32, ctypes.POINTER(_i64), ctypes.POINTER(ctypes.c_double)]),
+    "kv_profile_reset": (_i32, [_P]),
     "kv_pool_set_option": (_i32, [_P, ctypes.c_char_p, _i64]),
     "kv_last_cuda_error": (_i32, [_P]),
     "kv_strerror": (ctypes.c_char_p, [_i32]),
@@ -103,7 +107,9 @@ def _i32s(a) -> np.ndarray:
 
 
 def _ptrs(a) -> np.ndarray:
-    """list of tensors / ints -> uint64 array of device addresses."""
+    """list of tensors / ints, or an integer array of addresses -> uint64 array of addresses."""
+    if isinstance(a, np.ndarray):
+        return np.ascontiguousarray(a, dtype=np.uint64)
     return np.ascontiguousarray([x if isinstance(x, int) else x.data_ptr() for x in a], dtype=np.uint64)
 
 
@@ -165,6 +171,37 @@ def paged_decode_attention(handle: int, layer: int, req_ids, q_ptr: int, out_ptr
     ids = _ids(req_ids)
     _check(lib.paged_decode_attention(handle, layer, ids.size, _np(ids), q_ptr, out_ptr, sm_scale, stream or None),
            "paged_decode_attention")
+
+
+def kv_ingest_host(handle: int, req_ids, n_tokens, k_src, v_src, layer_begin: int, layer_count: int,
+                   staging_ptr: int, staging_bytes: int, stream: int = 0) -> None:
+    """k_src / v_src: HOST addresses (pinned tensors or ints)."""
+    ids, n, kp, vp = _ids(req_ids), _i32s(n_tokens), _ptrs(k_src), _ptrs(v_src)
+    assert ids.shape == n.shape == kp.shape == vp.shape
+    _check(lib.kv_ingest_host(handle, ids.size, _np(ids), _np(n), _np(kp), _np(vp), layer_begin, layer_count,
+                              staging_ptr, staging_bytes, stream or None), "kv_ingest_host")
+
+
+def paged_decode_attention_host(handle: int, layer: int, req_ids, q_host_ptr: int, out_host_ptr: int,
+                                sm_scale: float, staging_ptr: int, staging_bytes: int, stream: int = 0) -> None:
+    ids = _ids(req_ids)
+    _check(lib.paged_decode_attention_host(handle, layer, ids.size, _np(ids), q_host_ptr, out_host_ptr, sm_scale,
+                                           staging_ptr, staging_bytes, stream or None),
+           "paged_decode_attention_host")
+
+
+KERNEL_KINDS = {"attn": 0, "combine": 1, "ingest": 2, "gather": 3}
+
+
+def kv_profile_read(handle: int, kind: int):
+    """(launches, total milliseconds) of kernel `kind` since the last reset (needs option profile=1)."""
+    n, ms = _i64(), ctypes.c_double()
+    _check(lib.kv_profile_read(handle, kind, ctypes.byref(n), ctypes.byref(ms)), "kv_profile_read")
+    return int(n.value), float(ms.value)
+
+
+def kv_profile_reset(handle: int) -> None:
+    _check(lib.kv_profile_reset(handle), "kv_profile_reset")
 
 
 def kv_free(handle: int, req_ids) -> None:
@@ -281,6 +318,13 @@ class KVPool:
 
     def free(self, req_ids):
         kv_free(self.handle, req_ids)
+
+    def profile(self) -> dict:
+        """{kernel: (launches, total ms)} since the last profile_reset() (option profile=1)."""
+        return {k: kv_profile_read(self.handle, i) for k, i in KERNEL_KINDS.items()}
+
+    def profile_reset(self):
+        kv_profile_reset(self.handle)
 
     def block_table(self, req_id):
         return kv_block_table(self.handle, req_id)

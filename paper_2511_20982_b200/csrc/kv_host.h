@@ -8,7 +8,6 @@
 #include <algorithm>
 #include <cstdint>
 #include <unordered_map>
-#include <unordered_set>
 #include <vector>
 
 #include "../../include/kv_pool.h"
@@ -61,24 +60,28 @@ struct Request {
   int32_t slot = -1;    // row of the device block_table mirror
   int32_t len = 0;      // tokens stored (reserved)
   int32_t last_n = 0;   // size of the last reservation (for layer-sliced ingest)
+  mutable uint64_t plan_mark = 0;  // duplicate detection in plan_decode / batch validation
   std::vector<int32_t> blocks;
 };
 
-// One split-KV work item: a run of logical blocks of one (request, kv_head).
+// One split-KV work item: a run of logical blocks of one request, shared by all its KV heads.
+// The kernel expands item i into num_kv_heads units (unit = i * Hkv + kv_head, heads fastest, so
+// neighbouring warps stream neighbouring head tiles of the same physical blocks).
 struct WorkItem {
-  int32_t batch_idx;    // row of q / out
-  int32_t slot;         // row of the device block_table
-  int32_t kv_head;
-  int32_t blk_begin;    // first logical block
+  int32_t batch_idx;     // row of q / out
+  int32_t slot;          // row of the device block_table
+  int32_t blk_begin;     // first logical block
   int32_t n_blocks;
-  int32_t n_tokens;     // valid tokens in this run (last block of a request may be partial)
-  int32_t partial_idx;  // slot in the partials workspace, or -1: only chunk, writes `out`
-  int32_t pad;
+  int32_t n_tokens;      // valid tokens in this run (last block of a request may be partial)
+  int32_t partial_base;  // first partial slot of this request, or -1: only chunk, writes `out`
+  int32_t n_chunks;      // chunks of this request; partial slot of (kv_head h, chunk c) =
+  int32_t chunk_idx;     //   partial_base + h * n_chunks + c
 };
 static_assert(sizeof(WorkItem) == 32, "WorkItem is read by the kernel as two int4");
 
+// One request that was split: its Hkv * G heads each merge n_chunks partials.
 struct CombineEntry {
-  int32_t batch_idx, kv_head, partial_begin, n_chunks;
+  int32_t batch_idx, partial_begin, n_chunks, pad;
 };
 
 struct DecodePlan {
@@ -121,20 +124,29 @@ class HostState {
   // a1.  Atomic over the batch: validate everything, then mutate.
   int32_t reserve(int32_t n_req, const int64_t* ids, const int32_t* n_tokens) {
     if (n_req < 0 || (n_req > 0 && (!ids || !n_tokens))) return KV_ERR_INVALID;
-    std::unordered_set<int64_t> seen;
+    const uint64_t stamp = ++plan_stamp_;
+    fresh_.clear();
     int64_t need_blocks = 0;
-    int32_t need_slots = 0;
     for (int32_t i = 0; i < n_req; ++i) {
       if (n_tokens[i] < 0) return KV_ERR_INVALID;
-      if (!seen.insert(ids[i]).second) return KV_ERR_INVALID;
       auto it = reqs.find(ids[i]);
-      int64_t len = it == reqs.end() ? 0 : it->second.len;
+      int64_t len = 0;
+      if (it == reqs.end()) {
+        fresh_.push_back(ids[i]);
+      } else {
+        if (it->second.plan_mark == stamp) return KV_ERR_INVALID;  // duplicate id
+        it->second.plan_mark = stamp;
+        len = it->second.len;
+      }
       int64_t new_len = len + n_tokens[i];
       if (new_len > static_cast<int64_t>(cfg.max_blocks_per_request) * cfg.block_size) return KV_ERR_TOO_LONG;
       need_blocks += blocks_for(new_len) - blocks_for(len);
-      if (it == reqs.end()) ++need_slots;
     }
-    if (need_slots > static_cast<int32_t>(free_slots.size())) return KV_ERR_TOO_MANY_REQUESTS;
+    if (fresh_.size() > 1) {  // duplicates among the ids that are not live yet
+      std::sort(fresh_.begin(), fresh_.end());
+      if (std::adjacent_find(fresh_.begin(), fresh_.end()) != fresh_.end()) return KV_ERR_INVALID;
+    }
+    if (fresh_.size() > free_slots.size()) return KV_ERR_TOO_MANY_REQUESTS;
     if (need_blocks > alloc.free_count()) return KV_ERR_NO_BLOCKS;
     for (int32_t i = 0; i < n_req; ++i) {
       auto it = reqs.find(ids[i]);
@@ -157,10 +169,12 @@ class HostState {
   // a6.  Atomic: unknown or duplicate id => nothing freed.
   int32_t release(int32_t n_req, const int64_t* ids) {
     if (n_req < 0 || (n_req > 0 && !ids)) return KV_ERR_INVALID;
-    std::unordered_set<int64_t> seen;
+    const uint64_t stamp = ++plan_stamp_;
     for (int32_t i = 0; i < n_req; ++i) {
-      if (!seen.insert(ids[i]).second) return KV_ERR_INVALID;
-      if (reqs.find(ids[i]) == reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
+      auto it = reqs.find(ids[i]);
+      if (it == reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
+      if (it->second.plan_mark == stamp) return KV_ERR_INVALID;
+      it->second.plan_mark = stamp;
     }
     for (int32_t i = 0; i < n_req; ++i) {
       auto it = reqs.find(ids[i]);
@@ -173,66 +187,97 @@ class HostState {
     return KV_OK;
   }
 
+  // Every id live, none repeated (continuation ingest, host-buffer attention).  Optionally requires
+  // each request's last reservation to equal n_tokens[i].
+  int32_t check_batch(int32_t n_req, const int64_t* ids, const int32_t* last_n) const {
+    const uint64_t stamp = ++plan_stamp_;
+    for (int32_t i = 0; i < n_req; ++i) {
+      auto it = reqs.find(ids[i]);
+      if (it == reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
+      if (it->second.plan_mark == stamp) return KV_ERR_INVALID;
+      it->second.plan_mark = stamp;
+      if (last_n && it->second.last_n != last_n[i]) return KV_ERR_INVALID;
+    }
+    return KV_OK;
+  }
+
   // Work-list half of a4.  `slots` = resident warps the main kernel will run; the planner aims
-  // at `items_per_slot` near-uniform items per slot so that dynamic scheduling has a short tail,
+  // at `items_per_slot` near-uniform units per slot so that dynamic scheduling has a short tail,
   // while keeping chunks >= min_chunk_blocks so split-KV partial traffic stays << KV traffic.
+  // Cost matters (a 7B-MHA decode step is ~0.2 ms of GPU time): one pass over the batch, no hashing
+  // beyond the id lookup, counting sort.
   int32_t plan_decode(int32_t batch, const int64_t* ids, int32_t slots, int32_t items_per_slot,
                       int32_t min_chunk_blocks, int32_t max_partials, DecodePlan* plan) const {
     if (batch < 1 || !ids || batch > cfg.max_requests) return KV_ERR_INVALID;
-    std::vector<const Request*> rs(static_cast<size_t>(batch));
-    std::unordered_set<int64_t> seen;
+    scratch_.resize(static_cast<size_t>(batch));
+    const uint64_t stamp = ++plan_stamp_;
     int64_t total_blocks = 0;
     for (int32_t i = 0; i < batch; ++i) {
-      if (!seen.insert(ids[i]).second) return KV_ERR_INVALID;
       auto it = reqs.find(ids[i]);
       if (it == reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
-      if (it->second.len < 1) return KV_ERR_INVALID;
-      rs[static_cast<size_t>(i)] = &it->second;
-      total_blocks += blocks_for(it->second.len);
+      const Request& r = it->second;
+      if (r.len < 1 || r.plan_mark == stamp) return KV_ERR_INVALID;  // empty context (A11) / duplicate id
+      r.plan_mark = stamp;
+      scratch_[static_cast<size_t>(i)] = &r;
+      total_blocks += blocks_for(r.len);
     }
     const int64_t total_tiles = total_blocks * cfg.num_kv_heads;
     const int64_t target_items = std::max<int64_t>(1, static_cast<int64_t>(slots) * items_per_slot);
     int64_t chunk = std::max<int64_t>(min_chunk_blocks, (total_tiles + target_items - 1) / target_items);
     for (;;) {  // grow the chunk until the partials fit the workspace
       int64_t partials = 0;
-      for (const Request* r : rs) {
+      for (const Request* r : scratch_) {
         int64_t nc = (blocks_for(r->len) + chunk - 1) / chunk;
         if (nc > 1) partials += nc * cfg.num_kv_heads;
       }
       if (partials <= max_partials) break;
       chunk *= 2;
     }
-    plan->items.clear();
     plan->combines.clear();
     plan->chunk_blocks = static_cast<int32_t>(chunk);
-    int32_t next_partial = 0;
+    unsorted_.clear();
+    int32_t next_partial = 0, max_nb = 0;
     for (int32_t i = 0; i < batch; ++i) {
-      const Request* r = rs[static_cast<size_t>(i)];
+      const Request* r = scratch_[static_cast<size_t>(i)];
       const int32_t nb = blocks_for(r->len);
       const int32_t nc0 = static_cast<int32_t>((nb + chunk - 1) / chunk);
       const int32_t per = (nb + nc0 - 1) / nc0;  // even split: ceil(nb / nc0) <= chunk blocks per chunk
       const int32_t nc = (nb + per - 1) / per;   // <= nc0
-      for (int32_t h = 0; h < cfg.num_kv_heads; ++h) {
-        if (nc > 1) plan->combines.push_back({i, h, next_partial, nc});
-        for (int32_t c = 0; c < nc; ++c) {
-          WorkItem w;
-          w.batch_idx = i;
-          w.slot = r->slot;
-          w.kv_head = h;
-          w.blk_begin = c * per;
-          w.n_blocks = std::min(per, nb - c * per);
-          w.n_tokens = std::min(r->len - w.blk_begin * cfg.block_size, w.n_blocks * cfg.block_size);
-          w.partial_idx = nc > 1 ? next_partial++ : -1;
-          w.pad = 0;
-          plan->items.push_back(w);
-        }
+      const int32_t base = nc > 1 ? next_partial : -1;
+      if (nc > 1) {
+        plan->combines.push_back({i, base, nc, 0});
+        next_partial += nc * cfg.num_kv_heads;
+      }
+      for (int32_t c = 0; c < nc; ++c) {
+        WorkItem w;
+        w.batch_idx = i;
+        w.slot = r->slot;
+        w.blk_begin = c * per;
+        w.n_blocks = std::min(per, nb - c * per);
+        w.n_tokens = std::min(r->len - w.blk_begin * cfg.block_size, w.n_blocks * cfg.block_size);
+        w.partial_base = base;
+        w.n_chunks = nc;
+        w.chunk_idx = c;
+        max_nb = std::max(max_nb, w.n_blocks);
+        unsorted_.push_back(w);
       }
     }
     plan->n_partials = next_partial;
-    std::stable_sort(plan->items.begin(), plan->items.end(),
-                     [](const WorkItem& a, const WorkItem& b) { return a.n_blocks > b.n_blocks; });
+    // longest first, stable: counting sort on n_blocks
+    count_.assign(static_cast<size_t>(max_nb) + 2, 0);
+    for (const WorkItem& w : unsorted_) ++count_[static_cast<size_t>(max_nb - w.n_blocks) + 1];
+    for (size_t k = 1; k < count_.size(); ++k) count_[k] += count_[k - 1];
+    plan->items.resize(unsorted_.size());
+    for (const WorkItem& w : unsorted_) plan->items[static_cast<size_t>(count_[static_cast<size_t>(max_nb - w.n_blocks)]++)] = w;
     return KV_OK;
   }
+
+ private:
+  mutable std::vector<const Request*> scratch_;
+  mutable std::vector<WorkItem> unsorted_;
+  mutable std::vector<int32_t> count_;
+  std::vector<int64_t> fresh_;
+  mutable uint64_t plan_stamp_ = 0;
 };
 
 }  // namespace kvp

@@ -206,8 +206,8 @@ __global__ void __launch_bounds__(kIngestThreads) ingest_kernel(const IngestPara
 // a4 split-KV paged decode attention
 // ---------------------------------------------------------------------------------------------
 
-struct WorkItemDev {  // == kvp::WorkItem (kv_host.h)
-  int32_t batch_idx, slot, kv_head, blk_begin, n_blocks, n_tokens, partial_idx, pad;
+struct WorkItemDev {  // == kvp::WorkItem (kv_host.h); one item = num_kv_heads units, heads fastest
+  int32_t batch_idx, slot, blk_begin, n_blocks, n_tokens, partial_base, n_chunks, chunk_idx;
 };
 
 struct AttnParams {
@@ -215,7 +215,7 @@ struct AttnParams {
   const int32_t* block_table;
   int32_t bt_stride;
   const WorkItemDev* items;
-  int32_t n_items;
+  int32_t n_items, n_units;    // n_units = n_items * num_kv_heads
   const uint16_t* q;
   uint16_t* out;
   float* part_o;               // [n_partials][G][D]  un-normalised
@@ -266,11 +266,14 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
     int item = 0;
     if (lane == 0) item = atomicAdd(&p.counters[0], 1);
     item = __shfl_sync(0xffffffffu, item, 0);
-    if (item >= p.n_items) break;
-    const int4 w0 = __ldg(reinterpret_cast<const int4*>(p.items + item));
-    const int4 w1 = __ldg(reinterpret_cast<const int4*>(p.items + item) + 1);
-    const int batch_idx = w0.x, slot = w0.y, h = w0.z, blk_begin = w0.w;
-    const int n_blocks = w1.x, n_tokens = w1.y, pidx = w1.z;
+    if (item >= p.n_units) break;
+    const int h = item % p.num_kv_heads;
+    const WorkItemDev* wi = p.items + item / p.num_kv_heads;
+    const int4 w0 = __ldg(reinterpret_cast<const int4*>(wi));
+    const int4 w1 = __ldg(reinterpret_cast<const int4*>(wi) + 1);
+    const int batch_idx = w0.x, slot = w0.y, blk_begin = w0.z, n_blocks = w0.w;
+    const int n_tokens = w1.x;
+    const int pidx = w1.y < 0 ? -1 : w1.y + h * w1.z + w1.w;
 
     // q^T as B fragments: lane (g, c) holds head g, columns of chunk c + 4j (zero for g >= G)
     uint32_t qf[KS][2];
@@ -433,7 +436,7 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
 // a5 log-sum-exp combine: one warp per (combine entry, head of the group)
 // ---------------------------------------------------------------------------------------------
 
-struct CombineEntryDev { int32_t batch_idx, kv_head, partial_begin, n_chunks; };
+struct CombineEntryDev { int32_t batch_idx, partial_begin, n_chunks, pad; };  // == kvp::CombineEntry
 
 struct CombineParams {
   const CombineEntryDev* entries;
@@ -441,7 +444,7 @@ struct CombineParams {
   const float* part_o;
   const float* part_ml;
   uint16_t* out;
-  int32_t num_q_heads, group;
+  int32_t num_q_heads, num_kv_heads, group;
 };
 
 template <int D>
@@ -449,9 +452,11 @@ __global__ void __launch_bounds__(128) combine_kernel(const CombineParams p) {
   constexpr int V = D / 32;  // floats per lane
   const int lane = threadIdx.x & 31;
   const int w = blockIdx.x * 4 + (threadIdx.x >> 5);
-  if (w >= p.n_entries * p.group) return;
-  const int ei = w / p.group, head = w % p.group;
-  const CombineEntryDev e = p.entries[ei];
+  if (w >= p.n_entries * p.num_q_heads) return;
+  const int ei = w / p.num_q_heads, qh = w % p.num_q_heads;
+  const int kvh = qh / p.group, head = qh % p.group;
+  CombineEntryDev e = p.entries[ei];
+  e.partial_begin += kvh * e.n_chunks;                        // partials of (request, kv head): contiguous over chunks
   const float* ml = p.part_ml + (static_cast<int64_t>(e.partial_begin) * p.group + head) * 2;
   const int64_t ml_stride = static_cast<int64_t>(p.group) * 2;
   const float* po = p.part_o + (static_cast<int64_t>(e.partial_begin) * p.group + head) * D + lane * V;
@@ -480,7 +485,7 @@ __global__ void __launch_bounds__(128) combine_kernel(const CombineParams p) {
     }
   }
   const float inv = 1.f / den;
-  uint16_t* op = p.out + (static_cast<int64_t>(e.batch_idx) * p.num_q_heads + e.kv_head * p.group + head) * D + lane * V;
+  uint16_t* op = p.out + (static_cast<int64_t>(e.batch_idx) * p.num_q_heads + qh) * D + lane * V;
   if constexpr (V == 4) {
     *reinterpret_cast<uint2*>(op) = make_uint2(pack_bf16x2(acc[0] * inv, acc[1] * inv), pack_bf16x2(acc[2] * inv, acc[3] * inv));
   } else {

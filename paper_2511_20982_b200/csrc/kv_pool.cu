@@ -5,6 +5,7 @@
 
 #include <cmath>
 #include <cstring>
+#include <deque>
 #include <new>
 #include <vector>
 
@@ -17,8 +18,9 @@ namespace {
 using namespace kvp;
 
 constexpr int64_t kAlign = 256;
-constexpr int kRing = 4;                       // staging slots per blob kind
+constexpr int kRing = 4;                       // plan staging slots
 constexpr int64_t kIngestBlobBytes = 1 << 20;  // per ingest launch; larger calls are sub-batched
+constexpr int64_t kIngestRingBytes = 16 << 20; // descriptor staging ring: ~1000 decode appends in flight
 constexpr int32_t kMaxPartials = 32768;        // split-KV partial slots in the workspace
 
 inline int64_t align_up(int64_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
@@ -38,9 +40,9 @@ Layout make_layout(const kv_pool_config_t& c) {
   L.counters = off;
   off = align_up(off + 256);
   L.ingest_blobs = off;
-  off = align_up(off + kRing * kIngestBlobBytes);
-  const int64_t items_cap = static_cast<int64_t>(c.max_requests) * c.num_kv_heads + kMaxPartials;
-  const int64_t comb_cap = static_cast<int64_t>(c.max_requests) * c.num_kv_heads;
+  off = align_up(off + kIngestRingBytes);
+  const int64_t items_cap = static_cast<int64_t>(c.max_requests) + kMaxPartials;
+  const int64_t comb_cap = static_cast<int64_t>(c.max_requests);
   L.plan_blob_bytes = align_up(items_cap * static_cast<int64_t>(sizeof(WorkItem)) + comb_cap * static_cast<int64_t>(sizeof(CombineEntry)));
   L.plan_blobs = off;
   off = align_up(off + kRing * L.plan_blob_bytes);
@@ -59,6 +61,118 @@ struct StageSlot {
   bool in_flight = false;
 };
 
+// Descriptor staging for ingest launches: a byte ring in pinned host memory mirrored by a device
+// ring in the slab.  Segments are handed out in ring order; a segment is reused only after the
+// event recorded behind the launch that read it has completed, so the host never waits on
+// unrelated work (a decode append on stream A does not wait for a bulk ingest on stream B unless
+// the ring has wrapped all the way round to it).
+struct ByteRing {
+  struct Seg { int64_t begin, end; cudaEvent_t ev; };
+  char* host = nullptr;
+  char* dev = nullptr;
+  int64_t cap = 0, head = 0;
+  std::deque<Seg> inflight;
+  std::vector<cudaEvent_t> spare;
+
+  cudaError_t retire_front(bool wait) {
+    Seg& f = inflight.front();
+    cudaError_t e = wait ? cudaEventSynchronize(f.ev) : cudaEventQuery(f.ev);
+    if (e != cudaSuccess) return e;  // cudaErrorNotReady when !wait and still running
+    spare.push_back(f.ev);
+    inflight.pop_front();
+    return cudaSuccess;
+  }
+  // Reserve `bytes` (<= cap); *off receives the offset valid in both host and dev.
+  cudaError_t alloc(int64_t bytes, int64_t* off) {
+    bytes = align_up(bytes);
+    if (head + bytes > cap) head = 0;
+    const int64_t b = head, e = head + bytes;
+    for (;;) {
+      bool clash = false;
+      for (const Seg& s : inflight) if (s.begin < e && b < s.end) { clash = true; break; }
+      if (!clash) break;
+      cudaError_t err = retire_front(true);
+      if (err != cudaSuccess) return err;
+    }
+    while (!inflight.empty()) {  // opportunistic clean-up keeps the overlap scan short
+      cudaError_t err = retire_front(false);
+      if (err == cudaErrorNotReady) break;
+      if (err != cudaSuccess) return err;
+    }
+    head = e;
+    *off = b;
+    return cudaSuccess;
+  }
+  cudaError_t commit(int64_t off, int64_t bytes, cudaStream_t st) {
+    cudaEvent_t ev = nullptr;
+    if (!spare.empty()) { ev = spare.back(); spare.pop_back(); }
+    else {
+      cudaError_t e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+      if (e != cudaSuccess) return e;
+    }
+    cudaError_t e = cudaEventRecord(ev, st);
+    inflight.push_back({off, off + align_up(bytes), ev});
+    return e;
+  }
+  void destroy() {
+    for (Seg& s : inflight) cudaEventDestroy(s.ev);
+    for (cudaEvent_t e : spare) cudaEventDestroy(e);
+    inflight.clear(); spare.clear();
+    if (host) cudaFreeHost(host);
+    host = nullptr;
+  }
+};
+
+// Event pairs around the launches of one kernel kind (kv_profile_read).
+struct ProfRing {
+  std::vector<cudaEvent_t> a, b;
+  std::vector<char> live;
+  int next = 0;
+  int64_t launches = 0;
+  double ms = 0.0;
+
+  cudaError_t fold(int i) {
+    if (!live[static_cast<size_t>(i)]) return cudaSuccess;
+    cudaError_t e = cudaEventSynchronize(b[static_cast<size_t>(i)]);
+    float t = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&t, a[static_cast<size_t>(i)], b[static_cast<size_t>(i)]);
+    if (e == cudaSuccess) { ms += t; ++launches; }
+    live[static_cast<size_t>(i)] = 0;
+    return e;
+  }
+  cudaError_t begin(cudaStream_t st) {
+    if (a.empty()) {
+      a.resize(KV_PROFILE_RING); b.resize(KV_PROFILE_RING); live.assign(KV_PROFILE_RING, 0);
+      for (int i = 0; i < KV_PROFILE_RING; ++i) {
+        cudaError_t e = cudaEventCreate(&a[static_cast<size_t>(i)]);
+        if (e == cudaSuccess) e = cudaEventCreate(&b[static_cast<size_t>(i)]);
+        if (e != cudaSuccess) return e;
+      }
+    }
+    cudaError_t e = fold(next);
+    if (e != cudaSuccess) return e;
+    return cudaEventRecord(a[static_cast<size_t>(next)], st);
+  }
+  cudaError_t end(cudaStream_t st) {
+    cudaError_t e = cudaEventRecord(b[static_cast<size_t>(next)], st);
+    live[static_cast<size_t>(next)] = 1;
+    next = (next + 1) % KV_PROFILE_RING;
+    return e;
+  }
+  cudaError_t drain() {
+    for (int i = 0; i < static_cast<int>(live.size()); ++i) {
+      cudaError_t e = fold(i);
+      if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+  }
+  void destroy() {
+    for (cudaEvent_t e : a) if (e) cudaEventDestroy(e);
+    for (cudaEvent_t e : b) if (e) cudaEventDestroy(e);
+    a.clear(); b.clear(); live.clear();
+  }
+};
+
 }  // namespace
 
 struct kv_pool {
@@ -73,9 +187,12 @@ struct kv_pool {
   int32_t min_chunk_blocks = 16;
   int32_t ctas_per_sm = 2;
   int32_t items_per_slot = 8;
+  bool profile = false;
+  ProfRing prof[KV_KERNEL_KINDS];
   // staging
-  StageSlot ingest_ring[kRing], plan_ring[kRing];
-  int ingest_next = 0, plan_next = 0;
+  ByteRing ingest_ring;
+  StageSlot plan_ring[kRing];
+  int plan_next = 0;
   // cached decode plan (reused across the layers of one step)
   uint64_t plan_epoch = 0;
   std::vector<int64_t> plan_ids;
@@ -118,18 +235,20 @@ template <bool kGather>
 int32_t launch_ingest(kv_pool* pool, const std::vector<IngestReq>& reqs, const std::vector<int32_t>& ids,
                       int64_t total_units, int32_t layer_begin, int32_t layer_count, cudaStream_t stream) {
   if (total_units == 0) return KV_OK;
-  StageSlot* s = nullptr;
-  int32_t rc = acquire(pool, pool->ingest_ring, &pool->ingest_next, &s);
-  if (rc < 0) return rc;
   const size_t req_bytes = reqs.size() * sizeof(IngestReq);
   const size_t id_bytes = ids.size() * sizeof(int32_t);
-  std::memcpy(s->host, reqs.data(), req_bytes);
-  std::memcpy(s->host + req_bytes, ids.data(), id_bytes);
-  KV_CUDA(pool, cudaMemcpyAsync(s->dev, s->host, req_bytes + id_bytes, cudaMemcpyHostToDevice, stream));
+  ByteRing& ring = pool->ingest_ring;
+  int64_t off = 0;
+  KV_CUDA(pool, ring.alloc(static_cast<int64_t>(req_bytes + id_bytes), &off));
+  char* hbuf = ring.host + off;
+  char* dbuf = ring.dev + off;
+  std::memcpy(hbuf, reqs.data(), req_bytes);
+  std::memcpy(hbuf + req_bytes, ids.data(), id_bytes);
+  KV_CUDA(pool, cudaMemcpyAsync(dbuf, hbuf, req_bytes + id_bytes, cudaMemcpyHostToDevice, stream));
   const kv_pool_config_t& c = pool->hs.cfg;
   IngestParams p{};
-  p.reqs = reinterpret_cast<const IngestReq*>(s->dev);
-  p.blk_ids = reinterpret_cast<const int32_t*>(s->dev + req_bytes);
+  p.reqs = reinterpret_cast<const IngestReq*>(dbuf);
+  p.blk_ids = reinterpret_cast<const int32_t*>(dbuf + req_bytes);
   p.n_req = static_cast<int32_t>(reqs.size());
   p.total_units = total_units;
   p.kv = reinterpret_cast<uint16_t*>(pool->base);
@@ -140,14 +259,16 @@ int32_t launch_ingest(kv_pool* pool, const std::vector<IngestReq>& reqs, const s
   p.num_kv_heads = c.num_kv_heads;
   p.num_blocks = c.num_blocks;
   const unsigned grid = static_cast<unsigned>((total_units + kIngestWarps - 1) / kIngestWarps);
+  ProfRing& pr = pool->prof[kGather ? KV_KERNEL_GATHER : KV_KERNEL_INGEST];
+  if (pool->profile) KV_CUDA(pool, pr.begin(stream));
   if (c.head_dim == 128)
     ingest_kernel<128, kGather><<<grid, kIngestThreads, 0, stream>>>(p);
   else
     ingest_kernel<64, kGather><<<grid, kIngestThreads, 0, stream>>>(p);
   KV_CUDA(pool, cudaGetLastError());
+  if (pool->profile) KV_CUDA(pool, pr.end(stream));
   ++pool->launches;
-  KV_CUDA(pool, cudaEventRecord(s->ev, stream));
-  s->in_flight = true;
+  KV_CUDA(pool, ring.commit(off, static_cast<int64_t>(req_bytes + id_bytes), stream));
   return KV_OK;
 }
 
@@ -242,12 +363,12 @@ int32_t kv_pool_create(const kv_pool_config_t* cfg, kv_pool_t** out_pool) {
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&pool->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaHostAlloc(reinterpret_cast<void**>(&pool->ingest_ring.host), kIngestRingBytes, cudaHostAllocDefault);
+    pool->ingest_ring.dev = pool->base + lay.ingest_blobs;
+    pool->ingest_ring.cap = kIngestRingBytes;
     for (int i = 0; e == cudaSuccess && i < kRing; ++i) {
-      e = cudaHostAlloc(reinterpret_cast<void**>(&pool->ingest_ring[i].host), kIngestBlobBytes, cudaHostAllocDefault);
-      if (e == cudaSuccess) e = cudaHostAlloc(reinterpret_cast<void**>(&pool->plan_ring[i].host), lay.plan_blob_bytes, cudaHostAllocDefault);
-      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pool->ingest_ring[i].ev, cudaEventDisableTiming);
+      e = cudaHostAlloc(reinterpret_cast<void**>(&pool->plan_ring[i].host), lay.plan_blob_bytes, cudaHostAllocDefault);
       if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pool->plan_ring[i].ev, cudaEventDisableTiming);
-      pool->ingest_ring[i].dev = pool->base + lay.ingest_blobs + i * kIngestBlobBytes;
       pool->plan_ring[i].dev = pool->base + lay.plan_blobs + i * lay.plan_blob_bytes;
     }
     // work counters start at zero; the attention kernel rewinds them itself afterwards
@@ -263,12 +384,12 @@ int32_t kv_pool_create(const kv_pool_config_t* cfg, kv_pool_t** out_pool) {
 
 int32_t kv_pool_destroy(kv_pool_t* pool) {
   if (!pool) return KV_ERR_INVALID;
+  pool->ingest_ring.destroy();
   for (int i = 0; i < kRing; ++i) {
-    if (pool->ingest_ring[i].host) cudaFreeHost(pool->ingest_ring[i].host);
     if (pool->plan_ring[i].host) cudaFreeHost(pool->plan_ring[i].host);
-    if (pool->ingest_ring[i].ev) cudaEventDestroy(pool->ingest_ring[i].ev);
     if (pool->plan_ring[i].ev) cudaEventDestroy(pool->plan_ring[i].ev);
   }
+  for (ProfRing& r : pool->prof) r.destroy();
   delete pool;
   return KV_OK;
 }
@@ -294,13 +415,8 @@ int32_t kv_ingest(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const 
     int32_t rc = pool->hs.reserve(n_req, req_ids, n_tokens);
     if (rc != KV_OK) return rc;
   } else {  // continuation of the last reservation
-    std::unordered_set<int64_t> seen;
-    for (int32_t i = 0; i < n_req; ++i) {
-      if (!seen.insert(req_ids[i]).second) return KV_ERR_INVALID;
-      auto it = pool->hs.reqs.find(req_ids[i]);
-      if (it == pool->hs.reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
-      if (it->second.last_n != n_tokens[i]) return KV_ERR_INVALID;
-    }
+    int32_t rc = pool->hs.check_batch(n_req, req_ids, n_tokens);
+    if (rc != KV_OK) return rc;
   }
   std::vector<int32_t> start(static_cast<size_t>(n_req));
   for (int32_t i = 0; i < n_req; ++i) start[static_cast<size_t>(i)] = pool->hs.reqs.find(req_ids[i])->second.len - n_tokens[i];
@@ -355,11 +471,14 @@ int32_t kv_plan_decode(kv_pool_t* pool, int32_t batch, const int64_t* req_ids, i
   int32_t rc = pool->hs.plan_decode(batch, req_ids, pool->slots(), pool->items_per_slot, pool->min_chunk_blocks,
                                     kMaxPartials, &plan);
   if (rc != KV_OK) return rc;
-  const int32_t n = static_cast<int32_t>(plan.items.size());
-  for (int32_t i = 0; i < std::min(n, cap_items); ++i) {
-    const WorkItem& w = plan.items[static_cast<size_t>(i)];
-    int32_t* o = out_items + 5 * i;
-    o[0] = w.batch_idx; o[1] = w.kv_head; o[2] = w.blk_begin; o[3] = w.n_blocks; o[4] = w.partial_idx;
+  const int32_t Hkv = pool->hs.cfg.num_kv_heads;
+  const int32_t n = static_cast<int32_t>(plan.items.size()) * Hkv;  // one unit per (item, kv_head), heads fastest
+  for (int32_t u = 0; u < std::min(n, cap_items); ++u) {
+    const WorkItem& w = plan.items[static_cast<size_t>(u / Hkv)];
+    const int32_t h = u % Hkv;
+    int32_t* o = out_items + 5 * u;
+    o[0] = w.batch_idx; o[1] = h; o[2] = w.blk_begin; o[3] = w.n_blocks;
+    o[4] = w.partial_base < 0 ? -1 : w.partial_base + h * w.n_chunks + w.chunk_idx;
   }
   if (out_n_items) *out_n_items = n;
   if (out_chunk_blocks) *out_chunk_blocks = plan.chunk_blocks;
@@ -419,13 +538,16 @@ int32_t paged_decode_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
   p.num_kv_heads = c.num_kv_heads;
   p.group = G;
   p.scale_log2 = scale * 1.4426950408889634f;
-  const int32_t want = (p.n_items + kAttnWarps - 1) / kAttnWarps;
+  p.n_units = p.n_items * c.num_kv_heads;
+  const int32_t want = (p.n_units + kAttnWarps - 1) / kAttnWarps;
   const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * pool->ctas_per_sm)));
+  if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_ATTN].begin(stream));
   if (c.head_dim == 128)
     attn_splitkv_kernel<128><<<grid, kAttnThreads, 0, stream>>>(p);
   else
     attn_splitkv_kernel<64><<<grid, kAttnThreads, 0, stream>>>(p);
   KV_CUDA(pool, cudaGetLastError());
+  if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_ATTN].end(stream));
   ++pool->launches;
 
   if (pool->plan_n_combines > 0) {
@@ -437,16 +559,98 @@ int32_t paged_decode_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
     cp.out = p.out;
     cp.num_q_heads = c.num_q_heads;
     cp.group = G;
-    const unsigned cgrid = static_cast<unsigned>((static_cast<int64_t>(cp.n_entries) * G + 3) / 4);
+    cp.num_kv_heads = c.num_kv_heads;
+    const unsigned cgrid = static_cast<unsigned>((static_cast<int64_t>(cp.n_entries) * c.num_q_heads + 3) / 4);
+    if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_COMBINE].begin(stream));
     if (c.head_dim == 128)
       combine_kernel<128><<<cgrid, 128, 0, stream>>>(cp);
     else
       combine_kernel<64><<<cgrid, 128, 0, stream>>>(cp);
     KV_CUDA(pool, cudaGetLastError());
+    if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_COMBINE].end(stream));
     ++pool->launches;
   }
   KV_CUDA(pool, cudaEventRecord(s.ev, stream));
   s.in_flight = true;
+  return KV_OK;
+}
+
+int32_t kv_ingest_host(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const int32_t* n_tokens,
+                       const void* const* k_src, const void* const* v_src, int32_t layer_begin, int32_t layer_count,
+                       void* staging, int64_t staging_bytes, void* cuda_stream) {
+  if (!pool || n_req < 0) return KV_ERR_INVALID;
+  if (n_req > 0 && (!req_ids || !n_tokens || !k_src || !v_src)) return KV_ERR_INVALID;
+  const kv_pool_config_t& c = pool->hs.cfg;
+  if (layer_begin < 0 || layer_count < 1 || layer_begin + layer_count > c.num_layers) return KV_ERR_INVALID;
+  if (!pool->has_device) return KV_ERR_NO_DEVICE;
+  if (n_req > 0 && (!staging || (reinterpret_cast<uintptr_t>(staging) & (kAlign - 1)) != 0)) return KV_ERR_INVALID;
+  const int64_t row_bytes = static_cast<int64_t>(layer_count) * c.num_kv_heads * c.head_dim * 2;
+  int64_t need = 0;
+  for (int32_t i = 0; i < n_req; ++i) {
+    if (n_tokens[i] < 0) return KV_ERR_INVALID;
+    if (n_tokens[i] > 0 && (!k_src[i] || !v_src[i])) return KV_ERR_INVALID;
+    need += 2 * align_up(row_bytes * n_tokens[i]);
+  }
+  if (need > staging_bytes) return KV_ERR_INVALID;
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  // K tensors first, then V tensors; each at a 256-byte aligned offset.  A run of requests whose
+  // host ranges and staging ranges are both back to back moves with one copy.
+  std::vector<const void*> kd(static_cast<size_t>(n_req)), vd(static_cast<size_t>(n_req));
+  char* dst = static_cast<char*>(staging);
+  for (int pass = 0; pass < 2; ++pass) {
+    const void* const* src = pass ? v_src : k_src;
+    std::vector<const void*>& dev = pass ? vd : kd;
+    const char* run_src = nullptr;
+    char* run_dst = nullptr;
+    int64_t run_len = 0;
+    auto flush = [&]() -> cudaError_t {
+      cudaError_t e = run_len ? cudaMemcpyAsync(run_dst, run_src, static_cast<size_t>(run_len), cudaMemcpyHostToDevice, stream)
+                              : cudaSuccess;
+      run_len = 0;
+      return e;
+    };
+    for (int32_t i = 0; i < n_req; ++i) {
+      const int64_t bytes = row_bytes * n_tokens[i];
+      dev[static_cast<size_t>(i)] = dst;
+      if (bytes == 0) continue;
+      const char* sp = static_cast<const char*>(src[i]);
+      if (run_len && sp == run_src + run_len && dst == run_dst + run_len) {
+        run_len += bytes;
+      } else {
+        KV_CUDA(pool, flush());
+        run_src = sp; run_dst = dst; run_len = bytes;
+      }
+      dst += (bytes % kAlign == 0) ? bytes : align_up(bytes);
+    }
+    KV_CUDA(pool, flush());
+    dst = static_cast<char*>(staging) + align_up(dst - static_cast<char*>(staging));
+  }
+  return kv_ingest(pool, n_req, req_ids, n_tokens, kd.data(), vd.data(), layer_begin, layer_count, cuda_stream);
+}
+
+int32_t paged_decode_attention_host(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids,
+                                    const void* q, void* out, float sm_scale, void* staging, int64_t staging_bytes,
+                                    void* cuda_stream) {
+  if (!pool || !req_ids || !q || !out || !staging || batch < 1) return KV_ERR_INVALID;
+  if ((reinterpret_cast<uintptr_t>(staging) & (kAlign - 1)) != 0) return KV_ERR_INVALID;
+  if (!pool->has_device) return KV_ERR_NO_DEVICE;
+  const kv_pool_config_t& c = pool->hs.cfg;
+  const int64_t bytes = static_cast<int64_t>(batch) * c.num_q_heads * c.head_dim * 2;
+  if (2 * align_up(bytes) > staging_bytes) return KV_ERR_INVALID;
+  // validate the batch before any copy is issued, so an error leaves the stream untouched
+  {
+    int32_t rc = pool->hs.check_batch(batch, req_ids, nullptr);
+    if (rc != KV_OK) return rc;
+    for (int32_t i = 0; i < batch; ++i)
+      if (pool->hs.reqs.find(req_ids[i])->second.len < 1) return KV_ERR_INVALID;
+  }
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  char* dq = static_cast<char*>(staging);
+  char* dout = dq + align_up(bytes);
+  KV_CUDA(pool, cudaMemcpyAsync(dq, q, static_cast<size_t>(bytes), cudaMemcpyHostToDevice, stream));
+  int32_t rc = paged_decode_attention(pool, layer, batch, req_ids, dq, dout, sm_scale, cuda_stream);
+  if (rc != KV_OK) return rc;
+  KV_CUDA(pool, cudaMemcpyAsync(out, dout, static_cast<size_t>(bytes), cudaMemcpyDeviceToHost, stream));
   return KV_OK;
 }
 
@@ -458,7 +662,27 @@ int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
   if (!std::strcmp(key, "min_chunk_blocks") && value >= 1 && value <= 65536) { pool->min_chunk_blocks = static_cast<int32_t>(value); return KV_OK; }
   if (!std::strcmp(key, "ctas_per_sm") && value >= 1 && value <= 8) { pool->ctas_per_sm = static_cast<int32_t>(value); return KV_OK; }
   if (!std::strcmp(key, "items_per_slot") && value >= 1 && value <= 1024) { pool->items_per_slot = static_cast<int32_t>(value); return KV_OK; }
+  if (!std::strcmp(key, "profile") && (value == 0 || value == 1)) { pool->profile = value != 0; return KV_OK; }
   return KV_ERR_INVALID;
+}
+
+int32_t kv_profile_read(kv_pool_t* pool, int32_t kind, int64_t* out_launches, double* out_ms) {
+  if (!pool || kind < 0 || kind >= KV_KERNEL_KINDS) return KV_ERR_INVALID;
+  ProfRing& r = pool->prof[kind];
+  KV_CUDA(pool, r.drain());
+  if (out_launches) *out_launches = r.launches;
+  if (out_ms) *out_ms = r.ms;
+  return KV_OK;
+}
+
+int32_t kv_profile_reset(kv_pool_t* pool) {
+  if (!pool) return KV_ERR_INVALID;
+  for (ProfRing& r : pool->prof) {
+    KV_CUDA(pool, r.drain());
+    r.launches = 0;
+    r.ms = 0.0;
+  }
+  return KV_OK;
 }
 
 int32_t kv_last_cuda_error(const kv_pool_t* pool) { return pool ? pool->last_cuda : KV_ERR_INVALID; }

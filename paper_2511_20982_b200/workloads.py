@@ -105,6 +105,33 @@ def kv_values(seed: int, kind: int, uid: int, num_kv_heads: int, head_dim: int, 
     return out
 
 
+def stream_keys(seed: int, kind: int, uids) -> np.ndarray:
+    """Vectorised stream_key: int64 bit patterns of stream_key(seed, kind, uid) for each uid."""
+    def mix(x):
+        x = (x ^ (x >> np.uint64(30))) * np.uint64(_M1)
+        x = (x ^ (x >> np.uint64(27))) * np.uint64(_M2)
+        return x ^ (x >> np.uint64(31))
+    with np.errstate(over="ignore"):
+        base = np.uint64(mix64_i(seed * _GAMMA + kind))
+        return mix(base + np.asarray(uids, dtype=np.int64).astype(np.uint64)).astype(np.int64)
+
+
+def kv_values_at(seed: int, kind: int, uids, positions, num_kv_heads: int, head_dim: int, layer_begin: int,
+                 layer_count: int, device="cpu") -> torch.Tensor:
+    """bf16 [layer_count][B][num_kv_heads][head_dim]: for request i, the K/V row of logical token
+    positions[i] — element [ll][i][h][j] == kv_values(seed, kind, uids[i], ..., t, t+1)[ll][h][0][j]
+    with t = positions[i].  One call serves a whole decode batch's appended tokens."""
+    keys = torch.from_numpy(stream_keys(seed, kind, uids)).to(device).view(1, -1, 1, 1)
+    t = torch.as_tensor(np.asarray(positions, dtype=np.int64), device=device).view(1, -1, 1, 1)
+    assert int(t.max()) < (1 << 20) and head_dim <= 256
+    ll = torch.arange(layer_begin, layer_begin + layer_count, dtype=torch.int64, device=device).view(-1, 1, 1, 1)
+    h = torch.arange(num_kv_heads, dtype=torch.int64, device=device).view(1, 1, -1, 1)
+    j = torch.arange(head_dim, dtype=torch.int64, device=device).view(1, 1, 1, -1)
+    ctr = (((ll * num_kv_heads + h) << 20) | t) << 8 | j
+    bits = mix64_t(ctr * _s64(_GAMMA) + keys)
+    return normal_table(device)[_lsr(bits, 48)]
+
+
 def q_values(seed: int, step: int, layer: int, batch: int, num_q_heads: int, head_dim: int,
              device="cpu") -> torch.Tensor:
     """bf16 [batch][num_q_heads][head_dim] query of decode step `step`, layer `layer`."""
