@@ -52,6 +52,7 @@ def parse_args():
     ap.add_argument("--e2e-steps", type=int, default=4, help="timed steps of the host-buffer leg (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-isolated", action="store_true", help="skip the attention-alone / ingest-alone legs")
+    ap.add_argument("--unfused", action="store_true", help="append and attention as separate calls (a3, then a4+a5)")
     ap.add_argument("--opt", action="append", default=[], help="pool option key=value (tuning)")
     return ap.parse_args()
 
@@ -300,7 +301,7 @@ def run_cuda(args):
     opts = {k: int(v) for k, v in (o.split("=") for o in args.opt)}
     t_setup = time.time()
     loop = DecodeLoop(w, Wm + K, n_host_steps=e2e_w + args.e2e_steps, device=dev, streams=args.streams, salt=rank,
-                      options=opts)
+                      options=opts, fused=not args.unfused)
     t_setup = time.time() - t_setup
     pool = loop.pool
     phys = int(os.environ.get("CUDA_VISIBLE_DEVICES", "").split(",")[local]) if os.environ.get("CUDA_VISIBLE_DEVICES") else local
@@ -350,7 +351,8 @@ def run_cuda(args):
         "attn_splitkv_kernel": {"launches": attn_n, "ms": attn_ms},
         "combine_kernel": {"launches": comb_n, "ms": comb_ms},
         "ingest_kernel": {"launches": ing_n, "ms": ing_ms,
-                          "gbs": (by["ingest"] + by["append"]) / (ing_ms * 1e-3) / 1e9 if ing_ms > 0 else None},
+                          "gbs": (by["ingest"] + (0 if loop.fused else by["append"])) / (ing_ms * 1e-3) / 1e9
+                          if ing_ms > 0 else None},
         "attn_plus_combine_gbs": by["attn"] / ((attn_ms + comb_ms) * 1e-3) / 1e9 if attn_ms > 0 else None,
     }
 
@@ -405,6 +407,7 @@ def run_cuda(args):
             "config": {"workload": args.workload, "layers": w.num_layers, "q_heads": w.num_q_heads,
                        "kv_heads": w.num_kv_heads, "head_dim": w.head_dim, "block_size": w.block_size,
                        "batch": w.batch, "ingest_per_step": w.ingest_per_step, "streams": 2 if loop.two_streams else 1,
+                       "decode_call": "paged_decode_step (fused a3+a4+a5)" if loop.fused else "kv_ingest + paged_decode_attention",
                        "pool_blocks": loop.cfg.num_blocks, "pool_gb": pool.kv_bytes / 1e9,
                        "blocks_high_water": stats["blocks_high_water"],
                        "l2": f"inputs larger than L2: each layer's attention streams {kv_gb_layer:.2f} GB of KV",

@@ -151,6 +151,28 @@ int32_t paged_decode_attention(kv_pool_t* pool, int32_t layer, int32_t batch,
                                void* out /*device*/, float sm_scale, void* cuda_stream);
 
 /*
+ * a3 + a4 + a5 fused — one launch per layer and decode step.  Same result as
+ *     kv_ingest(n_tokens = 1 per request, layer_begin = layer, layer_count = 1)   then
+ *     paged_decode_attention(layer)
+ * but the new token's K/V row is appended by the attention kernel itself: the work unit that
+ * owns a request's last block reads that row from k_new / v_new, uses it, and writes it into
+ * the pool (every decode iteration adds one token to each in-flight request and
+ * re-reads its KV).  Protocol per decode step:
+ *     kv_reserve(pool, batch, req_ids, ones)           once, host only (a1)
+ *     for layer in 0 .. num_layers-1:
+ *         paged_decode_step(pool, layer, batch, req_ids, q, k_new, v_new, out, ...)
+ *   k_new, v_new: device, bf16, [batch][num_kv_heads][head_dim] — row i belongs to req_ids[i]
+ *   and lands at that request's last position (length - 1).
+ * Errors: as paged_decode_attention; additionally KV_ERR_INVALID unless every request's last
+ * reservation is exactly one token (no reservation since, no multi-token reservation).
+ * Calling it twice for the same layer and step rewrites the same row (idempotent).
+ */
+int32_t paged_decode_step(kv_pool_t* pool, int32_t layer, int32_t batch,
+                          const int64_t* req_ids /*host*/, const void* q /*device*/,
+                          const void* k_new /*device*/, const void* v_new /*device*/,
+                          void* out /*device*/, float sm_scale, void* cuda_stream);
+
+/*
  * a6 — free (a completed request releases consumer capacity).  Host only
  * and immediate: blocks return to the free list (LIFO) and the table row is dropped.  The
  * caller must not ingest into recycled blocks on a different stream before the attention
@@ -209,6 +231,13 @@ int32_t paged_decode_attention_host(kv_pool_t* pool, int32_t layer, int32_t batc
                                     const int64_t* req_ids /*host*/, const void* q /*HOST*/,
                                     void* out /*HOST*/, float sm_scale, void* staging /*device*/,
                                     int64_t staging_bytes, void* cuda_stream);
+/* paged_decode_step with q, k_new, v_new, out in HOST memory; staging needs
+ * 2 * batch*Hq*d*2 + 2 * batch*Hkv*d*2 bytes (each of the four rounded up to 256 B).       */
+int32_t paged_decode_step_host(kv_pool_t* pool, int32_t layer, int32_t batch,
+                               const int64_t* req_ids /*host*/, const void* q /*HOST*/,
+                               const void* k_new /*HOST*/, const void* v_new /*HOST*/,
+                               void* out /*HOST*/, float sm_scale, void* staging /*device*/,
+                               int64_t staging_bytes, void* cuda_stream);
 
 /* Number of kernels this pool has launched since creation (bench `gpu_launches`).         */
 int64_t kv_launch_count(const kv_pool_t* pool);
@@ -232,8 +261,9 @@ int32_t kv_profile_reset(kv_pool_t* pool);
 
 /* Tuning knobs (all optional; defaults chosen for B200).  key: "min_chunk_blocks" (smallest
  * split-KV chunk, in blocks), "ctas_per_sm" (resident attention CTAs per SM the planner
- * sizes the work list for), "items_per_slot" (work items per resident warp), "profile"
- * (0/1, see kv_profile_read).  Unknown key or out-of-range value => KV_ERR_INVALID.        */
+ * sizes the work list for), "items_per_slot" (work items per resident warp), "fuse_combine"
+ * (1, default: the split-KV merge runs inside the attention kernel; 0: separate combine
+ * kernel), "profile" (0/1, see kv_profile_read).  Unknown key or out-of-range value => KV_ERR_INVALID.        */
 int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value);
 
 /* Last CUDA error code seen by this pool (cudaError_t as int; 0 = none).                  */

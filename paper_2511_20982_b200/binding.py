@@ -47,6 +47,8 @@ _SIGS = {
     "kv_reserve": (_i32, [_P, _i32, _P, _P]),
     "kv_ingest": (_i32, [_P, _i32, _P, _P, _P, _P, _i32, _i32, _P]),
     "paged_decode_attention": (_i32, [_P, _i32, _i32, _P, _P, _P, ctypes.c_float, _P]),
+    "paged_decode_step": (_i32, [_P, _i32, _i32, _P, _P, _P, _P, _P, ctypes.c_float, _P]),
+    "paged_decode_step_host": (_i32, [_P, _i32, _i32, _P, _P, _P, _P, _P, ctypes.c_float, _P, _i64, _P]),
     "kv_free": (_i32, [_P, _i32, _P]),
     "kv_block_table": (_i32, [_P, _i64, _P, _i32, ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
     "kv_pool_stats": (_i32, [_P, ctypes.POINTER(_i64), ctypes.POINTER(_i64), ctypes.POINTER(_i32),
@@ -171,6 +173,23 @@ def paged_decode_attention(handle: int, layer: int, req_ids, q_ptr: int, out_ptr
     ids = _ids(req_ids)
     _check(lib.paged_decode_attention(handle, layer, ids.size, _np(ids), q_ptr, out_ptr, sm_scale, stream or None),
            "paged_decode_attention")
+
+
+def paged_decode_step(handle: int, layer: int, req_ids, q_ptr: int, k_new_ptr: int, v_new_ptr: int, out_ptr: int,
+                      sm_scale: float = 0.0, stream: int = 0) -> None:
+    """Fused a3 + a4 + a5 (after kv_reserve(req_ids, ones) for this step)."""
+    ids = _ids(req_ids)
+    _check(lib.paged_decode_step(handle, layer, ids.size, _np(ids), q_ptr, k_new_ptr, v_new_ptr, out_ptr, sm_scale,
+                                 stream or None), "paged_decode_step")
+
+
+def paged_decode_step_host(handle: int, layer: int, req_ids, q_host_ptr: int, k_new_host_ptr: int,
+                           v_new_host_ptr: int, out_host_ptr: int, sm_scale: float, staging_ptr: int,
+                           staging_bytes: int, stream: int = 0) -> None:
+    ids = _ids(req_ids)
+    _check(lib.paged_decode_step_host(handle, layer, ids.size, _np(ids), q_host_ptr, k_new_host_ptr, v_new_host_ptr,
+                                      out_host_ptr, sm_scale, staging_ptr, staging_bytes, stream or None),
+           "paged_decode_step_host")
 
 
 def kv_ingest_host(handle: int, req_ids, n_tokens, k_src, v_src, layer_begin: int, layer_count: int,
@@ -304,6 +323,18 @@ class KVPool:
         if out is None:
             out = torch.empty_like(q)
         paged_decode_attention(self.handle, layer, req_ids, q.data_ptr(), out.data_ptr(), sm_scale, self._stream(stream))
+        return out
+
+    def decode_step(self, layer, req_ids, q, k_new, v_new, out=None, sm_scale=0.0, stream=None):
+        """Fused append + attention for one layer; k_new / v_new: bf16 [batch][Hkv][d].  The caller has
+        reserved the step's token with ``reserve(req_ids, ones)``."""
+        import torch
+
+        assert q.is_contiguous() and k_new.is_contiguous() and v_new.is_contiguous()
+        if out is None:
+            out = torch.empty_like(q)
+        paged_decode_step(self.handle, layer, req_ids, q.data_ptr(), k_new.data_ptr(), v_new.data_ptr(),
+                          out.data_ptr(), sm_scale, self._stream(stream))
         return out
 
     def gather(self, req_id, stream=None):

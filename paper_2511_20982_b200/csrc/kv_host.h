@@ -74,8 +74,10 @@ struct WorkItem {
   int32_t n_blocks;
   int32_t n_tokens;      // valid tokens in this run (last block of a request may be partial)
   int32_t partial_base;  // first partial slot of this request, or -1: only chunk, writes `out`
-  int32_t n_chunks;      // chunks of this request; partial slot of (kv_head h, chunk c) =
-  int32_t chunk_idx;     //   partial_base + h * n_chunks + c
+  int32_t chunks;        // (n_chunks << 16) | chunk_idx; partial slot of (kv_head h, chunk c) =
+                         //   partial_base + h * n_chunks + c
+  int32_t last_blk;      // physical id of the request's LAST block (the fused decode step appends there
+                         //   before the device block_table mirror has seen it)
 };
 static_assert(sizeof(WorkItem) == 32, "WorkItem is read by the kernel as two int4");
 
@@ -243,6 +245,7 @@ class HostState {
       const int32_t nc0 = static_cast<int32_t>((nb + chunk - 1) / chunk);
       const int32_t per = (nb + nc0 - 1) / nc0;  // even split: ceil(nb / nc0) <= chunk blocks per chunk
       const int32_t nc = (nb + per - 1) / per;   // <= nc0
+      if (nc > 0xffff) return KV_ERR_TOO_LONG;   // (n_chunks, chunk_idx) are packed 16:16
       const int32_t base = nc > 1 ? next_partial : -1;
       if (nc > 1) {
         plan->combines.push_back({i, base, nc, 0});
@@ -256,8 +259,8 @@ class HostState {
         w.n_blocks = std::min(per, nb - c * per);
         w.n_tokens = std::min(r->len - w.blk_begin * cfg.block_size, w.n_blocks * cfg.block_size);
         w.partial_base = base;
-        w.n_chunks = nc;
-        w.chunk_idx = c;
+        w.chunks = (nc << 16) | c;
+        w.last_blk = r->blocks.back();
         max_nb = std::max(max_nb, w.n_blocks);
         unsorted_.push_back(w);
       }

@@ -207,21 +207,25 @@ __global__ void __launch_bounds__(kIngestThreads) ingest_kernel(const IngestPara
 // ---------------------------------------------------------------------------------------------
 
 struct WorkItemDev {  // == kvp::WorkItem (kv_host.h); one item = num_kv_heads units, heads fastest
-  int32_t batch_idx, slot, blk_begin, n_blocks, n_tokens, partial_base, n_chunks, chunk_idx;
+  int32_t batch_idx, slot, blk_begin, n_blocks, n_tokens, partial_base, chunks, last_blk;
 };
 
 struct AttnParams {
-  const uint16_t* kv_layer;    // &kv[layer][0]...
-  const int32_t* block_table;
+  uint16_t* kv_layer;          // &kv[layer][0]...  (written only by the fused append)
+  int32_t* block_table;        // device mirror (written only by the fused append)
   int32_t bt_stride;
   const WorkItemDev* items;
   int32_t n_items, n_units;    // n_units = n_items * num_kv_heads
   const uint16_t* q;
+  const uint16_t* k_new;       // fused decode step: [batch][Hkv][D] rows of the token being appended
+  const uint16_t* v_new;
   uint16_t* out;
   float* part_o;               // [n_partials][G][D]  un-normalised
   float* part_ml;              // [n_partials][G][2]  (m in log2 units, l)
   int32_t* counters;           // [0] next work item, [1] finished CTAs
+  int32_t* arrive;             // per split (request, kv_head): chunks finished (fused combine); self-resetting
   int32_t num_q_heads, num_kv_heads, group;
+  int32_t fuse_combine;
   float scale_log2;            // sm_scale * log2(e)
 };
 
@@ -250,7 +254,121 @@ __device__ __forceinline__ void load_tile(KVTile<D>& T, const uint16_t* tile, in
   }
 }
 
+// Fused decode step (a3 inside a4): the request's last tile with the row of the token being
+// appended (r_new = nv - 1) taken from k_new / v_new instead of the pool.  Same lanes, same
+// registers as load_tile, so the MMAs downstream do not know the difference.
 template <int D>
+__device__ __forceinline__ void load_tile_append(KVTile<D>& T, const uint16_t* tile, const uint16_t* k_new,
+                                                 const uint16_t* v_new, int nv, int g, int c) {
+  const int r_new = nv - 1;
+#pragma unroll
+  for (int rs = 0; rs < 2; ++rs) {
+    const int row = g + 8 * rs;
+    const uint16_t* kp = (row == r_new ? k_new : tile + row * D) + c * 8;
+#pragma unroll
+    for (int j = 0; j < D / 32; ++j) T.k[rs][j] = ldg_stream_pred(kp + j * 32, row < nv);
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int row = 2 * c + (i & 1) + 8 * (i >> 1);
+    const uint16_t* vp = (row == r_new ? v_new : tile + kBlockSize * D + row * D) + g * 8;
+#pragma unroll
+    for (int cs = 0; cs < D / 64; ++cs) T.v[i][cs] = ldg_stream_pred(vp + cs * 64, row < nv);
+  }
+}
+
+// ... and the append itself: the lanes that hold row r_new write it into the pool tile (a3).
+template <int D>
+__device__ __forceinline__ void store_new_row(const KVTile<D>& T, uint16_t* tile, int nv, int g, int c) {
+  const int r_new = nv - 1;
+#pragma unroll
+  for (int rs = 0; rs < 2; ++rs) {
+    if (g + 8 * rs == r_new) {
+      uint16_t* kp = tile + r_new * D + c * 8;
+#pragma unroll
+      for (int j = 0; j < D / 32; ++j) *reinterpret_cast<uint4*>(kp + j * 32) = T.k[rs][j];
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    if (2 * c + (i & 1) + 8 * (i >> 1) == r_new) {
+      uint16_t* vp = tile + kBlockSize * D + r_new * D + g * 8;
+#pragma unroll
+      for (int cs = 0; cs < D / 64; ++cs) *reinterpret_cast<uint4*>(vp + cs * 64) = T.v[i][cs];
+    }
+  }
+}
+
+// a5 for query heads [head0, head0 + NH) of one (request, kv head): out = sum_c 2^(m_c - M) O_c /
+// sum_c 2^(m_c - M) l_c over the n_chunks partials starting at partial slot pb (one slot per chunk).
+// One warp; lane owns D/32 columns of every head.  The merge is a running (online) one so the
+// loads of all heads and of several chunks are independent and in flight together — this code is
+// pure latency, it runs on warps that would otherwise be streaming KV.  Loads bypass L1 (.cg):
+// the partials were written by other SMs, possibly earlier in this same kernel.
+template <int D, int NH>
+__device__ __forceinline__ void combine_heads(const float* part_o, const float* part_ml, int pb, int n_chunks,
+                                              int G, int head0, uint16_t* out_row0, int lane) {
+  constexpr int V = D / 32;
+  const float* ml = part_ml + (static_cast<int64_t>(pb) * G + head0) * 2;
+  const int64_t ml_stride = static_cast<int64_t>(G) * 2;
+  const float* po = part_o + (static_cast<int64_t>(pb) * G + head0) * D + lane * V;
+  const int64_t po_stride = static_cast<int64_t>(G) * D;
+  float M[NH], den[NH], acc[NH][V];
+#pragma unroll
+  for (int hh = 0; hh < NH; ++hh) {
+    M[hh] = -INFINITY; den[hh] = 0.f;
+#pragma unroll
+    for (int k = 0; k < V; ++k) acc[hh][k] = 0.f;
+  }
+#pragma unroll 2
+  for (int ch = 0; ch < n_chunks; ++ch) {
+    float2 mlv[NH];
+    float x[NH][V];
+#pragma unroll
+    for (int hh = 0; hh < NH; ++hh) {
+      mlv[hh] = __ldcg(reinterpret_cast<const float2*>(ml + ch * ml_stride + hh * 2));
+      if constexpr (V == 4) {
+        const float4 t = __ldcg(reinterpret_cast<const float4*>(po + ch * po_stride + hh * D));
+        x[hh][0] = t.x; x[hh][1] = t.y; x[hh][2] = t.z; x[hh][3] = t.w;
+      } else {
+        const float2 t = __ldcg(reinterpret_cast<const float2*>(po + ch * po_stride + hh * D));
+        x[hh][0] = t.x; x[hh][1] = t.y;
+      }
+    }
+#pragma unroll
+    for (int hh = 0; hh < NH; ++hh) {
+      const float mn = fmaxf(M[hh], mlv[hh].x);                 // finite: every chunk holds >= 1 token
+      const float r = fast_exp2(M[hh] - mn), a = fast_exp2(mlv[hh].x - mn);
+      M[hh] = mn;
+      den[hh] = den[hh] * r + a * mlv[hh].y;
+#pragma unroll
+      for (int k = 0; k < V; ++k) acc[hh][k] = acc[hh][k] * r + a * x[hh][k];
+    }
+  }
+#pragma unroll
+  for (int hh = 0; hh < NH; ++hh) {
+    const float inv = 1.f / den[hh];
+    uint16_t* op = out_row0 + hh * D + lane * V;
+    if constexpr (V == 4) {
+      *reinterpret_cast<uint2*>(op) = make_uint2(pack_bf16x2(acc[hh][0] * inv, acc[hh][1] * inv),
+                                                 pack_bf16x2(acc[hh][2] * inv, acc[hh][3] * inv));
+    } else {
+      *reinterpret_cast<uint32_t*>(op) = pack_bf16x2(acc[hh][0] * inv, acc[hh][1] * inv);
+    }
+  }
+}
+
+// all G <= 8 heads of a (request, kv head), widest groups first
+template <int D>
+__device__ __forceinline__ void combine_group(const float* part_o, const float* part_ml, int pb, int n_chunks, int G,
+                                              uint16_t* out_row0, int lane) {
+  int head = 0;
+  for (; head + 4 <= G; head += 4) combine_heads<D, 4>(part_o, part_ml, pb, n_chunks, G, head, out_row0 + head * D, lane);
+  for (; head + 2 <= G; head += 2) combine_heads<D, 2>(part_o, part_ml, pb, n_chunks, G, head, out_row0 + head * D, lane);
+  for (; head < G; ++head) combine_heads<D, 1>(part_o, part_ml, pb, n_chunks, G, head, out_row0 + head * D, lane);
+}
+
+template <int D, bool kAppend>
 __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const AttnParams p) {
   constexpr int KJ = D / 32;   // K vectors per row per thread
   constexpr int KS = D / 16;   // MMA k-steps of S^T = K q^T
@@ -262,10 +380,10 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
   const int G = p.group;
   const int64_t blk_stride = static_cast<int64_t>(p.num_kv_heads) * kTileElems;
 
-  for (;;) {
-    int item = 0;
-    if (lane == 0) item = atomicAdd(&p.counters[0], 1);
-    item = __shfl_sync(0xffffffffu, item, 0);
+  // Dynamic scheduling: the first unit of every warp is its global warp index (no atomic on the way to
+  // the first byte), the rest come from a counter that starts at the number of warps.
+  const int n_warps = gridDim.x * kAttnWarps;
+  for (int item = blockIdx.x * kAttnWarps + (threadIdx.x >> 5);;) {
     if (item >= p.n_units) break;
     const int h = item % p.num_kv_heads;
     const WorkItemDev* wi = p.items + item / p.num_kv_heads;
@@ -273,7 +391,13 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
     const int4 w1 = __ldg(reinterpret_cast<const int4*>(wi) + 1);
     const int batch_idx = w0.x, slot = w0.y, blk_begin = w0.z, n_blocks = w0.w;
     const int n_tokens = w1.x;
-    const int pidx = w1.y < 0 ? -1 : w1.y + h * w1.z + w1.w;
+    const int n_chunks = w1.z >> 16, chunk_idx = w1.z & 0xffff, last_blk = w1.w;
+    const int pbase = w1.y < 0 ? -1 : w1.y + h * n_chunks;     // first partial slot of (request, kv head)
+    const int pidx = w1.y < 0 ? -1 : pbase + chunk_idx;
+    // Fused append: the unit that owns the request's last block takes that tile FIRST (the order of
+    // tiles does not matter to an online softmax), with the new token's row read from k_new / v_new.
+    const bool special = kAppend && chunk_idx == n_chunks - 1;
+    const int sp = special ? 1 : 0;
 
     // q^T as B fragments: lane (g, c) holds head g, columns of chunk c + 4j (zero for g >= G)
     uint32_t qf[KS][2];
@@ -294,7 +418,7 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
     for (int i = 0; i < MT; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
 
     const int32_t* bt = p.block_table + static_cast<int64_t>(slot) * p.bt_stride + blk_begin;
-    const uint16_t* kvh = p.kv_layer + static_cast<int64_t>(h) * kTileElems;
+    uint16_t* kvh = p.kv_layer + static_cast<int64_t>(h) * kTileElems;
     int32_t ids = lane < n_blocks ? __ldg(bt + lane) : 0;       // physical ids of blocks [32k, 32k+32)
     int32_t ids_next = 0;
 
@@ -339,9 +463,16 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
       l1 = l1 * a1 + (p1 + p3);
 #pragma unroll
       for (int i = 0; i < MT; ++i) { o[i][0] *= a0; o[i][1] *= a1; o[i][2] *= a0; o[i][3] *= a1; }
-      // ---- P^T as the B fragment: transpose the two 8x8 halves across the warp ----
-      const uint32_t b0 = movmatrix_trans(pack_bf16x2(p0, p1));  // tokens 2c, 2c+1   of head g
-      const uint32_t b1 = movmatrix_trans(pack_bf16x2(p2, p3));  // tokens 2c+8, 2c+9 of head g
+      // ---- P^T as the B fragment: transpose the two 8x8 halves across the warp.  P is fed to the
+      // tensor core as bf16 hi + bf16 lo (p = hi + lo up to 2^-17 p), so the weights keep ~16 mantissa
+      // bits and the only bf16-sized error left in the result is the final rounding of `out`.
+      const uint32_t ph01 = pack_bf16x2(p0, p1), ph23 = pack_bf16x2(p2, p3);
+      const uint32_t pl01 = pack_bf16x2(p0 - __uint_as_float(ph01 << 16), p1 - __uint_as_float(ph01 & 0xffff0000u));
+      const uint32_t pl23 = pack_bf16x2(p2 - __uint_as_float(ph23 << 16), p3 - __uint_as_float(ph23 & 0xffff0000u));
+      const uint32_t b0 = movmatrix_trans(ph01);                 // tokens 2c, 2c+1   of head g
+      const uint32_t b1 = movmatrix_trans(ph23);                 // tokens 2c+8, 2c+9 of head g
+      const uint32_t c0 = movmatrix_trans(pl01);
+      const uint32_t c1 = movmatrix_trans(pl23);
       // ---- O^T += V^T P^T : m-tile i takes d column e = i (row g) and e = i + NE/2 (row g+8) ----
 #pragma unroll
       for (int i = 0; i < MT; ++i) {
@@ -363,18 +494,33 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
           a3_ = pair_lo(u4_get(T.v[2][cs2], r2), u4_get(T.v[3][cs2], r2));
         }
         mma_bf16_m16n8k16(o[i], a0_, a1_, a2_, a3_, b0, b1);
+        mma_bf16_m16n8k16(o[i], a0_, a1_, a2_, a3_, c0, c1);
       }
     };
 
     KVTile<D> A, B;
-    issue(A, 0);
-    for (int t = 0; t < n_blocks; t += 2) {
-      const bool has_b = t + 1 < n_blocks;
-      if (has_b) issue(B, t + 1);
-      consume(A, t);
+    uint16_t* last_tile = kvh + last_blk * blk_stride;
+    const int nv_last = n_tokens - (n_blocks - 1) * kBlockSize;
+    if (special) {
+      const int64_t row = (static_cast<int64_t>(batch_idx) * p.num_kv_heads + h) * D;
+      load_tile_append<D>(A, last_tile, p.k_new + row, p.v_new + row, nv_last, g, c);
+      if (h == 0 && lane == 0) p.block_table[static_cast<int64_t>(slot) * p.bt_stride + blk_begin + n_blocks - 1] = last_blk;
+    } else {
+      issue(A, 0);
+    }
+    // virtual tile v -> real tile: special ? (v == 0 ? n_blocks - 1 : v - 1) : v
+    for (int v = 0; v < n_blocks; v += 2) {
+      const bool has_b = v + 1 < n_blocks;
+      if (has_b) issue(B, v + 1 - sp);
+      if (special && v == 0) {
+        consume(A, n_blocks - 1);
+        store_new_row<D>(A, last_tile, nv_last, g, c);
+      } else {
+        consume(A, v - sp);
+      }
       if (has_b) {
-        if (t + 2 < n_blocks) issue(A, t + 2);
-        consume(B, t + 1);
+        if (v + 2 < n_blocks) issue(A, v + 2 - sp);
+        consume(B, v + 1 - sp);
       }
     }
 
@@ -421,6 +567,24 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
         if (g == 0) *reinterpret_cast<float2*>(p.part_ml + (static_cast<int64_t>(pidx) * G + head) * 2) = make_float2(m, l);
       }
     }
+    // ---- fused a5: the unit that completes its (request, kv head) merges the partials ----
+    if (pidx >= 0 && p.fuse_combine) {
+      __threadfence();                                           // this lane's partial stores, device-wide
+      __syncwarp();
+      int last = 0;
+      if (lane == 0) {
+        last = atomicAdd(&p.arrive[pbase], 1) == n_chunks - 1;
+        if (last) p.arrive[pbase] = 0;                           // ready for the next launch
+      }
+      last = __shfl_sync(0xffffffffu, last, 0);
+      if (last) {
+        __threadfence();
+        combine_group<D>(p.part_o, p.part_ml, pbase, n_chunks, G,
+                         p.out + (static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G) * D, lane);
+      }
+    }
+    if (lane == 0) item = n_warps + atomicAdd(&p.counters[0], 1);
+    item = __shfl_sync(0xffffffffu, item, 0);
   }
 
   // Last CTA out rewinds the work counter for the next launch (launches on one pool are
@@ -449,48 +613,15 @@ struct CombineParams {
 
 template <int D>
 __global__ void __launch_bounds__(128) combine_kernel(const CombineParams p) {
-  constexpr int V = D / 32;  // floats per lane
   const int lane = threadIdx.x & 31;
   const int w = blockIdx.x * 4 + (threadIdx.x >> 5);
   if (w >= p.n_entries * p.num_q_heads) return;
   const int ei = w / p.num_q_heads, qh = w % p.num_q_heads;
   const int kvh = qh / p.group, head = qh % p.group;
-  CombineEntryDev e = p.entries[ei];
-  e.partial_begin += kvh * e.n_chunks;                        // partials of (request, kv head): contiguous over chunks
-  const float* ml = p.part_ml + (static_cast<int64_t>(e.partial_begin) * p.group + head) * 2;
-  const int64_t ml_stride = static_cast<int64_t>(p.group) * 2;
-  const float* po = p.part_o + (static_cast<int64_t>(e.partial_begin) * p.group + head) * D + lane * V;
-  const int64_t po_stride = static_cast<int64_t>(p.group) * D;
-
-  float M = -INFINITY;
-  for (int ch = lane; ch < e.n_chunks; ch += 32) M = fmaxf(M, __ldg(ml + ch * ml_stride));
-#pragma unroll
-  for (int off = 16; off > 0; off >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, off));
-
-  float acc[V];
-#pragma unroll
-  for (int k = 0; k < V; ++k) acc[k] = 0.f;
-  float den = 0.f;
-#pragma unroll 4
-  for (int ch = 0; ch < e.n_chunks; ++ch) {
-    const float2 mlv = __ldg(reinterpret_cast<const float2*>(ml + ch * ml_stride));
-    const float a = fast_exp2(mlv.x - M);
-    den += a * mlv.y;
-    if constexpr (V == 4) {
-      const float4 x = __ldg(reinterpret_cast<const float4*>(po + ch * po_stride));
-      acc[0] += a * x.x; acc[1] += a * x.y; acc[2] += a * x.z; acc[3] += a * x.w;
-    } else {
-      const float2 x = __ldg(reinterpret_cast<const float2*>(po + ch * po_stride));
-      acc[0] += a * x.x; acc[1] += a * x.y;
-    }
-  }
-  const float inv = 1.f / den;
-  uint16_t* op = p.out + (static_cast<int64_t>(e.batch_idx) * p.num_q_heads + qh) * D + lane * V;
-  if constexpr (V == 4) {
-    *reinterpret_cast<uint2*>(op) = make_uint2(pack_bf16x2(acc[0] * inv, acc[1] * inv), pack_bf16x2(acc[2] * inv, acc[3] * inv));
-  } else {
-    *reinterpret_cast<uint32_t*>(op) = pack_bf16x2(acc[0] * inv, acc[1] * inv);
-  }
+  const CombineEntryDev e = p.entries[ei];
+  // partials of (request, kv head) are contiguous over chunks
+  combine_heads<D, 1>(p.part_o, p.part_ml, e.partial_begin + kvh * e.n_chunks, e.n_chunks, p.group, head,
+                      p.out + (static_cast<int64_t>(e.batch_idx) * p.num_q_heads + qh) * D, lane);
 }
 
 }  // namespace kvp

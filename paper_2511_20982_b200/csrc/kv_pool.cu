@@ -26,7 +26,7 @@ constexpr int32_t kMaxPartials = 32768;        // split-KV partial slots in the 
 inline int64_t align_up(int64_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {  // byte offsets inside the caller's slab
-  int64_t kv_bytes, block_table, counters, ingest_blobs, plan_blobs, part_o, part_ml, total;
+  int64_t kv_bytes, block_table, counters, arrive, ingest_blobs, plan_blobs, part_o, part_ml, total;
   int64_t plan_blob_bytes;
 };
 
@@ -39,6 +39,8 @@ Layout make_layout(const kv_pool_config_t& c) {
   off = align_up(off + static_cast<int64_t>(c.max_requests) * c.max_blocks_per_request * 4);
   L.counters = off;
   off = align_up(off + 256);
+  L.arrive = off;
+  off = align_up(off + static_cast<int64_t>(kMaxPartials) * 4);
   L.ingest_blobs = off;
   off = align_up(off + kIngestRingBytes);
   const int64_t items_cap = static_cast<int64_t>(c.max_requests) + kMaxPartials;
@@ -187,6 +189,7 @@ struct kv_pool {
   int32_t min_chunk_blocks = 16;
   int32_t ctas_per_sm = 2;
   int32_t items_per_slot = 8;
+  bool fuse_combine = true;
   bool profile = false;
   ProfRing prof[KV_KERNEL_KINDS];
   // staging
@@ -198,6 +201,7 @@ struct kv_pool {
   std::vector<int64_t> plan_ids;
   int plan_slot = -1;
   int32_t plan_n_items = 0, plan_n_combines = 0;
+  int32_t plan_append_ok = -1;  // -1 unknown, 0 / 1: every request's last reservation is one token
   int64_t plan_combine_off = 0;
   kvp::DecodePlan plan;
 
@@ -319,12 +323,6 @@ int32_t run_ingest(kv_pool* pool, int32_t n_req, const int64_t* req_ids, const i
   return flush();
 }
 
-int32_t check_ids_known(const kv_pool* pool, int32_t n, const int64_t* ids) {
-  for (int32_t i = 0; i < n; ++i)
-    if (pool->hs.reqs.find(ids[i]) == pool->hs.reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
-  return KV_OK;
-}
-
 }  // namespace
 
 extern "C" {
@@ -373,6 +371,7 @@ int32_t kv_pool_create(const kv_pool_config_t* cfg, kv_pool_t** out_pool) {
     }
     // work counters start at zero; the attention kernel rewinds them itself afterwards
     if (e == cudaSuccess) e = cudaMemset(pool->base + lay.counters, 0, 256);
+    if (e == cudaSuccess) e = cudaMemset(pool->base + lay.arrive, 0, static_cast<size_t>(kMaxPartials) * 4);
     if (e != cudaSuccess) {
       kv_pool_destroy(pool);
       return KV_ERR_CUDA;
@@ -478,15 +477,16 @@ int32_t kv_plan_decode(kv_pool_t* pool, int32_t batch, const int64_t* req_ids, i
     const int32_t h = u % Hkv;
     int32_t* o = out_items + 5 * u;
     o[0] = w.batch_idx; o[1] = h; o[2] = w.blk_begin; o[3] = w.n_blocks;
-    o[4] = w.partial_base < 0 ? -1 : w.partial_base + h * w.n_chunks + w.chunk_idx;
+    o[4] = w.partial_base < 0 ? -1 : w.partial_base + h * (w.chunks >> 16) + (w.chunks & 0xffff);
   }
   if (out_n_items) *out_n_items = n;
   if (out_chunk_blocks) *out_chunk_blocks = plan.chunk_blocks;
   return KV_OK;
 }
 
-int32_t paged_decode_attention(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const void* q,
-                               void* out, float sm_scale, void* cuda_stream) {
+// a4 + a5 (and a3 when k_new / v_new are given): plan (cached across the layers of a step), upload, launch.
+static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const void* q,
+                                const void* k_new, const void* v_new, void* out, float sm_scale, void* cuda_stream) {
   if (!pool || !req_ids || !q || !out || !aligned16(q) || !aligned16(out)) return KV_ERR_INVALID;
   const kv_pool_config_t& c = pool->hs.cfg;
   if (layer < 0 || layer >= c.num_layers || batch < 1) return KV_ERR_INVALID;
@@ -512,11 +512,20 @@ int32_t paged_decode_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
     pool->plan_slot = -1;
     KV_CUDA(pool, cudaMemcpyAsync(s->dev, s->host, item_bytes + comb_bytes, cudaMemcpyHostToDevice, stream));
     pool->plan_slot = idx;
+    pool->plan_append_ok = -1;
     pool->plan_epoch = pool->hs.epoch;
     pool->plan_ids.assign(req_ids, req_ids + batch);
     pool->plan_n_items = static_cast<int32_t>(pool->plan.items.size());
     pool->plan_n_combines = static_cast<int32_t>(pool->plan.combines.size());
     pool->plan_combine_off = static_cast<int64_t>(item_bytes);
+  }
+  if (k_new) {  // fused append: every request's last reservation must be the one token being appended
+    if (!cached || pool->plan_append_ok != 1) {
+      pool->plan_append_ok = 1;
+      for (int32_t i = 0; i < batch; ++i)
+        if (pool->hs.reqs.find(req_ids[i])->second.last_n != 1) { pool->plan_append_ok = 0; break; }
+    }
+    if (!pool->plan_append_ok) return KV_ERR_INVALID;
   }
   StageSlot& s = pool->plan_ring[pool->plan_slot];
   const int32_t G = c.num_q_heads / c.num_kv_heads;
@@ -524,12 +533,16 @@ int32_t paged_decode_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
 
   AttnParams p{};
   const int64_t layer_elems = c.num_blocks * c.num_kv_heads * 2LL * c.block_size * c.head_dim;
-  p.kv_layer = reinterpret_cast<const uint16_t*>(pool->base) + static_cast<int64_t>(layer) * layer_elems;
-  p.block_table = reinterpret_cast<const int32_t*>(pool->base + pool->lay.block_table);
+  p.kv_layer = reinterpret_cast<uint16_t*>(pool->base) + static_cast<int64_t>(layer) * layer_elems;
+  p.block_table = reinterpret_cast<int32_t*>(pool->base + pool->lay.block_table);
   p.bt_stride = c.max_blocks_per_request;
   p.items = reinterpret_cast<const WorkItemDev*>(s.dev);
   p.n_items = pool->plan_n_items;
   p.q = static_cast<const uint16_t*>(q);
+  p.k_new = static_cast<const uint16_t*>(k_new);
+  p.v_new = static_cast<const uint16_t*>(v_new);
+  p.arrive = reinterpret_cast<int32_t*>(pool->base + pool->lay.arrive);
+  p.fuse_combine = pool->fuse_combine ? 1 : 0;
   p.out = static_cast<uint16_t*>(out);
   p.part_o = reinterpret_cast<float*>(pool->base + pool->lay.part_o);
   p.part_ml = reinterpret_cast<float*>(pool->base + pool->lay.part_ml);
@@ -542,15 +555,18 @@ int32_t paged_decode_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
   const int32_t want = (p.n_units + kAttnWarps - 1) / kAttnWarps;
   const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * pool->ctas_per_sm)));
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_ATTN].begin(stream));
-  if (c.head_dim == 128)
-    attn_splitkv_kernel<128><<<grid, kAttnThreads, 0, stream>>>(p);
-  else
-    attn_splitkv_kernel<64><<<grid, kAttnThreads, 0, stream>>>(p);
+  if (c.head_dim == 128) {
+    if (k_new) attn_splitkv_kernel<128, true><<<grid, kAttnThreads, 0, stream>>>(p);
+    else attn_splitkv_kernel<128, false><<<grid, kAttnThreads, 0, stream>>>(p);
+  } else {
+    if (k_new) attn_splitkv_kernel<64, true><<<grid, kAttnThreads, 0, stream>>>(p);
+    else attn_splitkv_kernel<64, false><<<grid, kAttnThreads, 0, stream>>>(p);
+  }
   KV_CUDA(pool, cudaGetLastError());
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_ATTN].end(stream));
   ++pool->launches;
 
-  if (pool->plan_n_combines > 0) {
+  if (pool->plan_n_combines > 0 && !pool->fuse_combine) {
     CombineParams cp{};
     cp.entries = reinterpret_cast<const CombineEntryDev*>(s.dev + pool->plan_combine_off);
     cp.n_entries = pool->plan_n_combines;
@@ -573,6 +589,17 @@ int32_t paged_decode_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
   KV_CUDA(pool, cudaEventRecord(s.ev, stream));
   s.in_flight = true;
   return KV_OK;
+}
+
+int32_t paged_decode_attention(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const void* q,
+                               void* out, float sm_scale, void* cuda_stream) {
+  return launch_attention(pool, layer, batch, req_ids, q, nullptr, nullptr, out, sm_scale, cuda_stream);
+}
+
+int32_t paged_decode_step(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const void* q,
+                          const void* k_new, const void* v_new, void* out, float sm_scale, void* cuda_stream) {
+  if (!k_new || !v_new || !aligned16(k_new) || !aligned16(v_new)) return KV_ERR_INVALID;
+  return launch_attention(pool, layer, batch, req_ids, q, k_new, v_new, out, sm_scale, cuda_stream);
 }
 
 int32_t kv_ingest_host(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const int32_t* n_tokens,
@@ -628,30 +655,54 @@ int32_t kv_ingest_host(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, c
   return kv_ingest(pool, n_req, req_ids, n_tokens, kd.data(), vd.data(), layer_begin, layer_count, cuda_stream);
 }
 
-int32_t paged_decode_attention_host(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids,
-                                    const void* q, void* out, float sm_scale, void* staging, int64_t staging_bytes,
-                                    void* cuda_stream) {
+static int32_t attention_host(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const void* q,
+                              const void* k_new, const void* v_new, void* out, float sm_scale, void* staging,
+                              int64_t staging_bytes, void* cuda_stream) {
   if (!pool || !req_ids || !q || !out || !staging || batch < 1) return KV_ERR_INVALID;
   if ((reinterpret_cast<uintptr_t>(staging) & (kAlign - 1)) != 0) return KV_ERR_INVALID;
   if (!pool->has_device) return KV_ERR_NO_DEVICE;
   const kv_pool_config_t& c = pool->hs.cfg;
-  const int64_t bytes = static_cast<int64_t>(batch) * c.num_q_heads * c.head_dim * 2;
-  if (2 * align_up(bytes) > staging_bytes) return KV_ERR_INVALID;
-  // validate the batch before any copy is issued, so an error leaves the stream untouched
-  {
+  const int64_t qb = static_cast<int64_t>(batch) * c.num_q_heads * c.head_dim * 2;
+  const int64_t kb = k_new ? static_cast<int64_t>(batch) * c.num_kv_heads * c.head_dim * 2 : 0;
+  if (2 * align_up(qb) + 2 * align_up(kb) > staging_bytes) return KV_ERR_INVALID;
+  {  // validate the batch before any copy is issued, so an error leaves the stream untouched
     int32_t rc = pool->hs.check_batch(batch, req_ids, nullptr);
     if (rc != KV_OK) return rc;
-    for (int32_t i = 0; i < batch; ++i)
-      if (pool->hs.reqs.find(req_ids[i])->second.len < 1) return KV_ERR_INVALID;
+    for (int32_t i = 0; i < batch; ++i) {
+      const Request& r = pool->hs.reqs.find(req_ids[i])->second;
+      if (r.len < 1 || (k_new && r.last_n != 1)) return KV_ERR_INVALID;
+    }
   }
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   char* dq = static_cast<char*>(staging);
-  char* dout = dq + align_up(bytes);
-  KV_CUDA(pool, cudaMemcpyAsync(dq, q, static_cast<size_t>(bytes), cudaMemcpyHostToDevice, stream));
-  int32_t rc = paged_decode_attention(pool, layer, batch, req_ids, dq, dout, sm_scale, cuda_stream);
+  char* dout = dq + align_up(qb);
+  char* dk = dout + align_up(qb);
+  char* dv = dk + align_up(kb);
+  KV_CUDA(pool, cudaMemcpyAsync(dq, q, static_cast<size_t>(qb), cudaMemcpyHostToDevice, stream));
+  if (k_new) {
+    KV_CUDA(pool, cudaMemcpyAsync(dk, k_new, static_cast<size_t>(kb), cudaMemcpyHostToDevice, stream));
+    KV_CUDA(pool, cudaMemcpyAsync(dv, v_new, static_cast<size_t>(kb), cudaMemcpyHostToDevice, stream));
+  }
+  int32_t rc = launch_attention(pool, layer, batch, req_ids, dq, k_new ? dk : nullptr, k_new ? dv : nullptr, dout,
+                                sm_scale, cuda_stream);
   if (rc != KV_OK) return rc;
-  KV_CUDA(pool, cudaMemcpyAsync(out, dout, static_cast<size_t>(bytes), cudaMemcpyDeviceToHost, stream));
+  KV_CUDA(pool, cudaMemcpyAsync(out, dout, static_cast<size_t>(qb), cudaMemcpyDeviceToHost, stream));
   return KV_OK;
+}
+
+int32_t paged_decode_attention_host(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids,
+                                    const void* q, void* out, float sm_scale, void* staging, int64_t staging_bytes,
+                                    void* cuda_stream) {
+  return attention_host(pool, layer, batch, req_ids, q, nullptr, nullptr, out, sm_scale, staging, staging_bytes,
+                        cuda_stream);
+}
+
+int32_t paged_decode_step_host(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const void* q,
+                               const void* k_new, const void* v_new, void* out, float sm_scale, void* staging,
+                               int64_t staging_bytes, void* cuda_stream) {
+  if (!k_new || !v_new) return KV_ERR_INVALID;
+  return attention_host(pool, layer, batch, req_ids, q, k_new, v_new, out, sm_scale, staging, staging_bytes,
+                        cuda_stream);
 }
 
 int64_t kv_launch_count(const kv_pool_t* pool) { return pool ? pool->launches : KV_ERR_INVALID; }
@@ -663,6 +714,7 @@ int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
   if (!std::strcmp(key, "ctas_per_sm") && value >= 1 && value <= 8) { pool->ctas_per_sm = static_cast<int32_t>(value); return KV_OK; }
   if (!std::strcmp(key, "items_per_slot") && value >= 1 && value <= 1024) { pool->items_per_slot = static_cast<int32_t>(value); return KV_OK; }
   if (!std::strcmp(key, "profile") && (value == 0 || value == 1)) { pool->profile = value != 0; return KV_OK; }
+  if (!std::strcmp(key, "fuse_combine") && (value == 0 || value == 1)) { pool->fuse_combine = value != 0; return KV_OK; }
   return KV_ERR_INVALID;
 }
 

@@ -9,8 +9,9 @@ One step (SURVEY §8(a), rows a1-a6; PAPER.md:200, :219-223 producer/consumer ba
     host      retire `ingest_per_step` finished requests           kv_free        (a6)
     stream B  ingest `ingest_per_step` prefill-completed requests  kv_ingest      (a1, a2)
               (they join the decode batch at the NEXT step, so the copy overlaps attention)
-    stream A  for each layer l:  append the new token's K/V        kv_ingest n=1  (a3)
-                                 attention over len+1 tokens       paged_decode_attention (a4, a5)
+    stream A  reserve the step's token for every request          kv_reserve     (a1, host)
+              for each layer l:  append + attention over len+1     paged_decode_step (a3, a4, a5: one launch)
+              (``fused=False``: kv_ingest n=1 then paged_decode_attention, two or three launches)
 The decode batch keeps its size: the requests retired at step s are replaced by the ones
 ingested during step s-1.  With ``streams=1`` everything runs on stream A in program order.
 
@@ -153,10 +154,10 @@ class DecodeLoop:
 
     def __init__(self, w: W.Workload, n_steps: int, n_host_steps: int = 0, device="cuda:0", streams: int = 2,
                  salt: int = 0, bank_bytes: int = 24 << 30, profile: bool = True, options: dict | None = None,
-                 sentinel: int | None = None):
+                 sentinel: int | None = None, fused: bool = True):
         """Steps [0, n_steps) take their inputs from device memory; steps [n_steps, n_steps + n_host_steps)
         take them from pinned host memory through the *_host entry points."""
-        self.w, self.dev, self.salt = w, torch.device(device), salt
+        self.w, self.dev, self.salt, self.fused = w, torch.device(device), salt, fused
         self.host_from, self.n_steps = n_steps, n_steps + n_host_steps
         self.two_streams = streams >= 2 and w.ingest_per_step > 0
         L, Hkv, Hq, d, k = w.num_layers, w.num_kv_heads, w.num_q_heads, w.head_dim, w.ingest_per_step
@@ -186,8 +187,9 @@ class DecodeLoop:
             self.pool.set_option(key, val)
         if profile:
             self.pool.set_option("profile", 1)
-        self.sA = torch.cuda.Stream(self.dev)
-        self.sB = torch.cuda.Stream(self.dev) if self.two_streams else self.sA
+        # decode (A) outranks bulk ingest (B): the block scheduler hands B's CTAs the SM time A leaves idle
+        self.sA = torch.cuda.Stream(self.dev, priority=-1)
+        self.sB = torch.cuda.Stream(self.dev, priority=0) if self.two_streams else self.sA
         self.evA = [torch.cuda.Event() for _ in range(4)]      # end of step on A (ring)
         self.evB = [torch.cuda.Event() for _ in range(4)]      # end of ingest on B (ring)
         self.step_idx = 0
@@ -290,7 +292,7 @@ class DecodeLoop:
         self._offs = np.arange(Bn, dtype=np.uint64) * np.uint64(self.row_new)
         self._ones = np.ones(Bn, dtype=np.int32)
         if self.n_steps > self.host_from:
-            self.stage_A = torch.empty(2 * _align(Bn * self.row_new) + 2 * _align(self.q_layer_bytes) + 1024,
+            self.stage_A = torch.empty(2 * _align(Bn * self.row_new) + 2 * _align(self.q_layer_bytes),
                                        dtype=torch.uint8, device=self.dev)
 
     # ---- one step ---------------------------------------------------------------------------
@@ -329,20 +331,27 @@ class DecodeLoop:
         kn, vn, q, out = self.k_new[s], self.v_new[s], self.q[s], self.out[s]
         a = A.cuda_stream
         lay_kv = self.w.batch * self.row_new
+        qb = self.q_layer_bytes
+        if self.fused:
+            B.kv_reserve(h, sp.batch, self._ones)                                                  # a1 (host)
         for l in range(L):
-            kp = self._offs + np.uint64(kn.data_ptr() + l * lay_kv)
-            vp = self._offs + np.uint64(vn.data_ptr() + l * lay_kv)
-            if host:
-                B.kv_ingest_host(h, sp.batch, self._ones, kp, vp, l, 1, self.stage_A.data_ptr(),
-                                 2 * _align(self.w.batch * self.row_new), a)                       # a3
-                off = 2 * _align(self.w.batch * self.row_new)
-                B.paged_decode_attention_host(h, l, sp.batch, q.data_ptr() + l * self.q_layer_bytes,
-                                              out.data_ptr() + l * self.q_layer_bytes, 0.0,
-                                              self.stage_A.data_ptr() + off, self.stage_A.numel() - off, a)
+            kl, vl = kn.data_ptr() + l * lay_kv, vn.data_ptr() + l * lay_kv
+            ql, ol = q.data_ptr() + l * qb, out.data_ptr() + l * qb
+            if self.fused and host:
+                B.paged_decode_step_host(h, l, sp.batch, ql, kl, vl, ol, 0.0, self.stage_A.data_ptr(),
+                                         self.stage_A.numel(), a)                                  # a3 + a4 + a5
+            elif self.fused:
+                B.paged_decode_step(h, l, sp.batch, ql, kl, vl, ol, 0.0, a)                        # a3 + a4 + a5
+            elif host:
+                off = 2 * _align(lay_kv)
+                B.kv_ingest_host(h, sp.batch, self._ones, self._offs + np.uint64(kl), self._offs + np.uint64(vl),
+                                 l, 1, self.stage_A.data_ptr(), off, a)                            # a3
+                B.paged_decode_attention_host(h, l, sp.batch, ql, ol, 0.0, self.stage_A.data_ptr() + off,
+                                              self.stage_A.numel() - off, a)                       # a4 + a5
             else:
-                B.kv_ingest(h, sp.batch, self._ones, kp, vp, l, 1, a)                             # a3
-                B.paged_decode_attention(h, l, sp.batch, q.data_ptr() + l * self.q_layer_bytes,
-                                         out.data_ptr() + l * self.q_layer_bytes, 0.0, a)         # a4 + a5
+                B.kv_ingest(h, sp.batch, self._ones, self._offs + np.uint64(kl), self._offs + np.uint64(vl),
+                            l, 1, a)                                                               # a3
+                B.paged_decode_attention(h, l, sp.batch, ql, ol, 0.0, a)                           # a4 + a5
         if self.two_streams:
             self.evA[s % 4].record(A)
         self.step_idx += 1
