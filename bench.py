@@ -54,6 +54,9 @@ def parse_args():
     ap.add_argument("--no-isolated", action="store_true", help="skip the attention-alone / ingest-alone legs")
     ap.add_argument("--unfused", action="store_true", help="append and attention as separate calls (a3, then a4+a5)")
     ap.add_argument("--opt", action="append", default=[], help="pool option key=value (tuning)")
+    ap.add_argument("--layers", type=int, default=0,
+                    help="profiling aid: run the workload with this many layers (a smaller pool for ncu replay); "
+                         "the line's config.layers says what ran")
     return ap.parse_args()
 
 
@@ -262,45 +265,25 @@ def cpu_baseline_and_check(loop, last_step: int, budget_s: float = 12.0):
 def run_cuda(args):
     import numpy as np
     import torch
-    import torch.distributed as dist
     import paper_2511_20982_b200 as kv              # ImportError if libkvpool.so is missing: no fallback
     from paper_2511_20982_b200 import binding as B
     from paper_2511_20982_b200 import workloads as W
     from paper_2511_20982_b200.engine import DecodeLoop
 
-    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
     assert torch.cuda.is_available(), "bench.py --impl cuda needs a GPU; there is no CPU fallback"
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-
-    def barrier():
-        if world > 1:
-            dist.barrier(device_ids=[local])
-        torch.cuda.synchronize(dev)
-
-    def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
-    def sum_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item())
+    from paper_2511_20982_b200 import replicas
+    rep = replicas.init("nccl")
+    rank, world, local, dev = rep.rank, rep.world, rep.local_rank, rep.device
+    barrier, max_over_ranks, sum_over_ranks = rep.barrier, rep.max, rep.sum
 
     w = W.CONFIGS[args.workload]
+    if args.layers > 0:
+        w = w.scaled(num_layers=args.layers)
     K, Wm = args.steps, args.warmup
     e2e_w = 3 if args.e2e_steps > 0 else 0
     opts = {k: int(v) for k, v in (o.split("=") for o in args.opt)}
     t_setup = time.time()
-    loop = DecodeLoop(w, Wm + K, n_host_steps=e2e_w + args.e2e_steps, device=dev, streams=args.streams, salt=rank,
+    loop = DecodeLoop(w, Wm + K, n_host_steps=e2e_w + args.e2e_steps, device=dev, streams=args.streams, salt=rep.salt,
                       options=opts, fused=not args.unfused)
     t_setup = time.time() - t_setup
     pool = loop.pool
@@ -420,8 +403,7 @@ def run_cuda(args):
             "cpu_baseline": cpu_base, "parity_sample": check, "e2e": e2e, "clocks": clocks,
         }))
     loop.close()
-    if world > 1:
-        dist.destroy_process_group()
+    rep.close()
 
 
 def isolated_legs(loop, last_step: int, peak: float, reps: int = 5):
