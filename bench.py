@@ -38,6 +38,11 @@ if ROOT not in sys.path:
 METRIC = "decode-attn + KV-ingest HBM GB/s"
 NOMINAL_HBM_GBS = 8000.0          # BASELINE.json north_star: "B200 HBM peak (~8 TB/s)"
 FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+# DRAM bytes per algorithmic byte of attn_splitkv_kernel, from the `ncu --set full` captures summarised in
+# profiles/README.md (dram__bytes_read.sum + dram__bytes_write.sum of one launch / that launch's algorithmic bytes).
+# The roofline's `traffic` is this ratio x the timed run's algorithmic bytes per launch.
+NCU_TRAFFIC_RATIO = {"cfg2_7b_mha": (1.0045, "profiles/r01 attn_cfg2"), "cfg3_8b_gqa": (1.0195, "profiles/r01 attn_cfg3"),
+                     "cfg4_70b_long": (1.0011, "profiles/r01 attn_cfg4")}
 DEFAULT_WORKLOAD = "cfg3_8b_gqa"  # first BASELINE.json config with both legs of the metric
 
 
@@ -330,6 +335,10 @@ def run_cuda(args):
                 "frac_of_nominal_8000": achieved / NOMINAL_HBM_GBS if achieved else None,
                 "launches": attn_n, "avg_launch_us": attn_ms / max(attn_n, 1) * 1e3,
                 "algorithmic_bytes_per_launch": attn_bytes_per_launch, "traffic": None}
+    if args.workload in NCU_TRAFFIC_RATIO:
+        ratio, src = NCU_TRAFFIC_RATIO[args.workload]
+        roofline.update({"traffic": attn_bytes_per_launch * ratio, "traffic_source": f"ncu --set full, {src}: "
+                         f"DRAM bytes = {ratio:.4f} x algorithmic bytes"})
     kernels = {
         "attn_splitkv_kernel": {"launches": attn_n, "ms": attn_ms},
         "combine_kernel": {"launches": comb_n, "ms": comb_ms},
