@@ -20,7 +20,9 @@ from helpers import bf16_bits, bits_of, bits_to_f64
 pytestmark = pytest.mark.gpu
 
 SPLIT_MODES = [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=1024),
-               dict(min_chunk_blocks=2, items_per_slot=1024, fuse_combine=0)]
+               dict(min_chunk_blocks=2, items_per_slot=1024, fuse_combine=0),
+               dict(stream_kernel=0), dict(stream_kernel=0, min_chunk_blocks=1, items_per_slot=1024),
+               dict(min_chunk_blocks=1, items_per_slot=1024, ctas_per_sm=1)]
 
 
 def from_bits(bits: np.ndarray) -> torch.Tensor:
