@@ -203,17 +203,22 @@ class HostState {
     return KV_OK;
   }
 
-  // Work-list half of a4.  `slots` = resident warps the main kernel will run; the planner aims
-  // at `items_per_slot` near-uniform units per slot so that dynamic scheduling has a short tail,
-  // while keeping chunks >= min_chunk_blocks so split-KV partial traffic stays << KV traffic.
-  // Cost matters (a 7B-MHA decode step is ~0.2 ms of GPU time): one pass over the batch, no hashing
-  // beyond the id lookup, counting sort.
+  // Work-list half of a4.  `slots` = resident warps the main kernel will run (one work unit at a
+  // time each; an item expands to num_kv_heads units).  Chunk sizes follow guided self-scheduling:
+  // requests are taken longest first and each chunk is sized to the work still unassigned,
+  //     c = max(min_chunk_blocks, remaining_tiles / (items_per_slot * slots))   blocks,
+  // so the list starts with few large units (few unit switches, few partials) and ends with small
+  // ones (the warps, which claim units dynamically in list order, all finish within one small
+  // unit of each other).  A request whose remainder is <= 1.25 c is not split further.
+  // Cost matters (a 7B-MHA decode step is ~0.2 ms of GPU time): two passes over the batch, no
+  // hashing beyond the id lookup, counting sorts.
   int32_t plan_decode(int32_t batch, const int64_t* ids, int32_t slots, int32_t items_per_slot,
                       int32_t min_chunk_blocks, int32_t max_partials, DecodePlan* plan) const {
     if (batch < 1 || !ids || batch > cfg.max_requests) return KV_ERR_INVALID;
     scratch_.resize(static_cast<size_t>(batch));
     const uint64_t stamp = ++plan_stamp_;
     int64_t total_blocks = 0;
+    int32_t longest = 0;
     for (int32_t i = 0; i < batch; ++i) {
       auto it = reqs.find(ids[i]);
       if (it == reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
@@ -221,52 +226,72 @@ class HostState {
       if (r.len < 1 || r.plan_mark == stamp) return KV_ERR_INVALID;  // empty context (A11) / duplicate id
       r.plan_mark = stamp;
       scratch_[static_cast<size_t>(i)] = &r;
-      total_blocks += blocks_for(r.len);
+      const int32_t nb = blocks_for(r.len);
+      total_blocks += nb;
+      longest = std::max(longest, nb);
     }
-    const int64_t total_tiles = total_blocks * cfg.num_kv_heads;
-    const int64_t target_items = std::max<int64_t>(1, static_cast<int64_t>(slots) * items_per_slot);
-    int64_t chunk = std::max<int64_t>(min_chunk_blocks, (total_tiles + target_items - 1) / target_items);
-    for (;;) {  // grow the chunk until the partials fit the workspace
-      int64_t partials = 0;
-      for (const Request* r : scratch_) {
-        int64_t nc = (blocks_for(r->len) + chunk - 1) / chunk;
-        if (nc > 1) partials += nc * cfg.num_kv_heads;
+    // batch rows, longest request first (stable counting sort on the block count)
+    order_.resize(static_cast<size_t>(batch));
+    count_.assign(static_cast<size_t>(longest) + 2, 0);
+    for (const Request* r : scratch_) ++count_[static_cast<size_t>(longest - blocks_for(r->len)) + 1];
+    for (size_t k = 1; k < count_.size(); ++k) count_[k] += count_[k - 1];
+    for (int32_t i = 0; i < batch; ++i)
+      order_[static_cast<size_t>(count_[static_cast<size_t>(longest - blocks_for(scratch_[static_cast<size_t>(i)]->len))]++)] = i;
+
+    const int64_t Hkv = cfg.num_kv_heads;
+    const int64_t denom = std::max<int64_t>(1, static_cast<int64_t>(slots) * items_per_slot);
+    int64_t floor_blocks = std::max<int32_t>(1, min_chunk_blocks);
+    int32_t max_nb = 0, next_partial = 0;
+    for (;;) {  // raise the smallest chunk until the partials fit the workspace
+      unsorted_.clear();
+      plan->combines.clear();
+      next_partial = 0;
+      max_nb = 0;
+      int64_t remaining = total_blocks * Hkv;  // tiles not yet assigned
+      bool overflow = false;
+      for (int32_t oi = 0; oi < batch && !overflow; ++oi) {
+        const int32_t i = order_[static_cast<size_t>(oi)];
+        const Request* r = scratch_[static_cast<size_t>(i)];
+        const int32_t nb = blocks_for(r->len);
+        const size_t first = unsorted_.size();
+        int32_t pos = 0;
+        while (pos < nb) {
+          const int64_t c = std::max<int64_t>(floor_blocks, remaining / denom);
+          const int32_t rem = nb - pos;
+          const int32_t take = rem <= c + c / 4 ? rem : static_cast<int32_t>(c);
+          WorkItem w;
+          w.batch_idx = i;
+          w.slot = r->slot;
+          w.blk_begin = pos;
+          w.n_blocks = take;
+          w.n_tokens = std::min(r->len - pos * cfg.block_size, take * cfg.block_size);
+          w.partial_base = -1;
+          w.chunks = 0;
+          w.last_blk = r->blocks.back();
+          unsorted_.push_back(w);
+          max_nb = std::max(max_nb, take);
+          pos += take;
+          remaining -= take * Hkv;
+        }
+        const int32_t nc = static_cast<int32_t>(unsorted_.size() - first);
+        if (nc > 0xffff) return KV_ERR_TOO_LONG;   // (n_chunks, chunk_idx) are packed 16:16
+        if (nc > 1) {
+          if (static_cast<int64_t>(next_partial) + static_cast<int64_t>(nc) * Hkv > max_partials) { overflow = true; break; }
+          plan->combines.push_back({i, next_partial, nc, 0});
+          for (int32_t c = 0; c < nc; ++c) unsorted_[first + static_cast<size_t>(c)].partial_base = next_partial;
+          next_partial += nc * static_cast<int32_t>(Hkv);
+        }
+        for (int32_t c = 0; c < nc; ++c) unsorted_[first + static_cast<size_t>(c)].chunks = (nc << 16) | c;
       }
-      if (partials <= max_partials) break;
-      chunk *= 2;
+      if (!overflow) break;
+      floor_blocks *= 2;
     }
-    plan->combines.clear();
-    plan->chunk_blocks = static_cast<int32_t>(chunk);
-    unsorted_.clear();
-    int32_t next_partial = 0, max_nb = 0;
-    for (int32_t i = 0; i < batch; ++i) {
-      const Request* r = scratch_[static_cast<size_t>(i)];
-      const int32_t nb = blocks_for(r->len);
-      const int32_t nc0 = static_cast<int32_t>((nb + chunk - 1) / chunk);
-      const int32_t per = (nb + nc0 - 1) / nc0;  // even split: ceil(nb / nc0) <= chunk blocks per chunk
-      const int32_t nc = (nb + per - 1) / per;   // <= nc0
-      if (nc > 0xffff) return KV_ERR_TOO_LONG;   // (n_chunks, chunk_idx) are packed 16:16
-      const int32_t base = nc > 1 ? next_partial : -1;
-      if (nc > 1) {
-        plan->combines.push_back({i, base, nc, 0});
-        next_partial += nc * cfg.num_kv_heads;
-      }
-      for (int32_t c = 0; c < nc; ++c) {
-        WorkItem w;
-        w.batch_idx = i;
-        w.slot = r->slot;
-        w.blk_begin = c * per;
-        w.n_blocks = std::min(per, nb - c * per);
-        w.n_tokens = std::min(r->len - w.blk_begin * cfg.block_size, w.n_blocks * cfg.block_size);
-        w.partial_base = base;
-        w.chunks = (nc << 16) | c;
-        w.last_blk = r->blocks.back();
-        max_nb = std::max(max_nb, w.n_blocks);
-        unsorted_.push_back(w);
-      }
+    {  // largest chunk this plan may contain (first chunk target, plus the no-split allowance)
+      const int64_t c0 = std::max<int64_t>(floor_blocks, total_blocks * Hkv / denom);
+      plan->chunk_blocks = static_cast<int32_t>(std::min<int64_t>(c0 + c0 / 4, 0x7fffffff));
     }
     plan->n_partials = next_partial;
-    // longest first, stable: counting sort on n_blocks
+    // largest units first, stable: counting sort on n_blocks
     count_.assign(static_cast<size_t>(max_nb) + 2, 0);
     for (const WorkItem& w : unsorted_) ++count_[static_cast<size_t>(max_nb - w.n_blocks) + 1];
     for (size_t k = 1; k < count_.size(); ++k) count_[k] += count_[k - 1];
@@ -278,7 +303,7 @@ class HostState {
  private:
   mutable std::vector<const Request*> scratch_;
   mutable std::vector<WorkItem> unsorted_;
-  mutable std::vector<int32_t> count_;
+  mutable std::vector<int32_t> count_, order_;
   std::vector<int64_t> fresh_;
   mutable uint64_t plan_stamp_ = 0;
 };

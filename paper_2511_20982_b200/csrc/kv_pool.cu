@@ -12,7 +12,6 @@
 #include "../../include/kv_pool.h"
 #include "kv_host.h"
 #include "kv_kernels.cuh"
-#include "kv_attn_stream.cuh"
 
 namespace {
 
@@ -187,11 +186,10 @@ struct kv_pool {
   int32_t last_cuda = 0;
   int64_t launches = 0;
   // tuning
-  int32_t min_chunk_blocks = 16;
+  int32_t min_chunk_blocks = 32;   // smallest split-KV chunk: 32 blocks = 256 KiB of KV per unit at d = 128
   int32_t ctas_per_sm = 2;
-  int32_t items_per_slot = 8;
+  int32_t items_per_slot = 2;     // guided chunking: first chunk = remaining work / (2 x resident warps)
   bool fuse_combine = true;
-  bool stream_kernel = true;   // attn_stream_kernel (cross-unit tile pipeline) vs attn_splitkv_kernel
   bool profile = false;
   ProfRing prof[KV_KERNEL_KINDS];
   // staging
@@ -557,15 +555,7 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, c
   const int32_t want = (p.n_units + kAttnWarps - 1) / kAttnWarps;
   const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * pool->ctas_per_sm)));
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_ATTN].begin(stream));
-  if (pool->stream_kernel) {
-    if (c.head_dim == 128) {
-      if (k_new) attn_stream_kernel<128, true><<<grid, kAttnThreads, 0, stream>>>(p);
-      else attn_stream_kernel<128, false><<<grid, kAttnThreads, 0, stream>>>(p);
-    } else {
-      if (k_new) attn_stream_kernel<64, true><<<grid, kAttnThreads, 0, stream>>>(p);
-      else attn_stream_kernel<64, false><<<grid, kAttnThreads, 0, stream>>>(p);
-    }
-  } else if (c.head_dim == 128) {
+  if (c.head_dim == 128) {
     if (k_new) attn_splitkv_kernel<128, true><<<grid, kAttnThreads, 0, stream>>>(p);
     else attn_splitkv_kernel<128, false><<<grid, kAttnThreads, 0, stream>>>(p);
   } else {
@@ -725,7 +715,6 @@ int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
   if (!std::strcmp(key, "items_per_slot") && value >= 1 && value <= 1024) { pool->items_per_slot = static_cast<int32_t>(value); return KV_OK; }
   if (!std::strcmp(key, "profile") && (value == 0 || value == 1)) { pool->profile = value != 0; return KV_OK; }
   if (!std::strcmp(key, "fuse_combine") && (value == 0 || value == 1)) { pool->fuse_combine = value != 0; return KV_OK; }
-  if (!std::strcmp(key, "stream_kernel") && (value == 0 || value == 1)) { pool->stream_kernel = value != 0; return KV_OK; }
   return KV_ERR_INVALID;
 }
 

@@ -21,7 +21,7 @@ pytestmark = pytest.mark.gpu
 
 SPLIT_MODES = [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=1024),
                dict(min_chunk_blocks=2, items_per_slot=1024, fuse_combine=0),
-               dict(stream_kernel=0), dict(stream_kernel=0, min_chunk_blocks=1, items_per_slot=1024),
+               dict(min_chunk_blocks=1, items_per_slot=2), dict(min_chunk_blocks=5, items_per_slot=1),
                dict(min_chunk_blocks=1, items_per_slot=1024, ctas_per_sm=1)]
 
 
