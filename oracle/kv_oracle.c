@@ -28,7 +28,11 @@
  * block-permutation invariance; GQA map; shift invariance / no overflow; agreement with
  * torch.nn.functional.scaled_dot_product_attention in fp64; an independent numpy
  * brute-force over gathered rows; chunk+combine == unsplit; scatter o gather == identity and
- * whole-slab equality with a numpy fancy-index scatter.  No function here is "parity unpinned".
+ * whole-slab equality with a numpy fancy-index scatter.  oracle_attention_varq
+ * (tests/test_oracle_varq_pins.py): q_len = 1 equals oracle_attention; full and chunked
+ * prefill equal torch SDPA with a causal (lower-right aligned) mask in fp64; first token of
+ * a fresh prefill returns V_0; q = 0 gives running means; each query row equals decode over
+ * the truncated sequence; future tokens do not matter.  No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -157,6 +161,69 @@ int oracle_attention(const uint16_t* kv, const oracle_dims_t* D, int32_t layer, 
       if (wsum) wsum[(int64_t)r * Hq + h] = ws;
       free(s);
     }
+  return bad ? -2 : 0;
+}
+
+/*
+ * Variable-q-length causal attention.  PAPER.md:443 (§V-E): "For
+ * ultra-short requests we employ PD-aggregation: merging their prefill with other requests'
+ * decoding on D-instances"; PAPER.md:94 (§II): such requests are executed "in-place (i.e.,
+ * without remote prefill)".  So one batch holds decode rows (one query token) and in-place
+ * prefill rows (q_len query tokens); Eq. 1 applies with Q = the LAST q_lens[r]
+ * tokens of request r.  Readings (B1-B3): the mask is causal — query token i, at
+ * absolute position P_i = seq_lens[r] - q_lens[r] + i, sees stored tokens 0..P_i inclusive (its
+ * own K/V is already in the pool); q_lens[r] = 1 is exactly oracle_attention's decode row.
+ *   q, out: [total_q][num_q_heads][head_dim], request r's rows start at q_off[r]
+ *   (q_off[batch] = total_q).  out is fp64, not rounded.  wsum optional as in oracle_attention.
+ * Returns 0; -1 if some request has q_lens[r] < 1 or q_lens[r] > seq_lens[r]; -2 out of memory.
+ */
+int oracle_attention_varq(const uint16_t* kv, const oracle_dims_t* D, int32_t layer,
+                          int32_t num_q_heads, int32_t batch, const int32_t* bt,
+                          const int64_t* bt_off, const int32_t* seq_lens, const int32_t* q_lens,
+                          const int64_t* q_off, const uint16_t* q, double scale, double* out,
+                          double* wsum) {
+  const int32_t d = D->head_dim, Hq = num_q_heads, G = num_q_heads / D->num_kv_heads;
+  for (int32_t r = 0; r < batch; ++r)
+    if (q_lens[r] < 1 || q_lens[r] > seq_lens[r]) return -1;
+  int bad = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int32_t r = 0; r < batch; ++r) {
+    const int32_t* blocks = bt + bt_off[r];
+    double* s = (double*)malloc(sizeof(double) * (size_t)seq_lens[r]);
+    if (!s) { bad = 1; continue; }
+    for (int32_t i = 0; i < q_lens[r]; ++i) {
+      const int32_t n = seq_lens[r] - q_lens[r] + i + 1;   /* tokens 0 .. P_i visible */
+      for (int32_t h = 0; h < Hq; ++h) {
+        const int32_t g = h / G;
+        const uint16_t* qv = q + ((q_off[r] + i) * Hq + h) * d;
+        double* o = out + ((q_off[r] + i) * Hq + h) * d;
+        for (int32_t t = 0; t < n; ++t) {
+          int64_t kb = kv_index(D, layer, blocks[t / D->block_size], g, 0, t % D->block_size, 0);
+          double acc = 0.0;
+          for (int32_t j = 0; j < d; ++j) acc += bf16_to_double(qv[j]) * bf16_to_double(kv[kb + j]);
+          s[t] = scale * acc;
+        }
+        double m = s[0];
+        for (int32_t t = 1; t < n; ++t)
+          if (s[t] > m) m = s[t];
+        double Z = 0.0;
+        for (int32_t t = 0; t < n; ++t) {
+          s[t] = exp(s[t] - m);
+          Z += s[t];
+        }
+        for (int32_t j = 0; j < d; ++j) o[j] = 0.0;
+        double ws = 0.0;
+        for (int32_t t = 0; t < n; ++t) {
+          int64_t vb = kv_index(D, layer, blocks[t / D->block_size], g, 1, t % D->block_size, 0);
+          double w = s[t] / Z;
+          ws += w;
+          for (int32_t j = 0; j < d; ++j) o[j] += w * bf16_to_double(kv[vb + j]);
+        }
+        if (wsum) wsum[(q_off[r] + i) * Hq + h] = ws;
+      }
+    }
+    free(s);
+  }
   return bad ? -2 : 0;
 }
 
