@@ -173,6 +173,31 @@ int32_t paged_decode_step(kv_pool_t* pool, int32_t layer, int32_t batch,
                           void* out /*device*/, float sm_scale, void* cuda_stream);
 
 /*
+ * NEXT-1 — variable-q-length causal paged attention: in-place prefill of ultra-short requests
+ * merged with decoding (§V-E: "For ultra-short requests we employ PD-aggregation:
+ * merging their prefill with other requests' decoding on D-instances avoids unnecessary
+ * KV-cache transfers"; such requests run "in-place (i.e., without remote
+ * prefill)").  One call serves a batch that mixes decode rows (q_lens[i] = 1) and prefill rows
+ * (q_lens[i] = number of prompt tokens computed in this step).  Request i's query tokens are
+ * its LAST q_lens[i] stored tokens — their K/V must already be in the pool (kv_ingest, possibly
+ * layer-sliced) — and query token t of request i, at absolute position P = len_i - q_lens[i] + t,
+ * attends stored tokens 0..P inclusive (Eq. 1, with a causal mask; readings
+ * DESIGN.md B1-B3):
+ *     out[row][h][:] = sum_{s <= P} softmax_s( sm_scale * <q[row][h], K_s> ) * V_s ,
+ *     row = sum_{k < i} q_lens[k] + t,   K_s, V_s of KV head h / G, layer `layer`.
+ *   q_lens: host int32[batch], 1 <= q_lens[i] <= len_i.
+ *   q, out: device, bf16, [sum_i q_lens[i]][num_q_heads][head_dim]; out RNE from fp32.
+ * With every q_lens[i] = 1 the result equals paged_decode_attention's.  One launch; split-KV
+ * partials are merged inside the kernel.  Errors: KV_ERR_UNKNOWN_REQUEST; q_lens[i] outside
+ * [1, len_i] or a duplicate id => KV_ERR_INVALID; more query tiles than the plan staging holds
+ * => KV_ERR_TOO_LONG; KV_ERR_NO_DEVICE; KV_ERR_CUDA.  Nothing changes on error.
+ */
+int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch,
+                               const int64_t* req_ids /*host*/, const int32_t* q_lens /*host*/,
+                               const void* q /*device*/, void* out /*device*/, float sm_scale,
+                               void* cuda_stream);
+
+/*
  * a6 — free (a completed request releases consumer capacity).  Host only
  * and immediate: blocks return to the free list (LIFO) and the table row is dropped.  The
  * caller must not ingest into recycled blocks on a different stream before the attention
@@ -254,7 +279,8 @@ int64_t kv_launch_count(const kv_pool_t* pool);
 #define KV_KERNEL_COMBINE  1   /* combine_kernel (a5)               */
 #define KV_KERNEL_INGEST   2   /* ingest_kernel, scatter (a2 / a3)  */
 #define KV_KERNEL_GATHER   3   /* ingest_kernel, gather direction   */
-#define KV_KERNEL_KINDS    4
+#define KV_KERNEL_VARQ     4   /* attn_splitkv_kernel, variable-q   */
+#define KV_KERNEL_KINDS    5
 #define KV_PROFILE_RING    1024
 int32_t kv_profile_read(kv_pool_t* pool, int32_t kind, int64_t* out_launches, double* out_ms);
 int32_t kv_profile_reset(kv_pool_t* pool);

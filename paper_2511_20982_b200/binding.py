@@ -49,6 +49,7 @@ _SIGS = {
     "paged_decode_attention": (_i32, [_P, _i32, _i32, _P, _P, _P, ctypes.c_float, _P]),
     "paged_decode_step": (_i32, [_P, _i32, _i32, _P, _P, _P, _P, _P, ctypes.c_float, _P]),
     "paged_decode_step_host": (_i32, [_P, _i32, _i32, _P, _P, _P, _P, _P, ctypes.c_float, _P, _i64, _P]),
+    "paged_varlen_attention": (_i32, [_P, _i32, _i32, _P, _P, _P, _P, ctypes.c_float, _P]),
     "kv_free": (_i32, [_P, _i32, _P]),
     "kv_block_table": (_i32, [_P, _i64, _P, _i32, ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
     "kv_pool_stats": (_i32, [_P, ctypes.POINTER(_i64), ctypes.POINTER(_i64), ctypes.POINTER(_i32),
@@ -209,7 +210,16 @@ def paged_decode_attention_host(handle: int, layer: int, req_ids, q_host_ptr: in
            "paged_decode_attention_host")
 
 
-KERNEL_KINDS = {"attn": 0, "combine": 1, "ingest": 2, "gather": 3}
+def paged_varlen_attention(handle: int, layer: int, req_ids, q_lens, q_ptr: int, out_ptr: int, sm_scale: float = 0.0,
+                           stream: int = 0) -> None:
+    """Variable-q-length causal attention: request i's last q_lens[i] tokens are its query tokens."""
+    ids, ql = _ids(req_ids), _i32s(q_lens)
+    assert ids.shape == ql.shape
+    _check(lib.paged_varlen_attention(handle, layer, ids.size, _np(ids), _np(ql), q_ptr, out_ptr, sm_scale,
+                                      stream or None), "paged_varlen_attention")
+
+
+KERNEL_KINDS = {"attn": 0, "combine": 1, "ingest": 2, "gather": 3, "varq": 4}
 
 
 def kv_profile_read(handle: int, kind: int):
@@ -335,6 +345,17 @@ class KVPool:
             out = torch.empty_like(q)
         paged_decode_step(self.handle, layer, req_ids, q.data_ptr(), k_new.data_ptr(), v_new.data_ptr(),
                           out.data_ptr(), sm_scale, self._stream(stream))
+        return out
+
+    def varlen_attention(self, layer, req_ids, q_lens, q, out=None, sm_scale=0.0, stream=None):
+        """q: bf16 [sum(q_lens)][Hq][d]; decode rows have q_len 1, in-place prefill rows their prompt length."""
+        import torch
+
+        assert q.is_contiguous() and q.dtype == torch.bfloat16 and q.shape[0] == int(sum(int(x) for x in q_lens))
+        if out is None:
+            out = torch.empty_like(q)
+        paged_varlen_attention(self.handle, layer, req_ids, q_lens, q.data_ptr(), out.data_ptr(), sm_scale,
+                               self._stream(stream))
         return out
 
     def gather(self, req_id, stream=None):

@@ -88,6 +88,7 @@ struct CombineEntry {
 
 struct DecodePlan {
   std::vector<WorkItem> items;
+  std::vector<int32_t> item_span;   // index of the planned span (request / query tile) of each item
   std::vector<CombineEntry> combines;
   int32_t chunk_blocks = 0;
   int32_t n_partials = 0;
@@ -203,40 +204,93 @@ class HostState {
     return KV_OK;
   }
 
-  // Work-list half of a4.  `slots` = resident warps the main kernel will run (one work unit at a
-  // time each; an item expands to num_kv_heads units).  Chunk sizes follow guided self-scheduling:
-  // requests are taken longest first and each chunk is sized to the work still unassigned,
-  //     c = max(min_chunk_blocks, remaining_tiles / (items_per_slot * slots))   blocks,
-  // so the list starts with few large units (few unit switches, few partials) and ends with small
-  // ones (the warps, which claim units dynamically in list order, all finish within one small
-  // unit of each other).  A request whose remainder is <= 1.25 c is not split further.
-  // Cost matters (a 7B-MHA decode step is ~0.2 ms of GPU time): two passes over the batch, no
-  // hashing beyond the id lookup, counting sorts.
+  // Work-list half of a4: decode.  One span per request (row = batch index), all its blocks.
   int32_t plan_decode(int32_t batch, const int64_t* ids, int32_t slots, int32_t items_per_slot,
                       int32_t min_chunk_blocks, int32_t max_partials, DecodePlan* plan) const {
     if (batch < 1 || !ids || batch > cfg.max_requests) return KV_ERR_INVALID;
-    scratch_.resize(static_cast<size_t>(batch));
+    spans_.resize(static_cast<size_t>(batch));
     const uint64_t stamp = ++plan_stamp_;
-    int64_t total_blocks = 0;
-    int32_t longest = 0;
     for (int32_t i = 0; i < batch; ++i) {
       auto it = reqs.find(ids[i]);
       if (it == reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
       const Request& r = it->second;
       if (r.len < 1 || r.plan_mark == stamp) return KV_ERR_INVALID;  // empty context (A11) / duplicate id
       r.plan_mark = stamp;
-      scratch_[static_cast<size_t>(i)] = &r;
-      const int32_t nb = blocks_for(r.len);
-      total_blocks += nb;
-      longest = std::max(longest, nb);
+      spans_[static_cast<size_t>(i)] = {i, r.slot, blocks_for(r.len), r.len, r.blocks.back()};
     }
-    // batch rows, longest request first (stable counting sort on the block count)
-    order_.resize(static_cast<size_t>(batch));
+    return plan_spans(slots, items_per_slot, min_chunk_blocks, max_partials, plan);
+  }
+
+  // Work-list half of the variable-q-length call: request i's
+  // LAST q_lens[i] tokens are query tokens (a decode row has q_lens[i] = 1, an in-place prefill row
+  // q_lens[i] = its prompt length).  The kernel packs (query token, head) pairs into its 8 MMA
+  // columns, so the unit of planning is a QUERY TILE of 8 / G consecutive query tokens: one span per
+  // tile, covering the blocks that hold tokens 0 .. position of the tile's last query token (causal).
+  // plan->items[k].batch_idx = first row of the tile in q / out; tiles[k] = {pos0, n_qtok} for the
+  // same k (pos0 = absolute position of the tile's first query token).
+  struct QueryTile { int32_t pos0, n_qtok; };
+  int32_t plan_varq(int32_t batch, const int64_t* ids, const int32_t* q_lens, int32_t slots, int32_t items_per_slot,
+                    int32_t min_chunk_blocks, int32_t max_partials, DecodePlan* plan,
+                    std::vector<QueryTile>* tiles) const {
+    if (batch < 1 || !ids || !q_lens || batch > cfg.max_requests) return KV_ERR_INVALID;
+    const int32_t G = cfg.num_q_heads / cfg.num_kv_heads;
+    const int32_t tpt = std::max(1, 8 / G);   // query tokens per tile
+    spans_.clear();
+    span_tiles_.clear();
+    const uint64_t stamp = ++plan_stamp_;
+    int64_t row = 0;
+    for (int32_t i = 0; i < batch; ++i) {
+      auto it = reqs.find(ids[i]);
+      if (it == reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
+      const Request& r = it->second;
+      if (q_lens[i] < 1 || q_lens[i] > r.len || r.plan_mark == stamp) return KV_ERR_INVALID;
+      r.plan_mark = stamp;
+      const int32_t p0 = r.len - q_lens[i];
+      for (int32_t k = 0; k < q_lens[i]; k += tpt) {
+        const int32_t nq = std::min(tpt, q_lens[i] - k);
+        const int32_t visible = p0 + k + nq;                      // tokens 0 .. position of the tile's last query
+        if (row + k > 0x7fffffff) return KV_ERR_TOO_LONG;
+        spans_.push_back({static_cast<int32_t>(row + k), r.slot, blocks_for(visible), visible, r.blocks.back()});
+        span_tiles_.push_back({p0 + k, nq});
+      }
+      row += q_lens[i];
+    }
+    int32_t rc = plan_spans(slots, items_per_slot, min_chunk_blocks, max_partials, plan);
+    if (rc != KV_OK) return rc;
+    tiles->resize(plan->items.size());
+    for (size_t k = 0; k < plan->items.size(); ++k) (*tiles)[k] = span_tiles_[static_cast<size_t>(plan->item_span[k])];
+    return KV_OK;
+  }
+
+ private:
+  // One independently planned run of blocks [0, nb) with n_tokens valid tokens: a request (decode)
+  // or a query tile (variable-q).  `row` lands in WorkItem::batch_idx.
+  struct Span { int32_t row, slot, nb, n_tokens, last_blk; };
+
+  // `slots` = resident warps the main kernel will run (one work unit at a time each; an item expands
+  // to num_kv_heads units).  Chunk sizes follow guided self-scheduling: spans are taken longest
+  // first and each chunk is sized to the work still unassigned,
+  //     c = max(min_chunk_blocks, remaining_tiles / (items_per_slot * slots))   blocks,
+  // so the list starts with few large units (few unit switches, few partials) and ends with small
+  // ones (the warps, which claim units dynamically in list order, all finish within one small
+  // unit of each other).  A span whose remainder is <= 1.25 c is not split further.
+  // Cost matters (a 7B-MHA decode step is ~0.2 ms of GPU time): two passes over the spans, counting sorts.
+  int32_t plan_spans(int32_t slots, int32_t items_per_slot, int32_t min_chunk_blocks, int32_t max_partials,
+                     DecodePlan* plan) const {
+    const int32_t n_spans = static_cast<int32_t>(spans_.size());
+    int64_t total_blocks = 0;
+    int32_t longest = 0;
+    for (const Span& sp : spans_) {
+      total_blocks += sp.nb;
+      longest = std::max(longest, sp.nb);
+    }
+    // longest span first (stable counting sort on the block count)
+    order_.resize(static_cast<size_t>(n_spans));
     count_.assign(static_cast<size_t>(longest) + 2, 0);
-    for (const Request* r : scratch_) ++count_[static_cast<size_t>(longest - blocks_for(r->len)) + 1];
+    for (const Span& sp : spans_) ++count_[static_cast<size_t>(longest - sp.nb) + 1];
     for (size_t k = 1; k < count_.size(); ++k) count_[k] += count_[k - 1];
-    for (int32_t i = 0; i < batch; ++i)
-      order_[static_cast<size_t>(count_[static_cast<size_t>(longest - blocks_for(scratch_[static_cast<size_t>(i)]->len))]++)] = i;
+    for (int32_t i = 0; i < n_spans; ++i)
+      order_[static_cast<size_t>(count_[static_cast<size_t>(longest - spans_[static_cast<size_t>(i)].nb)]++)] = i;
 
     const int64_t Hkv = cfg.num_kv_heads;
     const int64_t denom = std::max<int64_t>(1, static_cast<int64_t>(slots) * items_per_slot);
@@ -244,31 +298,32 @@ class HostState {
     int32_t max_nb = 0, next_partial = 0;
     for (;;) {  // raise the smallest chunk until the partials fit the workspace
       unsorted_.clear();
+      unsorted_span_.clear();
       plan->combines.clear();
       next_partial = 0;
       max_nb = 0;
       int64_t remaining = total_blocks * Hkv;  // tiles not yet assigned
       bool overflow = false;
-      for (int32_t oi = 0; oi < batch && !overflow; ++oi) {
+      for (int32_t oi = 0; oi < n_spans && !overflow; ++oi) {
         const int32_t i = order_[static_cast<size_t>(oi)];
-        const Request* r = scratch_[static_cast<size_t>(i)];
-        const int32_t nb = blocks_for(r->len);
+        const Span& sp = spans_[static_cast<size_t>(i)];
         const size_t first = unsorted_.size();
         int32_t pos = 0;
-        while (pos < nb) {
+        while (pos < sp.nb) {
           const int64_t c = std::max<int64_t>(floor_blocks, remaining / denom);
-          const int32_t rem = nb - pos;
+          const int32_t rem = sp.nb - pos;
           const int32_t take = rem <= c + c / 4 ? rem : static_cast<int32_t>(c);
           WorkItem w;
-          w.batch_idx = i;
-          w.slot = r->slot;
+          w.batch_idx = sp.row;
+          w.slot = sp.slot;
           w.blk_begin = pos;
           w.n_blocks = take;
-          w.n_tokens = std::min(r->len - pos * cfg.block_size, take * cfg.block_size);
+          w.n_tokens = std::min(sp.n_tokens - pos * cfg.block_size, take * cfg.block_size);
           w.partial_base = -1;
           w.chunks = 0;
-          w.last_blk = r->blocks.back();
+          w.last_blk = sp.last_blk;
           unsorted_.push_back(w);
+          unsorted_span_.push_back(i);
           max_nb = std::max(max_nb, take);
           pos += take;
           remaining -= take * Hkv;
@@ -277,13 +332,14 @@ class HostState {
         if (nc > 0xffff) return KV_ERR_TOO_LONG;   // (n_chunks, chunk_idx) are packed 16:16
         if (nc > 1) {
           if (static_cast<int64_t>(next_partial) + static_cast<int64_t>(nc) * Hkv > max_partials) { overflow = true; break; }
-          plan->combines.push_back({i, next_partial, nc, 0});
+          plan->combines.push_back({sp.row, next_partial, nc, 0});
           for (int32_t c = 0; c < nc; ++c) unsorted_[first + static_cast<size_t>(c)].partial_base = next_partial;
           next_partial += nc * static_cast<int32_t>(Hkv);
         }
         for (int32_t c = 0; c < nc; ++c) unsorted_[first + static_cast<size_t>(c)].chunks = (nc << 16) | c;
       }
       if (!overflow) break;
+      if (floor_blocks > longest) return KV_ERR_TOO_LONG;   // even unsplit spans do not fit: cannot happen (no partials then)
       floor_blocks *= 2;
     }
     {  // largest chunk this plan may contain (first chunk target, plus the no-split allowance)
@@ -296,12 +352,18 @@ class HostState {
     for (const WorkItem& w : unsorted_) ++count_[static_cast<size_t>(max_nb - w.n_blocks) + 1];
     for (size_t k = 1; k < count_.size(); ++k) count_[k] += count_[k - 1];
     plan->items.resize(unsorted_.size());
-    for (const WorkItem& w : unsorted_) plan->items[static_cast<size_t>(count_[static_cast<size_t>(max_nb - w.n_blocks)]++)] = w;
+    plan->item_span.resize(unsorted_.size());
+    for (size_t k = 0; k < unsorted_.size(); ++k) {
+      const int32_t dst = count_[static_cast<size_t>(max_nb - unsorted_[k].n_blocks)]++;
+      plan->items[static_cast<size_t>(dst)] = unsorted_[k];
+      plan->item_span[static_cast<size_t>(dst)] = unsorted_span_[k];
+    }
     return KV_OK;
   }
 
- private:
-  mutable std::vector<const Request*> scratch_;
+  mutable std::vector<Span> spans_;
+  mutable std::vector<QueryTile> span_tiles_;
+  mutable std::vector<int32_t> unsorted_span_;
   mutable std::vector<WorkItem> unsorted_;
   mutable std::vector<int32_t> count_, order_;
   std::vector<int64_t> fresh_;

