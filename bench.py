@@ -438,6 +438,7 @@ def isolated_legs(loop, last_step: int, peak: float, reps: int = 5):
     t_attn = float(np.median(times[1:]))
     res = {"attention_gbs": sp.attn_bytes_layer * L / (t_attn * 1e-3) / 1e9, "attention_ms": t_attn}
     res["attention_frac"] = res["attention_gbs"] / peak
+    res.update(varlen_leg(loop, last_step, peak, reps))
     if w.ingest_per_step and loop.bank:
         k = w.ingest_per_step
         ents = list(range(k))
@@ -460,6 +461,81 @@ def isolated_legs(loop, last_step: int, peak: float, reps: int = 5):
                         "ingest_frac": nbytes / (t_ing * 1e-3) / 1e9 / peak, "ingest_bytes": nbytes})
         except B.KVError as e:
             res["ingest_error"] = str(e)
+    return res
+
+
+ULTRA_SHORT = (16, 128)   # prompt lengths of the in-place prefill rows (the paper gives no threshold; its
+N_ULTRA_SHORT = 16        # shortest profiled length is 100): 16 such requests join a step
+
+
+def varlen_leg(loop, last_step: int, peak: float, reps: int = 5):
+    """NEXT-1: the last step's decode batch (q_len 1) plus N_ULTRA_SHORT fresh requests prefilled
+    in place (q_len = prompt length), all layers through paged_varlen_attention, timed with CUDA events on
+    stream A; the prefill rows of the last layer are checked against oracle_attention_varq."""
+    import numpy as np
+    import torch
+    from paper_2511_20982_b200 import binding as B
+    from paper_2511_20982_b200 import workloads as W
+    from paper_2511_20982_b200.engine import attention_bytes
+    w, sp, h, A = loop.w, loop.sched.steps[last_step], loop.pool.handle, loop.sA
+    L, Hq, Hkv, d = w.num_layers, w.num_q_heads, w.num_kv_heads, w.head_dim
+    rng = np.random.default_rng(w.seed + 31)
+    plen = rng.integers(ULTRA_SHORT[0], ULTRA_SHORT[1] + 1, size=N_ULTRA_SHORT).astype(np.int32)
+    uid0 = 1 << 22
+    pids = np.arange(N_ULTRA_SHORT, dtype=np.int64) + (1 << 41)
+    try:
+        with torch.cuda.stream(A):
+            src = [(W.kv_values(w.seed, W.KIND_K, uid0 + i, Hkv, d, 0, L, 0, int(n), loop.dev),
+                    W.kv_values(w.seed, W.KIND_V, uid0 + i, Hkv, d, 0, L, 0, int(n), loop.dev)) for i, n in enumerate(plen)]
+            B.kv_ingest(h, pids, plen, [s[0] for s in src], [s[1] for s in src], 0, L, A.cuda_stream)
+            nq = len(sp.batch) + int(plen.sum())
+            q = torch.empty((L, nq, Hq, d), dtype=torch.bfloat16, device=loop.dev)
+            q[:, : len(sp.batch)] = loop.q[last_step]
+            for l in range(L):
+                q[l, len(sp.batch):] = W.q_values(w.seed, 1 << 20, l, int(plen.sum()), Hq, d, loop.dev)
+            out = torch.empty_like(q)
+    except B.KVError as e:
+        return {"varlen_error": str(e)}
+    ids = np.concatenate([sp.batch, pids])
+    qlens = np.concatenate([np.ones(len(sp.batch), np.int32), plen])
+    lb = nq * Hq * d * 2
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    times = []
+    for r in range(reps + 1):
+        e0.record(A)
+        for l in range(L):
+            B.paged_varlen_attention(h, l, ids, qlens, q.data_ptr() + l * lb, out.data_ptr() + l * lb, 0.0, A.cuda_stream)
+        e1.record(A)
+        A.synchronize()
+        times.append(e0.elapsed_time(e1))
+    t = float(np.median(times[1:]))
+    # algorithmic bytes: every request's visible KV once, every q / out row once, block tables once
+    by = attention_bytes(w, np.concatenate([sp.lens_after, plen.astype(np.int64)])) + 2 * (nq - len(ids)) * Hq * d * 2
+    res = {"varlen_gbs": by * L / (t * 1e-3) / 1e9, "varlen_ms": t, "varlen_frac": by * L / (t * 1e-3) / 1e9 / peak,
+           "varlen_rows": {"decode": len(sp.batch), "prefill_requests": N_ULTRA_SHORT, "prefill_tokens": int(plen.sum())}}
+    # parity of the in-place prefill rows, last layer
+    import oracle
+    layer = L - 1
+    bits = lambda x: x.detach().cpu().contiguous().view(torch.int16).numpy().view(np.uint16).copy()
+    nblk = [(int(n) + w.block_size - 1) // w.block_size for n in plen]
+    dims = oracle.Dims(1, Hkv, d, w.block_size, sum(nblk))
+    slab = oracle.new_slab(dims, 0x7FC0)
+    lists, off = [], 0
+    for i, n in enumerate(plen):
+        lists.append(np.arange(off, off + nblk[i], dtype=np.int32)); off += nblk[i]
+        oracle.scatter(slab, dims, lists[-1], 0,
+                       bits(W.kv_values(w.seed, W.KIND_K, uid0 + i, Hkv, d, layer, 1, 0, int(n), "cpu")),
+                       bits(W.kv_values(w.seed, W.KIND_V, uid0 + i, Hkv, d, layer, 1, 0, int(n), "cpu")))
+    want = oracle.attention_varq(slab, dims, 0, Hq, lists, plen, plen, bits(q[layer, len(sp.batch):]))
+    got = (bits(out[layer, len(sp.batch):]).astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+    err = np.abs(got - want)
+    res["varlen_parity"] = {"rows": int(plen.sum()), "max_abs_err": float(err.max()), "mean_abs_err": float(err.mean()),
+                            "pass": bool(err.max() <= 1e-2 and err.mean() <= 1e-3)}
+    # decode rows must agree with the decode call's output of the same batch (computed by the attention-alone leg)
+    same = torch.equal(out[layer, : len(sp.batch)].view(torch.int16), loop.out[last_step][layer].view(torch.int16))
+    dmax = float((out[layer, : len(sp.batch)].float() - loop.out[last_step][layer].float()).abs().max())
+    res["varlen_decode_rows_vs_decode_call"] = {"bit_identical": bool(same), "max_abs_diff": dmax}
+    B.kv_free(h, pids)
     return res
 
 

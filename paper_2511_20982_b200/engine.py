@@ -177,7 +177,7 @@ class DecodeLoop:
         else:
             num_blocks = max(int(self.sched.peak_blocks * w.pool_slack), self.sched.peak_blocks + 64)
         self.cfg = B.PoolConfig(num_layers=L, num_q_heads=Hq, num_kv_heads=Hkv, head_dim=d, num_blocks=num_blocks,
-                                max_requests=w.batch + 3 * k + 8,
+                                max_requests=w.batch + 3 * k + 32,
                                 max_blocks_per_request=(w.max_len + self.n_steps + w.block_size) // w.block_size + 1,
                                 alloc_seed=w.seed + salt)
         self.pool = B.KVPool(self.cfg, device=self.dev)
