@@ -264,6 +264,55 @@ int32_t paged_decode_step_host(kv_pool_t* pool, int32_t layer, int32_t batch,
                                void* out /*HOST*/, float sm_scale, void* staging /*device*/,
                                int64_t staging_bytes, void* cuda_stream);
 
+/* ---- NEXT-3: D-instance capacity model (host only, closed forms) ------------------------ */
+
+/*
+ * What the measured bandwidth of this path is FOR in DOPD (§IV-B-2): sizing a
+ * D-instance.  Plain fp64 evaluation of
+ *     V_mem = (M_gpu - M') x TP - M_model                                  (Eq. 11)
+ *     V_BW  = t_d^SLO x alpha x TP x BW                                    (Eq. 12)
+ *     cc_d  = min(V_mem, V_BW) / ((ISL + OSL/2) x M_token)                 (Eq. 13)
+ * Readings (A10): alpha, undefined in the text, is the achieved fraction of the HBM
+ * bandwidth BW (what bench.py measures for the KV part); M_token, undefined in the text, is the KV
+ * bytes of one token over the whole model, 2 x layers x kv_heads x head_dim x bytes/element
+ * (kv_token_bytes); M_gpu, M', BW are per GPU, M_model and M_token for the whole model.
+ * All byte quantities in bytes, times in seconds, lengths in tokens.
+ */
+typedef struct kv_capacity_model {
+  double  m_gpu;       /* HBM bytes per GPU (M_gpu)                                         */
+  double  m_reserved;  /* M': peak activation + ancillary bytes per GPU                     */
+  double  m_model;     /* model weight bytes, whole model (M_model)                         */
+  int32_t tp;          /* tensor-parallel size of the D-instance (TP >= 1)                  */
+  double  bw;          /* HBM bytes/s per GPU (BW)                                          */
+  double  alpha;       /* achieved fraction of BW, in (0, 1.5]                              */
+  double  t_d_slo;     /* TPOT SLO limit, seconds                                           */
+  double  isl, osl;    /* input / output sequence length, tokens (isl >= 0, osl > 0)        */
+  double  m_token;     /* KV bytes per token, whole model (M_token > 0)                     */
+} kv_capacity_model_t;
+
+typedef struct kv_capacity {
+  double  v_mem;            /* Eq. 11 (may be <= 0: the model does not fit)                 */
+  double  v_bw;             /* Eq. 12                                                       */
+  double  cc_d;             /* Eq. 13, not rounded; 0 when v_mem <= 0                       */
+  int32_t bandwidth_bound;  /* 1 if v_bw < v_mem (the TPOT SLO, not capacity, limits cc_d)  */
+} kv_capacity_t;
+
+/* KV_ERR_INVALID on a null pointer or an argument outside the ranges above; nothing written then. */
+int32_t kv_capacity(const kv_capacity_model_t* model, kv_capacity_t* out);
+
+/*
+ * Optimal P/D ratio (Eq. 14: n_p x (t_d x OSL / t_p) = n_d x cc_d; the closed form the
+ * text announces at PAPER.md:225 is missing from the extraction and is read as)
+ *     R_opt = n_p / n_d = cc_d x t_p / (t_d x OSL),
+ * t_p = time of one prefill, t_d = time of one decode step at concurrency cc_d, both seconds.
+ * All arguments must be > 0, else KV_ERR_INVALID.
+ */
+int32_t kv_optimal_pd_ratio(double cc_d, double t_p, double t_d, double osl, double* out_ratio);
+
+/* M_token of a pool geometry: 2 x num_layers x num_kv_heads x head_dim x 2 bytes (bf16); < 0 on an
+ * invalid config.                                                                           */
+int64_t kv_token_bytes(const kv_pool_config_t* cfg);
+
 /* Number of kernels this pool has launched since creation (bench `gpu_launches`).         */
 int64_t kv_launch_count(const kv_pool_t* pool);
 

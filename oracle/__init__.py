@@ -86,6 +86,11 @@ def _load():
         lib.oracle_attention_varq.restype = ctypes.c_int
         lib.oracle_attention_varq.argtypes = [P, ctypes.POINTER(_Dims), ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
                                               P, P, P, P, P, P, ctypes.c_double, P, P]
+        D = ctypes.c_double
+        lib.oracle_capacity.restype = None
+        lib.oracle_capacity.argtypes = [D] * 10 + [P]
+        lib.oracle_pd_ratio.restype = D
+        lib.oracle_pd_ratio.argtypes = [D] * 4
         lib.oracle_chunk.restype = None
         lib.oracle_chunk.argtypes = [P, ctypes.POINTER(_Dims), ctypes.c_int32, ctypes.c_int32, P, ctypes.c_int32,
                                      ctypes.c_int32, P, ctypes.c_double, P, P, P]
@@ -230,3 +235,16 @@ def combine(m, l, O) -> np.ndarray:
     out = np.empty(d, dtype=np.float64)
     _load().oracle_combine(n, d, _ptr(m), _ptr(l), _ptr(O), _ptr(out))
     return out
+
+
+def capacity(M_gpu, M_prime, M_model, TP, BW, alpha, t_d_slo, ISL, OSL, M_token):
+    """(V_mem, V_BW, cc_d) by Eq. 11-13 as printed."""
+    out = np.empty(3, dtype=np.float64)
+    _load().oracle_capacity(float(M_gpu), float(M_prime), float(M_model), float(TP), float(BW), float(alpha),
+                            float(t_d_slo), float(ISL), float(OSL), float(M_token), _ptr(out))
+    return tuple(float(x) for x in out)
+
+
+def pd_ratio(cc_d, t_p, t_d, OSL) -> float:
+    """n_p / n_d by Eq. 14."""
+    return float(_load().oracle_pd_ratio(float(cc_d), float(t_p), float(t_d), float(OSL)))

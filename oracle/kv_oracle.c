@@ -32,7 +32,10 @@
  * (tests/test_oracle_varq_pins.py): q_len = 1 equals oracle_attention; full and chunked
  * prefill equal torch SDPA with a causal (lower-right aligned) mask in fp64; first token of
  * a fresh prefill returns V_0; q = 0 gives running means; each query row equals decode over
- * the truncated sequence; future tokens do not matter.  No function here is "parity unpinned".
+ * the truncated sequence; future tokens do not matter.  oracle_capacity / oracle_pd_ratio
+ * (tests/test_capacity_model.py): exact-fraction hand values; Eq. 14 with Table I's printed T_p
+ * and T_d brackets the printed optimum 4.58.  No function here is
+ * "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -225,6 +228,30 @@ int oracle_attention_varq(const uint16_t* kv, const oracle_dims_t* D, int32_t la
     free(s);
   }
   return bad ? -2 : 0;
+}
+
+/*
+ * D-instance capacity model, the formulas as printed:
+ *   PAPER.md:206 Eq. 11  V_mem = (M_gpu - M') x TP - M_model
+ *   PAPER.md:212 Eq. 12  V_BW  = t_d^SLO x alpha x TP x BW
+ *   PAPER.md:216 Eq. 13  cc_d  = min(V_mem, V_BW) / ((ISL + OSL/2) x M_token)
+ * out[0..2] = V_mem, V_BW, cc_d (cc_d = 0 if the smaller volume is not positive).
+ */
+void oracle_capacity(double M_gpu, double M_prime, double M_model, double TP, double BW, double alpha,
+                     double t_d_slo, double ISL, double OSL, double M_token, double* out) {
+  double V_mem = (M_gpu - M_prime) * TP - M_model;
+  double V_BW = t_d_slo * alpha * TP * BW;
+  double V = V_mem < V_BW ? V_mem : V_BW;
+  out[0] = V_mem;
+  out[1] = V_BW;
+  out[2] = V > 0.0 ? V / ((ISL + OSL / 2.0) * M_token) : 0.0;
+}
+
+/* PAPER.md:223 Eq. 14  n_p x (t_d x OSL / t_p) = n_d x cc_d, solved for n_p / n_d (the closed form
+ * announced at PAPER.md:225 is missing from the extraction; reading A10). */
+double oracle_pd_ratio(double cc_d, double t_p, double t_d, double OSL) {
+  double per_p = t_d * OSL / t_p; /* concurrency one P-instance can drive on a D-instance */
+  return cc_d / per_p;
 }
 
 /*

@@ -58,6 +58,9 @@ _SIGS = {
     "kv_plan_decode": (_i32, [_P, _i32, _P, _P, _i32, ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
     "kv_ingest_host": (_i32, [_P, _i32, _P, _P, _P, _P, _i32, _i32, _P, _i64, _P]),
     "paged_decode_attention_host": (_i32, [_P, _i32, _i32, _P, _P, _P, ctypes.c_float, _P, _i64, _P]),
+    "kv_capacity": (_i32, [_P, _P]),
+    "kv_optimal_pd_ratio": (_i32, [ctypes.c_double] * 4 + [ctypes.POINTER(ctypes.c_double)]),
+    "kv_token_bytes": (_i64, [_CFG]),
     "kv_launch_count": (_i64, [_P]),
     "kv_profile_read": (_i32, [_P, _i32, ctypes.POINTER(_i64), ctypes.POINTER(ctypes.c_double)]),
     "kv_profile_reset": (_i32, [_P]),
@@ -268,6 +271,41 @@ def kv_plan_decode(handle: int, req_ids):
     _check(lib.kv_plan_decode(handle, ids.size, _np(ids), _np(items), n.value, ctypes.byref(n), ctypes.byref(ch)),
            "kv_plan_decode")
     return items, ch.value
+
+
+class _CapacityModel(ctypes.Structure):
+    _fields_ = [("m_gpu", ctypes.c_double), ("m_reserved", ctypes.c_double), ("m_model", ctypes.c_double),
+                ("tp", ctypes.c_int32), ("bw", ctypes.c_double), ("alpha", ctypes.c_double),
+                ("t_d_slo", ctypes.c_double), ("isl", ctypes.c_double), ("osl", ctypes.c_double),
+                ("m_token", ctypes.c_double)]
+
+
+class _Capacity(ctypes.Structure):
+    _fields_ = [("v_mem", ctypes.c_double), ("v_bw", ctypes.c_double), ("cc_d", ctypes.c_double),
+                ("bandwidth_bound", ctypes.c_int32)]
+
+
+def kv_capacity(m_gpu, m_reserved, m_model, tp, bw, alpha, t_d_slo, isl, osl, m_token) -> dict:
+    """Eq. 11-13 (PAPER.md:206-216): {v_mem, v_bw, cc_d, bandwidth_bound}."""
+    m = _CapacityModel(m_gpu, m_reserved, m_model, tp, bw, alpha, t_d_slo, isl, osl, m_token)
+    r = _Capacity()
+    _check(lib.kv_capacity(ctypes.byref(m), ctypes.byref(r)), "kv_capacity")
+    return {"v_mem": r.v_mem, "v_bw": r.v_bw, "cc_d": r.cc_d, "bandwidth_bound": bool(r.bandwidth_bound)}
+
+
+def kv_optimal_pd_ratio(cc_d, t_p, t_d, osl) -> float:
+    """Eq. 14 (PAPER.md:223): n_p / n_d = cc_d * t_p / (t_d * OSL)."""
+    r = ctypes.c_double()
+    _check(lib.kv_optimal_pd_ratio(cc_d, t_p, t_d, osl, ctypes.byref(r)), "kv_optimal_pd_ratio")
+    return float(r.value)
+
+
+def kv_token_bytes(cfg: PoolConfig) -> int:
+    c = cfg._c()
+    n = lib.kv_token_bytes(ctypes.byref(c))
+    if n < 0:
+        raise KVError(int(n), "kv_token_bytes")
+    return int(n)
 
 
 def kv_launch_count(handle: int) -> int:

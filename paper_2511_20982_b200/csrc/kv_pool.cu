@@ -776,6 +776,34 @@ int32_t paged_decode_step_host(kv_pool_t* pool, int32_t layer, int32_t batch, co
                         cuda_stream);
 }
 
+int32_t kv_capacity(const kv_capacity_model_t* m, kv_capacity_t* out) {
+  if (!m || !out) return KV_ERR_INVALID;
+  const bool ok = m->m_gpu > 0 && m->m_reserved >= 0 && m->m_model >= 0 && m->tp >= 1 && m->bw > 0 && m->alpha > 0 &&
+                  m->alpha <= 1.5 && m->t_d_slo > 0 && m->isl >= 0 && m->osl > 0 && m->m_token > 0;
+  if (!ok) return KV_ERR_INVALID;   // NaNs fail every comparison above
+  kv_capacity_t r{};
+  r.v_mem = (m->m_gpu - m->m_reserved) * m->tp - m->m_model;          // Eq. 11
+  r.v_bw = m->t_d_slo * m->alpha * m->tp * m->bw;                     // Eq. 12
+  r.bandwidth_bound = r.v_bw < r.v_mem ? 1 : 0;
+  const double v = r.v_bw < r.v_mem ? r.v_bw : r.v_mem;
+  r.cc_d = v > 0 ? v / ((m->isl + m->osl / 2) * m->m_token) : 0.0;    // Eq. 13
+  *out = r;
+  return KV_OK;
+}
+
+int32_t kv_optimal_pd_ratio(double cc_d, double t_p, double t_d, double osl, double* out_ratio) {
+  if (!out_ratio || !(cc_d > 0) || !(t_p > 0) || !(t_d > 0) || !(osl > 0)) return KV_ERR_INVALID;
+  *out_ratio = cc_d * t_p / (t_d * osl);                              // Eq. 14 solved for n_p / n_d
+  return KV_OK;
+}
+
+int64_t kv_token_bytes(const kv_pool_config_t* cfg) {
+  if (!cfg) return KV_ERR_INVALID;
+  int32_t rc = HostState::validate(*cfg);
+  if (rc != KV_OK) return rc;
+  return 2LL * cfg->num_layers * cfg->num_kv_heads * cfg->head_dim * 2;
+}
+
 int64_t kv_launch_count(const kv_pool_t* pool) { return pool ? pool->launches : KV_ERR_INVALID; }
 
 int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
