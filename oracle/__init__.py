@@ -27,7 +27,7 @@ def build(force: bool = False) -> str:
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + f".{os.getpid()}.tmp"
         subprocess.run(
-            ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-Wall", "-Wextra",
+            ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-Wall", "-Wextra", "-ffp-contract=off",
              "-o", tmp, _SRC, "-lm"],
             check=True,
         )
@@ -58,6 +58,15 @@ class Dims:
     @property
     def kv_elems(self) -> int:
         return self.num_layers * self.num_blocks * self.num_kv_heads * 2 * self.block_size * self.head_dim
+
+    @property
+    def fp8_tile_bytes(self) -> int:
+        """FP8 pool: K8[16][d] | V8[16][d] | sc[16][2] fp32 per (layer, block, kv head)."""
+        return 32 * self.head_dim + 128
+
+    @property
+    def fp8_bytes(self) -> int:
+        return self.num_layers * self.num_blocks * self.num_kv_heads * self.fp8_tile_bytes
 
     def shape(self):
         return (self.num_layers, self.num_blocks, self.num_kv_heads, 2, self.block_size, self.head_dim)
@@ -91,6 +100,18 @@ def _load():
         lib.oracle_capacity.argtypes = [D] * 10 + [P]
         lib.oracle_pd_ratio.restype = D
         lib.oracle_pd_ratio.argtypes = [D] * 4
+        lib.oracle_e4m3_decode_table.restype = None
+        lib.oracle_e4m3_decode_table.argtypes = [P]
+        lib.oracle_e4m3_encode_many.restype = None
+        lib.oracle_e4m3_encode_many.argtypes = [P, ctypes.c_int64, P]
+        lib.oracle_scatter_fp8.restype = None
+        lib.oracle_scatter_fp8.argtypes = [P, ctypes.POINTER(_Dims), P, ctypes.c_int32, ctypes.c_int32, P, P,
+                                           ctypes.c_int32, ctypes.c_int32]
+        lib.oracle_dequant_fp8.restype = None
+        lib.oracle_dequant_fp8.argtypes = [P, ctypes.POINTER(_Dims), ctypes.c_int32, P, ctypes.c_int32, P, P]
+        lib.oracle_attention_fp8.restype = ctypes.c_int
+        lib.oracle_attention_fp8.argtypes = [P, ctypes.POINTER(_Dims), ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
+                                             P, P, P, P, ctypes.c_double, P, P]
         lib.oracle_chunk.restype = None
         lib.oracle_chunk.argtypes = [P, ctypes.POINTER(_Dims), ctypes.c_int32, ctypes.c_int32, P, ctypes.c_int32,
                                      ctypes.c_int32, P, ctypes.c_double, P, P, P]
@@ -248,3 +269,77 @@ def capacity(M_gpu, M_prime, M_model, TP, BW, alpha, t_d_slo, ISL, OSL, M_token)
 def pd_ratio(cc_d, t_p, t_d, OSL) -> float:
     """n_p / n_d by Eq. 14."""
     return float(_load().oracle_pd_ratio(float(cc_d), float(t_p), float(t_d), float(OSL)))
+
+
+# ---- NEXT-2: FP8 (e4m3) KV pool -------------------------------------------------------------
+
+def e4m3_decode_table() -> np.ndarray:
+    out = np.empty(256, dtype=np.float64)
+    _load().oracle_e4m3_decode_table(_ptr(out))
+    return out
+
+
+def e4m3_encode(y) -> np.ndarray:
+    """float32 array -> e4m3 codes (uint8), round-to-nearest-even, saturating at +-448."""
+    y = np.ascontiguousarray(y, dtype=np.float32)
+    out = np.empty(y.shape, dtype=np.uint8)
+    _load().oracle_e4m3_encode_many(_ptr(y), y.size, _ptr(out))
+    return out
+
+
+def new_slab_fp8(dims: Dims, fill: int = 0) -> np.ndarray:
+    """A host FP8 KV region, flat uint8, pre-filled with a byte pattern."""
+    return np.full(dims.fp8_bytes, fill, dtype=np.uint8)
+
+
+def scatter_fp8(kv8: np.ndarray, dims: Dims, blocks, start_pos: int, k_src, v_src, layer_begin: int = 0) -> None:
+    """In place: quantising scatter of bf16 rows (uint16 [layer_count][Hkv][n][d]) into the FP8 pool."""
+    assert kv8.dtype == np.uint8 and kv8.flags.c_contiguous and kv8.size == dims.fp8_bytes and dims.block_size == 16
+    k_src, v_src = _u16(k_src, "k_src"), _u16(v_src, "v_src")
+    layer_count, hkv, n, d = k_src.shape
+    assert v_src.shape == k_src.shape and hkv == dims.num_kv_heads and d == dims.head_dim
+    assert 0 <= layer_begin and layer_begin + layer_count <= dims.num_layers
+    blocks = np.ascontiguousarray(blocks, dtype=np.int32)
+    assert (start_pos + n + dims.block_size - 1) // dims.block_size <= blocks.size
+    assert blocks.size == 0 or (0 <= blocks.min() and blocks.max() < dims.num_blocks)
+    c = dims._c()
+    _load().oracle_scatter_fp8(_ptr(kv8), ctypes.byref(c), _ptr(blocks), start_pos, n, _ptr(k_src), _ptr(v_src),
+                               layer_begin, layer_count)
+
+
+def dequant_fp8(kv8: np.ndarray, dims: Dims, layer: int, blocks, length: int):
+    """Dequantised (k, v) float64 [Hkv][length][d] of one request's layer."""
+    assert kv8.dtype == np.uint8 and kv8.size == dims.fp8_bytes
+    blocks = np.ascontiguousarray(blocks, dtype=np.int32)
+    k = np.empty((dims.num_kv_heads, length, dims.head_dim), dtype=np.float64)
+    v = np.empty_like(k)
+    c = dims._c()
+    _load().oracle_dequant_fp8(_ptr(kv8), ctypes.byref(c), layer, _ptr(blocks), length, _ptr(k), _ptr(v))
+    return k, v
+
+
+def attention_fp8(kv8: np.ndarray, dims: Dims, layer: int, num_q_heads: int, block_lists, seq_lens, q,
+                  scale: float | None = None, return_wsum: bool = False):
+    """Decode attention over an FP8 pool (definition on the dequantised values).  q: uint16 [B][Hq][d]."""
+    assert kv8.dtype == np.uint8 and kv8.flags.c_contiguous and kv8.size == dims.fp8_bytes
+    q = _u16(q, "q")
+    batch = q.shape[0]
+    assert q.shape == (batch, num_q_heads, dims.head_dim)
+    seq_lens = np.ascontiguousarray(seq_lens, dtype=np.int32)
+    lists = [np.ascontiguousarray(b, dtype=np.int32) for b in block_lists]
+    for b, n in zip(lists, seq_lens):
+        assert (int(n) + dims.block_size - 1) // dims.block_size <= b.size
+        assert b.size == 0 or (0 <= b.min() and b.max() < dims.num_blocks)
+    off = np.zeros(batch + 1, dtype=np.int64)
+    off[1:] = np.cumsum([b.size for b in lists])
+    bt = np.ascontiguousarray(np.concatenate(lists) if lists else np.zeros(0, np.int32), dtype=np.int32)
+    if scale is None:
+        scale = 1.0 / float(np.sqrt(np.float64(dims.head_dim)))
+    out = np.empty((batch, num_q_heads, dims.head_dim), dtype=np.float64)
+    wsum = np.empty((batch, num_q_heads), dtype=np.float64)
+    c = dims._c()
+    rc = _load().oracle_attention_fp8(_ptr(kv8), ctypes.byref(c), layer, num_q_heads, batch, _ptr(bt), _ptr(off),
+                                      _ptr(seq_lens), _ptr(q), float(scale), _ptr(out), _ptr(wsum))
+    if rc != 0:
+        raise ValueError(f"oracle_attention_fp8 failed ({rc})")
+    return (out, wsum) if return_wsum else out

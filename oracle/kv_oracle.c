@@ -34,8 +34,13 @@
  * a fresh prefill returns V_0; q = 0 gives running means; each query row equals decode over
  * the truncated sequence; future tokens do not matter.  oracle_capacity / oracle_pd_ratio
  * (tests/test_capacity_model.py): exact-fraction hand values; Eq. 14 with Table I's printed T_p
- * and T_d brackets the printed optimum 4.58.  No function here is
- * "parity unpinned".
+ * and T_d brackets the printed optimum 4.58.  FP8 functions
+ * (tests/test_oracle_fp8_pins.py): the e4m3 decode table and the RNE encoder equal
+ * torch.float8_e4m3fn on every code, every midpoint and a dense random sweep; the quantising
+ * scatter equals an independent numpy/torch-float8 statement over the whole slab, a brute-force
+ * nearest-code search and the |x - x^| <= 16 scale bound; attention over an FP8 pool equals
+ * oracle_attention when the data is exactly representable and torch SDPA (fp64) on the
+ * dequantised values otherwise.  No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -298,4 +303,181 @@ void oracle_combine(int32_t n_chunks, int32_t d, const double* m, const double* 
     for (int32_t j = 0; j < d; ++j) out[j] += a * O[(int64_t)c * d + j];
   }
   for (int32_t j = 0; j < d; ++j) out[j] /= den;
+}
+
+/* =============================================================================================
+ * NEXT-2: FP8 (e4m3) KV pool.  The paper's models are FP8 and
+ * the KV bytes per token M_token are the denominator of Eq. 13: halving them doubles
+ * cc_d under both Eq. 11 and Eq. 12.  The paper fixes no KV quantisation; the reading taken
+ * (C1-C4) is stated here step by step, in the precision both sides use (fp32 for the
+ * two roundings that decide a code):
+ *   per token row x[0..d) of one (layer, kv head, K|V):
+ *     amax  = max_j |x_j|                          (exact: bf16 magnitudes)
+ *     scale = amax == 0 ? 1 : fl32(amax / 448)     stored beside the row, fp32
+ *     inv   = amax == 0 ? 1 : fl32(448 / amax)
+ *     code_j = RNE_e4m3( fl32(x_j * inv) )         e4m3 "fn": 1-4-3 bits, bias 7, no infinities,
+ *                                                  S.1111.111 = NaN, max finite 448; saturating
+ *   dequantised value  x^_j = e4m3(code_j) * scale  (exact in fp64)
+ * Attention over an FP8 pool is Eq. 1 on the dequantised values (oracle_attention_fp8, fp64).
+ *
+ * FP8 slab layout (restated independently from include/kv_pool.h): per (layer, block, kv head) one
+ * tile of 32 d + 128 bytes:  K8[16][d] codes | V8[16][d] codes | sc[16][2] fp32 (ks_t, vs_t);
+ * tiles ordered [layer][block][kv_head].
+ * ============================================================================================= */
+
+static double e4m3_decode(uint8_t c) {
+  int sign = c >> 7, e = (c >> 3) & 15, m = c & 7;
+  double v;
+  if (e == 15 && m == 7) return NAN;
+  if (e == 0) v = ldexp((double)m, -9);            /* subnormal: m/8 * 2^-6 */
+  else v = ldexp(1.0 + m / 8.0, e - 7);
+  return sign ? -v : v;
+}
+
+void oracle_e4m3_decode_table(double* out256) {
+  for (int c = 0; c < 256; ++c) out256[c] = e4m3_decode((uint8_t)c);
+}
+
+/* Round-to-nearest-even onto the e4m3 grid, saturating at +-448; NaN -> 0x7f. */
+uint8_t oracle_e4m3_encode(float yf) {
+  double y = (double)yf;
+  if (y != y) return 0x7f;
+  uint8_t sign = (uint8_t)(signbit(y) ? 0x80 : 0);
+  double a = fabs(y);
+  if (a >= 448.0) return (uint8_t)(sign | 0x7e);   /* satfinite (also covers inf) */
+  int e;
+  (void)frexp(a, &e);                               /* a = f * 2^e, f in [0.5, 1)  ->  floor(log2 a) = e - 1 */
+  int ex = a == 0.0 ? -6 : e - 1;
+  if (ex < -6) ex = -6;                             /* subnormal range shares the quantum of 2^-6 */
+  double quantum = ldexp(1.0, ex - 3);              /* spacing of the grid in [2^ex, 2^(ex+1)) */
+  double n = nearbyint(a / quantum);                /* exact division by a power of two; ties to even */
+  double r = n * quantum;                           /* may round up into the next binade: still on the grid */
+  if (r > 448.0) r = 448.0;
+  if (r == 0.0) return sign;
+  (void)frexp(r, &e);
+  ex = e - 1;
+  if (ex < -6) return (uint8_t)(sign | (uint8_t)(r / ldexp(1.0, -9)));          /* subnormal: m = r / 2^-9 */
+  int m = (int)((r / ldexp(1.0, ex) - 1.0) * 8.0);
+  return (uint8_t)(sign | ((ex + 7) << 3) | m);
+}
+
+void oracle_e4m3_encode_many(const float* y, int64_t n, uint8_t* out) {
+  for (int64_t i = 0; i < n; ++i) out[i] = oracle_e4m3_encode(y[i]);
+}
+
+static int64_t kv8_tile_bytes(const oracle_dims_t* D) { return 32 * (int64_t)D->head_dim + 128; }
+static int64_t kv8_tile(const oracle_dims_t* D, int64_t layer, int64_t block, int64_t head) {
+  return ((layer * D->num_blocks + block) * D->num_kv_heads + head) * kv8_tile_bytes(D);
+}
+
+static float bf16_to_float(uint16_t b) {
+  uint32_t u = ((uint32_t)b) << 16;
+  float f;
+  memcpy(&f, &u, sizeof f);
+  return f;
+}
+
+/* one row: codes[d] and the fp32 scale, by the steps in the header comment */
+static float quantise_row(const uint16_t* x, int32_t d, uint8_t* codes) {
+  float amax = 0.0f;
+  for (int32_t j = 0; j < d; ++j) {
+    float a = fabsf(bf16_to_float(x[j]));
+    if (a > amax) amax = a;
+  }
+  volatile float scale = amax == 0.0f ? 1.0f : amax / 448.0f;   /* volatile: force the fp32 rounding */
+  volatile float inv = amax == 0.0f ? 1.0f : 448.0f / amax;
+  for (int32_t j = 0; j < d; ++j) {
+    volatile float y = bf16_to_float(x[j]) * inv;
+    codes[j] = oracle_e4m3_encode(y);
+  }
+  return scale;
+}
+
+/* Quantising scatter: oracle_scatter's relocation with each row quantised on the way. */
+void oracle_scatter_fp8(uint8_t* kv8, const oracle_dims_t* D, const int32_t* blocks, int32_t start_pos,
+                        int32_t n, const uint16_t* k_src, const uint16_t* v_src, int32_t layer_begin,
+                        int32_t layer_count) {
+  const int32_t d = D->head_dim;
+  for (int32_t ll = 0; ll < layer_count; ++ll)
+    for (int32_t h = 0; h < D->num_kv_heads; ++h)
+      for (int32_t t = 0; t < n; ++t) {
+        int32_t pos = start_pos + t;
+        int32_t slot = pos % D->block_size;
+        uint8_t* tile = kv8 + kv8_tile(D, layer_begin + ll, blocks[pos / D->block_size], h);
+        int64_t s = (((int64_t)ll * D->num_kv_heads + h) * n + t) * d;
+        float ks = quantise_row(k_src + s, d, tile + (int64_t)slot * d);
+        float vs = quantise_row(v_src + s, d, tile + 16 * (int64_t)d + (int64_t)slot * d);
+        memcpy(tile + 32 * (int64_t)d + slot * 8, &ks, 4);
+        memcpy(tile + 32 * (int64_t)d + slot * 8 + 4, &vs, 4);
+      }
+}
+
+/* Dequantised row of one token as doubles: c = 0 K, 1 V. */
+static void dequant_row(const uint8_t* kv8, const oracle_dims_t* D, int32_t layer, int32_t block, int32_t head,
+                        int32_t c, int32_t slot, double* out) {
+  const int32_t d = D->head_dim;
+  const uint8_t* tile = kv8 + kv8_tile(D, layer, block, head);
+  float sc;
+  memcpy(&sc, tile + 32 * (int64_t)d + slot * 8 + 4 * c, 4);
+  const uint8_t* codes = tile + (int64_t)c * 16 * d + (int64_t)slot * d;
+  for (int32_t j = 0; j < d; ++j) out[j] = e4m3_decode(codes[j]) * (double)sc;
+}
+
+/* Gather + dequantise one request's layer: k_out / v_out fp64 [num_kv_heads][len][d] (test support). */
+void oracle_dequant_fp8(const uint8_t* kv8, const oracle_dims_t* D, int32_t layer, const int32_t* blocks,
+                        int32_t len, double* k_out, double* v_out) {
+  const int32_t d = D->head_dim;
+  for (int32_t h = 0; h < D->num_kv_heads; ++h)
+    for (int32_t t = 0; t < len; ++t) {
+      int64_t o = ((int64_t)h * len + t) * d;
+      dequant_row(kv8, D, layer, blocks[t / D->block_size], h, 0, t % D->block_size, k_out + o);
+      dequant_row(kv8, D, layer, blocks[t / D->block_size], h, 1, t % D->block_size, v_out + o);
+    }
+}
+
+/* oracle_attention over an FP8 pool: the same definition on the dequantised values. */
+int oracle_attention_fp8(const uint8_t* kv8, const oracle_dims_t* D, int32_t layer, int32_t num_q_heads,
+                         int32_t batch, const int32_t* bt, const int64_t* bt_off, const int32_t* seq_lens,
+                         const uint16_t* q, double scale, double* out, double* wsum) {
+  const int32_t d = D->head_dim, Hq = num_q_heads, G = num_q_heads / D->num_kv_heads;
+  for (int32_t r = 0; r < batch; ++r)
+    if (seq_lens[r] < 1) return -1;
+  int bad = 0;
+#pragma omp parallel for collapse(2) schedule(dynamic, 1)
+  for (int32_t r = 0; r < batch; ++r)
+    for (int32_t h = 0; h < Hq; ++h) {
+      const int32_t g = h / G, n = seq_lens[r];
+      const int32_t* blocks = bt + bt_off[r];
+      const uint16_t* qv = q + ((int64_t)r * Hq + h) * d;
+      double* s = (double*)malloc(sizeof(double) * (size_t)n);
+      double* row = (double*)malloc(sizeof(double) * (size_t)d);
+      double* o = out + ((int64_t)r * Hq + h) * d;
+      if (!s || !row) { bad = 1; free(s); free(row); continue; }
+      for (int32_t t = 0; t < n; ++t) {
+        dequant_row(kv8, D, layer, blocks[t / D->block_size], g, 0, t % D->block_size, row);
+        double acc = 0.0;
+        for (int32_t j = 0; j < d; ++j) acc += bf16_to_double(qv[j]) * row[j];
+        s[t] = scale * acc;
+      }
+      double m = s[0];
+      for (int32_t t = 1; t < n; ++t)
+        if (s[t] > m) m = s[t];
+      double Z = 0.0;
+      for (int32_t t = 0; t < n; ++t) {
+        s[t] = exp(s[t] - m);
+        Z += s[t];
+      }
+      for (int32_t j = 0; j < d; ++j) o[j] = 0.0;
+      double ws = 0.0;
+      for (int32_t t = 0; t < n; ++t) {
+        dequant_row(kv8, D, layer, blocks[t / D->block_size], g, 1, t % D->block_size, row);
+        double w = s[t] / Z;
+        ws += w;
+        for (int32_t j = 0; j < d; ++j) o[j] += w * row[j];
+      }
+      if (wsum) wsum[(int64_t)r * Hq + h] = ws;
+      free(s);
+      free(row);
+    }
+  return bad ? -2 : 0;
 }
