@@ -63,6 +63,11 @@ extern "C" {
 #define KV_ERR_TOO_MANY_REQUESTS  -5  /* more than max_requests live requests                */
 #define KV_ERR_CUDA               -6  /* a CUDA runtime call failed; see kv_last_cuda_error  */
 #define KV_ERR_NO_DEVICE          -7  /* pool was created without a device slab (host-only)  */
+#define KV_ERR_UNSUPPORTED        -8  /* call not available for this pool's kv_dtype         */
+
+/* ---- KV element types ---------------------------------------------------------------- */
+#define KV_DTYPE_BF16              0  /* bf16 pool (the BASELINE.json configs)               */
+#define KV_DTYPE_FP8_E4M3          1  /* NEXT-2: e4m3 codes + per-token fp32 scales          */
 
 typedef struct kv_pool kv_pool_t; /* opaque, library-owned host object */
 
@@ -87,7 +92,26 @@ typedef struct kv_pool_config {
                                        NULL => host-only pool: allocator and planner work,
                                        calls that launch kernels return KV_ERR_NO_DEVICE    */
   int64_t  device_bytes;            /* size of the slab at device_base                      */
+  int32_t  kv_dtype;                /* KV_DTYPE_BF16 (0) or KV_DTYPE_FP8_E4M3                */
 } kv_pool_config_t;
+
+/*
+ * NEXT-2 — FP8 pool (kv_dtype = KV_DTYPE_FP8_E4M3).  The paper's models are FP8 and
+ * M_token, the KV bytes per token, is the denominator of Eq. 13: an FP8 pool holds and
+ * streams about twice the tokens per byte (cc_d x 1.94 at head_dim 128).  The paper fixes no KV
+ * quantisation; the one used (C1-C4), per token row x[0..head_dim) of one
+ * (layer, kv head, K|V), with every rounding in fp32:
+ *     amax = max_j |x_j|;  scale = amax / 448;  inv = 448 / amax   (scale = inv = 1 if amax = 0)
+ *     code_j = e4m3_rne_saturating(x_j * inv);        dequantised x^_j = e4m3(code_j) * scale
+ * (e4m3 = OCP FP8 E4M3 "fn": 1-4-3 bits, bias 7, no infinities, max 448).  Sources and queries stay
+ * bf16; kv_ingest quantises on the way in; paged_decode_attention evaluates Eq. 1 on the dequantised
+ * values.  KV region layout, one tile of 32*head_dim + 128 bytes per (layer, block, kv_head), tiles
+ * ordered [layer][block][kv_head]:
+ *     K8[16][head_dim] codes | V8[16][head_dim] codes | sc[16][2] fp32 = (k scale, v scale) of slot t
+ * Available on an FP8 pool: kv_reserve, kv_ingest(_host), paged_decode_attention(_host), kv_free and
+ * the introspection / profiling calls.  paged_decode_step(_host), paged_varlen_attention and kv_gather
+ * return KV_ERR_UNSUPPORTED (the decode loop appends with kv_ingest, n_tokens = 1).
+ */
 
 /* Bytes of the KV region / of the whole slab (KV region + private metadata) for `cfg`
  * (device_base / device_bytes ignored).  Return < 0 (a KV_ERR_*) on an invalid config.    */

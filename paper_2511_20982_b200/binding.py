@@ -24,7 +24,8 @@ lib = ctypes.CDLL(lib_path)
 
 KV_OK = 0
 KV_ERR_INVALID, KV_ERR_NO_BLOCKS, KV_ERR_UNKNOWN_REQUEST, KV_ERR_TOO_LONG = -1, -2, -3, -4
-KV_ERR_TOO_MANY_REQUESTS, KV_ERR_CUDA, KV_ERR_NO_DEVICE = -5, -6, -7
+KV_ERR_TOO_MANY_REQUESTS, KV_ERR_CUDA, KV_ERR_NO_DEVICE, KV_ERR_UNSUPPORTED = -5, -6, -7, -8
+KV_DTYPE_BF16, KV_DTYPE_FP8_E4M3 = 0, 1
 
 
 class _Config(ctypes.Structure):
@@ -33,6 +34,7 @@ class _Config(ctypes.Structure):
         ("head_dim", ctypes.c_int32), ("block_size", ctypes.c_int32), ("num_blocks", ctypes.c_int64),
         ("max_requests", ctypes.c_int32), ("max_blocks_per_request", ctypes.c_int32),
         ("alloc_seed", ctypes.c_uint64), ("device_base", ctypes.c_void_p), ("device_bytes", ctypes.c_int64),
+        ("kv_dtype", ctypes.c_int32),
     ]
 
 
@@ -97,11 +99,12 @@ class PoolConfig:
     max_blocks_per_request: int
     block_size: int = 16
     alloc_seed: int = 0
+    kv_dtype: int = KV_DTYPE_BF16
 
     def _c(self, device_base: int = 0, device_bytes: int = 0) -> _Config:
         return _Config(self.num_layers, self.num_q_heads, self.num_kv_heads, self.head_dim, self.block_size,
                        self.num_blocks, self.max_requests, self.max_blocks_per_request, self.alloc_seed,
-                       device_base or None, device_bytes)
+                       device_base or None, device_bytes, self.kv_dtype)
 
 
 def _ids(a) -> np.ndarray:

@@ -106,6 +106,7 @@ class HostState {
     if (c.num_layers < 1 || c.num_q_heads < 1 || c.num_kv_heads < 1) return KV_ERR_INVALID;
     if (c.head_dim != 64 && c.head_dim != 128) return KV_ERR_INVALID;
     if (c.block_size != 16) return KV_ERR_INVALID;
+    if (c.kv_dtype != KV_DTYPE_BF16 && c.kv_dtype != KV_DTYPE_FP8_E4M3) return KV_ERR_INVALID;
     if (c.num_q_heads % c.num_kv_heads != 0 || c.num_q_heads / c.num_kv_heads > 8) return KV_ERR_INVALID;
     if (c.num_blocks < 1 || c.num_blocks > 0x7fffffffLL) return KV_ERR_INVALID;
     if (c.max_requests < 1 || c.max_blocks_per_request < 1) return KV_ERR_INVALID;

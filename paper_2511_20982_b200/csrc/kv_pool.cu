@@ -12,6 +12,7 @@
 #include "../../include/kv_pool.h"
 #include "kv_host.h"
 #include "kv_kernels.cuh"
+#include "kv_fp8.cuh"
 
 namespace {
 
@@ -33,7 +34,9 @@ struct Layout {  // byte offsets inside the caller's slab
 Layout make_layout(const kv_pool_config_t& c) {
   Layout L{};
   const int64_t G = c.num_q_heads / c.num_kv_heads;
-  L.kv_bytes = static_cast<int64_t>(c.num_layers) * c.num_blocks * c.num_kv_heads * 2 * c.block_size * c.head_dim * 2;
+  L.kv_bytes = c.kv_dtype == KV_DTYPE_FP8_E4M3
+                   ? static_cast<int64_t>(c.num_layers) * c.num_blocks * c.num_kv_heads * (32LL * c.head_dim + 128)
+                   : static_cast<int64_t>(c.num_layers) * c.num_blocks * c.num_kv_heads * 2 * c.block_size * c.head_dim * 2;
   int64_t off = align_up(L.kv_bytes);
   L.block_table = off;
   off = align_up(off + static_cast<int64_t>(c.max_requests) * c.max_blocks_per_request * 4);
@@ -268,7 +271,13 @@ int32_t launch_ingest(kv_pool* pool, const std::vector<IngestReq>& reqs, const s
   const unsigned grid = static_cast<unsigned>((total_units + kIngestWarps - 1) / kIngestWarps);
   ProfRing& pr = pool->prof[kGather ? KV_KERNEL_GATHER : KV_KERNEL_INGEST];
   if (pool->profile) KV_CUDA(pool, pr.begin(stream));
-  if (c.head_dim == 128)
+  if (c.kv_dtype == KV_DTYPE_FP8_E4M3) {
+    if (kGather) return KV_ERR_UNSUPPORTED;
+    if (c.head_dim == 128)
+      ingest_fp8_kernel<128><<<grid, kIngestThreads, 0, stream>>>(p);
+    else
+      ingest_fp8_kernel<64><<<grid, kIngestThreads, 0, stream>>>(p);
+  } else if (c.head_dim == 128)
     ingest_kernel<128, kGather><<<grid, kIngestThreads, 0, stream>>>(p);
   else
     ingest_kernel<64, kGather><<<grid, kIngestThreads, 0, stream>>>(p);
@@ -428,6 +437,7 @@ int32_t kv_ingest(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const 
 
 int32_t kv_gather(kv_pool_t* pool, int64_t req_id, void* k_dst, void* v_dst, void* cuda_stream) {
   if (!pool || !k_dst || !v_dst || !aligned16(k_dst) || !aligned16(v_dst)) return KV_ERR_INVALID;
+  if (pool->hs.cfg.kv_dtype != KV_DTYPE_BF16) return KV_ERR_UNSUPPORTED;
   if (!pool->has_device) return KV_ERR_NO_DEVICE;
   auto it = pool->hs.reqs.find(req_id);
   if (it == pool->hs.reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
@@ -493,8 +503,8 @@ static AttnParams attn_params(kv_pool_t* pool, int32_t layer, const void* q, voi
   const kv_pool_config_t& c = pool->hs.cfg;
   const float scale = sm_scale > 0.f ? sm_scale : 1.0f / std::sqrt(static_cast<float>(c.head_dim));
   AttnParams p{};
-  const int64_t layer_elems = c.num_blocks * c.num_kv_heads * 2LL * c.block_size * c.head_dim;
-  p.kv_layer = reinterpret_cast<uint16_t*>(pool->base) + static_cast<int64_t>(layer) * layer_elems;
+  const int64_t layer_bytes = pool->lay.kv_bytes / c.num_layers;
+  p.kv_layer = reinterpret_cast<uint16_t*>(pool->base + static_cast<int64_t>(layer) * layer_bytes);
   p.block_table = reinterpret_cast<int32_t*>(pool->base + pool->lay.block_table);
   p.bt_stride = c.max_blocks_per_request;
   p.items = reinterpret_cast<const WorkItemDev*>(s.dev);
@@ -520,6 +530,7 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, c
   if (!pool || !req_ids || !q || !out || !aligned16(q) || !aligned16(out)) return KV_ERR_INVALID;
   const kv_pool_config_t& c = pool->hs.cfg;
   if (layer < 0 || layer >= c.num_layers || batch < 1) return KV_ERR_INVALID;
+  if (k_new && c.kv_dtype != KV_DTYPE_BF16) return KV_ERR_UNSUPPORTED;
   if (!pool->has_device) return KV_ERR_NO_DEVICE;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
 
@@ -566,7 +577,10 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, c
   const int32_t want = (p.n_units + kAttnWarps - 1) / kAttnWarps;
   const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * pool->ctas_per_sm)));
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_ATTN].begin(stream));
-  if (c.head_dim == 128) {
+  if (c.kv_dtype == KV_DTYPE_FP8_E4M3) {
+    if (c.head_dim == 128) attn_fp8_kernel<128><<<grid, kAttnThreads, 0, stream>>>(p);
+    else attn_fp8_kernel<64><<<grid, kAttnThreads, 0, stream>>>(p);
+  } else if (c.head_dim == 128) {
     if (k_new) attn_splitkv_kernel<128, true><<<grid, kAttnThreads, 0, stream>>>(p);
     else attn_splitkv_kernel<128, false><<<grid, kAttnThreads, 0, stream>>>(p);
   } else {
@@ -620,6 +634,7 @@ int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
   if (!pool || !req_ids || !q_lens || !q || !out || !aligned16(q) || !aligned16(out)) return KV_ERR_INVALID;
   const kv_pool_config_t& c = pool->hs.cfg;
   if (layer < 0 || layer >= c.num_layers || batch < 1) return KV_ERR_INVALID;
+  if (c.kv_dtype != KV_DTYPE_BF16) return KV_ERR_UNSUPPORTED;
   if (!pool->has_device) return KV_ERR_NO_DEVICE;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const int32_t G = c.num_q_heads / c.num_kv_heads;
@@ -848,6 +863,7 @@ const char* kv_strerror(int32_t status) {
     case KV_ERR_TOO_MANY_REQUESTS: return "more than max_requests live requests";
     case KV_ERR_CUDA: return "CUDA runtime error (see kv_last_cuda_error)";
     case KV_ERR_NO_DEVICE: return "pool has no device slab (host-only)";
+    case KV_ERR_UNSUPPORTED: return "call not available for this pool's kv_dtype";
     default: return "unknown status";
   }
 }

@@ -1,0 +1,181 @@
+"""-m gpu parity of the FP8 (e4m3) KV pool through the C-ABI:
+  * kv_ingest into an FP8 pool == oracle.scatter_fp8, BYTE-exact over the whole KV region (codes, scales,
+    sentinel everywhere else), for one-shot, split and token-by-token ingests (per-token scales make a
+    row's bytes independent of how it arrived);
+  * paged_decode_attention over the FP8 pool == oracle.attention_fp8 (Eq. 1 on the dequantised values)
+    within the bf16-output tolerance, for every split mode and GQA group size, including rows whose
+    magnitudes span e^-6 .. e^6 (the V scale rides in the softmax reference, not in the f16 weights)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2511_20982_b200 as kv
+from paper_2511_20982_b200 import binding as B
+from paper_2511_20982_b200 import workloads as W
+from gpu_harness import DEV, compare_attention, dims_of, kv_src
+from helpers import bf16_bits, bits_of, bits_to_f64
+
+pytestmark = pytest.mark.gpu
+
+MODES = [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=1024),
+         dict(min_chunk_blocks=2, items_per_slot=2, fuse_combine=0), dict(min_chunk_blocks=5, items_per_slot=1, ctas_per_sm=1)]
+SENT = 0xFF   # e4m3 NaN code / NaN scale bytes: an unmasked read poisons the output
+
+
+def make_fp8_pool(L, Hq, Hkv, d, num_blocks, max_requests=16, max_len=4096, alloc_seed=11):
+    cfg = kv.PoolConfig(num_layers=L, num_q_heads=Hq, num_kv_heads=Hkv, head_dim=d, num_blocks=num_blocks,
+                        max_requests=max_requests, max_blocks_per_request=(max_len + 15) // 16, alloc_seed=alloc_seed,
+                        kv_dtype=B.KV_DTYPE_FP8_E4M3)
+    pool = kv.KVPool(cfg, device=DEV)
+    assert pool.kv_bytes == L * num_blocks * Hkv * (32 * d + 128)
+    pool.slab[: pool.kv_bytes].fill_(SENT)
+    return pool
+
+
+def pool_bytes(pool) -> np.ndarray:
+    return pool.slab[: pool.kv_bytes].cpu().numpy()
+
+
+def tb(bits):
+    return torch.from_numpy(bits.view(np.int16).copy()).view(torch.bfloat16).to(DEV)
+
+
+def wide_rows(rng, L, Hkv, n, d):
+    """N(0,1) rows with per-row magnitudes e^U(-6, 6), a zero row and a row with one huge element."""
+    x = rng.standard_normal((L, Hkv, n, d)) * np.exp(rng.uniform(-6, 6, (L, Hkv, n, 1)))
+    if n > 3:
+        x[:, :, 2] = 0.0
+        x[:, :, 3, 5] = 3.0e4
+    return bf16_bits(x)
+
+
+@pytest.mark.parametrize("d,Hkv,L", [(128, 8, 2), (64, 2, 3), (128, 32, 1)])
+def test_ingest_is_byte_exact(d, Hkv, L):
+    rng = np.random.default_rng(d + Hkv)
+    lens = [17, 64, 130, 255, 1, 16, 33]
+    ids = list(range(100, 100 + len(lens)))
+    NB = sum((n + 15) // 16 for n in lens) + 5
+    K = [wide_rows(rng, L, Hkv, n, d) for n in lens]
+    V = [wide_rows(rng, L, Hkv, n, d) for n in lens]
+    for mode in ("once", "split", "tokens"):
+        pool = make_fp8_pool(L, Hkv, Hkv, d, NB)
+        slab = oracle.new_slab_fp8(dims_of(pool), SENT)
+        if mode == "once":
+            pool.ingest(ids, [tb(k) for k in K], [tb(v) for v in V])
+        else:
+            for i, n in enumerate(lens):
+                cuts = [0, n] if n < 3 else ([0, n // 3, n // 3 + 1, n] if mode == "split" else list(range(n + 1)))
+                for a, b in zip(cuts[:-1], cuts[1:]):
+                    pool.ingest([ids[i]], [tb(K[i][:, :, a:b].copy())], [tb(V[i][:, :, a:b].copy())])
+        torch.cuda.synchronize()
+        for i, n in enumerate(lens):
+            oracle.scatter_fp8(slab, dims_of(pool), pool.block_table(ids[i])[0], 0, K[i], V[i])
+        got = pool_bytes(pool)
+        assert np.array_equal(got, slab), f"{mode}: FP8 ingest is not byte-exact ({int((got != slab).sum())} bytes differ)"
+        pool.close()
+
+
+@pytest.mark.parametrize("opts", MODES)
+@pytest.mark.parametrize("Hq,Hkv,d", [(8, 2, 64), (32, 32, 128), (64, 8, 128), (32, 8, 128)])
+def test_attention_matches_oracle(Hq, Hkv, d, opts):
+    rng = np.random.default_rng(7)
+    lens = [17, 64, 130, 255, 1, 16, 33, 700, 1900, 5]
+    ids = list(range(300, 300 + len(lens)))
+    pool = make_fp8_pool(1, Hq, Hkv, d, sum((n + 15) // 16 for n in lens) + 8)
+    for k_, v_ in opts.items():
+        pool.set_option(k_, v_)
+    w = W.Workload("fp8", 1, Hq, Hkv, d, len(lens), None, 99, max_len=4096)
+    srcs = [kv_src(w, uid, 0, n, DEV) for uid, n in zip(ids, lens)]
+    pool.ingest(ids, [s[0] for s in srcs], [s[1] for s in srcs])
+    slab = oracle.new_slab_fp8(dims_of(pool), SENT)
+    for uid, n, (k, v) in zip(ids, lens, srcs):
+        oracle.scatter_fp8(slab, dims_of(pool), pool.block_table(uid)[0], 0, bits_of(k), bits_of(v))
+    q = W.q_values(w.seed, 1, 0, len(lens), Hq, d, DEV)
+    out = pool.attention(0, ids, q)
+    torch.cuda.synchronize()
+    assert np.array_equal(pool_bytes(pool), slab)
+    lists = [pool.block_table(u)[0] for u in ids]
+    want = oracle.attention_fp8(slab, dims_of(pool), 0, Hq, lists, lens, bits_of(q))
+    compare_attention(out, want)
+    # the quantisation itself: close to the bf16 oracle on the unquantised values (sanity, loose)
+    s16 = oracle.new_slab(dims_of(pool), 0)
+    for uid, n, (k, v) in zip(ids, lens, srcs):
+        oracle.scatter(s16, dims_of(pool), pool.block_table(uid)[0], 0, bits_of(k), bits_of(v))
+    exact = oracle.attention(s16, dims_of(pool), 0, Hq, lists, lens, bits_of(q))
+    assert np.abs(want - exact).max() < 0.15 and np.abs(want - exact).mean() < 0.01
+
+
+@pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=2, items_per_slot=1024)])
+def test_attention_wide_dynamic_range(opts):
+    """Row magnitudes from e^-6 to e^6 in K and V, scaled-up queries, a zero row and an outlier element."""
+    rng = np.random.default_rng(8)
+    Hq, Hkv, d = 16, 4, 128
+    lens = [40, 333, 1000]
+    ids = [1, 2, 3]
+    pool = make_fp8_pool(1, Hq, Hkv, d, 100)
+    for k_, v_ in opts.items():
+        pool.set_option(k_, v_)
+    K = [bf16_bits(rng.standard_normal((1, Hkv, n, d)) * 0.3) for n in lens]      # keep the scores moderate
+    V = [wide_rows(rng, 1, Hkv, n, d) for n in lens]
+    pool.ingest(ids, [tb(k) for k in K], [tb(v) for v in V])
+    slab = oracle.new_slab_fp8(dims_of(pool), SENT)
+    for uid, k, v in zip(ids, K, V):
+        oracle.scatter_fp8(slab, dims_of(pool), pool.block_table(uid)[0], 0, k, v)
+    for qscale in (1.0, 2.0 ** 40, 2.0 ** -40):
+        qb = bf16_bits(rng.standard_normal((3, Hq, d)) * qscale)
+        sm = 0.0883883 / qscale                                   # exact power-of-two compensation in the scale
+        out = pool.attention(0, ids, tb(qb), sm_scale=sm)
+        torch.cuda.synchronize()
+        lists = [pool.block_table(u)[0] for u in ids]
+        want = oracle.attention_fp8(slab, dims_of(pool), 0, Hq, lists, lens, qb, scale=float(np.float32(sm)))
+        got = bits_to_f64(bits_of(out))
+        assert np.all(np.isfinite(got))
+        err = np.abs(got - want)
+        tol = 2.0 ** -7 * np.abs(want) + 1e-3 * np.sqrt((want ** 2).mean(axis=-1, keepdims=True)) + 1e-30
+        assert np.all(err <= tol), float((err / tol).max())
+
+
+def test_decode_loop_appends_with_ingest():
+    Hq, Hkv, d, L = 32, 8, 128, 2
+    lens = [15, 16, 31, 500, 1]
+    ids = list(range(5))
+    w = W.Workload("fp8d", L, Hq, Hkv, d, len(lens), None, 5, max_len=1024)
+    pool = make_fp8_pool(L, Hq, Hkv, d, 64)
+    slab = oracle.new_slab_fp8(dims_of(pool), SENT)
+    srcs = [kv_src(w, u, 0, n, DEV) for u, n in zip(ids, lens)]
+    pool.ingest(ids, [s[0] for s in srcs], [s[1] for s in srcs])
+    for u, n, (k, v) in zip(ids, lens, srcs):
+        oracle.scatter_fp8(slab, dims_of(pool), pool.block_table(u)[0], 0, bits_of(k), bits_of(v))
+    for step in range(3):
+        new = [kv_src(w, u, n + step, n + step + 1, DEV) for u, n in zip(ids, lens)]
+        pool.ingest(ids, [s[0] for s in new], [s[1] for s in new])
+        for u, n, (k, v) in zip(ids, lens, new):
+            oracle.scatter_fp8(slab, dims_of(pool), pool.block_table(u)[0], n + step, bits_of(k), bits_of(v))
+        for l in range(L):
+            q = W.q_values(w.seed, step, l, len(ids), Hq, d, DEV)
+            out = pool.attention(l, ids, q)
+            torch.cuda.synchronize()
+            lists = [pool.block_table(u)[0] for u in ids]
+            want = oracle.attention_fp8(slab, dims_of(pool), l, Hq, lists, [n + step + 1 for n in lens], bits_of(q))
+            compare_attention(out, want)
+    assert np.array_equal(pool_bytes(pool), slab)
+
+
+def test_unsupported_calls():
+    pool = make_fp8_pool(1, 8, 2, 64, 16)
+    w = W.Workload("fp8u", 1, 8, 2, 64, 1, None, 5, max_len=256)
+    k, v = kv_src(w, 1, 0, 20, DEV)
+    pool.ingest([1], [k], [v])
+    q = torch.zeros((1, 8, 64), dtype=torch.bfloat16, device=DEV)
+    with pytest.raises(B.KVError) as e:
+        pool.gather(1)
+    assert e.value.status == B.KV_ERR_UNSUPPORTED
+    with pytest.raises(B.KVError) as e:
+        pool.varlen_attention(0, [1], [1], q)
+    assert e.value.status == B.KV_ERR_UNSUPPORTED
+    pool.reserve([1], [1])
+    with pytest.raises(B.KVError) as e:
+        pool.decode_step(0, [1], q, torch.zeros((1, 2, 64), dtype=torch.bfloat16, device=DEV),
+                         torch.zeros((1, 2, 64), dtype=torch.bfloat16, device=DEV))
+    assert e.value.status == B.KV_ERR_UNSUPPORTED
