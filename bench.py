@@ -59,6 +59,8 @@ def parse_args():
     ap.add_argument("--no-isolated", action="store_true", help="skip the attention-alone / ingest-alone legs")
     ap.add_argument("--unfused", action="store_true", help="append and attention as separate calls (a3, then a4+a5)")
     ap.add_argument("--opt", action="append", default=[], help="pool option key=value (tuning)")
+    ap.add_argument("--kv-dtype", choices=["bf16", "fp8"], default="bf16",
+                    help="fp8: NEXT-2, e4m3 KV pool with per-token scales (append by kv_ingest, not fused)")
     ap.add_argument("--layers", type=int, default=0,
                     help="profiling aid: run the workload with this many layers (a smaller pool for ncu replay); "
                          "the line's config.layers says what ran")
@@ -145,11 +147,11 @@ class OracleSample:
     Builds a private host slab with sequential block lists, times oracle.scatter (ingest) and
     oracle.attention, and returns the algorithmic bytes moved."""
 
-    def __init__(self, w, reqs, layer: int, q_bits):
+    def __init__(self, w, reqs, layer: int, q_bits, fp8: bool = False):
         import numpy as np
         import oracle
         from paper_2511_20982_b200 import workloads as W
-        self.w, self.reqs, self.layer, self.q_bits = w, reqs, layer, q_bits
+        self.w, self.reqs, self.layer, self.q_bits, self.fp8 = w, reqs, layer, q_bits, fp8
         bs = w.block_size
         nblk = [(n + bs - 1) // bs for _, n in reqs]
         self.dims = oracle.Dims(1, w.num_kv_heads, w.head_dim, bs, max(1, sum(nblk)))
@@ -165,21 +167,21 @@ class OracleSample:
     def run(self):
         """-> (seconds scatter, seconds attention, out float64 [R][Hq][d])."""
         import oracle
-        slab = oracle.new_slab(self.dims, 0x7FC0)
+        slab = oracle.new_slab_fp8(self.dims, 0xFF) if self.fp8 else oracle.new_slab(self.dims, 0x7FC0)
+        scatter, attention = (oracle.scatter_fp8, oracle.attention_fp8) if self.fp8 else (oracle.scatter, oracle.attention)
         t0 = time.perf_counter()
         for (k, v), bl in zip(self.src, self.lists):
-            oracle.scatter(slab, self.dims, bl, 0, k, v)
+            scatter(slab, self.dims, bl, 0, k, v)
         t1 = time.perf_counter()
-        out = oracle.attention(slab, self.dims, 0, self.w.num_q_heads, self.lists, [n for _, n in self.reqs],
-                               self.q_bits)
+        out = attention(slab, self.dims, 0, self.w.num_q_heads, self.lists, [n for _, n in self.reqs], self.q_bits)
         t2 = time.perf_counter()
         return t1 - t0, t2 - t1, out
 
     def bytes(self):
-        from paper_2511_20982_b200.engine import attention_bytes
+        from paper_2511_20982_b200.engine import attention_bytes, kv_token_bytes_layer
         lens = [n for _, n in self.reqs]
-        ingest = 2 * sum(lens) * 2 * self.w.num_kv_heads * self.w.head_dim * 2
-        return attention_bytes(self.w, lens), ingest
+        ingest = sum(lens) * (2 * self.w.num_kv_heads * self.w.head_dim * 2 + kv_token_bytes_layer(self.w, self.fp8))
+        return attention_bytes(self.w, lens, self.fp8), ingest
 
 
 def run_reference(args):
@@ -200,7 +202,7 @@ def run_reference(args):
         reqs.append((i, n)); tot += n
     q = W.q_values(w.seed, 0, 0, w.batch, w.num_q_heads, w.head_dim, "cpu")[: len(reqs)]
     q_bits = q.contiguous().view(__import__("torch").int16).numpy().view(np.uint16).copy()
-    smp = OracleSample(w, reqs, 0, q_bits)
+    smp = OracleSample(w, reqs, 0, q_bits, fp8=args.kv_dtype == "fp8")
     for _ in range(args.warmup):
         smp.run()
     t = time.perf_counter()
@@ -214,7 +216,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": "GB/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "sample": sample},
+        "config": {"workload": args.workload, "sample": sample, "kv_dtype": args.kv_dtype},
         "cpu_baseline": {"value": val, "unit": "GB/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -244,7 +246,7 @@ def cpu_baseline_and_check(loop, last_step: int, budget_s: float = 12.0):
     for c0 in range(0, len(order), chunk):
         rows = order[c0:c0 + chunk]
         reqs = [(loop.sched.content_uid[int(sp.batch[r])], int(sp.lens_after[r])) for r in rows]
-        smp = OracleSample(w, reqs, layer, bits(q[rows]))
+        smp = OracleSample(w, reqs, layer, bits(q[rows]), fp8=loop.fp8)
         a, b, want = smp.run()
         t_sc += a; t_at += b
         x, y = smp.bytes(); ab += x; ib += y
@@ -288,8 +290,9 @@ def run_cuda(args):
     e2e_w = 3 if args.e2e_steps > 0 else 0
     opts = {k: int(v) for k, v in (o.split("=") for o in args.opt)}
     t_setup = time.time()
+    fp8 = args.kv_dtype == "fp8"
     loop = DecodeLoop(w, Wm + K, n_host_steps=e2e_w + args.e2e_steps, device=dev, streams=args.streams, salt=rep.salt,
-                      options=opts, fused=not args.unfused)
+                      options=opts, fused=not args.unfused, kv_dtype=B.KV_DTYPE_FP8_E4M3 if fp8 else B.KV_DTYPE_BF16)
     t_setup = time.time() - t_setup
     pool = loop.pool
     phys = int(os.environ.get("CUDA_VISIBLE_DEVICES", "").split(",")[local]) if os.environ.get("CUDA_VISIBLE_DEVICES") else local
@@ -330,12 +333,12 @@ def run_cuda(args):
     ing_n, ing_ms = prof["ingest"]
     attn_bytes_per_launch = by["attn"] / max(attn_n, 1)
     achieved = attn_bytes_per_launch / (attn_ms / max(attn_n, 1) * 1e-3) / 1e9 if attn_ms > 0 else None
-    roofline = {"kernel": "attn_splitkv_kernel", "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    roofline = {"kernel": "attn_fp8_kernel" if fp8 else "attn_splitkv_kernel", "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak if achieved else None, "peak_source": peak_src,
                 "frac_of_nominal_8000": achieved / NOMINAL_HBM_GBS if achieved else None,
                 "launches": attn_n, "avg_launch_us": attn_ms / max(attn_n, 1) * 1e3,
                 "algorithmic_bytes_per_launch": attn_bytes_per_launch, "traffic": None}
-    if args.workload in NCU_TRAFFIC_RATIO:
+    if args.workload in NCU_TRAFFIC_RATIO and not fp8:
         ratio, src = NCU_TRAFFIC_RATIO[args.workload]
         roofline.update({"traffic": attn_bytes_per_launch * ratio, "traffic_source": f"ncu --set full, {src}: "
                          f"DRAM bytes = {ratio:.4f} x algorithmic bytes"})
@@ -395,8 +398,8 @@ def run_cuda(args):
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "bf16 (fp32 accumulate)", "data": "synthetic",
-            "config": {"workload": args.workload, "layers": w.num_layers, "q_heads": w.num_q_heads,
+            "dtype": "fp8 e4m3 KV, bf16 q/out (fp32 accumulate)" if fp8 else "bf16 (fp32 accumulate)", "data": "synthetic",
+            "config": {"workload": args.workload, "kv_dtype": args.kv_dtype, "layers": w.num_layers, "q_heads": w.num_q_heads,
                        "kv_heads": w.num_kv_heads, "head_dim": w.head_dim, "block_size": w.block_size,
                        "batch": w.batch, "ingest_per_step": w.ingest_per_step, "streams": 2 if loop.two_streams else 1,
                        "decode_call": "paged_decode_step (fused a3+a4+a5)" if loop.fused else "kv_ingest + paged_decode_attention",
@@ -438,7 +441,8 @@ def isolated_legs(loop, last_step: int, peak: float, reps: int = 5):
     t_attn = float(np.median(times[1:]))
     res = {"attention_gbs": sp.attn_bytes_layer * L / (t_attn * 1e-3) / 1e9, "attention_ms": t_attn}
     res["attention_frac"] = res["attention_gbs"] / peak
-    res.update(varlen_leg(loop, last_step, peak, reps))
+    if not loop.fp8:
+        res.update(varlen_leg(loop, last_step, peak, reps))
     if w.ingest_per_step and loop.bank:
         k = w.ingest_per_step
         ents = list(range(k))
@@ -446,7 +450,8 @@ def isolated_legs(loop, last_step: int, peak: float, reps: int = 5):
         kp = np.asarray([loop.bank[e][0].data_ptr() for e in ents], dtype=np.uint64)
         vp = np.asarray([loop.bank[e][1].data_ptr() for e in ents], dtype=np.uint64)
         ids = np.arange(k, dtype=np.int64) + (1 << 40)
-        nbytes = 2 * 2 * loop.tok_bytes * int(nt.sum())
+        from paper_2511_20982_b200.engine import kv_token_bytes_layer
+        nbytes = (2 * loop.tok_bytes + L * kv_token_bytes_layer(w, loop.fp8)) * int(nt.sum())   # source read + pool written
         times = []
         try:
             for r in range(reps + 1):

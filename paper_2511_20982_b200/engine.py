@@ -66,18 +66,24 @@ class Schedule:
     peak_blocks: int = 0
 
 
-def attention_bytes(w: W.Workload, lens) -> int:
+def kv_token_bytes_layer(w: W.Workload, fp8: bool = False) -> int:
+    """Pool bytes of one token in one layer: K and V rows of every kv head — bf16, or e4m3 codes plus the
+    two fp32 row scales (FP8 pool, NEXT-2)."""
+    return w.num_kv_heads * ((2 * w.head_dim + 8) if fp8 else (2 * w.head_dim * 2))
+
+
+def attention_bytes(w: W.Workload, lens, fp8: bool = False) -> int:
     """Algorithmic bytes of one layer's decode attention: every resident K and V element once, q in and
     out once, the block_table once per request, seq_lens."""
     lens = np.asarray(lens, dtype=np.int64)
-    kv = int(lens.sum()) * 2 * w.num_kv_heads * w.head_dim * 2
+    kv = int(lens.sum()) * kv_token_bytes_layer(w, fp8)
     qo = 2 * len(lens) * w.num_q_heads * w.head_dim * 2
     bt = 4 * int(((lens + w.block_size - 1) // w.block_size).sum()) + 4 * len(lens)
     return kv + qo + bt
 
 
 def build_schedule(w: W.Workload, n_steps: int, bank_steps: int, salt: int = 0, host_from: int | None = None,
-                   host_bank_steps: int = 2) -> Schedule:
+                   host_bank_steps: int = 2, fp8: bool = False) -> Schedule:
     """Seeded, host-only simulation of which requests retire / arrive / decode at every step.
     Steps >= host_from (the host-buffer steps) cycle over the first `host_bank_steps` bank steps only,
     which are the ones mirrored in pinned host memory."""
@@ -92,7 +98,8 @@ def build_schedule(w: W.Workload, n_steps: int, bank_steps: int, salt: int = 0, 
         sch.content_uid[i] = i
     order = list(range(w.batch))          # FIFO arrival order of the decode batch
     next_id = w.batch
-    row = 2 * (2 * w.num_layers * w.num_kv_heads * w.head_dim * 2)  # per token: K+V source bytes, read + written
+    # per token: K+V bf16 source bytes read + pool bytes written (all layers)
+    row = 2 * w.num_layers * w.num_kv_heads * w.head_dim * 2 + w.num_layers * kv_token_bytes_layer(w, fp8)
     blocks = lambda n: (n + w.block_size - 1) // w.block_size
     live_blocks = sum(blocks(n) for n in lens.values())
     sch.peak_blocks = live_blocks
@@ -141,7 +148,7 @@ def build_schedule(w: W.Workload, n_steps: int, bank_steps: int, salt: int = 0, 
         la = np.asarray([lens[i] for i in order], np.int64)
         sch.peak_blocks = max(sch.peak_blocks, live_blocks)
         sch.steps.append(StepPlan(np.asarray(retire, np.int64), np.asarray(ids, np.int64),
-                                  np.asarray(banks, np.int64), batch, la, attention_bytes(w, la),
+                                  np.asarray(banks, np.int64), batch, la, attention_bytes(w, la, fp8),
                                   len(order) * row, sum(lens[i] for i in ids) * row,
                                   sum(lens[i] for i in ids)))
     return sch
@@ -154,10 +161,11 @@ class DecodeLoop:
 
     def __init__(self, w: W.Workload, n_steps: int, n_host_steps: int = 0, device="cuda:0", streams: int = 2,
                  salt: int = 0, bank_bytes: int = 24 << 30, profile: bool = True, options: dict | None = None,
-                 sentinel: int | None = None, fused: bool = True):
+                 sentinel: int | None = None, fused: bool = True, kv_dtype: int = B.KV_DTYPE_BF16):
         """Steps [0, n_steps) take their inputs from device memory; steps [n_steps, n_steps + n_host_steps)
         take them from pinned host memory through the *_host entry points."""
-        self.w, self.dev, self.salt, self.fused = w, torch.device(device), salt, fused
+        self.fp8 = kv_dtype == B.KV_DTYPE_FP8_E4M3
+        self.w, self.dev, self.salt, self.fused = w, torch.device(device), salt, fused and not self.fp8
         self.host_from, self.n_steps = n_steps, n_steps + n_host_steps
         self.two_streams = streams >= 2 and w.ingest_per_step > 0
         L, Hkv, Hq, d, k = w.num_layers, w.num_kv_heads, w.num_q_heads, w.head_dim, w.ingest_per_step
@@ -166,10 +174,10 @@ class DecodeLoop:
         per_step = max(1.0, 2 * self.tok_bytes * mean_len * max(k, 1))
         self.bank_steps = int(min(8, max(2, bank_bytes // per_step))) if k else 0
         self.sched = build_schedule(w, self.n_steps, max(self.bank_steps, 1), salt, self.host_from,
-                                    self.HOST_BANK_STEPS)
+                                    self.HOST_BANK_STEPS, self.fp8)
 
         # ---- pool ----
-        block_bytes = L * Hkv * 2 * w.block_size * d * 2
+        block_bytes = L * w.block_size * kv_token_bytes_layer(w, self.fp8)
         if w.pool_hbm_frac > 0:
             total = torch.cuda.get_device_properties(self.dev).total_memory
             num_blocks = int(total * w.pool_hbm_frac) // block_bytes
@@ -179,7 +187,7 @@ class DecodeLoop:
         self.cfg = B.PoolConfig(num_layers=L, num_q_heads=Hq, num_kv_heads=Hkv, head_dim=d, num_blocks=num_blocks,
                                 max_requests=w.batch + 3 * k + 32,
                                 max_blocks_per_request=(w.max_len + self.n_steps + w.block_size) // w.block_size + 1,
-                                alloc_seed=w.seed + salt)
+                                alloc_seed=w.seed + salt, kv_dtype=kv_dtype)
         self.pool = B.KVPool(self.cfg, device=self.dev)
         if sentinel is not None:
             self.pool.slab[: self.pool.kv_bytes].view(torch.int16).fill_(sentinel)
