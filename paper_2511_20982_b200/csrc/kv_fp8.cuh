@@ -308,14 +308,17 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_fp8_kernel(const AttnPar
         mx1 = fmaxf(mx1, __shfl_xor_sync(kFull, mx1, off));
       }
       const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);   // finite: every tile has >= 1 valid token
+      const bool moved = mn0 != m0 || mn1 != m1;
       const float a0 = fast_exp2(m0 - mn0), a1 = fast_exp2(m1 - mn1);
       m0 = mn0; m1 = mn1;
       const float p0 = fast_exp2(t0 - mn0), p1 = fast_exp2(t1 - mn1);   // p'_t = p_t * vs_t  in (0, 1]
       const float p2 = fast_exp2(t2 - mn0), p3 = fast_exp2(t3 - mn1);
       l0 = l0 * a0 + (p0 * iv0 + p2 * iv1);
       l1 = l1 * a1 + (p1 * iv0 + p3 * iv1);
+      if (__any_sync(kFull, moved)) {                            // the running maximum settles after a few tiles
 #pragma unroll
-      for (int i = 0; i < MT; ++i) { o[i][0] *= a0; o[i][1] *= a1; o[i][2] *= a0; o[i][3] *= a1; }
+        for (int i = 0; i < MT; ++i) { o[i][0] *= a0; o[i][1] *= a1; o[i][2] *= a0; o[i][3] *= a1; }
+      }
       // ---- P'^T as the f16 B fragment (11-bit weights in (0, 1]: 2^-12 relative, below the final bf16 rounding) ----
       const uint32_t b0 = movmatrix_trans(pack_f16x2(p0, p1));  // tokens 2c, 2c+1   of head g
       const uint32_t b1 = movmatrix_trans(pack_f16x2(p2, p3));  // tokens 2c+8, 2c+9 of head g
