@@ -41,6 +41,12 @@ __device__ __forceinline__ uint2 ldg_stream8_pred(const void* ptr, bool pred) {
   return r;
 }
 
+__device__ __forceinline__ uint4 lds128(uint32_t smem_addr) {
+  uint4 r;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(smem_addr));
+  return r;
+}
+
 // two e4m3 codes (low 16 bits / high 16 bits of w) -> f16x2, exact
 __device__ __forceinline__ uint32_t e4m3x2_lo_to_f16x2(uint32_t w) {
   uint32_t d;
@@ -359,6 +365,286 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_fp8_kernel(const AttnPar
         consume(E, v + 3);
       }
     }
+
+    // ---- epilogue: finish l over the token lanes, then store ----
+#pragma unroll
+    for (int off = 4; off < 32; off <<= 1) {
+      l0 += __shfl_xor_sync(kFull, l0, off);
+      l1 += __shfl_xor_sync(kFull, l1, off);
+    }
+#pragma unroll
+    for (int hh = 0; hh < 2; ++hh) {
+      const int head = 2 * c + hh;
+      if (head >= G) continue;
+      const float l = hh ? l1 : l0, m = hh ? m1 : m0;
+      // element e of this lane: d column g * NE + e, register o[e % (NE/2)][2*(e/(NE/2)) + hh]
+      if (pidx < 0) {
+        const float inv = 1.f / l;
+        uint16_t* op = p.out + (static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G + head) * D + g * NE;
+#pragma unroll
+        for (int e = 0; e < NE; e += 8) {
+          uint32_t w[4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const int ea = e + 2 * k, eb2 = ea + 1;
+            w[k] = pack_bf16x2(o[ea % (NE / 2)][2 * (ea / (NE / 2)) + hh] * inv, o[eb2 % (NE / 2)][2 * (eb2 / (NE / 2)) + hh] * inv);
+          }
+          *reinterpret_cast<uint4*>(op + e) = make_uint4(w[0], w[1], w[2], w[3]);
+        }
+      } else {
+        float* po = p.part_o + (static_cast<int64_t>(pidx) * G + head) * D + g * NE;
+#pragma unroll
+        for (int e = 0; e < NE; e += 4) {
+          float f[4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) f[k] = o[(e + k) % (NE / 2)][2 * ((e + k) / (NE / 2)) + hh];
+          *reinterpret_cast<float4*>(po + e) = make_float4(f[0], f[1], f[2], f[3]);
+        }
+        if (g == 0) *reinterpret_cast<float2*>(p.part_ml + (static_cast<int64_t>(pidx) * G + head) * 2) = make_float2(m, l);
+      }
+    }
+    // ---- fused a5: the unit that completes its (request, kv head) merges the partials ----
+    if (pidx >= 0 && p.fuse_combine) {
+      __threadfence();
+      __syncwarp();
+      int last = 0;
+      if (lane == 0) {
+        last = atomicAdd(&p.arrive[pbase], 1) == n_chunks - 1;
+        if (last) p.arrive[pbase] = 0;                           // ready for the next launch
+      }
+      last = __shfl_sync(kFull, last, 0);
+      if (last) {
+        __threadfence();
+        combine_group<D>(p.part_o, p.part_ml, pbase, n_chunks, G,
+                         p.out + (static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G) * D, lane);
+      }
+    }
+    if (lane == 0) item = n_warps + atomicAdd(&p.counters[0], 1);
+    item = __shfl_sync(kFull, item, 0);
+  }
+
+  // Last CTA out rewinds the work counter for the next launch
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const unsigned prev = atomicInc(reinterpret_cast<unsigned*>(&p.counters[1]), gridDim.x - 1);
+    if (prev == gridDim.x - 1) p.counters[0] = 0;
+  }
+}
+
+// Shared-memory ring variant.  ncu on attn_fp8_kernel (profiles/r01) shows what half-size tiles do to the
+// register-direct design: the warp spends as long computing a 4 KiB tile as the memory system needs to
+// deliver it, four tile buffers (144 registers) are all the prefetch depth 254 registers can pay for, and
+// 8 warps per SM cannot cover the rest — 0.88 of the copy ceiling where a load-only version of the same
+// kernel reaches 1.02.  Here the tiles wait in shared memory instead: every warp owns a private ring of R
+// tile slots filled by 16-byte cp.async (zero-filled for rows past the request's end), so the prefetch depth
+// costs no registers, the kernel fits 3 CTAs = 12 warps per SM, and a tile is pulled into fragment
+// registers only when it is consumed.  Slot layout = tile layout with the 16-byte chunks of every 128-byte
+// row XOR-swizzled, chunk' = chunk ^ (row bit 1) << 1 ^ (row bit 2 ^ row bit 0) << 2, which makes both
+// fragment access patterns bank-conflict free: K reads (rows g, g+1 x chunks c + 4j) and V reads
+// (rows 2c + const x chunks g).  No block-wide barrier: a ring is private to its warp (cp.async groups +
+// __syncwarp).
+template <int D>
+__device__ __forceinline__ uint32_t ring_chunk_off(int row, int chunk) {   // byte offset of a 16-byte chunk of a code row
+  if constexpr (D == 128) return row * 128 + ((chunk ^ (((row >> 1) & 1) << 1) ^ ((((row >> 2) ^ row) & 1) << 2)) << 4);
+  else return row * 64 + ((chunk ^ ((row >> 1) & 3)) << 4);               // 4 chunks per row: rows pair up per 128 bytes
+}
+
+template <int D, int R>
+__global__ void __launch_bounds__(kAttnThreads, 3) attn_fp8_ring_kernel(const AttnParams p) {
+  extern __shared__ __align__(128) unsigned char ring_smem[];
+  const uint32_t ring = static_cast<uint32_t>(__cvta_generic_to_shared(ring_smem)) +
+                        (threadIdx.x >> 5) * static_cast<uint32_t>(R * fp8_tile_bytes<D>());
+  constexpr int KS = D / 16;   // MMA k-steps of S^T = K q^T
+  constexpr int MT = D / 16;   // MMA m-tiles of O^T = V^T P^T
+  constexpr int NE = D / 8;    // d columns owned per lane: g * NE + e
+  constexpr int64_t kTile = fp8_tile_bytes<D>();
+  constexpr unsigned kFull = 0xffffffffu;
+  const int lane = threadIdx.x & 31;
+  const int g = lane >> 2, c = lane & 3;
+  const int G = p.group;
+  const int64_t blk_stride = static_cast<int64_t>(p.num_kv_heads) * kTile;
+  const uint8_t* kv8 = reinterpret_cast<const uint8_t*>(p.kv_layer);
+
+  const int n_warps = gridDim.x * kAttnWarps;
+  for (int item = blockIdx.x * kAttnWarps + (threadIdx.x >> 5);;) {
+    if (item >= p.n_units) break;
+    const int h = item % p.num_kv_heads;
+    const int4* wi = reinterpret_cast<const int4*>(p.items) + (item / p.num_kv_heads) * 2;
+    const int4 w0 = __ldg(wi);
+    const int4 w1 = __ldg(wi + 1);
+    const int batch_idx = w0.x, slot = w0.y, blk_begin = w0.z, n_blocks = w0.w;
+    const int n_tokens = w1.x;
+    const int n_chunks = w1.z >> 16, chunk_idx = w1.z & 0xffff;
+    const int pbase = w1.y < 0 ? -1 : w1.y + h * n_chunks;     // first partial slot of (request, kv head)
+    const int pidx = w1.y < 0 ? -1 : pbase + chunk_idx;
+
+    // q^T as f16 B fragments: lane (g, c) holds head g, d columns (c + 4j) * 16 + [0, 16), scaled by a
+    // power of two so that the row maximum lies in [1, 2); cs0 / cs1 give the factor back to the scores
+    uint32_t qf[KS][2];
+    float cs0, cs1;
+    {
+      const bool ok = g < G;
+      const uint16_t* qp = p.q + (static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G + (ok ? g : 0)) * D + c * 16;
+      uint4 raw[D / 64][2];
+      uint32_t mx = 0;
+#pragma unroll
+      for (int j = 0; j < D / 64; ++j)
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          raw[j][k] = ldg_stream_pred(qp + j * 64 + k * 8, ok);
+          mx = __vmaxu2(mx, __vmaxu2(__vmaxu2(raw[j][k].x & 0x7fff7fffu, raw[j][k].y & 0x7fff7fffu),
+                                     __vmaxu2(raw[j][k].z & 0x7fff7fffu, raw[j][k].w & 0x7fff7fffu)));
+        }
+      mx = max(mx & 0xffffu, mx >> 16);
+      mx = max(mx, __shfl_xor_sync(kFull, mx, 1));
+      mx = max(mx, __shfl_xor_sync(kFull, mx, 2));
+      const uint32_t eb = min(max(mx >> 7, 1u), 253u);           // biased exponent of the row maximum
+      const float sf = __uint_as_float((254u - eb) << 23);        // 2^(127 - eb)
+      const float back = __uint_as_float(eb << 23) * p.scale_log2;
+      cs0 = __shfl_sync(kFull, back, (2 * c) * 4);
+      cs1 = __shfl_sync(kFull, back, (2 * c + 1) * 4);
+#pragma unroll
+      for (int j = 0; j < D / 64; ++j)
+#pragma unroll
+        for (int k = 0; k < 2; ++k)
+#pragma unroll
+          for (int w = 0; w < 4; w += 2) {                       // words (w, w+1) = 4 bf16 = one k-step's (b0, b1)
+            const uint32_t e0 = u4_get(raw[j][k], w), e1 = u4_get(raw[j][k], w + 1);
+            qf[4 * j + 2 * k + w / 2][0] = pack_f16x2(__uint_as_float(e0 << 16) * sf, __uint_as_float(e0 & 0xffff0000u) * sf);
+            qf[4 * j + 2 * k + w / 2][1] = pack_f16x2(__uint_as_float(e1 << 16) * sf, __uint_as_float(e1 & 0xffff0000u) * sf);
+          }
+    }
+
+    float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;  // heads 2c, 2c+1 (l: this lane's rows only)
+    float o[MT][4];
+#pragma unroll
+    for (int i = 0; i < MT; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
+
+    const int32_t* bt = p.block_table + static_cast<int64_t>(slot) * p.bt_stride + blk_begin;
+    const uint8_t* kvh = kv8 + static_cast<int64_t>(h) * kTile;
+    int32_t ids = lane < n_blocks ? __ldg(bt + lane) : 0;       // physical ids of blocks [32k, 32k+32)
+    int32_t ids_next = 0;
+
+    // start the copies of tile t into ring slot t % R (one cp.async group per tile, empty past the unit's end)
+    auto issue = [&](int t) {
+      if (t < n_blocks) {
+        if ((t & 31) == 0 && t > 0) ids = ids_next;
+        if ((t & 31) == 8 && t + 24 + lane < n_blocks) ids_next = __ldg(bt + t + 24 + lane);
+        const int blk = __shfl_sync(kFull, ids, t & 31);
+        const uint8_t* tile = kvh + blk * blk_stride;
+        const uint32_t slot = ring + (t % R) * static_cast<uint32_t>(kTile);
+        const int nv = n_tokens - t * kBlockSize;
+        constexpr int kChunksPerRow = D / 16;
+#pragma unroll
+        for (int i = 0; i < 2 * kBlockSize * kChunksPerRow / 32; ++i) {          // the K8 | V8 code rows
+          const int idx = lane + 32 * i, row32 = idx / kChunksPerRow, ch = idx % kChunksPerRow;
+          const int row = row32 & (kBlockSize - 1);
+          const uint32_t dst = slot + (row32 >> 4) * (kBlockSize * D) + ring_chunk_off<D>(row, ch);
+          const int sz = row < nv ? 16 : 0;                                      // zero-fill rows past the end
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(tile + idx * 16), "r"(sz) : "memory");
+        }
+        if (lane < 8) {                                                           // sc[16] {ks, vs}: 8 chunks of 2 rows
+          const int sz = 2 * lane < nv ? (2 * lane + 1 < nv ? 16 : 8) : 0;
+          asm volatile("cp.async.ca.shared.global [%0], [%1], 16, %2;" ::"r"(slot + 2 * kBlockSize * D + lane * 16),
+                       "l"(tile + 2 * kBlockSize * D + lane * 16), "r"(sz) : "memory");
+        }
+      }
+      asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    auto consume = [&](int t) {
+      KV8Tile<D> T;                                              // fragments of ring slot t % R
+      {
+        const uint32_t slot = ring + (t % R) * static_cast<uint32_t>(kTile);
+#pragma unroll
+        for (int rs = 0; rs < 2; ++rs) {
+          const int row = g + 8 * rs;
+#pragma unroll
+          for (int j = 0; j < D / 64; ++j) T.k[rs][j] = lds128(slot + ring_chunk_off<D>(row, c + 4 * j));
+          asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(T.sc[rs].x), "=f"(T.sc[rs].y) : "r"(slot + 2 * kBlockSize * D + row * 8));
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int row = 2 * c + (i & 1) + 8 * (i >> 1);
+          if constexpr (D == 128) {
+            const uint4 x = lds128(slot + kBlockSize * D + ring_chunk_off<D>(row, g));
+            T.v[i][0] = x.x; T.v[i][1] = x.y; T.v[i][2] = x.z; T.v[i][3] = x.w;
+          } else {
+            asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(T.v[i][0]), "=r"(T.v[i][1])
+                         : "r"(slot + kBlockSize * D + ring_chunk_off<D>(row, g >> 1) + (g & 1) * 8));
+          }
+        }
+      }
+      // ---- S^T = K8 q~^T : word w of vector j feeds k-step 4j + w; two accumulation chains ----
+      float sa[4] = {0.f, 0.f, 0.f, 0.f}, sb[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int j = 0; j < D / 64; ++j)
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+          const uint32_t r0 = u4_get(T.k[0][j], w), r1 = u4_get(T.k[1][j], w);
+          mma_f16_m16n8k16((w & 1) ? sb : sa, e4m3x2_lo_to_f16x2(r0), e4m3x2_lo_to_f16x2(r1), e4m3x2_hi_to_f16x2(r0),
+                           e4m3x2_hi_to_f16x2(r1), qf[4 * j + w][0], qf[4 * j + w][1]);
+        }
+      // s[0], s[1]: token g, heads 2c, 2c+1;  s[2], s[3]: token g+8   (log2 units)
+      float s[4];
+      s[0] = (sa[0] + sb[0]) * (T.sc[0].x * cs0);
+      s[1] = (sa[1] + sb[1]) * (T.sc[0].x * cs1);
+      s[2] = (sa[2] + sb[2]) * (T.sc[1].x * cs0);
+      s[3] = (sa[3] + sb[3]) * (T.sc[1].x * cs1);
+      const int nv = n_tokens - t * kBlockSize;
+      const bool ok0 = g < nv, ok1 = g + 8 < nv;                 // ragged last block: mask by index, not value
+      // ---- online softmax with the V scale folded into the reference: t = s + log2(vs) ----
+      const float lv0 = ok0 ? fast_log2(T.sc[0].y) : -INFINITY, lv1 = ok1 ? fast_log2(T.sc[1].y) : -INFINITY;
+      const float iv0 = ok0 ? __frcp_rn(T.sc[0].y) : 0.f, iv1 = ok1 ? __frcp_rn(T.sc[1].y) : 0.f;
+      const float t0 = s[0] + lv0, t1 = s[1] + lv0, t2 = s[2] + lv1, t3 = s[3] + lv1;
+      float mx0 = fmaxf(t0, t2), mx1 = fmaxf(t1, t3);
+#pragma unroll
+      for (int off = 4; off < 32; off <<= 1) {
+        mx0 = fmaxf(mx0, __shfl_xor_sync(kFull, mx0, off));
+        mx1 = fmaxf(mx1, __shfl_xor_sync(kFull, mx1, off));
+      }
+      const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);   // finite: every tile has >= 1 valid token
+      const bool moved = mn0 != m0 || mn1 != m1;
+      const float a0 = fast_exp2(m0 - mn0), a1 = fast_exp2(m1 - mn1);
+      m0 = mn0; m1 = mn1;
+      const float p0 = fast_exp2(t0 - mn0), p1 = fast_exp2(t1 - mn1);   // p'_t = p_t * vs_t  in (0, 1]
+      const float p2 = fast_exp2(t2 - mn0), p3 = fast_exp2(t3 - mn1);
+      l0 = l0 * a0 + (p0 * iv0 + p2 * iv1);
+      l1 = l1 * a1 + (p1 * iv0 + p3 * iv1);
+      if (__any_sync(kFull, moved)) {                            // the running maximum settles after a few tiles
+#pragma unroll
+        for (int i = 0; i < MT; ++i) { o[i][0] *= a0; o[i][1] *= a1; o[i][2] *= a0; o[i][3] *= a1; }
+      }
+      // ---- P'^T as the f16 B fragment (11-bit weights in (0, 1]: 2^-12 relative, below the final bf16 rounding) ----
+      const uint32_t b0 = movmatrix_trans(pack_f16x2(p0, p1));  // tokens 2c, 2c+1   of head g
+      const uint32_t b1 = movmatrix_trans(pack_f16x2(p2, p3));  // tokens 2c+8, 2c+9 of head g
+      // ---- O^T += V8^T P'^T : m-tile i takes the lane's column e = i (row g) and e = i + NE/2 (row g+8);
+      // one PRMT pairs the codes of two tokens for two neighbouring columns, one F2FP per pair ----
+#pragma unroll
+      for (int i = 0; i < MT; i += 2) {                          // columns (i, i+1) and (i + NE/2, i + 1 + NE/2)
+        const int e1 = i, e2 = i + NE / 2;
+        const uint32_t sel = (e1 & 2) ? 0x7362u : 0x5140u;      // bytes (b, b+1) of both rows: [A.b, B.b, A.b+1, B.b+1]
+        const uint32_t x01 = __byte_perm(T.v[0][e1 >> 2], T.v[1][e1 >> 2], sel);   // tokens 2c, 2c+1; columns e1, e1+1
+        const uint32_t x23 = __byte_perm(T.v[2][e1 >> 2], T.v[3][e1 >> 2], sel);   // tokens 2c+8, 2c+9
+        const uint32_t y01 = __byte_perm(T.v[0][e2 >> 2], T.v[1][e2 >> 2], sel);   // columns e2, e2+1
+        const uint32_t y23 = __byte_perm(T.v[2][e2 >> 2], T.v[3][e2 >> 2], sel);
+        mma_f16_m16n8k16(o[i], e4m3x2_lo_to_f16x2(x01), e4m3x2_lo_to_f16x2(y01), e4m3x2_lo_to_f16x2(x23),
+                         e4m3x2_lo_to_f16x2(y23), b0, b1);
+        mma_f16_m16n8k16(o[i + 1], e4m3x2_hi_to_f16x2(x01), e4m3x2_hi_to_f16x2(y01), e4m3x2_hi_to_f16x2(x23),
+                         e4m3x2_hi_to_f16x2(y23), b0, b1);
+      }
+    };
+
+#pragma unroll
+    for (int t = 0; t < R - 1; ++t) issue(t);                    // R - 1 tiles ahead
+    for (int t = 0; t < n_blocks; ++t) {
+      asm volatile("cp.async.wait_group %0;" ::"n"(R - 2) : "memory");   // tile t has landed (this lane's copies)
+      __syncwarp();                                              // ... everyone's; and slot (t - 1) % R is free
+      issue(t + R - 1);
+      consume(t);
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncwarp();
 
     // ---- epilogue: finish l over the token lanes, then store ----
 #pragma unroll

@@ -193,6 +193,8 @@ struct kv_pool {
   int32_t ctas_per_sm = 2;
   int32_t items_per_slot = 2;     // guided chunking: first chunk = remaining work / (2 x resident warps)
   bool fuse_combine = true;
+  bool fp8_ring = true;           // FP8 pool: attn_fp8_ring_kernel (shared-memory tile ring) vs attn_fp8_kernel (register tiles)
+  bool fp8_ring_ready = false;    // dynamic shared-memory attribute set
   bool profile = false;
   ProfRing prof[KV_KERNEL_KINDS];
   // staging
@@ -215,7 +217,10 @@ struct kv_pool {
     last_cuda = static_cast<int32_t>(e);
     return KV_ERR_CUDA;
   }
-  int32_t slots() const { return num_sms * ctas_per_sm * kvp::kAttnWarps; }
+  int32_t slots() const {
+    const int32_t ctas = (hs.cfg.kv_dtype == KV_DTYPE_FP8_E4M3 && fp8_ring) ? 3 : ctas_per_sm;
+    return num_sms * ctas * kvp::kAttnWarps;
+  }
 };
 
 namespace {
@@ -577,7 +582,20 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, c
   const int32_t want = (p.n_units + kAttnWarps - 1) / kAttnWarps;
   const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * pool->ctas_per_sm)));
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_ATTN].begin(stream));
-  if (c.kv_dtype == KV_DTYPE_FP8_E4M3) {
+  if (c.kv_dtype == KV_DTYPE_FP8_E4M3 && pool->fp8_ring) {
+    constexpr int kR = 4;                                        // ring slots per warp
+    const size_t smem = static_cast<size_t>(kAttnWarps) * kR * (32 * c.head_dim + 128);
+    if (!pool->fp8_ring_ready) {
+      KV_CUDA(pool, cudaFuncSetAttribute(attn_fp8_ring_kernel<128, kR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         kAttnWarps * kR * (32 * 128 + 128)));
+      KV_CUDA(pool, cudaFuncSetAttribute(attn_fp8_ring_kernel<64, kR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         kAttnWarps * kR * (32 * 64 + 128)));
+      pool->fp8_ring_ready = true;
+    }
+    const unsigned rgrid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * 3)));
+    if (c.head_dim == 128) attn_fp8_ring_kernel<128, kR><<<rgrid, kAttnThreads, smem, stream>>>(p);
+    else attn_fp8_ring_kernel<64, kR><<<rgrid, kAttnThreads, smem, stream>>>(p);
+  } else if (c.kv_dtype == KV_DTYPE_FP8_E4M3) {
     if (c.head_dim == 128) attn_fp8_kernel<128><<<grid, kAttnThreads, 0, stream>>>(p);
     else attn_fp8_kernel<64><<<grid, kAttnThreads, 0, stream>>>(p);
   } else if (c.head_dim == 128) {
@@ -829,6 +847,7 @@ int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
   if (!std::strcmp(key, "items_per_slot") && value >= 1 && value <= 1024) { pool->items_per_slot = static_cast<int32_t>(value); return KV_OK; }
   if (!std::strcmp(key, "profile") && (value == 0 || value == 1)) { pool->profile = value != 0; return KV_OK; }
   if (!std::strcmp(key, "fuse_combine") && (value == 0 || value == 1)) { pool->fuse_combine = value != 0; return KV_OK; }
+  if (!std::strcmp(key, "fp8_ring") && (value == 0 || value == 1)) { pool->fp8_ring = value != 0; return KV_OK; }
   return KV_ERR_INVALID;
 }
 
