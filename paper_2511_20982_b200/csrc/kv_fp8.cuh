@@ -92,14 +92,19 @@ template <int D>
 __host__ __device__ constexpr int64_t fp8_tile_bytes() { return 32 * D + 128; }
 
 // ---------------------------------------------------------------------------------------------
-// quantising scatter: same units, same descriptors as ingest_kernel (IngestParams::kv = the FP8 region)
+// quantising scatter: same units, same descriptors as ingest_kernel (IngestParams::kv = the FP8 region),
+// but one warp per (unit, K|V): the quantisation arithmetic sits between a warp's loads and its stores,
+// so the kernel wants many light warps (4 KiB in flight each, ~50 registers) rather than few heavy ones.
+// Launch with 2 * total_units warps.
 // ---------------------------------------------------------------------------------------------
 template <int D>
 __global__ void __launch_bounds__(kIngestThreads) ingest_fp8_kernel(const IngestParams p) {
   constexpr int kPiecesPerRow = D / 8;                          // 16-byte source pieces (8 bf16) per token row
   constexpr int kMaxPerLane = kBlockSize * kPiecesPerRow / 32;  // 8 at D=128, 4 at D=64
   const int lane = threadIdx.x & 31;
-  const int64_t u = static_cast<int64_t>(blockIdx.x) * kIngestWarps + (threadIdx.x >> 5);
+  const int64_t u2 = static_cast<int64_t>(blockIdx.x) * kIngestWarps + (threadIdx.x >> 5);
+  const int64_t u = u2 >> 1;
+  const int c = static_cast<int>(u2 & 1);                        // 0: the K rows of the unit, 1: the V rows
   if (u >= p.total_units) return;
 
   int lo = 0, hi = p.n_req - 1;                                 // request of this unit: last i with unit_begin <= u
@@ -121,49 +126,40 @@ __global__ void __launch_bounds__(kIngestThreads) ingest_fp8_kernel(const Ingest
   const int pieces = (row1 - row0) * kPiecesPerRow;
 
   const int64_t src_off = ((static_cast<int64_t>(ll) * p.num_kv_heads + h) * r.n_tokens + t0) * D;
-  const uint4* lin_k = reinterpret_cast<const uint4*>(reinterpret_cast<const uint16_t*>(r.k_src) + src_off);
-  const uint4* lin_v = reinterpret_cast<const uint4*>(reinterpret_cast<const uint16_t*>(r.v_src) + src_off);
+  const uint4* lin = reinterpret_cast<const uint4*>(reinterpret_cast<const uint16_t*>(c ? r.v_src : r.k_src) + src_off);
   uint8_t* tile = reinterpret_cast<uint8_t*>(p.kv) +
                   ((static_cast<int64_t>(p.layer_begin + ll) * p.num_blocks + blk) * p.num_kv_heads + h) * fp8_tile_bytes<D>();
 
-  uint4 bk[kMaxPerLane], bv[kMaxPerLane];
+  uint4 buf[kMaxPerLane];
 #pragma unroll
-  for (int i = 0; i < kMaxPerLane; ++i) {                       // all loads first
-    const int idx = lane + 32 * i;
-    const bool ok = idx < pieces;
-    bk[i] = ldg_copy_pred(lin_k + idx, ok);
-    bv[i] = ldg_copy_pred(lin_v + idx, ok);
-  }
+  for (int i = 0; i < kMaxPerLane; ++i) buf[i] = ldg_copy_pred(lin + lane + 32 * i, lane + 32 * i < pieces);   // all loads first
 #pragma unroll
   for (int i = 0; i < kMaxPerLane; ++i) {
     const int idx = lane + 32 * i;
     const bool ok = idx < pieces;
     const int row = row0 + idx / kPiecesPerRow, cp = idx % kPiecesPerRow;
+    const uint4 x = buf[i];
+    // row amax: bf16 magnitudes compare like unsigned integers
+    uint32_t mx = __vmaxu2(__vmaxu2(x.x & 0x7fff7fffu, x.y & 0x7fff7fffu), __vmaxu2(x.z & 0x7fff7fffu, x.w & 0x7fff7fffu));
+    mx = max(mx & 0xffffu, mx >> 16);
 #pragma unroll
-    for (int c = 0; c < 2; ++c) {
-      const uint4 x = c ? bv[i] : bk[i];
-      // row amax: bf16 magnitudes compare like unsigned integers
-      uint32_t mx = __vmaxu2(__vmaxu2(x.x & 0x7fff7fffu, x.y & 0x7fff7fffu), __vmaxu2(x.z & 0x7fff7fffu, x.w & 0x7fff7fffu));
-      mx = max(mx & 0xffffu, mx >> 16);
+    for (int off = kPiecesPerRow / 2; off > 0; off >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, off));
+    const float amax = __uint_as_float(mx << 16);
+    const float scale = mx == 0 ? 1.f : __fdiv_rn(amax, 448.f);
+    const float inv = mx == 0 ? 1.f : __fdiv_rn(448.f, amax);
+    uint32_t w[4];
 #pragma unroll
-      for (int off = kPiecesPerRow / 2; off > 0; off >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, off));
-      const float amax = __uint_as_float(mx << 16);
-      const float scale = mx == 0 ? 1.f : __fdiv_rn(amax, 448.f);
-      const float inv = mx == 0 ? 1.f : __fdiv_rn(448.f, amax);
-      uint32_t w[4];
-#pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        const uint32_t e = u4_get(x, k);
-        w[k] = f32x2_to_e4m3x2(__fmul_rn(__uint_as_float(e << 16), inv), __fmul_rn(__uint_as_float(e & 0xffff0000u), inv));
-      }
-      if (ok) {
-        uint8_t* dst = tile + c * (kBlockSize * D) + row * D + cp * 8;
-        *reinterpret_cast<uint2*>(dst) = make_uint2(w[0] | (w[1] << 16), w[2] | (w[3] << 16));
-        if (cp == 0) *reinterpret_cast<float*>(tile + 2 * kBlockSize * D + row * 8 + c * 4) = scale;
-      }
+    for (int k = 0; k < 4; ++k) {
+      const uint32_t e = u4_get(x, k);
+      w[k] = f32x2_to_e4m3x2(__fmul_rn(__uint_as_float(e << 16), inv), __fmul_rn(__uint_as_float(e & 0xffff0000u), inv));
+    }
+    if (ok) {
+      uint8_t* dst = tile + c * (kBlockSize * D) + row * D + cp * 8;
+      *reinterpret_cast<uint2*>(dst) = make_uint2(w[0] | (w[1] << 16), w[2] | (w[3] << 16));
+      if (cp == 0) *reinterpret_cast<float*>(tile + 2 * kBlockSize * D + row * 8 + c * 4) = scale;
     }
   }
-  if (ll == 0 && h == 0 && lane == 0)                           // device block_table mirror (a1, device half)
+  if (c == 0 && ll == 0 && h == 0 && lane == 0)                 // device block_table mirror (a1, device half)
     p.block_table[static_cast<int64_t>(r.slot) * p.bt_stride + lb] = blk;
 }
 

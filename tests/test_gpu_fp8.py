@@ -19,7 +19,8 @@ from helpers import bf16_bits, bits_of, bits_to_f64
 pytestmark = pytest.mark.gpu
 
 MODES = [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=1024),
-         dict(min_chunk_blocks=2, items_per_slot=2, fuse_combine=0), dict(min_chunk_blocks=5, items_per_slot=1, ctas_per_sm=1)]
+         dict(min_chunk_blocks=2, items_per_slot=2, fuse_combine=0), dict(min_chunk_blocks=5, items_per_slot=1, ctas_per_sm=1),
+         dict(fp8_ring=0), dict(fp8_ring=0, min_chunk_blocks=2, items_per_slot=1024)]
 SENT = 0xFF   # e4m3 NaN code / NaN scale bytes: an unmasked read poisons the output
 
 
