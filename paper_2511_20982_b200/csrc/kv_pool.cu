@@ -13,6 +13,7 @@
 #include "kv_host.h"
 #include "kv_kernels.cuh"
 #include "kv_fp8.cuh"
+#include "kv_attn_ring.cuh"
 
 namespace {
 
@@ -194,6 +195,7 @@ struct kv_pool {
   int32_t items_per_slot = 2;     // guided chunking: first chunk = remaining work / (2 x resident warps)
   bool items_per_slot_set = false;  // FP8 ring kernel (12 warps per SM): 1 measured best unless the caller chose
   bool fuse_combine = true;
+  int32_t ring = 3;               // bf16 pool: 3 (default) / 2: attn_ring_kernel with that many slots per warp (2 / 3 CTAs per SM); 0: register-tile attn_splitkv_kernel
   bool fp8_ring = true;           // FP8 pool: attn_fp8_ring_kernel (shared-memory tile ring) vs attn_fp8_kernel (register tiles)
   bool fp8_ring_ready = false;    // dynamic shared-memory attribute set
   bool profile = false;
@@ -219,7 +221,8 @@ struct kv_pool {
     return KV_ERR_CUDA;
   }
   int32_t slots() const {
-    const int32_t ctas = (hs.cfg.kv_dtype == KV_DTYPE_FP8_E4M3 && fp8_ring) ? 3 : ctas_per_sm;
+    const int32_t ctas = (hs.cfg.kv_dtype == KV_DTYPE_FP8_E4M3 && fp8_ring) ? 3
+                         : (hs.cfg.kv_dtype == KV_DTYPE_BF16 && ring == 2) ? 3 : ctas_per_sm;
     return num_sms * ctas * kvp::kAttnWarps;
   }
   int32_t ips() const {
@@ -343,6 +346,32 @@ int32_t run_ingest(kv_pool* pool, int32_t n_req, const int64_t* req_ids, const i
     units += static_cast<int64_t>(touched) * layer_count * c.num_kv_heads;
   }
   return flush();
+}
+
+// attn_ring_kernel launch: R slots per warp, kCtas CTAs per SM; dynamic shared memory above 48 KiB needs the opt-in.
+template <int D, bool kAppend, bool kVarQ, int R, int kCtas>
+static cudaError_t launch_ring(const AttnParams& p, int num_sms, int want, cudaStream_t stream) {
+  static bool ready = false;
+  constexpr size_t smem = static_cast<size_t>(kAttnWarps) * R * (2 * kBlockSize * D * 2);
+  if (!ready) {
+    cudaError_t e = cudaFuncSetAttribute(attn_ring_kernel<D, kAppend, kVarQ, R, kCtas>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    if (e != cudaSuccess) return e;
+    ready = true;
+  }
+  const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, num_sms * kCtas)));
+  attn_ring_kernel<D, kAppend, kVarQ, R, kCtas><<<grid, kAttnThreads, smem, stream>>>(p);
+  return cudaGetLastError();
+}
+
+template <bool kAppend, bool kVarQ>
+static cudaError_t launch_ring_any(int head_dim, int ring, const AttnParams& p, int num_sms, int want, cudaStream_t stream) {
+  if (head_dim == 128) {
+    if (ring == 2) return launch_ring<128, kAppend, kVarQ, 2, 3>(p, num_sms, want, stream);
+    return launch_ring<128, kAppend, kVarQ, 3, 2>(p, num_sms, want, stream);
+  }
+  if (ring == 2) return launch_ring<64, kAppend, kVarQ, 2, 3>(p, num_sms, want, stream);
+  return launch_ring<64, kAppend, kVarQ, 3, 2>(p, num_sms, want, stream);
 }
 
 }  // namespace
@@ -603,6 +632,10 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, c
   } else if (c.kv_dtype == KV_DTYPE_FP8_E4M3) {
     if (c.head_dim == 128) attn_fp8_kernel<128><<<grid, kAttnThreads, 0, stream>>>(p);
     else attn_fp8_kernel<64><<<grid, kAttnThreads, 0, stream>>>(p);
+  } else if (pool->ring) {
+    const cudaError_t re = k_new ? launch_ring_any<true, false>(c.head_dim, pool->ring, p, pool->num_sms, want, stream)
+                                 : launch_ring_any<false, false>(c.head_dim, pool->ring, p, pool->num_sms, want, stream);
+    KV_CUDA(pool, re);
   } else if (c.head_dim == 128) {
     if (k_new) attn_splitkv_kernel<128, true><<<grid, kAttnThreads, 0, stream>>>(p);
     else attn_splitkv_kernel<128, false><<<grid, kAttnThreads, 0, stream>>>(p);
@@ -699,7 +732,10 @@ int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
   const int32_t want = (p.n_units + kAttnWarps - 1) / kAttnWarps;
   const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * pool->ctas_per_sm)));
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_VARQ].begin(stream));
-  if (c.head_dim == 128)
+  if (pool->ring) {
+    const cudaError_t re = launch_ring_any<false, true>(c.head_dim, pool->ring, p, pool->num_sms, want, stream);
+    KV_CUDA(pool, re);
+  } else if (c.head_dim == 128)
     attn_splitkv_kernel<128, false, true><<<grid, kAttnThreads, 0, stream>>>(p);
   else
     attn_splitkv_kernel<64, false, true><<<grid, kAttnThreads, 0, stream>>>(p);
@@ -852,6 +888,7 @@ int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
   if (!std::strcmp(key, "items_per_slot") && value >= 1 && value <= 1024) { pool->items_per_slot = static_cast<int32_t>(value); pool->items_per_slot_set = true; return KV_OK; }
   if (!std::strcmp(key, "profile") && (value == 0 || value == 1)) { pool->profile = value != 0; return KV_OK; }
   if (!std::strcmp(key, "fuse_combine") && (value == 0 || value == 1)) { pool->fuse_combine = value != 0; return KV_OK; }
+  if (!std::strcmp(key, "ring") && (value == 0 || value == 2 || value == 3)) { pool->ring = static_cast<int32_t>(value); return KV_OK; }
   if (!std::strcmp(key, "fp8_ring") && (value == 0 || value == 1)) { pool->fp8_ring = value != 0; return KV_OK; }
   return KV_ERR_INVALID;
 }
