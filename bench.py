@@ -13,7 +13,7 @@ every layer append the new token's K/V and run paged decode attention + LSE comb
   e2e       the same metric through the host-buffer C-ABI calls (kv_ingest_host,
             paged_decode_attention_host): every step's q, appended K/V and arriving requests' K/V
             come from pinned host memory and the outputs go back to it, inside the timed region
-  roofline  attn_splitkv_kernel: algorithmic bytes per launch / mean launch duration (CUDA event
+  roofline  the attention kernel (attn_ring_kernel): algorithmic bytes per launch / mean launch duration (CUDA event
             pairs recorded by the library around every launch of the timed region)
   cpu_baseline  the fp64 oracle timed on this box's host cores on a bounded sample
 
@@ -38,11 +38,11 @@ if ROOT not in sys.path:
 METRIC = "decode-attn + KV-ingest HBM GB/s"
 NOMINAL_HBM_GBS = 8000.0          # BASELINE.json north_star: "B200 HBM peak (~8 TB/s)"
 FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
-# DRAM bytes per algorithmic byte of attn_splitkv_kernel, from the `ncu --set full` captures summarised in
+# DRAM bytes per algorithmic byte of attn_ring_kernel, from the `ncu --set full` captures summarised in
 # profiles/README.md (dram__bytes_read.sum + dram__bytes_write.sum of one launch / that launch's algorithmic bytes).
 # The roofline's `traffic` is this ratio x the timed run's algorithmic bytes per launch.
-NCU_TRAFFIC_RATIO = {"cfg2_7b_mha": (1.0045, "profiles/r01 attn_cfg2"), "cfg3_8b_gqa": (1.0195, "profiles/r01 attn_cfg3"),
-                     "cfg4_70b_long": (1.0011, "profiles/r01 attn_cfg4")}
+NCU_TRAFFIC_RATIO = {"cfg2_7b_mha": (1.0058, "profiles/r01 attn_ring_cfg2"), "cfg3_8b_gqa": (1.0110, "profiles/r01 attn_ring_cfg3"),
+                     "cfg4_70b_long": (1.0073, "profiles/r01 attn_ring_cfg4")}
 DEFAULT_WORKLOAD = "cfg3_8b_gqa"  # first BASELINE.json config with both legs of the metric
 
 
@@ -333,17 +333,19 @@ def run_cuda(args):
     ing_n, ing_ms = prof["ingest"]
     attn_bytes_per_launch = by["attn"] / max(attn_n, 1)
     achieved = attn_bytes_per_launch / (attn_ms / max(attn_n, 1) * 1e-3) / 1e9 if attn_ms > 0 else None
-    roofline = {"kernel": "attn_fp8_kernel" if fp8 else "attn_splitkv_kernel", "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    ring = opts.get("fp8_ring", 1) if fp8 else opts.get("ring", 3)
+    attn_kernel = ("attn_fp8_ring_kernel" if ring else "attn_fp8_kernel") if fp8 else ("attn_ring_kernel" if ring else "attn_splitkv_kernel")
+    roofline = {"kernel": attn_kernel, "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak if achieved else None, "peak_source": peak_src,
                 "frac_of_nominal_8000": achieved / NOMINAL_HBM_GBS if achieved else None,
                 "launches": attn_n, "avg_launch_us": attn_ms / max(attn_n, 1) * 1e3,
                 "algorithmic_bytes_per_launch": attn_bytes_per_launch, "traffic": None}
-    if args.workload in NCU_TRAFFIC_RATIO and not fp8:
+    if args.workload in NCU_TRAFFIC_RATIO and not fp8 and ring == 3:
         ratio, src = NCU_TRAFFIC_RATIO[args.workload]
         roofline.update({"traffic": attn_bytes_per_launch * ratio, "traffic_source": f"ncu --set full, {src}: "
                          f"DRAM bytes = {ratio:.4f} x algorithmic bytes"})
     kernels = {
-        "attn_splitkv_kernel": {"launches": attn_n, "ms": attn_ms},
+        attn_kernel: {"launches": attn_n, "ms": attn_ms},
         "combine_kernel": {"launches": comb_n, "ms": comb_ms},
         "ingest_kernel": {"launches": ing_n, "ms": ing_ms,
                           "gbs": (by["ingest"] + (0 if loop.fused else by["append"])) / (ing_ms * 1e-3) / 1e9
