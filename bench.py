@@ -536,8 +536,12 @@ def varlen_leg(loop, last_step: int, peak: float, reps: int = 5):
     want = oracle.attention_varq(slab, dims, 0, Hq, lists, plen, plen, bits(q[layer, len(sp.batch):]))
     got = (bits(out[layer, len(sp.batch):]).astype(np.uint32) << 16).view(np.float32).astype(np.float64)
     err = np.abs(got - want)
+    # a fresh prefill row sees 1, 2, 3, ... tokens: its output is (nearly) a V row, |x| up to ~4.5 for N(0,1) values, and
+    # the final bf16 rounding alone is then up to 2^-8 |x| = 0.0176 > 1e-2.  The absolute bar applies beyond that rounding.
+    beyond = np.maximum(err - np.abs(want) * 2.0 ** -8, 0.0)
     res["varlen_parity"] = {"rows": int(plen.sum()), "max_abs_err": float(err.max()), "mean_abs_err": float(err.mean()),
-                            "pass": bool(err.max() <= 1e-2 and err.mean() <= 1e-3)}
+                            "max_abs_err_beyond_bf16_rounding_of_the_element": float(beyond.max()),
+                            "pass": bool(float(np.max(err - np.maximum(1e-2, np.abs(want) * 2.0 ** -8))) <= 0 and err.mean() <= 1e-3)}
     # decode rows must agree with the decode call's output of the same batch (computed by the attention-alone leg)
     same = torch.equal(out[layer, : len(sp.batch)].view(torch.int16), loop.out[last_step][layer].view(torch.int16))
     dmax = float((out[layer, : len(sp.batch)].float() - loop.out[last_step][layer].float()).abs().max())
