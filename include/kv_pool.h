@@ -27,7 +27,8 @@
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All
  *     GPU work of a call is enqueued on it and the call returns without synchronising;
  *     source buffers may be released once the stream has passed the call.
- *   - bf16 = IEEE bfloat16 bit patterns (uint16_t).  No other KV dtype in this version.
+ *   - bf16 = IEEE bfloat16 bit patterns (uint16_t).  Sources, queries and outputs are always bf16;
+ *     the pool is bf16 or, with kv_dtype = KV_DTYPE_FP8_E4M3, e4m3 codes + scales (see below).
  *   - One host thread per pool.  Pools are independent.
  *
  * Slab layout (caller-visible so that an independent checker can read the pool).
@@ -108,9 +109,10 @@ typedef struct kv_pool_config {
  * values.  KV region layout, one tile of 32*head_dim + 128 bytes per (layer, block, kv_head), tiles
  * ordered [layer][block][kv_head]:
  *     K8[16][head_dim] codes | V8[16][head_dim] codes | sc[16][2] fp32 = (k scale, v scale) of slot t
- * Available on an FP8 pool: kv_reserve, kv_ingest(_host), paged_decode_attention(_host), kv_free and
- * the introspection / profiling calls.  paged_decode_step(_host), paged_varlen_attention and kv_gather
- * return KV_ERR_UNSUPPORTED (the decode loop appends with kv_ingest, n_tokens = 1).
+ * Available on an FP8 pool: kv_reserve, kv_ingest(_host), paged_decode_attention(_host),
+ * paged_decode_step(_host) (the fused append quantises the new row exactly as kv_ingest does: same
+ * bytes), kv_free and the introspection / profiling calls.  paged_varlen_attention and kv_gather
+ * return KV_ERR_UNSUPPORTED.
  */
 
 /* Bytes of the KV region / of the whole slab (KV region + private metadata) for `cfg`

@@ -445,7 +445,7 @@ __device__ __forceinline__ uint32_t ring_chunk_off(int row, int chunk) {   // by
   else return row * 64 + ((chunk ^ ((row >> 1) & 3)) << 4);               // 4 chunks per row: rows pair up per 128 bytes
 }
 
-template <int D, int R>
+template <int D, int R, bool kAppend>
 __global__ void __launch_bounds__(kAttnThreads, 3) attn_fp8_ring_kernel(const AttnParams p) {
   extern __shared__ __align__(128) unsigned char ring_smem[];
   const uint32_t ring = static_cast<uint32_t>(__cvta_generic_to_shared(ring_smem)) +
@@ -473,6 +473,14 @@ __global__ void __launch_bounds__(kAttnThreads, 3) attn_fp8_ring_kernel(const At
     const int n_chunks = w1.z >> 16, chunk_idx = w1.z & 0xffff;
     const int pbase = w1.y < 0 ? -1 : w1.y + h * n_chunks;     // first partial slot of (request, kv head)
     const int pidx = w1.y < 0 ? -1 : pbase + chunk_idx;
+    // Fused append (a3 inside a4): the unit that owns the request's last block takes that tile FIRST; the new
+    // token's K / V rows are quantised here exactly as ingest_fp8_kernel does (same fp32 roundings, same codes),
+    // written into the pool, and patched into the ring slot once the tile's stale bytes have landed.
+    const bool special = kAppend && chunk_idx == n_chunks - 1;
+    const int sp = special ? 1 : 0;
+    const int last_blk = w1.w;
+    uint2 new_codes = make_uint2(0u, 0u);
+    float new_scale = 0.f;
 
     // q^T as f16 B fragments: lane (g, c) holds head g, d columns (c + 4j) * 16 + [0, 16), scaled by a
     // power of two so that the row maximum lies in [1, 2); cs0 / cs1 give the factor back to the scores
@@ -522,36 +530,85 @@ __global__ void __launch_bounds__(kAttnThreads, 3) attn_fp8_ring_kernel(const At
     int32_t ids_next = 0;
 
     // start the copies of tile t into ring slot t % R (one cp.async group per tile, empty past the unit's end)
-    auto issue = [&](int t) {
-      if (t < n_blocks) {
-        if ((t & 31) == 0 && t > 0) ids = ids_next;
-        if ((t & 31) == 8 && t + 24 + lane < n_blocks) ids_next = __ldg(bt + t + 24 + lane);
-        const int blk = __shfl_sync(kFull, ids, t & 31);
-        const uint8_t* tile = kvh + blk * blk_stride;
-        const uint32_t slot = ring + (t % R) * static_cast<uint32_t>(kTile);
+    // virtual tile v -> real tile: special ? (v == 0 ? n_blocks - 1 : v - 1) : v
+    auto issue = [&](int v) {
+      if (v < n_blocks) {
+        const bool first_special = special && v == 0;
+        const int t = first_special ? n_blocks - 1 : v - sp;
+        const uint8_t* tile;
+        if (first_special) {
+          tile = kvh + last_blk * blk_stride;
+        } else {
+          if ((t & 31) == 0 && t > 0) ids = ids_next;
+          if ((t & 31) == 8 && t + 24 + lane < n_blocks) ids_next = __ldg(bt + t + 24 + lane);
+          tile = kvh + __shfl_sync(kFull, ids, t & 31) * blk_stride;
+        }
+        const uint32_t sl = ring + (v % R) * static_cast<uint32_t>(kTile);
         const int nv = n_tokens - t * kBlockSize;
         constexpr int kChunksPerRow = D / 16;
 #pragma unroll
         for (int i = 0; i < 2 * kBlockSize * kChunksPerRow / 32; ++i) {          // the K8 | V8 code rows
           const int idx = lane + 32 * i, row32 = idx / kChunksPerRow, ch = idx % kChunksPerRow;
           const int row = row32 & (kBlockSize - 1);
-          const uint32_t dst = slot + (row32 >> 4) * (kBlockSize * D) + ring_chunk_off<D>(row, ch);
+          const uint32_t dst = sl + (row32 >> 4) * (kBlockSize * D) + ring_chunk_off<D>(row, ch);
           const int sz = row < nv ? 16 : 0;                                      // zero-fill rows past the end
           asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(tile + idx * 16), "r"(sz) : "memory");
         }
         if (lane < 8) {                                                           // sc[16] {ks, vs}: 8 chunks of 2 rows
           const int sz = 2 * lane < nv ? (2 * lane + 1 < nv ? 16 : 8) : 0;
-          asm volatile("cp.async.ca.shared.global [%0], [%1], 16, %2;" ::"r"(slot + 2 * kBlockSize * D + lane * 16),
+          asm volatile("cp.async.ca.shared.global [%0], [%1], 16, %2;" ::"r"(sl + 2 * kBlockSize * D + lane * 16),
                        "l"(tile + 2 * kBlockSize * D + lane * 16), "r"(sz) : "memory");
+        }
+        if constexpr (kAppend) {
+          if (first_special) {                                    // quantise the new row: lanes [0, D/8) K pieces, [D/8, D/4) V pieces
+            constexpr int kP = D / 8;
+            const int cc = lane / kP, cp = lane % kP, r_new = nv - 1;
+            const bool on = lane < 2 * kP;
+            const uint16_t* srow = (cc ? p.v_new : p.k_new) + (static_cast<int64_t>(batch_idx) * p.num_kv_heads + h) * D;
+            const uint4 x = ldg_stream_pred(srow + cp * 8, on);
+            uint32_t mx = __vmaxu2(__vmaxu2(x.x & 0x7fff7fffu, x.y & 0x7fff7fffu), __vmaxu2(x.z & 0x7fff7fffu, x.w & 0x7fff7fffu));
+            mx = max(mx & 0xffffu, mx >> 16);
+#pragma unroll
+            for (int off = kP / 2; off > 0; off >>= 1) mx = max(mx, __shfl_xor_sync(kFull, mx, off));
+            const float amax = __uint_as_float(mx << 16);
+            new_scale = mx == 0 ? 1.f : __fdiv_rn(amax, 448.f);
+            const float inv = mx == 0 ? 1.f : __fdiv_rn(448.f, amax);
+            uint32_t w[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              const uint32_t e = u4_get(x, k);
+              w[k] = f32x2_to_e4m3x2(__fmul_rn(__uint_as_float(e << 16), inv), __fmul_rn(__uint_as_float(e & 0xffff0000u), inv));
+            }
+            new_codes = make_uint2(w[0] | (w[1] << 16), w[2] | (w[3] << 16));
+            if (on) {
+              uint8_t* wt = const_cast<uint8_t*>(tile);
+              *reinterpret_cast<uint2*>(wt + cc * (kBlockSize * D) + r_new * D + cp * 8) = new_codes;
+              if (cp == 0) *reinterpret_cast<float*>(wt + 2 * kBlockSize * D + r_new * 8 + cc * 4) = new_scale;
+            }
+            if (h == 0 && lane == 0) p.block_table[static_cast<int64_t>(slot) * p.bt_stride + blk_begin + n_blocks - 1] = last_blk;
+          }
         }
       }
       asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
-    auto consume = [&](int t) {
-      KV8Tile<D> T;                                              // fragments of ring slot t % R
+    auto consume = [&](int v) {
+      const int t = (special && v == 0) ? n_blocks - 1 : v - sp;
+      KV8Tile<D> T;                                              // fragments of ring slot v % R
       {
-        const uint32_t slot = ring + (t % R) * static_cast<uint32_t>(kTile);
+        const uint32_t slot = ring + (v % R) * static_cast<uint32_t>(kTile);
+        if constexpr (kAppend) {
+          if (special && v == 0) {                               // the tile's stale row r_new has landed: patch in the new row
+            constexpr int kP = D / 8;
+            const int cc = lane / kP, cp = lane % kP, r_new = n_tokens - t * kBlockSize - 1;
+            if (lane < 2 * kP) {
+              asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(slot + cc * (kBlockSize * D) + ring_chunk_off<D>(r_new, cp >> 1) + (cp & 1) * 8),
+                           "r"(new_codes.x), "r"(new_codes.y) : "memory");
+              if (cp == 0) asm volatile("st.shared.f32 [%0], %1;" ::"r"(slot + 2 * kBlockSize * D + r_new * 8 + cc * 4), "f"(new_scale) : "memory");
+            }
+            __syncwarp();
+          }
+        }
 #pragma unroll
         for (int rs = 0; rs < 2; ++rs) {
           const int row = g + 8 * rs;

@@ -569,7 +569,7 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, c
   if (!pool || !req_ids || !q || !out || !aligned16(q) || !aligned16(out)) return KV_ERR_INVALID;
   const kv_pool_config_t& c = pool->hs.cfg;
   if (layer < 0 || layer >= c.num_layers || batch < 1) return KV_ERR_INVALID;
-  if (k_new && c.kv_dtype != KV_DTYPE_BF16) return KV_ERR_UNSUPPORTED;
+  if (k_new && c.kv_dtype != KV_DTYPE_BF16 && !pool->fp8_ring) return KV_ERR_UNSUPPORTED;   // register-tile FP8 kernel: no fused append
   if (!pool->has_device) return KV_ERR_NO_DEVICE;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
 
@@ -620,15 +620,21 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, c
     constexpr int kR = 4;                                        // ring slots per warp
     const size_t smem = static_cast<size_t>(kAttnWarps) * kR * (32 * c.head_dim + 128);
     if (!pool->fp8_ring_ready) {
-      KV_CUDA(pool, cudaFuncSetAttribute(attn_fp8_ring_kernel<128, kR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         kAttnWarps * kR * (32 * 128 + 128)));
-      KV_CUDA(pool, cudaFuncSetAttribute(attn_fp8_ring_kernel<64, kR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         kAttnWarps * kR * (32 * 64 + 128)));
+      const int s128 = kAttnWarps * kR * (32 * 128 + 128), s64 = kAttnWarps * kR * (32 * 64 + 128);
+      KV_CUDA(pool, cudaFuncSetAttribute(attn_fp8_ring_kernel<128, kR, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s128));
+      KV_CUDA(pool, cudaFuncSetAttribute(attn_fp8_ring_kernel<128, kR, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s128));
+      KV_CUDA(pool, cudaFuncSetAttribute(attn_fp8_ring_kernel<64, kR, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s64));
+      KV_CUDA(pool, cudaFuncSetAttribute(attn_fp8_ring_kernel<64, kR, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s64));
       pool->fp8_ring_ready = true;
     }
     const unsigned rgrid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * 3)));
-    if (c.head_dim == 128) attn_fp8_ring_kernel<128, kR><<<rgrid, kAttnThreads, smem, stream>>>(p);
-    else attn_fp8_ring_kernel<64, kR><<<rgrid, kAttnThreads, smem, stream>>>(p);
+    if (c.head_dim == 128) {
+      if (k_new) attn_fp8_ring_kernel<128, kR, true><<<rgrid, kAttnThreads, smem, stream>>>(p);
+      else attn_fp8_ring_kernel<128, kR, false><<<rgrid, kAttnThreads, smem, stream>>>(p);
+    } else {
+      if (k_new) attn_fp8_ring_kernel<64, kR, true><<<rgrid, kAttnThreads, smem, stream>>>(p);
+      else attn_fp8_ring_kernel<64, kR, false><<<rgrid, kAttnThreads, smem, stream>>>(p);
+    }
   } else if (c.kv_dtype == KV_DTYPE_FP8_E4M3) {
     if (c.head_dim == 128) attn_fp8_kernel<128><<<grid, kAttnThreads, 0, stream>>>(p);
     else attn_fp8_kernel<64><<<grid, kAttnThreads, 0, stream>>>(p);

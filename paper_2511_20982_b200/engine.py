@@ -165,7 +165,7 @@ class DecodeLoop:
         """Steps [0, n_steps) take their inputs from device memory; steps [n_steps, n_steps + n_host_steps)
         take them from pinned host memory through the *_host entry points."""
         self.fp8 = kv_dtype == B.KV_DTYPE_FP8_E4M3
-        self.w, self.dev, self.salt, self.fused = w, torch.device(device), salt, fused and not self.fp8
+        self.w, self.dev, self.salt, self.fused = w, torch.device(device), salt, fused
         self.host_from, self.n_steps = n_steps, n_steps + n_host_steps
         self.two_streams = streams >= 2 and w.ingest_per_step > 0
         L, Hkv, Hq, d, k = w.num_layers, w.num_kv_heads, w.num_q_heads, w.head_dim, w.ingest_per_step

@@ -175,8 +175,46 @@ def test_unsupported_calls():
     with pytest.raises(B.KVError) as e:
         pool.varlen_attention(0, [1], [1], q)
     assert e.value.status == B.KV_ERR_UNSUPPORTED
+    pool.set_option("fp8_ring", 0)                                 # the register-tile variant has no fused append
     pool.reserve([1], [1])
     with pytest.raises(B.KVError) as e:
         pool.decode_step(0, [1], q, torch.zeros((1, 2, 64), dtype=torch.bfloat16, device=DEV),
                          torch.zeros((1, 2, 64), dtype=torch.bfloat16, device=DEV))
     assert e.value.status == B.KV_ERR_UNSUPPORTED
+
+
+@pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=2)])
+@pytest.mark.parametrize("Hq,Hkv,d", [(32, 8, 128), (8, 2, 64), (32, 32, 128)])
+def test_fused_decode_step_quantises_like_ingest(Hq, Hkv, d, opts):
+    """paged_decode_step on an FP8 pool: the appended row's codes and scales are the bytes kv_ingest would have
+    written (whole pool == oracle.scatter_fp8), and the output is attention over len + 1 tokens."""
+    L = 2
+    lens = [15, 16, 31, 500, 1, 0, 1029, 47]          # fill a block, open a new one, empty request, split contexts
+    ids = list(range(len(lens)))
+    w = W.Workload("fp8s", L, Hq, Hkv, d, len(lens), None, 6, max_len=2048)
+    pool = make_fp8_pool(L, Hq, Hkv, d, 160)
+    for k_, v_ in opts.items():
+        pool.set_option(k_, v_)
+    slab = oracle.new_slab_fp8(dims_of(pool), SENT)
+    live = [(u, n) for u, n in zip(ids, lens) if n]
+    srcs = [kv_src(w, u, 0, n, DEV) for u, n in live]
+    pool.ingest([u for u, _ in live], [s[0] for s in srcs], [s[1] for s in srcs])
+    for (u, n), (k, v) in zip(live, srcs):
+        oracle.scatter_fp8(slab, dims_of(pool), pool.block_table(u)[0], 0, bits_of(k), bits_of(v))
+    for step in range(3):
+        pool.reserve(ids, [1] * len(ids))
+        n_launch = pool.launches
+        for l in range(L):
+            new = [kv_src(w, u, n + step, n + step + 1, DEV, layer_begin=l, layer_count=1) for u, n in zip(ids, lens)]
+            k_new = torch.stack([s[0][0, :, 0] for s in new]).contiguous()          # [B][Hkv][d]
+            v_new = torch.stack([s[1][0, :, 0] for s in new]).contiguous()
+            q = W.q_values(w.seed, step, l, len(ids), Hq, d, DEV)
+            out = pool.decode_step(l, ids, q, k_new, v_new)
+            torch.cuda.synchronize()
+            for u, n, (k, v) in zip(ids, lens, new):
+                oracle.scatter_fp8(slab, dims_of(pool), pool.block_table(u)[0], n + step, bits_of(k), bits_of(v), layer_begin=l)
+            lists = [pool.block_table(u)[0] for u in ids]
+            want = oracle.attention_fp8(slab, dims_of(pool), l, Hq, lists, [n + step + 1 for n in lens], bits_of(q))
+            compare_attention(out, want)
+        assert pool.launches - n_launch == L                          # one launch per layer
+        assert np.array_equal(pool_bytes(pool), slab), f"step {step}: fused FP8 append is not byte-exact"
