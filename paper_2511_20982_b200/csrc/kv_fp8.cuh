@@ -107,10 +107,14 @@ __global__ void __launch_bounds__(kIngestThreads) ingest_fp8_kernel(const Ingest
   const int c = static_cast<int>(u2 & 1);                        // 0: the K rows of the unit, 1: the V rows
   if (u >= p.total_units) return;
 
-  int lo = 0, hi = p.n_req - 1;                                 // request of this unit: last i with unit_begin <= u
-  while (lo < hi) {
-    int mid = (lo + hi + 1) >> 1;
-    if (__ldg(&p.reqs[mid].unit_begin) <= u) lo = mid; else hi = mid - 1;
+  // request of this unit: last i with unit_begin <= u.  The lanes test 32 candidates at a time (independent
+  // loads, one ballot each) instead of walking a binary search of dependent loads: the warp's few-hundred-cycle
+  // quantisation already sits between its loads and its stores, so its prologue should not add more dead time.
+  int lo = -1;
+  for (int base = 0; base < p.n_req; base += 32) {
+    const int i = base + lane;
+    const bool le = i < p.n_req && __ldg(&p.reqs[i].unit_begin) <= u;
+    lo += __popc(__ballot_sync(0xffffffffu, le));
   }
   const IngestReq r = p.reqs[lo];
   const int64_t local = u - r.unit_begin;
