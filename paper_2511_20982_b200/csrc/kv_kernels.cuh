@@ -154,11 +154,13 @@ __global__ void __launch_bounds__(kIngestThreads) ingest_kernel(const IngestPara
   const int64_t u = static_cast<int64_t>(blockIdx.x) * kIngestWarps + (threadIdx.x >> 5);
   if (u >= p.total_units) return;
 
-  // request of this unit: last i with unit_begin <= u
-  int lo = 0, hi = p.n_req - 1;
-  while (lo < hi) {
-    int mid = (lo + hi + 1) >> 1;
-    if (__ldg(&p.reqs[mid].unit_begin) <= u) lo = mid; else hi = mid - 1;
+  // request of this unit: last i with unit_begin <= u.  The lanes test 32 candidates at a time (independent
+  // loads, one ballot each) rather than walk a binary search of dependent loads.
+  int lo = -1;
+  for (int base = 0; base < p.n_req; base += 32) {
+    const int i = base + lane;
+    const bool le = i < p.n_req && __ldg(&p.reqs[i].unit_begin) <= u;
+    lo += __popc(__ballot_sync(0xffffffffu, le));
   }
   const IngestReq r = p.reqs[lo];
   const int64_t local = u - r.unit_begin;
