@@ -112,6 +112,9 @@ def _load():
         lib.oracle_attention_fp8.restype = ctypes.c_int
         lib.oracle_attention_fp8.argtypes = [P, ctypes.POINTER(_Dims), ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
                                              P, P, P, P, ctypes.c_double, P, P]
+        lib.oracle_attention_varq_fp8.restype = ctypes.c_int
+        lib.oracle_attention_varq_fp8.argtypes = [P, ctypes.POINTER(_Dims), ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
+                                                  P, P, P, P, P, P, ctypes.c_double, P, P]
         lib.oracle_chunk.restype = None
         lib.oracle_chunk.argtypes = [P, ctypes.POINTER(_Dims), ctypes.c_int32, ctypes.c_int32, P, ctypes.c_int32,
                                      ctypes.c_int32, P, ctypes.c_double, P, P, P]
@@ -342,4 +345,36 @@ def attention_fp8(kv8: np.ndarray, dims: Dims, layer: int, num_q_heads: int, blo
                                       _ptr(seq_lens), _ptr(q), float(scale), _ptr(out), _ptr(wsum))
     if rc != 0:
         raise ValueError(f"oracle_attention_fp8 failed ({rc})")
+    return (out, wsum) if return_wsum else out
+
+
+def attention_varq_fp8(kv8: np.ndarray, dims: Dims, layer: int, num_q_heads: int, block_lists, seq_lens, q_lens, q,
+                       scale: float | None = None, return_wsum: bool = False):
+    """attention_varq over an FP8 pool (causal definition on the dequantised values)."""
+    assert kv8.dtype == np.uint8 and kv8.flags.c_contiguous and kv8.size == dims.fp8_bytes
+    q = _u16(q, "q")
+    seq_lens = np.ascontiguousarray(seq_lens, dtype=np.int32)
+    q_lens = np.ascontiguousarray(q_lens, dtype=np.int32)
+    batch = seq_lens.size
+    total_q = int(q_lens.sum())
+    assert q.shape == (total_q, num_q_heads, dims.head_dim) and len(block_lists) == batch
+    lists = [np.ascontiguousarray(b, dtype=np.int32) for b in block_lists]
+    for b, n in zip(lists, seq_lens):
+        assert (int(n) + dims.block_size - 1) // dims.block_size <= b.size
+        assert b.size == 0 or (0 <= b.min() and b.max() < dims.num_blocks)
+    off = np.zeros(batch + 1, dtype=np.int64)
+    off[1:] = np.cumsum([b.size for b in lists])
+    q_off = np.zeros(batch + 1, dtype=np.int64)
+    q_off[1:] = np.cumsum(q_lens)
+    bt = np.ascontiguousarray(np.concatenate(lists) if lists else np.zeros(0, np.int32), dtype=np.int32)
+    if scale is None:
+        scale = 1.0 / float(np.sqrt(np.float64(dims.head_dim)))
+    out = np.empty((total_q, num_q_heads, dims.head_dim), dtype=np.float64)
+    wsum = np.empty((total_q, num_q_heads), dtype=np.float64)
+    c = dims._c()
+    rc = _load().oracle_attention_varq_fp8(_ptr(kv8), ctypes.byref(c), layer, num_q_heads, batch, _ptr(bt), _ptr(off),
+                                           _ptr(seq_lens), _ptr(q_lens), _ptr(q_off), _ptr(q), float(scale), _ptr(out),
+                                           _ptr(wsum))
+    if rc != 0:
+        raise ValueError(f"oracle_attention_varq_fp8 failed ({rc})")
     return (out, wsum) if return_wsum else out

@@ -40,7 +40,9 @@
  * scatter equals an independent numpy/torch-float8 statement over the whole slab, a brute-force
  * nearest-code search and the |x - x^| <= 16 scale bound; attention over an FP8 pool equals
  * oracle_attention when the data is exactly representable and torch SDPA (fp64) on the
- * dequantised values otherwise.  No function here is "parity unpinned".
+ * dequantised values otherwise; oracle_attention_varq_fp8 equals oracle_attention_fp8 at q_len = 1,
+ * oracle_attention_varq on exactly representable rows and torch SDPA (causal, fp64) on the
+ * dequantised values.  No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -479,5 +481,60 @@ int oracle_attention_fp8(const uint8_t* kv8, const oracle_dims_t* D, int32_t lay
       free(s);
       free(row);
     }
+  return bad ? -2 : 0;
+}
+
+/* oracle_attention_varq over an FP8 pool: the variable-q-length causal definition (readings B1-B3) on the
+ * dequantised values (readings C1-C4).  Same arguments as oracle_attention_varq. */
+int oracle_attention_varq_fp8(const uint8_t* kv8, const oracle_dims_t* D, int32_t layer, int32_t num_q_heads,
+                              int32_t batch, const int32_t* bt, const int64_t* bt_off, const int32_t* seq_lens,
+                              const int32_t* q_lens, const int64_t* q_off, const uint16_t* q, double scale,
+                              double* out, double* wsum) {
+  const int32_t d = D->head_dim, Hq = num_q_heads, G = num_q_heads / D->num_kv_heads;
+  for (int32_t r = 0; r < batch; ++r)
+    if (q_lens[r] < 1 || q_lens[r] > seq_lens[r]) return -1;
+  int bad = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int32_t r = 0; r < batch; ++r) {
+    const int32_t* blocks = bt + bt_off[r];
+    const int32_t len = seq_lens[r];
+    /* dequantise the request's layer once: [kv head][token][d] */
+    double* kd = (double*)malloc(sizeof(double) * (size_t)D->num_kv_heads * (size_t)len * (size_t)d);
+    double* vd = (double*)malloc(sizeof(double) * (size_t)D->num_kv_heads * (size_t)len * (size_t)d);
+    double* s = (double*)malloc(sizeof(double) * (size_t)len);
+    if (!kd || !vd || !s) { bad = 1; free(kd); free(vd); free(s); continue; }
+    oracle_dequant_fp8(kv8, D, layer, blocks, len, kd, vd);
+    for (int32_t i = 0; i < q_lens[r]; ++i) {
+      const int32_t n = len - q_lens[r] + i + 1;   /* tokens 0 .. P_i visible */
+      for (int32_t h = 0; h < Hq; ++h) {
+        const double* kh = kd + (int64_t)(h / G) * len * d;
+        const double* vh = vd + (int64_t)(h / G) * len * d;
+        const uint16_t* qv = q + ((q_off[r] + i) * Hq + h) * d;
+        double* o = out + ((q_off[r] + i) * Hq + h) * d;
+        for (int32_t t = 0; t < n; ++t) {
+          double acc = 0.0;
+          for (int32_t j = 0; j < d; ++j) acc += bf16_to_double(qv[j]) * kh[(int64_t)t * d + j];
+          s[t] = scale * acc;
+        }
+        double m = s[0];
+        for (int32_t t = 1; t < n; ++t)
+          if (s[t] > m) m = s[t];
+        double Z = 0.0;
+        for (int32_t t = 0; t < n; ++t) {
+          s[t] = exp(s[t] - m);
+          Z += s[t];
+        }
+        for (int32_t j = 0; j < d; ++j) o[j] = 0.0;
+        double ws = 0.0;
+        for (int32_t t = 0; t < n; ++t) {
+          double w = s[t] / Z;
+          ws += w;
+          for (int32_t j = 0; j < d; ++j) o[j] += w * vh[(int64_t)t * d + j];
+        }
+        if (wsum) wsum[(q_off[r] + i) * Hq + h] = ws;
+      }
+    }
+    free(kd); free(vd); free(s);
+  }
   return bad ? -2 : 0;
 }

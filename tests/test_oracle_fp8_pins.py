@@ -165,3 +165,50 @@ def test_f4_sdpa_on_dequantised_values():
     # n = 1: the output is the dequantised V_0 exactly
     _, vd = oracle.dequant_fp8(kv8, dims, 0, blocks[0], 1)
     assert np.array_equal(got[0], np.repeat(vd[:, 0], Hq // Hkv, axis=0))
+
+
+def test_f5_varq_over_fp8_pool():
+    """oracle_attention_varq_fp8: q_len = 1 == attention_fp8 (bit for bit); exactly representable rows ==
+    attention_varq on the bf16 pool; random data == torch SDPA (causal, lower-right aligned, fp64) on the
+    dequantised values."""
+    rng = np.random.default_rng(4)
+    Hq, Hkv, d, NB = 8, 2, 64, 40
+    lens, qls = [37, 100, 9, 260], [37, 13, 1, 130]
+    dims = oracle.Dims(1, Hkv, d, 16, NB)
+    kv8 = oracle.new_slab_fp8(dims, 0xFF)
+    perm, blocks, p = rng.permutation(NB), [], 0
+    for n in lens:
+        nb = (n + 15) // 16
+        blocks.append(perm[p:p + nb].astype(np.int32)); p += nb
+        oracle.scatter_fp8(kv8, dims, blocks[-1], 0, bf16_bits(rng.standard_normal((1, Hkv, n, d))),
+                           bf16_bits(rng.standard_normal((1, Hkv, n, d))))
+    q1 = bf16_bits(rng.standard_normal((len(lens), Hq, d)))
+    assert np.array_equal(oracle.attention_varq_fp8(kv8, dims, 0, Hq, blocks, lens, [1] * len(lens), q1),
+                          oracle.attention_fp8(kv8, dims, 0, Hq, blocks, lens, q1))
+    q = bf16_bits(rng.standard_normal((sum(qls), Hq, d)))
+    got, wsum = oracle.attention_varq_fp8(kv8, dims, 0, Hq, blocks, lens, qls, q, return_wsum=True)
+    assert np.all(np.abs(wsum - 1) < 1e-12)
+    off = 0
+    for r, (n, ql) in enumerate(zip(lens, qls)):
+        kd, vd = oracle.dequant_fp8(kv8, dims, 0, blocks[r], n)
+        kk = torch.from_numpy(kd).repeat_interleave(Hq // Hkv, 0)[None]
+        vv = torch.from_numpy(vd).repeat_interleave(Hq // Hkv, 0)[None]
+        qq = torch.from_numpy(bits_to_f64(q[off:off + ql])).permute(1, 0, 2)[None]
+        mask = torch.arange(n)[None, :] <= (torch.arange(ql)[:, None] + (n - ql))
+        want = torch.nn.functional.scaled_dot_product_attention(qq, kk, vv, attn_mask=mask)[0].permute(1, 0, 2).numpy()
+        assert np.max(np.abs(got[off:off + ql] - want)) < 1e-10
+        off += ql
+    # exactly representable rows: the FP8 pool and the bf16 pool hold the same values
+    kv8b, kv16 = oracle.new_slab_fp8(dims, 0xFF), oracle.new_slab(dims, 0x7FC0)
+    grid = oracle.e4m3_decode_table()[:0x7f]
+    for b, n in zip(blocks, lens):
+        def rows():
+            x = rng.choice(grid, size=(1, Hkv, n, d)) * rng.choice([-1.0, 1.0], size=(1, Hkv, n, d))
+            x[..., 0] = 448.0
+            return x * 2.0 ** rng.integers(-12, -5, size=(1, Hkv, n, 1))
+        k, v = bf16_bits(rows()), bf16_bits(rows())
+        oracle.scatter_fp8(kv8b, dims, b, 0, k, v)
+        oracle.scatter(kv16, dims, b, 0, k, v)
+    a = oracle.attention_varq_fp8(kv8b, dims, 0, Hq, blocks, lens, qls, q)
+    c = oracle.attention_varq(kv16, dims, 0, Hq, blocks, lens, qls, q)
+    assert np.max(np.abs(a - c)) < 1e-13
