@@ -111,8 +111,8 @@ typedef struct kv_pool_config {
  *     K8[16][head_dim] codes | V8[16][head_dim] codes | sc[16][2] fp32 = (k scale, v scale) of slot t
  * Available on an FP8 pool: kv_reserve, kv_ingest(_host), paged_decode_attention(_host),
  * paged_decode_step(_host) (the fused append quantises the new row exactly as kv_ingest does: same
- * bytes), kv_free and the introspection / profiling calls.  paged_varlen_attention and kv_gather
- * return KV_ERR_UNSUPPORTED.
+ * bytes), paged_varlen_attention, kv_free and the introspection / profiling calls.  kv_gather returns
+ * KV_ERR_UNSUPPORTED.
  */
 
 /* Bytes of the KV region / of the whole slab (KV region + private metadata) for `cfg`

@@ -449,7 +449,9 @@ __device__ __forceinline__ uint32_t ring_chunk_off(int row, int chunk) {   // by
   else return row * 64 + ((chunk ^ ((row >> 1) & 3)) << 4);               // 4 chunks per row: rows pair up per 128 bytes
 }
 
-template <int D, int R, bool kAppend>
+// kVarQ: the variable-q-length causal call on an FP8 pool — columns are (query token, head) pairs, 48-byte items,
+// causal mask per column, -inf guards (see attn_splitkv_kernel, kVarQ).
+template <int D, int R, bool kAppend, bool kVarQ = false>
 __global__ void __launch_bounds__(kAttnThreads, 3) attn_fp8_ring_kernel(const AttnParams p) {
   extern __shared__ __align__(128) unsigned char ring_smem[];
   const uint32_t ring = static_cast<uint32_t>(__cvta_generic_to_shared(ring_smem)) +
@@ -469,7 +471,7 @@ __global__ void __launch_bounds__(kAttnThreads, 3) attn_fp8_ring_kernel(const At
   for (int item = blockIdx.x * kAttnWarps + (threadIdx.x >> 5);;) {
     if (item >= p.n_units) break;
     const int h = item % p.num_kv_heads;
-    const int4* wi = reinterpret_cast<const int4*>(p.items) + (item / p.num_kv_heads) * 2;
+    const int4* wi = reinterpret_cast<const int4*>(p.items) + (item / p.num_kv_heads) * (kVarQ ? 3 : 2);
     const int4 w0 = __ldg(wi);
     const int4 w1 = __ldg(wi + 1);
     const int batch_idx = w0.x, slot = w0.y, blk_begin = w0.z, n_blocks = w0.w;
@@ -485,14 +487,28 @@ __global__ void __launch_bounds__(kAttnThreads, 3) attn_fp8_ring_kernel(const At
     const int last_blk = w1.w;
     uint2 new_codes = make_uint2(0u, 0u);
     float new_scale = 0.f;
+    // kVarQ: tokens in the tile, and the last visible token of columns 2c, 2c+1 relative to the chunk start
+    int n_qtok = 1, rel0 = 0, rel1 = 0;
+    if constexpr (kVarQ) {
+      const int4 w2 = __ldg(wi + 2);
+      n_qtok = w2.y;
+      const int t0 = (2 * c) / G, t1 = (2 * c + 1) / G;
+      rel0 = t0 < n_qtok ? w2.x + t0 - blk_begin * kBlockSize : 0x3fffffff;   // unused columns: q = 0, never stored
+      rel1 = t1 < n_qtok ? w2.x + t1 - blk_begin * kBlockSize : 0x3fffffff;
+    }
 
     // q^T as f16 B fragments: lane (g, c) holds head g, d columns (c + 4j) * 16 + [0, 16), scaled by a
     // power of two so that the row maximum lies in [1, 2); cs0 / cs1 give the factor back to the scores
     uint32_t qf[KS][2];
     float cs0, cs1;
     {
-      const bool ok = g < G;
+      bool ok = g < G;
       const uint16_t* qp = p.q + (static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G + (ok ? g : 0)) * D + c * 16;
+      if constexpr (kVarQ) {                                     // column g = (query token g / G, head g % G)
+        const int qt = g / G;
+        ok = qt < n_qtok;
+        qp = p.q + (static_cast<int64_t>(batch_idx + (ok ? qt : 0)) * p.num_q_heads + h * G + (ok ? g - qt * G : 0)) * D + c * 16;
+      }
       uint4 raw[D / 64][2];
       uint32_t mx = 0;
 #pragma unroll
@@ -653,19 +669,31 @@ __global__ void __launch_bounds__(kAttnThreads, 3) attn_fp8_ring_kernel(const At
       // ---- online softmax with the V scale folded into the reference: t = s + log2(vs) ----
       const float lv0 = ok0 ? fast_log2(T.sc[0].y) : -INFINITY, lv1 = ok1 ? fast_log2(T.sc[1].y) : -INFINITY;
       const float iv0 = ok0 ? __frcp_rn(T.sc[0].y) : 0.f, iv1 = ok1 ? __frcp_rn(T.sc[1].y) : 0.f;
-      const float t0 = s[0] + lv0, t1 = s[1] + lv0, t2 = s[2] + lv1, t3 = s[3] + lv1;
+      float t0 = s[0] + lv0, t1 = s[1] + lv0, t2 = s[2] + lv1, t3 = s[3] + lv1;
+      if constexpr (kVarQ) {                                    // causal: a column sees tokens <= its own position
+        const int tok = t * kBlockSize + g;
+        if (tok > rel0) t0 = -INFINITY;
+        if (tok > rel1) t1 = -INFINITY;
+        if (tok + 8 > rel0) t2 = -INFINITY;
+        if (tok + 8 > rel1) t3 = -INFINITY;
+      }
       float mx0 = fmaxf(t0, t2), mx1 = fmaxf(t1, t3);
 #pragma unroll
       for (int off = 4; off < 32; off <<= 1) {
         mx0 = fmaxf(mx0, __shfl_xor_sync(kFull, mx0, off));
         mx1 = fmaxf(mx1, __shfl_xor_sync(kFull, mx1, off));
       }
-      const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);   // finite: every tile has >= 1 valid token
+      const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);   // finite: every tile has >= 1 valid token ...
       const bool moved = mn0 != m0 || mn1 != m1;
-      const float a0 = fast_exp2(m0 - mn0), a1 = fast_exp2(m1 - mn1);
+      float ms0 = mn0, ms1 = mn1;
+      if constexpr (kVarQ) {                                    // ... except for a column that sees nothing yet
+        ms0 = mn0 == -INFINITY ? 0.f : mn0;
+        ms1 = mn1 == -INFINITY ? 0.f : mn1;
+      }
+      const float a0 = fast_exp2(m0 - ms0), a1 = fast_exp2(m1 - ms1);
       m0 = mn0; m1 = mn1;
-      const float p0 = fast_exp2(t0 - mn0), p1 = fast_exp2(t1 - mn1);   // p'_t = p_t * vs_t  in (0, 1]
-      const float p2 = fast_exp2(t2 - mn0), p3 = fast_exp2(t3 - mn1);
+      const float p0 = fast_exp2(t0 - ms0), p1 = fast_exp2(t1 - ms1);   // p'_t = p_t * vs_t  in (0, 1]
+      const float p2 = fast_exp2(t2 - ms0), p3 = fast_exp2(t3 - ms1);
       l0 = l0 * a0 + (p0 * iv0 + p2 * iv1);
       l1 = l1 * a1 + (p1 * iv0 + p3 * iv1);
       if (__any_sync(kFull, moved)) {                            // the running maximum settles after a few tiles
@@ -709,15 +737,24 @@ __global__ void __launch_bounds__(kAttnThreads, 3) attn_fp8_ring_kernel(const At
       l0 += __shfl_xor_sync(kFull, l0, off);
       l1 += __shfl_xor_sync(kFull, l1, off);
     }
+    const int PG = kVarQ ? 8 : G;                                // columns per partial slot
 #pragma unroll
     for (int hh = 0; hh < 2; ++hh) {
-      const int head = 2 * c + hh;
-      if (head >= G) continue;
+      const int head = 2 * c + hh;                               // MMA column
+      int64_t out_row;
+      if constexpr (kVarQ) {
+        const int qt = head / G;
+        if (qt >= n_qtok) continue;
+        out_row = static_cast<int64_t>(batch_idx + qt) * p.num_q_heads + h * G + (head - qt * G);
+      } else {
+        if (head >= G) continue;
+        out_row = static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G + head;
+      }
       const float l = hh ? l1 : l0, m = hh ? m1 : m0;
       // element e of this lane: d column g * NE + e, register o[e % (NE/2)][2*(e/(NE/2)) + hh]
       if (pidx < 0) {
         const float inv = 1.f / l;
-        uint16_t* op = p.out + (static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G + head) * D + g * NE;
+        uint16_t* op = p.out + out_row * D + g * NE;
 #pragma unroll
         for (int e = 0; e < NE; e += 8) {
           uint32_t w[4];
@@ -729,7 +766,7 @@ __global__ void __launch_bounds__(kAttnThreads, 3) attn_fp8_ring_kernel(const At
           *reinterpret_cast<uint4*>(op + e) = make_uint4(w[0], w[1], w[2], w[3]);
         }
       } else {
-        float* po = p.part_o + (static_cast<int64_t>(pidx) * G + head) * D + g * NE;
+        float* po = p.part_o + (static_cast<int64_t>(pidx) * PG + head) * D + g * NE;
 #pragma unroll
         for (int e = 0; e < NE; e += 4) {
           float f[4];
@@ -737,11 +774,11 @@ __global__ void __launch_bounds__(kAttnThreads, 3) attn_fp8_ring_kernel(const At
           for (int k = 0; k < 4; ++k) f[k] = o[(e + k) % (NE / 2)][2 * ((e + k) / (NE / 2)) + hh];
           *reinterpret_cast<float4*>(po + e) = make_float4(f[0], f[1], f[2], f[3]);
         }
-        if (g == 0) *reinterpret_cast<float2*>(p.part_ml + (static_cast<int64_t>(pidx) * G + head) * 2) = make_float2(m, l);
+        if (g == 0) *reinterpret_cast<float2*>(p.part_ml + (static_cast<int64_t>(pidx) * PG + head) * 2) = make_float2(m, l);
       }
     }
     // ---- fused a5: the unit that completes its (request, kv head) merges the partials ----
-    if (pidx >= 0 && p.fuse_combine) {
+    if (pidx >= 0 && (kVarQ || p.fuse_combine)) {
       __threadfence();
       __syncwarp();
       int last = 0;
@@ -752,8 +789,14 @@ __global__ void __launch_bounds__(kAttnThreads, 3) attn_fp8_ring_kernel(const At
       last = __shfl_sync(kFull, last, 0);
       if (last) {
         __threadfence();
-        combine_group<D>(p.part_o, p.part_ml, pbase, n_chunks, G,
-                         p.out + (static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G) * D, lane);
+        if constexpr (kVarQ) {
+          for (int qt = 0; qt < n_qtok; ++qt)
+            combine_cols<D>(p.part_o, p.part_ml, pbase, n_chunks, 8, qt * G, G,
+                            p.out + (static_cast<int64_t>(batch_idx + qt) * p.num_q_heads + h * G) * D, lane);
+        } else {
+          combine_group<D>(p.part_o, p.part_ml, pbase, n_chunks, G,
+                           p.out + (static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G) * D, lane);
+        }
       }
     }
     if (lane == 0) item = n_warps + atomicAdd(&p.counters[0], 1);

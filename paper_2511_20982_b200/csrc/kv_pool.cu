@@ -197,7 +197,6 @@ struct kv_pool {
   bool fuse_combine = true;
   int32_t ring = 3;               // bf16 pool: 3 (default) / 2: attn_ring_kernel with that many slots per warp (2 / 3 CTAs per SM); 0: register-tile attn_splitkv_kernel
   bool fp8_ring = true;           // FP8 pool: attn_fp8_ring_kernel (shared-memory tile ring) vs attn_fp8_kernel (register tiles)
-  bool fp8_ring_ready = false;    // dynamic shared-memory attribute set
   bool profile = false;
   ProfRing prof[KV_KERNEL_KINDS];
   // staging
@@ -346,6 +345,23 @@ int32_t run_ingest(kv_pool* pool, int32_t n_req, const int64_t* req_ids, const i
     units += static_cast<int64_t>(touched) * layer_count * c.num_kv_heads;
   }
   return flush();
+}
+
+// attn_fp8_ring_kernel launch: 4 ring slots per warp, 3 CTAs per SM.
+constexpr int kFp8RingSlots = 4;
+template <int D, bool kAppend, bool kVarQ>
+static cudaError_t launch_fp8_ring(const AttnParams& p, int num_sms, int want, cudaStream_t stream) {
+  static bool ready = false;
+  constexpr size_t smem = static_cast<size_t>(kAttnWarps) * kFp8RingSlots * (32 * D + 128);
+  if (!ready) {
+    cudaError_t e = cudaFuncSetAttribute(attn_fp8_ring_kernel<D, kFp8RingSlots, kAppend, kVarQ>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    if (e != cudaSuccess) return e;
+    ready = true;
+  }
+  const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, num_sms * 3)));
+  attn_fp8_ring_kernel<D, kFp8RingSlots, kAppend, kVarQ><<<grid, kAttnThreads, smem, stream>>>(p);
+  return cudaGetLastError();
 }
 
 // attn_ring_kernel launch: R slots per warp, kCtas CTAs per SM; dynamic shared memory above 48 KiB needs the opt-in.
@@ -617,24 +633,12 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, c
   const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * pool->ctas_per_sm)));
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_ATTN].begin(stream));
   if (c.kv_dtype == KV_DTYPE_FP8_E4M3 && pool->fp8_ring) {
-    constexpr int kR = 4;                                        // ring slots per warp
-    const size_t smem = static_cast<size_t>(kAttnWarps) * kR * (32 * c.head_dim + 128);
-    if (!pool->fp8_ring_ready) {
-      const int s128 = kAttnWarps * kR * (32 * 128 + 128), s64 = kAttnWarps * kR * (32 * 64 + 128);
-      KV_CUDA(pool, cudaFuncSetAttribute(attn_fp8_ring_kernel<128, kR, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s128));
-      KV_CUDA(pool, cudaFuncSetAttribute(attn_fp8_ring_kernel<128, kR, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s128));
-      KV_CUDA(pool, cudaFuncSetAttribute(attn_fp8_ring_kernel<64, kR, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s64));
-      KV_CUDA(pool, cudaFuncSetAttribute(attn_fp8_ring_kernel<64, kR, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s64));
-      pool->fp8_ring_ready = true;
-    }
-    const unsigned rgrid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * 3)));
-    if (c.head_dim == 128) {
-      if (k_new) attn_fp8_ring_kernel<128, kR, true><<<rgrid, kAttnThreads, smem, stream>>>(p);
-      else attn_fp8_ring_kernel<128, kR, false><<<rgrid, kAttnThreads, smem, stream>>>(p);
-    } else {
-      if (k_new) attn_fp8_ring_kernel<64, kR, true><<<rgrid, kAttnThreads, smem, stream>>>(p);
-      else attn_fp8_ring_kernel<64, kR, false><<<rgrid, kAttnThreads, smem, stream>>>(p);
-    }
+    const cudaError_t re = c.head_dim == 128
+                               ? (k_new ? launch_fp8_ring<128, true, false>(p, pool->num_sms, want, stream)
+                                        : launch_fp8_ring<128, false, false>(p, pool->num_sms, want, stream))
+                               : (k_new ? launch_fp8_ring<64, true, false>(p, pool->num_sms, want, stream)
+                                        : launch_fp8_ring<64, false, false>(p, pool->num_sms, want, stream));
+    KV_CUDA(pool, re);
   } else if (c.kv_dtype == KV_DTYPE_FP8_E4M3) {
     if (c.head_dim == 128) attn_fp8_kernel<128><<<grid, kAttnThreads, 0, stream>>>(p);
     else attn_fp8_kernel<64><<<grid, kAttnThreads, 0, stream>>>(p);
@@ -696,7 +700,7 @@ int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
   if (!pool || !req_ids || !q_lens || !q || !out || !aligned16(q) || !aligned16(out)) return KV_ERR_INVALID;
   const kv_pool_config_t& c = pool->hs.cfg;
   if (layer < 0 || layer >= c.num_layers || batch < 1) return KV_ERR_INVALID;
-  if (c.kv_dtype != KV_DTYPE_BF16) return KV_ERR_UNSUPPORTED;
+  if (c.kv_dtype != KV_DTYPE_BF16 && !pool->fp8_ring) return KV_ERR_UNSUPPORTED;   // register-tile FP8 kernel: decode only
   if (!pool->has_device) return KV_ERR_NO_DEVICE;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const int32_t G = c.num_q_heads / c.num_kv_heads;
@@ -738,7 +742,11 @@ int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
   const int32_t want = (p.n_units + kAttnWarps - 1) / kAttnWarps;
   const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * pool->ctas_per_sm)));
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_VARQ].begin(stream));
-  if (pool->ring) {
+  if (c.kv_dtype == KV_DTYPE_FP8_E4M3) {
+    const cudaError_t re = c.head_dim == 128 ? launch_fp8_ring<128, false, true>(p, pool->num_sms, want, stream)
+                                             : launch_fp8_ring<64, false, true>(p, pool->num_sms, want, stream);
+    KV_CUDA(pool, re);
+  } else if (pool->ring) {
     const cudaError_t re = launch_ring_any<false, true>(c.head_dim, pool->ring, p, pool->num_sms, want, stream);
     KV_CUDA(pool, re);
   } else if (c.head_dim == 128)

@@ -172,10 +172,10 @@ def test_unsupported_calls():
     with pytest.raises(B.KVError) as e:
         pool.gather(1)
     assert e.value.status == B.KV_ERR_UNSUPPORTED
+    pool.set_option("fp8_ring", 0)                                 # the register-tile variant: decode attention only
     with pytest.raises(B.KVError) as e:
         pool.varlen_attention(0, [1], [1], q)
     assert e.value.status == B.KV_ERR_UNSUPPORTED
-    pool.set_option("fp8_ring", 0)                                 # the register-tile variant has no fused append
     pool.reserve([1], [1])
     with pytest.raises(B.KVError) as e:
         pool.decode_step(0, [1], q, torch.zeros((1, 2, 64), dtype=torch.bfloat16, device=DEV),
@@ -218,3 +218,28 @@ def test_fused_decode_step_quantises_like_ingest(Hq, Hkv, d, opts):
             compare_attention(out, want)
         assert pool.launches - n_launch == L                          # one launch per layer
         assert np.array_equal(pool_bytes(pool), slab), f"step {step}: fused FP8 append is not byte-exact"
+
+
+@pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=2)])
+@pytest.mark.parametrize("Hq,Hkv,d", [(8, 2, 64), (32, 32, 128), (64, 8, 128), (6, 2, 64)])
+def test_varlen_attention_on_fp8_pool(Hq, Hkv, d, opts):
+    """In-place prefill rows + decode rows over an FP8 pool == oracle.attention_varq_fp8."""
+    lens = [17, 64, 130, 255, 1, 16, 33, 700, 1100, 5, 48, 100]
+    q_lens = [17, 1, 130, 7, 1, 16, 1, 1, 300, 5, 31, 100]
+    ids = list(range(700, 700 + len(lens)))
+    pool = make_fp8_pool(1, Hq, Hkv, d, sum((n + 15) // 16 for n in lens) + 8)
+    for k_, v_ in opts.items():
+        pool.set_option(k_, v_)
+    w = W.Workload("fp8v", 1, Hq, Hkv, d, len(lens), None, 98, max_len=4096)
+    srcs = [kv_src(w, uid, 0, n, DEV) for uid, n in zip(ids, lens)]
+    pool.ingest(ids, [s[0] for s in srcs], [s[1] for s in srcs])
+    slab = oracle.new_slab_fp8(dims_of(pool), SENT)
+    for uid, n, (k, v) in zip(ids, lens, srcs):
+        oracle.scatter_fp8(slab, dims_of(pool), pool.block_table(uid)[0], 0, bits_of(k), bits_of(v))
+    q = W.q_values(w.seed, 2, 0, sum(q_lens), Hq, d, DEV)
+    out = pool.varlen_attention(0, ids, q_lens, q)
+    torch.cuda.synchronize()
+    assert np.array_equal(pool_bytes(pool), slab)
+    lists = [pool.block_table(u)[0] for u in ids]
+    want = oracle.attention_varq_fp8(slab, dims_of(pool), 0, Hq, lists, lens, q_lens, bits_of(q))
+    compare_attention(out, want)
