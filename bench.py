@@ -443,8 +443,7 @@ def isolated_legs(loop, last_step: int, peak: float, reps: int = 5):
     t_attn = float(np.median(times[1:]))
     res = {"attention_gbs": sp.attn_bytes_layer * L / (t_attn * 1e-3) / 1e9, "attention_ms": t_attn}
     res["attention_frac"] = res["attention_gbs"] / peak
-    if not loop.fp8:
-        res.update(varlen_leg(loop, last_step, peak, reps))
+    res.update(varlen_leg(loop, last_step, peak, reps))
     if w.ingest_per_step and loop.bank:
         k = w.ingest_per_step
         ents = list(range(k))
@@ -517,7 +516,7 @@ def varlen_leg(loop, last_step: int, peak: float, reps: int = 5):
         times.append(e0.elapsed_time(e1))
     t = float(np.median(times[1:]))
     # algorithmic bytes: every request's visible KV once, every q / out row once, block tables once
-    by = attention_bytes(w, np.concatenate([sp.lens_after, plen.astype(np.int64)])) + 2 * (nq - len(ids)) * Hq * d * 2
+    by = attention_bytes(w, np.concatenate([sp.lens_after, plen.astype(np.int64)]), loop.fp8) + 2 * (nq - len(ids)) * Hq * d * 2
     res = {"varlen_gbs": by * L / (t * 1e-3) / 1e9, "varlen_ms": t, "varlen_frac": by * L / (t * 1e-3) / 1e9 / peak,
            "varlen_rows": {"decode": len(sp.batch), "prefill_requests": N_ULTRA_SHORT, "prefill_tokens": int(plen.sum())}}
     # parity of the in-place prefill rows, last layer
@@ -526,14 +525,15 @@ def varlen_leg(loop, last_step: int, peak: float, reps: int = 5):
     bits = lambda x: x.detach().cpu().contiguous().view(torch.int16).numpy().view(np.uint16).copy()
     nblk = [(int(n) + w.block_size - 1) // w.block_size for n in plen]
     dims = oracle.Dims(1, Hkv, d, w.block_size, sum(nblk))
-    slab = oracle.new_slab(dims, 0x7FC0)
+    slab = oracle.new_slab_fp8(dims, 0xFF) if loop.fp8 else oracle.new_slab(dims, 0x7FC0)
     lists, off = [], 0
     for i, n in enumerate(plen):
         lists.append(np.arange(off, off + nblk[i], dtype=np.int32)); off += nblk[i]
-        oracle.scatter(slab, dims, lists[-1], 0,
+        (oracle.scatter_fp8 if loop.fp8 else oracle.scatter)(slab, dims, lists[-1], 0,
                        bits(W.kv_values(w.seed, W.KIND_K, uid0 + i, Hkv, d, layer, 1, 0, int(n), "cpu")),
                        bits(W.kv_values(w.seed, W.KIND_V, uid0 + i, Hkv, d, layer, 1, 0, int(n), "cpu")))
-    want = oracle.attention_varq(slab, dims, 0, Hq, lists, plen, plen, bits(q[layer, len(sp.batch):]))
+    want = (oracle.attention_varq_fp8 if loop.fp8 else oracle.attention_varq)(slab, dims, 0, Hq, lists, plen, plen,
+                                                                           bits(q[layer, len(sp.batch):]))
     got = (bits(out[layer, len(sp.batch):]).astype(np.uint32) << 16).view(np.float32).astype(np.float64)
     err = np.abs(got - want)
     # a fresh prefill row sees 1, 2, 3, ... tokens: its output is (nearly) a V row, |x| up to ~4.5 for N(0,1) values, and
