@@ -167,8 +167,9 @@ int32_t kv_ingest(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids /*host*
  *     K_t, V_t = token t of request req_ids[i], KV head h / G, layer `layer`, t < len_i.
  *   q, out: device, bf16, [batch][num_q_heads][head_dim]; out is written RNE-rounded from
  *   fp32 accumulation.  sm_scale <= 0 selects 1/sqrt(head_dim).
- * Runs a split-KV main kernel (per (request, kv_head, chunk) online softmax -> partial
- * (m, l, O)) and an LSE combine kernel; both on `cuda_stream`.
+ * One launch on `cuda_stream`: a split-KV kernel (per (request, kv_head, chunk) online softmax -> partial
+ * (m, l, O)) whose last-arriving chunk merges the partials (LSE combine); with option fuse_combine = 0 the
+ * merge is a second launch.
  * Errors: KV_ERR_UNKNOWN_REQUEST; a request of length 0 or a duplicate id => KV_ERR_INVALID;
  * batch > max_requests => KV_ERR_INVALID; KV_ERR_NO_DEVICE; KV_ERR_CUDA.
  */
@@ -364,7 +365,10 @@ int32_t kv_profile_reset(kv_pool_t* pool);
  * split-KV chunk, in blocks), "ctas_per_sm" (resident attention CTAs per SM the planner
  * sizes the work list for), "items_per_slot" (work items per resident warp), "fuse_combine"
  * (1, default: the split-KV merge runs inside the attention kernel; 0: separate combine
- * kernel), "profile" (0/1, see kv_profile_read).  Unknown key or out-of-range value => KV_ERR_INVALID.        */
+ * kernel), "ring" (bf16 pools: 3, default, or 2 = shared-memory tile ring with that many slots per warp and
+ * 2 / 3 CTAs per SM; 0 = register-tile kernel), "fp8_ring" (FP8 pools: 1, default, ring kernel; 0 = register-tile
+ * kernel, decode attention only), "profile" (0/1, see kv_profile_read).
+ * Unknown key or out-of-range value => KV_ERR_INVALID.                                                          */
 int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value);
 
 /* Last CUDA error code seen by this pool (cudaError_t as int; 0 = none).                  */

@@ -8,12 +8,14 @@
 //
 // Tile of one (layer, block, kv head), 32 D + 128 bytes:  K8[16][D] | V8[16][D] | sc[16] {ks_t, vs_t} fp32.
 //
-//   ingest_fp8_kernel<D>   quantising scatter (a2 / a3 for an FP8 pool)
-//   attn_fp8_kernel<D>     split-KV paged decode attention over an FP8 pool (a4 + a5)
+//   ingest_fp8_kernel<D>                          quantising scatter (a2 / a3 for an FP8 pool)
+//   attn_fp8_ring_kernel<D, R, kAppend, kVarQ>    split-KV paged attention over an FP8 pool (a4 + a5 [+ a3], NEXT-1 rows):
+//                                                 the default — tiles staged through a per-warp cp.async shared-memory ring
+//   attn_fp8_kernel<D>                            the first version (option fp8_ring = 0): tiles in register buffers, decode only
 //
-// attn_fp8_kernel keeps the register-direct tiles of attn_splitkv_kernel (16 tokens on M, the <= 8 heads
-// of the group on N, every global load a 16-byte vector whose bytes feed MMA fragments after one
-// F2FP.F16.E4M3.UNPACK per pair) but runs the MMAs in f16: e4m3 -> f16 is exact and one instruction.
+// Both attention kernels keep the fragment mapping of the bf16 kernels (16 tokens on M, the <= 8 heads of the
+// group on N, a fragment register is a plain 16-byte piece of a K or V row, turned into f16x2 by one
+// F2FP.F16.E4M3.UNPACK per code pair) and run the MMAs in f16: e4m3 -> f16 is exact and one instruction.
 //   * q rows are pre-scaled by a power of two so their largest element lies in [1, 2) and converted to
 //     f16 (exact for every element within 2^-14 of the row maximum); the factor returns through the
 //     per-column score scale.
@@ -22,7 +24,6 @@
 //     so the weights fed to the PV MMA, p'_t = 2^(s_t + log2 vs_t - m') = p_t * vs_t, lie in (0, 1]
 //     whatever the magnitude of V — no f16 overflow or underflow to manage — while l accumulates
 //     p'_t / vs_t.  O and l share the reference m', so O / l and the LSE merge are unchanged.
-// Half-size tiles need twice as many in flight: four tile buffers per warp (~17 KB).
 #pragma once
 
 #include <cuda_fp16.h>

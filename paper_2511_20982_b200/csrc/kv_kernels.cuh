@@ -1,8 +1,10 @@
 // kv_kernels.cuh — sm_100a kernels of the D-instance KV path.
 //
 //   ingest_kernel<D, kGather>   a2/a3 (and its inverse): contiguous [L][Hkv][n][d] <-> paged blocks
-//   attn_splitkv_kernel<D>      a4: split-KV paged decode attention, one warp per work item
-//   combine_kernel<D>           a5: log-sum-exp merge of split-KV partials
+//   attn_splitkv_kernel<D,..>   a4 (+ a3, a5): split-KV paged attention, one warp per work item, KV tiles in REGISTER
+//                               buffers — the round's first design, kept behind option ring = 0.  The default kernel,
+//                               attn_ring_kernel (kv_attn_ring.cuh), shares everything below except the staging.
+//   combine_kernel<D>           a5: log-sum-exp merge of split-KV partials (stand-alone form, option fuse_combine = 0)
 //
 // Both data-moving kernels are HBM-bound (0 and G <= 8 flop/byte), so the design
 // targets bytes in flight, sector-exact 16-byte accesses and no re-reads; tensor cores
