@@ -367,7 +367,12 @@ int32_t kv_profile_reset(kv_pool_t* pool);
  * (1, default: the split-KV merge runs inside the attention kernel; 0: separate combine
  * kernel), "ring" (bf16 pools: 3, default, or 2 = shared-memory tile ring with that many slots per warp and
  * 2 / 3 CTAs per SM; 0 = register-tile kernel), "fp8_ring" (FP8 pools: 1, default, ring kernel; 0 = register-tile
- * kernel, decode attention only), "profile" (0/1, see kv_profile_read).
+ * kernel, decode attention only), "profile" (0/1, see kv_profile_read);
+ * KV-head sharding of a TP-sharded D-instance: "src_kv_heads" = H (0 = off) then
+ * "src_head_begin" = h0 declare that the contiguous side of kv_ingest(_host) / kv_gather is the FULL-width tensor
+ * [layer_count][H][n_tokens][head_dim] of which this pool holds heads [h0, h0 + num_kv_heads): every GPU of the
+ * instance ingests its slice from the same producer buffer, runs attention on its own query heads, and no
+ * collective is needed inside this path (q, k_new, v_new, out stay local-width).
  * Unknown key or out-of-range value => KV_ERR_INVALID.                                                          */
 int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value);
 

@@ -130,7 +130,7 @@ __global__ void __launch_bounds__(kIngestThreads) ingest_fp8_kernel(const Ingest
   const int t0 = lb * kBlockSize + row0 - r.start_pos;          // first source token of this unit
   const int pieces = (row1 - row0) * kPiecesPerRow;
 
-  const int64_t src_off = ((static_cast<int64_t>(ll) * p.num_kv_heads + h) * r.n_tokens + t0) * D;
+  const int64_t src_off = ((static_cast<int64_t>(ll) * p.src_kv_heads + p.src_head_begin + h) * r.n_tokens + t0) * D;
   const uint4* lin = reinterpret_cast<const uint4*>(reinterpret_cast<const uint16_t*>(c ? r.v_src : r.k_src) + src_off);
   uint8_t* tile = reinterpret_cast<uint8_t*>(p.kv) +
                   ((static_cast<int64_t>(p.layer_begin + ll) * p.num_blocks + blk) * p.num_kv_heads + h) * fp8_tile_bytes<D>();

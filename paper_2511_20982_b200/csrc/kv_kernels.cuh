@@ -146,6 +146,9 @@ struct IngestParams {
   int32_t bt_stride;
   int32_t layer_begin, layer_count, num_kv_heads;
   int64_t num_blocks;
+  // KV-head sharding: the contiguous side is [layer_count][src_kv_heads][n][D] and this
+  // pool's head h is its head src_head_begin + h.  Unsharded: src_kv_heads = num_kv_heads, src_head_begin = 0.
+  int32_t src_kv_heads, src_head_begin;
 };
 
 template <int D, bool kGather>
@@ -178,7 +181,7 @@ __global__ void __launch_bounds__(kIngestThreads) ingest_kernel(const IngestPara
   const int pieces = (row1 - row0) * kPiecesPerRow;
 
   // rows row0..row1-1 are contiguous both in the source run and inside the block
-  const int64_t src_off = ((static_cast<int64_t>(ll) * p.num_kv_heads + h) * r.n_tokens + t0) * D;
+  const int64_t src_off = ((static_cast<int64_t>(ll) * p.src_kv_heads + p.src_head_begin + h) * r.n_tokens + t0) * D;
   const int64_t dst_off =
       ((((static_cast<int64_t>(p.layer_begin + ll) * p.num_blocks + blk) * p.num_kv_heads + h) * 2) * kBlockSize +
        row0) * D;

@@ -195,6 +195,8 @@ struct kv_pool {
   int32_t items_per_slot = 2;     // guided chunking: first chunk = remaining work / (2 x resident warps)
   bool items_per_slot_set = false;  // FP8 ring kernel (12 warps per SM): 1 measured best unless the caller chose
   bool fuse_combine = true;
+  int32_t src_kv_heads = 0;       // KV-head sharding: heads of the contiguous side of ingest / gather (0: this pool's own)
+  int32_t src_head_begin = 0;     //                   this pool's head 0 is that side's head src_head_begin
   int32_t ring = 3;               // bf16 pool: 3 (default) / 2: attn_ring_kernel with that many slots per warp (2 / 3 CTAs per SM); 0: register-tile attn_splitkv_kernel
   bool fp8_ring = true;           // FP8 pool: attn_fp8_ring_kernel (shared-memory tile ring) vs attn_fp8_kernel (register tiles)
   bool profile = false;
@@ -224,6 +226,7 @@ struct kv_pool {
                          : (hs.cfg.kv_dtype == KV_DTYPE_BF16 && ring == 2) ? 3 : ctas_per_sm;
     return num_sms * ctas * kvp::kAttnWarps;
   }
+  int32_t src_heads() const { return src_kv_heads > 0 ? src_kv_heads : hs.cfg.num_kv_heads; }
   int32_t ips() const {
     return (hs.cfg.kv_dtype == KV_DTYPE_FP8_E4M3 && fp8_ring && !items_per_slot_set) ? 1 : items_per_slot;
   }
@@ -279,6 +282,8 @@ int32_t launch_ingest(kv_pool* pool, const std::vector<IngestReq>& reqs, const s
   p.layer_count = layer_count;
   p.num_kv_heads = c.num_kv_heads;
   p.num_blocks = c.num_blocks;
+  p.src_kv_heads = pool->src_heads();
+  p.src_head_begin = pool->src_head_begin;
   const unsigned grid = static_cast<unsigned>((total_units + kIngestWarps - 1) / kIngestWarps);
   ProfRing& pr = pool->prof[kGather ? KV_KERNEL_GATHER : KV_KERNEL_INGEST];
   if (pool->profile) KV_CUDA(pool, pr.begin(stream));
@@ -770,7 +775,7 @@ int32_t kv_ingest_host(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, c
   if (layer_begin < 0 || layer_count < 1 || layer_begin + layer_count > c.num_layers) return KV_ERR_INVALID;
   if (!pool->has_device) return KV_ERR_NO_DEVICE;
   if (n_req > 0 && (!staging || (reinterpret_cast<uintptr_t>(staging) & (kAlign - 1)) != 0)) return KV_ERR_INVALID;
-  const int64_t row_bytes = static_cast<int64_t>(layer_count) * c.num_kv_heads * c.head_dim * 2;
+  const int64_t row_bytes = static_cast<int64_t>(layer_count) * pool->src_heads() * c.head_dim * 2;   // full-width source rows
   int64_t need = 0;
   for (int32_t i = 0; i < n_req; ++i) {
     if (n_tokens[i] < 0) return KV_ERR_INVALID;
@@ -903,6 +908,15 @@ int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
   if (!std::strcmp(key, "profile") && (value == 0 || value == 1)) { pool->profile = value != 0; return KV_OK; }
   if (!std::strcmp(key, "fuse_combine") && (value == 0 || value == 1)) { pool->fuse_combine = value != 0; return KV_OK; }
   if (!std::strcmp(key, "ring") && (value == 0 || value == 2 || value == 3)) { pool->ring = static_cast<int32_t>(value); return KV_OK; }
+  if (!std::strcmp(key, "src_kv_heads") && (value == 0 || (value >= pool->hs.cfg.num_kv_heads + pool->src_head_begin && value <= 65536))) {
+    pool->src_kv_heads = static_cast<int32_t>(value);
+    if (value == 0) pool->src_head_begin = 0;
+    return KV_OK;
+  }
+  if (!std::strcmp(key, "src_head_begin") && value >= 0 && value + pool->hs.cfg.num_kv_heads <= pool->src_heads()) {
+    pool->src_head_begin = static_cast<int32_t>(value);
+    return KV_OK;
+  }
   if (!std::strcmp(key, "fp8_ring") && (value == 0 || value == 1)) { pool->fp8_ring = value != 0; return KV_OK; }
   return KV_ERR_INVALID;
 }

@@ -223,3 +223,36 @@ def test_plan_respects_partials_workspace():
     p.set_option("items_per_slot", 1024)                # asks for ~1.2M items: must be clamped
     items, chunk = check_plan(p, ids, lens, Hkv)
     assert (items[:, 4] >= 0).sum() <= 32768
+
+
+def test_kv_head_shards_take_identical_allocator_decisions():
+    """the shards of a TP-sharded D-instance hold different KV heads of the SAME blocks, so their
+    allocators must decide identically — same seed, same op sequence => same block lists, whatever the head count;
+    and the sharding options validate their range."""
+    rng = np.random.default_rng(11)
+    full = host_pool(num_q_heads=32, num_kv_heads=8, head_dim=128, num_blocks=512, alloc_seed=5, max_requests=32)
+    shards = [host_pool(num_q_heads=8, num_kv_heads=2, head_dim=128, num_blocks=512, alloc_seed=5, max_requests=32)
+              for _ in range(4)]
+    for r, s in enumerate(shards):
+        s.set_option("src_kv_heads", 8)
+        s.set_option("src_head_begin", 2 * r)
+    live = []
+    for step in range(60):
+        if live and rng.random() < 0.3:
+            victim = live.pop(int(rng.integers(len(live))))
+            for p in [full] + shards:
+                p.free([victim])
+        else:
+            uid, n = 1000 + step, int(rng.integers(1, 200))
+            for p in [full] + shards:
+                p.reserve([uid], [n])
+            live.append(uid)
+        for uid in live:
+            want = full.block_table(uid)
+            for s in shards:
+                got = s.block_table(uid)
+                assert np.array_equal(got[0], want[0]) and got[1] == want[1]
+    with pytest.raises(kv.KVError):
+        shards[0].set_option("src_head_begin", 7)            # heads [7, 9) do not exist in an 8-head source
+    with pytest.raises(kv.KVError):
+        full.set_option("src_kv_heads", 4)                   # narrower than the pool itself
