@@ -98,12 +98,14 @@ __host__ __device__ constexpr int64_t fp8_tile_bytes() { return 32 * D + 128; }
 // so the kernel wants many light warps (4 KiB in flight each, ~50 registers) rather than few heavy ones.
 // Launch with 2 * total_units warps.
 // ---------------------------------------------------------------------------------------------
+constexpr int kIngest8Threads = 64;   // small CTAs: an SM slot frees as soon as two warps are done (one-shot warps of uneven length)
+constexpr int kIngest8Warps = kIngest8Threads / 32;
 template <int D>
-__global__ void __launch_bounds__(kIngestThreads) ingest_fp8_kernel(const IngestParams p) {
+__global__ void __launch_bounds__(kIngest8Threads) ingest_fp8_kernel(const IngestParams p) {
   constexpr int kPiecesPerRow = D / 8;                          // 16-byte source pieces (8 bf16) per token row
   constexpr int kMaxPerLane = kBlockSize * kPiecesPerRow / 32;  // 8 at D=128, 4 at D=64
   const int lane = threadIdx.x & 31;
-  const int64_t u2 = static_cast<int64_t>(blockIdx.x) * kIngestWarps + (threadIdx.x >> 5);
+  const int64_t u2 = static_cast<int64_t>(blockIdx.x) * kIngest8Warps + (threadIdx.x >> 5);
   const int64_t u = u2 >> 1;
   const int c = static_cast<int>(u2 & 1);                        // 0: the K rows of the unit, 1: the V rows
   if (u >= p.total_units) return;

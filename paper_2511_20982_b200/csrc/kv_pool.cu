@@ -289,11 +289,11 @@ int32_t launch_ingest(kv_pool* pool, const std::vector<IngestReq>& reqs, const s
   if (pool->profile) KV_CUDA(pool, pr.begin(stream));
   if (c.kv_dtype == KV_DTYPE_FP8_E4M3) {
     if (kGather) return KV_ERR_UNSUPPORTED;
-    const unsigned grid8 = static_cast<unsigned>((2 * total_units + kIngestWarps - 1) / kIngestWarps);   // a warp per (unit, K|V)
+    const unsigned grid8 = static_cast<unsigned>((2 * total_units + kIngest8Warps - 1) / kIngest8Warps);   // a warp per (unit, K|V)
     if (c.head_dim == 128)
-      ingest_fp8_kernel<128><<<grid8, kIngestThreads, 0, stream>>>(p);
+      ingest_fp8_kernel<128><<<grid8, kIngest8Threads, 0, stream>>>(p);
     else
-      ingest_fp8_kernel<64><<<grid8, kIngestThreads, 0, stream>>>(p);
+      ingest_fp8_kernel<64><<<grid8, kIngest8Threads, 0, stream>>>(p);
   } else if (c.head_dim == 128)
     ingest_kernel<128, kGather><<<grid, kIngestThreads, 0, stream>>>(p);
   else
