@@ -351,11 +351,11 @@ int64_t kv_launch_count(const kv_pool_t* pool);
  * outstanding samples of `kind`, returns the number of launches and their summed duration in
  * milliseconds since the last kv_profile_reset, and leaves the sums in place.
  */
-#define KV_KERNEL_ATTN     0   /* attn_splitkv_kernel (a4)          */
+#define KV_KERNEL_ATTN     0   /* the decode attention kernel (a4)  */
 #define KV_KERNEL_COMBINE  1   /* combine_kernel (a5)               */
 #define KV_KERNEL_INGEST   2   /* ingest_kernel, scatter (a2 / a3)  */
 #define KV_KERNEL_GATHER   3   /* ingest_kernel, gather direction   */
-#define KV_KERNEL_VARQ     4   /* attn_splitkv_kernel, variable-q   */
+#define KV_KERNEL_VARQ     4   /* the attention kernel, variable-q  */
 #define KV_KERNEL_KINDS    5
 #define KV_PROFILE_RING    1024
 int32_t kv_profile_read(kv_pool_t* pool, int32_t kind, int64_t* out_launches, double* out_ms);
