@@ -356,7 +356,10 @@ int32_t run_ingest(kv_pool* pool, int32_t n_req, const int64_t* req_ids, const i
 constexpr int kFp8RingSlots = 4;
 template <int D, bool kAppend, bool kVarQ>
 static cudaError_t launch_fp8_ring(const AttnParams& p, int num_sms, int want, cudaStream_t stream) {
-  static bool ready = false;
+  static bool ready_dev[64] = {};                               // the opt-in is per device
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return cudaGetLastError();
+  bool& ready = ready_dev[dev & 63];
   constexpr size_t smem = static_cast<size_t>(kAttnWarps) * kFp8RingSlots * (32 * D + 128);
   if (!ready) {
     cudaError_t e = cudaFuncSetAttribute(attn_fp8_ring_kernel<D, kFp8RingSlots, kAppend, kVarQ>,
@@ -372,7 +375,10 @@ static cudaError_t launch_fp8_ring(const AttnParams& p, int num_sms, int want, c
 // attn_ring_kernel launch: R slots per warp, kCtas CTAs per SM; dynamic shared memory above 48 KiB needs the opt-in.
 template <int D, bool kAppend, bool kVarQ, int R, int kCtas>
 static cudaError_t launch_ring(const AttnParams& p, int num_sms, int want, cudaStream_t stream) {
-  static bool ready = false;
+  static bool ready_dev[64] = {};                               // the opt-in is per device
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return cudaGetLastError();
+  bool& ready = ready_dev[dev & 63];
   constexpr size_t smem = static_cast<size_t>(kAttnWarps) * R * (2 * kBlockSize * D * 2);
   if (!ready) {
     cudaError_t e = cudaFuncSetAttribute(attn_ring_kernel<D, kAppend, kVarQ, R, kCtas>,
