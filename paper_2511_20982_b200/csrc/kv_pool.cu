@@ -190,7 +190,8 @@ struct kv_pool {
   int32_t last_cuda = 0;
   int64_t launches = 0;
   // tuning
-  int32_t min_chunk_blocks = 32;   // smallest split-KV chunk: 32 blocks = 256 KiB of KV per unit at d = 128
+  int32_t min_chunk_blocks = 64;   // smallest split-KV chunk: 64 blocks = 512 KiB of KV per unit at d = 128 (bf16);
+  bool min_chunk_set = false;      //   FP8 pools default to 32 blocks (tiles are half the bytes) unless the caller chose
   int32_t ctas_per_sm = 2;
   int32_t items_per_slot = 2;     // guided chunking: first chunk = remaining work / (2 x resident warps)
   bool items_per_slot_set = false;  // FP8 ring kernel (12 warps per SM): 1 measured best unless the caller chose
@@ -227,6 +228,9 @@ struct kv_pool {
     return num_sms * ctas * kvp::kAttnWarps;
   }
   int32_t src_heads() const { return src_kv_heads > 0 ? src_kv_heads : hs.cfg.num_kv_heads; }
+  int32_t min_chunk() const {
+    return (hs.cfg.kv_dtype == KV_DTYPE_FP8_E4M3 && !min_chunk_set) ? 32 : min_chunk_blocks;
+  }
   int32_t ips() const {
     return (hs.cfg.kv_dtype == KV_DTYPE_FP8_E4M3 && fp8_ring && !items_per_slot_set) ? 1 : items_per_slot;
   }
@@ -546,7 +550,7 @@ int32_t kv_plan_decode(kv_pool_t* pool, int32_t batch, const int64_t* req_ids, i
                        int32_t* out_n_items, int32_t* out_chunk_blocks) {
   if (!pool || cap_items < 0 || (cap_items > 0 && !out_items)) return KV_ERR_INVALID;
   DecodePlan plan;
-  int32_t rc = pool->hs.plan_decode(batch, req_ids, pool->slots(), pool->ips(), pool->min_chunk_blocks,
+  int32_t rc = pool->hs.plan_decode(batch, req_ids, pool->slots(), pool->ips(), pool->min_chunk(),
                                     kMaxPartials, &plan);
   if (rc != KV_OK) return rc;
   const int32_t Hkv = pool->hs.cfg.num_kv_heads;
@@ -605,7 +609,7 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, c
                       static_cast<int32_t>(pool->plan_ids.size()) == batch &&
                       std::memcmp(pool->plan_ids.data(), req_ids, sizeof(int64_t) * static_cast<size_t>(batch)) == 0;
   if (!cached) {
-    int32_t rc = pool->hs.plan_decode(batch, req_ids, pool->slots(), pool->ips(), pool->min_chunk_blocks,
+    int32_t rc = pool->hs.plan_decode(batch, req_ids, pool->slots(), pool->ips(), pool->min_chunk(),
                                       kMaxPartials, &pool->plan);
     if (rc != KV_OK) return rc;
     StageSlot* s = nullptr;
@@ -723,7 +727,7 @@ int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
   if (!cached) {
     // a partial slot of this kernel is 8 columns wide; the workspace is sized in G-column slots
     const int32_t max_partials = static_cast<int32_t>(static_cast<int64_t>(kMaxPartials) * G / 8);
-    int32_t rc = pool->hs.plan_varq(batch, req_ids, q_lens, pool->slots(), pool->ips(), pool->min_chunk_blocks,
+    int32_t rc = pool->hs.plan_varq(batch, req_ids, q_lens, pool->slots(), pool->ips(), pool->min_chunk(),
                                     max_partials, &pool->plan, &pool->plan_tiles);
     if (rc != KV_OK) return rc;
     const size_t n_items = pool->plan.items.size();
@@ -908,7 +912,7 @@ int64_t kv_launch_count(const kv_pool_t* pool) { return pool ? pool->launches : 
 int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
   if (!pool || !key) return KV_ERR_INVALID;
   pool->plan_slot = -1;  // any option may change the plan
-  if (!std::strcmp(key, "min_chunk_blocks") && value >= 1 && value <= 65536) { pool->min_chunk_blocks = static_cast<int32_t>(value); return KV_OK; }
+  if (!std::strcmp(key, "min_chunk_blocks") && value >= 1 && value <= 65536) { pool->min_chunk_blocks = static_cast<int32_t>(value); pool->min_chunk_set = true; return KV_OK; }
   if (!std::strcmp(key, "ctas_per_sm") && value >= 1 && value <= 8) { pool->ctas_per_sm = static_cast<int32_t>(value); return KV_OK; }
   if (!std::strcmp(key, "items_per_slot") && value >= 1 && value <= 1024) { pool->items_per_slot = static_cast<int32_t>(value); pool->items_per_slot_set = true; return KV_OK; }
   if (!std::strcmp(key, "profile") && (value == 0 || value == 1)) { pool->profile = value != 0; return KV_OK; }
