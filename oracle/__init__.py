@@ -115,6 +115,13 @@ def _load():
         lib.oracle_attention_varq_fp8.restype = ctypes.c_int
         lib.oracle_attention_varq_fp8.argtypes = [P, ctypes.POINTER(_Dims), ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
                                                   P, P, P, P, P, P, ctypes.c_double, P, P]
+        lib.oracle_transfer.restype = None
+        lib.oracle_transfer.argtypes = [P, ctypes.POINTER(_Dims), P, P, ctypes.POINTER(_Dims), P, ctypes.c_int32,
+                                        ctypes.c_int32, ctypes.c_int32]
+        lib.oracle_transfer_fp8.restype = None
+        lib.oracle_transfer_fp8.argtypes = lib.oracle_transfer.argtypes
+        lib.oracle_gather_fp8.restype = None
+        lib.oracle_gather_fp8.argtypes = [P, ctypes.POINTER(_Dims), P, ctypes.c_int32, P, P, P, P]
         lib.oracle_chunk.restype = None
         lib.oracle_chunk.argtypes = [P, ctypes.POINTER(_Dims), ctypes.c_int32, ctypes.c_int32, P, ctypes.c_int32,
                                      ctypes.c_int32, P, ctypes.c_double, P, P, P]
@@ -378,3 +385,62 @@ def attention_varq_fp8(kv8: np.ndarray, dims: Dims, layer: int, num_q_heads: int
     if rc != 0:
         raise ValueError(f"oracle_attention_varq_fp8 failed ({rc})")
     return (out, wsum) if return_wsum else out
+
+
+# ---- NEXT-4: producer -> consumer transfer, FP8 gather ---------------------------------------
+
+def _same_geometry(a: Dims, b: Dims) -> bool:
+    return (a.num_layers, a.num_kv_heads, a.head_dim, a.block_size) == (b.num_layers, b.num_kv_heads, b.head_dim, b.block_size)
+
+
+def transfer(src_kv: np.ndarray, src_dims: Dims, src_blocks, dst_kv: np.ndarray, dst_dims: Dims, dst_blocks,
+             length: int, layer_begin: int = 0, layer_count: int | None = None) -> None:
+    """In place on dst_kv: tokens [0, length) of a request move from pool A (src) to pool B (dst), each side
+    addressed through its own block list.  bf16 pools (uint16 slabs)."""
+    assert src_kv.dtype == np.uint16 and src_kv.size == src_dims.kv_elems
+    assert dst_kv.dtype == np.uint16 and dst_kv.flags.c_contiguous and dst_kv.size == dst_dims.kv_elems
+    assert _same_geometry(src_dims, dst_dims)
+    lc = src_dims.num_layers - layer_begin if layer_count is None else layer_count
+    assert 0 <= layer_begin and lc >= 0 and layer_begin + lc <= src_dims.num_layers
+    sb = np.ascontiguousarray(src_blocks, dtype=np.int32)
+    db = np.ascontiguousarray(dst_blocks, dtype=np.int32)
+    nb = (length + src_dims.block_size - 1) // src_dims.block_size
+    assert nb <= sb.size and nb <= db.size
+    assert nb == 0 or (0 <= sb[:nb].min() and sb[:nb].max() < src_dims.num_blocks)
+    assert nb == 0 or (0 <= db[:nb].min() and db[:nb].max() < dst_dims.num_blocks)
+    cs, cd = src_dims._c(), dst_dims._c()
+    _load().oracle_transfer(_ptr(np.ascontiguousarray(src_kv)), ctypes.byref(cs), _ptr(sb), _ptr(dst_kv),
+                            ctypes.byref(cd), _ptr(db), length, layer_begin, lc)
+
+
+def transfer_fp8(src_kv8: np.ndarray, src_dims: Dims, src_blocks, dst_kv8: np.ndarray, dst_dims: Dims, dst_blocks,
+                 length: int, layer_begin: int = 0, layer_count: int | None = None) -> None:
+    """transfer() between two FP8 pools (uint8 slabs): codes and row scales move verbatim."""
+    assert src_kv8.dtype == np.uint8 and src_kv8.size == src_dims.fp8_bytes and src_dims.block_size == 16
+    assert dst_kv8.dtype == np.uint8 and dst_kv8.flags.c_contiguous and dst_kv8.size == dst_dims.fp8_bytes
+    assert _same_geometry(src_dims, dst_dims)
+    lc = src_dims.num_layers - layer_begin if layer_count is None else layer_count
+    assert 0 <= layer_begin and lc >= 0 and layer_begin + lc <= src_dims.num_layers
+    sb = np.ascontiguousarray(src_blocks, dtype=np.int32)
+    db = np.ascontiguousarray(dst_blocks, dtype=np.int32)
+    nb = (length + 15) // 16
+    assert nb <= sb.size and nb <= db.size
+    assert nb == 0 or (0 <= sb[:nb].min() and sb[:nb].max() < src_dims.num_blocks)
+    assert nb == 0 or (0 <= db[:nb].min() and db[:nb].max() < dst_dims.num_blocks)
+    cs, cd = src_dims._c(), dst_dims._c()
+    _load().oracle_transfer_fp8(_ptr(np.ascontiguousarray(src_kv8)), ctypes.byref(cs), _ptr(sb), _ptr(dst_kv8),
+                                ctypes.byref(cd), _ptr(db), length, layer_begin, lc)
+
+
+def gather_fp8(kv8: np.ndarray, dims: Dims, blocks, length: int):
+    """Stored codes and scales of tokens [0, length), all layers:
+    (k_codes uint8 [L][Hkv][length][d], k_scales float32 [L][Hkv][length], v_codes, v_scales)."""
+    assert kv8.dtype == np.uint8 and kv8.flags.c_contiguous and kv8.size == dims.fp8_bytes and dims.block_size == 16
+    blocks = np.ascontiguousarray(blocks, dtype=np.int32)
+    assert (length + 15) // 16 <= blocks.size
+    shape = (dims.num_layers, dims.num_kv_heads, length, dims.head_dim)
+    kc, vc = np.empty(shape, dtype=np.uint8), np.empty(shape, dtype=np.uint8)
+    ks, vs = np.empty(shape[:3], dtype=np.float32), np.empty(shape[:3], dtype=np.float32)
+    c = dims._c()
+    _load().oracle_gather_fp8(_ptr(kv8), ctypes.byref(c), _ptr(blocks), length, _ptr(kc), _ptr(ks), _ptr(vc), _ptr(vs))
+    return kc, ks, vc, vs

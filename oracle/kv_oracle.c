@@ -42,7 +42,13 @@
  * oracle_attention when the data is exactly representable and torch SDPA (fp64) on the
  * dequantised values otherwise; oracle_attention_varq_fp8 equals oracle_attention_fp8 at q_len = 1,
  * oracle_attention_varq on exactly representable rows and torch SDPA (causal, fp64) on the
- * dequantised values.  No function here is "parity unpinned".
+ * dequantised values.  NEXT-4 functions (tests/test_oracle_transfer_pins.py): oracle_transfer into a
+ * sentinel-filled pool B equals oracle_scatter of the ORIGINAL source through B's block list over the
+ * whole slab (and an independent numpy fancy-index statement), A is untouched, slots past the
+ * request's end keep the sentinel, gather(B) returns the source; oracle_transfer_fp8 likewise against
+ * oracle_scatter_fp8 and a numpy byte-view statement; oracle_gather_fp8's codes x scales equal
+ * oracle_dequant_fp8 and a numpy index statement of the tile layout.
+ * No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -537,4 +543,74 @@ int oracle_attention_varq_fp8(const uint8_t* kv8, const oracle_dims_t* D, int32_
     free(kd); free(vd); free(s);
   }
   return bad ? -2 : 0;
+}
+
+/* =============================================================================================
+ * NEXT-4: producer -> consumer KV transfer.  PAPER.md:82 (§II): "KV-cache
+ * transmission can add on the order of 15-80ms depending on block fragmentation and count";
+ * PAPER.md:360 (§V-C): the KV-cache transmitter moves a prefill-completed request's KV out of the
+ * producer's KV-cache blocks into KV-cache blocks registered on the consumer.  Both sides are
+ * paged pools with their OWN block lists (and their own num_blocks), so the operation is, by
+ * definition, "gather from pool A through A's block list, then scatter into pool B through B's":
+ * token t of the request moves from A's block src_blocks[t / bs], slot t % bs, to B's block
+ * dst_blocks[t / bs], slot t % bs, for every layer in [layer_begin, layer_begin + layer_count),
+ * every kv head, K and V.  Pure bit copies; A is read-only; bytes of B outside the n written
+ * token slots keep their contents (reading A5).  The two pools share layer count, kv heads,
+ * head_dim and block_size (checked by the caller); num_blocks may differ.
+ * ============================================================================================= */
+void oracle_transfer(const uint16_t* src_kv, const oracle_dims_t* Ds, const int32_t* src_blocks,
+                     uint16_t* dst_kv, const oracle_dims_t* Dd, const int32_t* dst_blocks, int32_t n,
+                     int32_t layer_begin, int32_t layer_count) {
+  for (int32_t l = layer_begin; l < layer_begin + layer_count; ++l)
+    for (int32_t h = 0; h < Ds->num_kv_heads; ++h)
+      for (int32_t t = 0; t < n; ++t) {
+        int32_t slot = t % Ds->block_size;
+        int32_t sb = src_blocks[t / Ds->block_size], db = dst_blocks[t / Dd->block_size];
+        for (int32_t c = 0; c < 2; ++c)
+          for (int32_t j = 0; j < Ds->head_dim; ++j)
+            dst_kv[kv_index(Dd, l, db, h, c, slot, j)] = src_kv[kv_index(Ds, l, sb, h, c, slot, j)];
+      }
+}
+
+/* The same relocation between two FP8 pools: a token's d codes of K, d codes of V and its two fp32
+ * row scales (ks_t, vs_t) move verbatim — no re-quantisation (a code row and its scale are a pure
+ * function of the token row, reading C2, so they mean the same in any pool). */
+void oracle_transfer_fp8(const uint8_t* src_kv8, const oracle_dims_t* Ds, const int32_t* src_blocks,
+                         uint8_t* dst_kv8, const oracle_dims_t* Dd, const int32_t* dst_blocks, int32_t n,
+                         int32_t layer_begin, int32_t layer_count) {
+  const int64_t d = Ds->head_dim;
+  for (int32_t l = layer_begin; l < layer_begin + layer_count; ++l)
+    for (int32_t h = 0; h < Ds->num_kv_heads; ++h)
+      for (int32_t t = 0; t < n; ++t) {
+        int32_t slot = t % 16;
+        const uint8_t* st = src_kv8 + kv8_tile(Ds, l, src_blocks[t / 16], h);
+        uint8_t* dt = dst_kv8 + kv8_tile(Dd, l, dst_blocks[t / 16], h);
+        for (int64_t j = 0; j < d; ++j) {
+          dt[slot * d + j] = st[slot * d + j];                       /* K codes */
+          dt[16 * d + slot * d + j] = st[16 * d + slot * d + j];     /* V codes */
+        }
+        for (int32_t b = 0; b < 8; ++b) dt[32 * d + slot * 8 + b] = st[32 * d + slot * 8 + b];  /* ks_t, vs_t */
+      }
+}
+
+/* Inverse of oracle_scatter_fp8's relocation (NOT of its quantisation): the stored codes and scales of
+ * tokens [0, len), all layers, in contiguous form — the producer-side paged -> contiguous step on an FP8
+ * pool.  k_codes / v_codes: [num_layers][num_kv_heads][len][d] bytes; k_scales / v_scales:
+ * [num_layers][num_kv_heads][len] fp32. */
+void oracle_gather_fp8(const uint8_t* kv8, const oracle_dims_t* D, const int32_t* blocks, int32_t len,
+                       uint8_t* k_codes, float* k_scales, uint8_t* v_codes, float* v_scales) {
+  const int64_t d = D->head_dim;
+  for (int32_t l = 0; l < D->num_layers; ++l)
+    for (int32_t h = 0; h < D->num_kv_heads; ++h)
+      for (int32_t t = 0; t < len; ++t) {
+        int32_t slot = t % 16;
+        const uint8_t* tile = kv8 + kv8_tile(D, l, blocks[t / 16], h);
+        int64_t row = ((int64_t)l * D->num_kv_heads + h) * len + t;
+        for (int64_t j = 0; j < d; ++j) {
+          k_codes[row * d + j] = tile[slot * d + j];
+          v_codes[row * d + j] = tile[16 * d + slot * d + j];
+        }
+        memcpy(&k_scales[row], tile + 32 * d + slot * 8, 4);
+        memcpy(&v_scales[row], tile + 32 * d + slot * 8 + 4, 4);
+      }
 }
