@@ -30,6 +30,14 @@
  *   - bf16 = IEEE bfloat16 bit patterns (uint16_t).  Sources, queries and outputs are always bf16;
  *     the pool is bf16 or, with kv_dtype = KV_DTYPE_FP8_E4M3, e4m3 codes + scales (see below).
  *   - One host thread per pool.  Pools are independent.
+ *   - One attention stream per pool at a time: paged_decode_attention / paged_decode_step(_layers) /
+ *     paged_varlen_attention launches of ONE pool share a device workspace (work and arrival counters,
+ *     split-KV partials, the staged plan), so they must execute one after the other.  Calls on one stream
+ *     do; when a call arrives on a different stream than the pool's previous attention launch the library
+ *     orders it behind that launch itself (cudaStreamWaitEvent), so the result is still correct but the two
+ *     do not overlap.  kv_ingest / kv_transfer / kv_gather have no such workspace and may run on any stream.
+ *   - A pool belongs to the device its slab is on; calls made while another device is current switch to the
+ *     pool's device for their duration.
  *
  * Slab layout (caller-visible so that an independent checker can read the pool).
  *   The caller allocates `kv_pool_required_bytes(cfg)` bytes at `device_base`.  The first
@@ -111,8 +119,8 @@ typedef struct kv_pool_config {
  *     K8[16][head_dim] codes | V8[16][head_dim] codes | sc[16][2] fp32 = (k scale, v scale) of slot t
  * Available on an FP8 pool: kv_reserve, kv_ingest(_host), paged_decode_attention(_host),
  * paged_decode_step(_host) (the fused append quantises the new row exactly as kv_ingest does: same
- * bytes), paged_varlen_attention, kv_free and the introspection / profiling calls.  kv_gather returns
- * KV_ERR_UNSUPPORTED.
+ * bytes), paged_varlen_attention, kv_free, kv_transfer (FP8 -> FP8), kv_gather (codes + scales, see there)
+ * and the introspection / profiling calls.
  */
 
 /* Bytes of the KV region / of the whole slab (KV region + private metadata) for `cfg`
@@ -152,6 +160,8 @@ int32_t kv_reserve(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids /*host
  *                      KV layer by layer, and a decode loop append per layer.
  * A pure bit copy: no arithmetic, no conversion.  Bytes outside the written slots keep
  * their previous contents.  Errors as kv_reserve, plus KV_ERR_NO_DEVICE / KV_ERR_CUDA.
+ * Atomic: if the call fails for any reason — including a CUDA error while enqueuing — the
+ * reservation it made is rolled back and no request is modified.
  */
 int32_t kv_ingest(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids /*host*/,
                   const int32_t* n_tokens /*host*/,
@@ -200,6 +210,33 @@ int32_t paged_decode_step(kv_pool_t* pool, int32_t layer, int32_t batch,
                           void* out /*device*/, float sm_scale, void* cuda_stream);
 
 /*
+ * One decode step's attention for layers [layer_begin, layer_begin + layer_count) in ONE host call
+ * (PAPER.md:204 names the "CUDA graph inference configuration" as the deployed form of the decode step:
+ * the step is enqueued as a unit, not layer by layer from the host).  Equivalent to
+ *     if (flags & KV_STEP_RESERVE) kv_reserve(pool, batch, req_ids, ones);          (layer_begin must be 0)
+ *     for l in layer_begin .. layer_begin + layer_count - 1:
+ *         k_new ? paged_decode_step(pool, l, batch, req_ids, q_l, k_new_l, v_new_l, out_l, sm_scale, stream)
+ *               : paged_decode_attention(pool, l, batch, req_ids, q_l, out_l, sm_scale, stream)
+ * with q_l = q + (l - layer_begin) * q_layer_stride_bytes (out_l likewise) and k_new_l = k_new +
+ * (l - layer_begin) * kv_layer_stride_bytes (v_new_l likewise); strides in bytes, multiples of 16.
+ * One plan, one upload; the layer launches are issued back to back with the programmatic-dependent-launch
+ * attribute (option "pdl", default 1), so the CTAs of layer l+1 take over SMs as layer l drains and their
+ * work-item and block-id reads overlap its tail; every read of q, k_new, v_new and every write happens
+ * after layer l (and whatever produced q) has completed (griddepcontrol.wait).  It is for callers that hold
+ * the queries of several layers at once (bench, replay, a captured graph whose other kernels sit in
+ * between); a model that computes q_l from out_(l-1) calls it with layer_count = 1 per layer and still gets
+ * the one-plan-per-step and PDL behaviour.  k_new = v_new = NULL selects attention without append.
+ * Errors: as paged_decode_step / paged_decode_attention / kv_reserve; KV_STEP_RESERVE with layer_begin != 0 or
+ * without k_new => KV_ERR_INVALID.  On error nothing changes (a reservation made by this call is rolled back).
+ */
+#define KV_STEP_RESERVE 1
+int32_t paged_decode_step_layers(kv_pool_t* pool, int32_t layer_begin, int32_t layer_count, int32_t batch,
+                                 const int64_t* req_ids /*host*/, const void* q /*device*/,
+                                 const void* k_new /*device or NULL*/, const void* v_new /*device or NULL*/,
+                                 void* out /*device*/, int64_t q_layer_stride_bytes, int64_t kv_layer_stride_bytes,
+                                 float sm_scale, int32_t flags, void* cuda_stream);
+
+/*
  * NEXT-1 — variable-q-length causal paged attention: in-place prefill of ultra-short requests
  * merged with decoding (§V-E: "For ultra-short requests we employ PD-aggregation:
  * merging their prefill with other requests' decoding on D-instances avoids unnecessary
@@ -242,11 +279,41 @@ int32_t kv_block_table(const kv_pool_t* pool, int64_t req_id, int32_t* out_block
 int32_t kv_pool_stats(const kv_pool_t* pool, int64_t* blocks_total, int64_t* blocks_free,
                       int32_t* live_requests, int64_t* blocks_high_water);
 
-/* Inverse of ingest for one request, all layers: k_dst/v_dst device bf16
- * [num_layers][num_kv_heads][len][head_dim].  Test support; also the producer-side
- * paged->contiguous step of SURVEY §8(f) NEXT-4.                                           */
+/* Inverse of ingest's relocation for one request, all layers (test support; also the producer-side
+ * paged->contiguous step of SURVEY §8(f) NEXT-4).
+ *   bf16 pool: k_dst / v_dst device bf16 [num_layers][num_kv_heads][len][head_dim].
+ *   FP8 pool:  the STORED codes and row scales, not re-quantised and not dequantised.  k_dst (v_dst likewise):
+ *              e4m3 codes u8 [num_layers][num_kv_heads][len][head_dim], then, at the next 16-byte boundary,
+ *              fp32 scales [num_layers][num_kv_heads][len]; kv_gather_bytes() is the size of each of the two.
+ * With option src_kv_heads = H the contiguous side is H heads wide (this pool's heads at src_head_begin).   */
 int32_t kv_gather(kv_pool_t* pool, int64_t req_id, void* k_dst /*device*/,
                   void* v_dst /*device*/, void* cuda_stream);
+/* Bytes kv_gather writes to EACH of k_dst and v_dst for a request of n_tokens tokens; < 0 on an invalid config. */
+int64_t kv_gather_bytes(const kv_pool_config_t* cfg, int32_t n_tokens);
+
+/*
+ * NEXT-4 — producer -> consumer transfer, paged -> paged (§II: "KV-cache transmission can add on
+ * the order of 15-80ms depending on block fragmentation and count"; §V-C: the KV-cache
+ * transmitter moves a prefill-completed request's KV into KV-cache blocks registered on the consumer).
+ * For i in [0, n_req): request src_req_ids[i] of `src` (the producer's pool), all its len_i tokens, becomes
+ * request dst_req_ids[i] of `dst` (this D-instance's pool), layers [layer_begin, layer_begin + layer_count):
+ *     dst.kv[l][dst_table_i[t / bs]][h][c][t % bs][:] = src.kv[l][src_table_i[t / bs]][h][c][t % bs][:]
+ * — each side addressed through its own block list, block to block, no contiguous staging buffer, ONE launch
+ * for all requests (on `dst`'s device, pulling: a src slab that is peer-mapped memory of the producer GPU makes
+ * this the NVLink hop and the scatter in one kernel).  src is read-only.  The pools must agree in num_layers,
+ * num_kv_heads, head_dim, block_size and kv_dtype (FP8 pools move codes and row scales verbatim); num_blocks,
+ * alloc_seed and the block lists are independent.
+ *   layer_begin == 0 : dst_req_ids[i] must not be live in dst; it is created with length len_i (kv_reserve).
+ *   layer_begin  > 0 : continuation (a producer streaming layer by layer): dst_req_ids[i] must be live with
+ *                      length len_i and a last reservation of len_i tokens.
+ * Bytes of dst outside the written token slots keep their contents.  Atomic: on any error nothing changes in
+ * either pool.  Errors: KV_ERR_UNKNOWN_REQUEST (src id not live), KV_ERR_INVALID (geometry mismatch, src == dst,
+ * duplicate ids, dst id live at layer_begin 0), KV_ERR_NO_BLOCKS, KV_ERR_TOO_LONG, KV_ERR_TOO_MANY_REQUESTS,
+ * KV_ERR_NO_DEVICE, KV_ERR_CUDA.  The caller orders the call after whatever wrote the src blocks.
+ */
+int32_t kv_transfer(kv_pool_t* dst, const kv_pool_t* src, int32_t n_req, const int64_t* dst_req_ids /*host*/,
+                    const int64_t* src_req_ids /*host*/, int32_t layer_begin, int32_t layer_count,
+                    void* cuda_stream);
 
 /*
  * Host-only view of the split-KV plan paged_decode_attention would use for this batch
@@ -336,8 +403,9 @@ int32_t kv_capacity(const kv_capacity_model_t* model, kv_capacity_t* out);
  */
 int32_t kv_optimal_pd_ratio(double cc_d, double t_p, double t_d, double osl, double* out_ratio);
 
-/* M_token of a pool geometry: 2 x num_layers x num_kv_heads x head_dim x 2 bytes (bf16); < 0 on an
- * invalid config.                                                                           */
+/* M_token of a pool geometry, the KV bytes one token occupies over the whole model: bf16 pool
+ * 2 x num_layers x num_kv_heads x head_dim x 2; FP8 pool num_layers x num_kv_heads x (2 x head_dim + 8)
+ * (codes + the two fp32 row scales); < 0 on an invalid config.                               */
 int64_t kv_token_bytes(const kv_pool_config_t* cfg);
 
 /* Number of kernels this pool has launched since creation (bench `gpu_launches`).         */
@@ -345,7 +413,8 @@ int64_t kv_launch_count(const kv_pool_t* pool);
 
 /*
  * Per-kernel device timing (bench `roofline`).  With option "profile" = 1 every kernel
- * launch is bracketed by a pair of CUDA events on its own stream (a ring of
+ * launch (paged_decode_step_layers: every group of layer_count launches, counted as layer_count) is
+ * bracketed by a pair of CUDA events on its own stream (a ring of
  * KV_PROFILE_RING pairs per kind; older samples are folded into the running sums when their
  * slot is reused, which synchronises on that sample).  kv_profile_read synchronises on the
  * outstanding samples of `kind`, returns the number of launches and their summed duration in
@@ -356,7 +425,8 @@ int64_t kv_launch_count(const kv_pool_t* pool);
 #define KV_KERNEL_INGEST   2   /* ingest_kernel, scatter (a2 / a3)  */
 #define KV_KERNEL_GATHER   3   /* ingest_kernel, gather direction   */
 #define KV_KERNEL_VARQ     4   /* the attention kernel, variable-q  */
-#define KV_KERNEL_KINDS    5
+#define KV_KERNEL_TRANSFER 5   /* transfer_kernel (NEXT-4)          */
+#define KV_KERNEL_KINDS    6
 #define KV_PROFILE_RING    1024
 int32_t kv_profile_read(kv_pool_t* pool, int32_t kind, int64_t* out_launches, double* out_ms);
 int32_t kv_profile_reset(kv_pool_t* pool);
@@ -366,8 +436,8 @@ int32_t kv_profile_reset(kv_pool_t* pool);
  * sizes the work list for), "items_per_slot" (work items per resident warp), "fuse_combine"
  * (1, default: the split-KV merge runs inside the attention kernel; 0: separate combine
  * kernel), "ring" (bf16 pools: 3, default, or 2 = shared-memory tile ring with that many slots per warp and
- * 2 / 3 CTAs per SM; 0 = register-tile kernel), "fp8_ring" (FP8 pools: 1, default, ring kernel; 0 = register-tile
- * kernel, decode attention only), "profile" (0/1, see kv_profile_read);
+ * 2 / 3 CTAs per SM), "pdl" (1, default: attention launches carry the programmatic-dependent-launch attribute;
+ * 0: plain launches), "profile" (0/1, see kv_profile_read);
  * KV-head sharding of a TP-sharded D-instance: "src_kv_heads" = H (0 = off) then
  * "src_head_begin" = h0 declare that the contiguous side of kv_ingest(_host) / kv_gather is the FULL-width tensor
  * [layer_count][H][n_tokens][head_dim] of which this pool holds heads [h0, h0 + num_kv_heads): every GPU of the

@@ -20,6 +20,13 @@ if not os.path.exists(lib_path):
         f"{lib_path} is missing: build it with `python -m paper_2511_20982_b200.build` "
         "(nvcc, sm_100a).  There is no CPU or PyTorch fallback for this path.")
 
+from . import build as _build
+
+if _build.stale():
+    raise ImportError(
+        f"{lib_path} was not built from the sources in this tree (source hash mismatch): rebuild it with "
+        "`python -m paper_2511_20982_b200.build --force`.  A stale library is refused rather than loaded.")
+
 lib = ctypes.CDLL(lib_path)
 
 KV_OK = 0
@@ -51,12 +58,15 @@ _SIGS = {
     "paged_decode_attention": (_i32, [_P, _i32, _i32, _P, _P, _P, ctypes.c_float, _P]),
     "paged_decode_step": (_i32, [_P, _i32, _i32, _P, _P, _P, _P, _P, ctypes.c_float, _P]),
     "paged_decode_step_host": (_i32, [_P, _i32, _i32, _P, _P, _P, _P, _P, ctypes.c_float, _P, _i64, _P]),
+    "paged_decode_step_layers": (_i32, [_P, _i32, _i32, _i32, _P, _P, _P, _P, _P, _i64, _i64, ctypes.c_float, _i32, _P]),
     "paged_varlen_attention": (_i32, [_P, _i32, _i32, _P, _P, _P, _P, ctypes.c_float, _P]),
     "kv_free": (_i32, [_P, _i32, _P]),
     "kv_block_table": (_i32, [_P, _i64, _P, _i32, ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
     "kv_pool_stats": (_i32, [_P, ctypes.POINTER(_i64), ctypes.POINTER(_i64), ctypes.POINTER(_i32),
                              ctypes.POINTER(_i64)]),
     "kv_gather": (_i32, [_P, _i64, _P, _P, _P]),
+    "kv_gather_bytes": (_i64, [_CFG, _i32]),
+    "kv_transfer": (_i32, [_P, _P, _i32, _P, _P, _i32, _i32, _P]),
     "kv_plan_decode": (_i32, [_P, _i32, _P, _P, _i32, ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
     "kv_ingest_host": (_i32, [_P, _i32, _P, _P, _P, _P, _i32, _i32, _P, _i64, _P]),
     "paged_decode_attention_host": (_i32, [_P, _i32, _i32, _P, _P, _P, ctypes.c_float, _P, _i64, _P]),
@@ -190,6 +200,19 @@ def paged_decode_step(handle: int, layer: int, req_ids, q_ptr: int, k_new_ptr: i
                                  stream or None), "paged_decode_step")
 
 
+KV_STEP_RESERVE = 1
+
+
+def paged_decode_step_layers(handle: int, layer_begin: int, layer_count: int, req_ids, q_ptr: int, k_new_ptr: int,
+                             v_new_ptr: int, out_ptr: int, q_layer_stride_bytes: int, kv_layer_stride_bytes: int,
+                             sm_scale: float = 0.0, flags: int = 0, stream: int = 0) -> None:
+    """One decode step's (append +) attention for layer_count layers in one call; k_new_ptr = 0: no append."""
+    ids = _ids(req_ids)
+    _check(lib.paged_decode_step_layers(handle, layer_begin, layer_count, ids.size, _np(ids), q_ptr, k_new_ptr or None,
+                                        v_new_ptr or None, out_ptr, q_layer_stride_bytes, kv_layer_stride_bytes,
+                                        sm_scale, flags, stream or None), "paged_decode_step_layers")
+
+
 def paged_decode_step_host(handle: int, layer: int, req_ids, q_host_ptr: int, k_new_host_ptr: int,
                            v_new_host_ptr: int, out_host_ptr: int, sm_scale: float, staging_ptr: int,
                            staging_bytes: int, stream: int = 0) -> None:
@@ -225,7 +248,7 @@ def paged_varlen_attention(handle: int, layer: int, req_ids, q_lens, q_ptr: int,
                                       stream or None), "paged_varlen_attention")
 
 
-KERNEL_KINDS = {"attn": 0, "combine": 1, "ingest": 2, "gather": 3, "varq": 4}
+KERNEL_KINDS = {"attn": 0, "combine": 1, "ingest": 2, "gather": 3, "varq": 4, "transfer": 5}
 
 
 def kv_profile_read(handle: int, kind: int):
@@ -262,6 +285,23 @@ def kv_pool_stats(handle: int) -> dict:
 
 def kv_gather(handle: int, req_id: int, k_dst_ptr: int, v_dst_ptr: int, stream: int = 0) -> None:
     _check(lib.kv_gather(handle, req_id, k_dst_ptr, v_dst_ptr, stream or None), "kv_gather")
+
+
+def kv_gather_bytes(cfg: PoolConfig, n_tokens: int) -> int:
+    c = cfg._c()
+    n = lib.kv_gather_bytes(ctypes.byref(c), n_tokens)
+    if n < 0:
+        raise KVError(int(n), "kv_gather_bytes")
+    return int(n)
+
+
+def kv_transfer(dst_handle: int, src_handle: int, dst_req_ids, src_req_ids, layer_begin: int = 0, layer_count: int = 1,
+                stream: int = 0) -> None:
+    """NEXT-4: requests src_req_ids of the producer pool become requests dst_req_ids of the consumer pool."""
+    d, s_ = _ids(dst_req_ids), _ids(src_req_ids)
+    assert d.shape == s_.shape
+    _check(lib.kv_transfer(dst_handle, src_handle, d.size, _np(d), _np(s_), layer_begin, layer_count, stream or None),
+           "kv_transfer")
 
 
 def kv_plan_decode(handle: int, req_ids):
@@ -399,15 +439,33 @@ class KVPool:
                                self._stream(stream))
         return out
 
-    def gather(self, req_id, stream=None):
+    def gather(self, req_id, stream=None, src_kv_heads=None):
+        """bf16 pool: (k, v) bf16 [L][H][n][d].  FP8 pool: (k_codes u8 [L][H][n][d], k_scales f32 [L][H][n],
+        v_codes, v_scales) — views of the two buffers kv_gather fills.  H = src_kv_heads or the pool's kv heads."""
         import torch
 
         _, n = kv_block_table(self.handle, req_id)
         c = self.cfg
-        k = torch.empty((c.num_layers, c.num_kv_heads, n, c.head_dim), dtype=torch.bfloat16, device=self.slab.device)
-        v = torch.empty_like(k)
-        kv_gather(self.handle, req_id, k.data_ptr(), v.data_ptr(), self._stream(stream))
-        return k, v
+        H = src_kv_heads or c.num_kv_heads
+        dev = self.slab.device
+        if c.kv_dtype == KV_DTYPE_BF16:
+            k = torch.empty((c.num_layers, H, n, c.head_dim), dtype=torch.bfloat16, device=dev)
+            v = torch.empty_like(k)
+            kv_gather(self.handle, req_id, k.data_ptr(), v.data_ptr(), self._stream(stream))
+            return k, v
+        rows = c.num_layers * H * n
+        codes = (rows * c.head_dim + 15) // 16 * 16
+        kb = torch.empty(codes + 4 * rows, dtype=torch.uint8, device=dev)
+        vb = torch.empty_like(kb)
+        kv_gather(self.handle, req_id, kb.data_ptr(), vb.data_ptr(), self._stream(stream))
+        split = lambda b: (b[: rows * c.head_dim].view(c.num_layers, H, n, c.head_dim),
+                           b[codes:].view(torch.float32).view(c.num_layers, H, n))
+        return (*split(kb), *split(vb))
+
+    def transfer_from(self, src: "KVPool", dst_req_ids, src_req_ids, layer_begin=0, layer_count=None, stream=None):
+        """NEXT-4: pull requests out of the producer pool `src` into this pool, block to block."""
+        lc = self.cfg.num_layers - layer_begin if layer_count is None else layer_count
+        kv_transfer(self.handle, src.handle, dst_req_ids, src_req_ids, layer_begin, lc, self._stream(stream))
 
     def free(self, req_ids):
         kv_free(self.handle, req_ids)

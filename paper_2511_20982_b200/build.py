@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libkvpool.so")
 SOURCES = ["kv_pool.cu"]
-DEPS = SOURCES + ["kv_kernels.cuh", "kv_fp8.cuh", "kv_attn_ring.cuh", "kv_host.h", os.path.join("..", "..", "include", "kv_pool.h")]
+DEPS = SOURCES + ["kv_common.cuh", "kv_copy.cuh", "kv_attn.cuh", "kv_host.h", os.path.join("..", "..", "include", "kv_pool.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -22,11 +22,26 @@ NVCC_FLAGS = [
 ]
 
 
+STAMP = LIB + ".srchash"
+
+
+def source_hash() -> str:
+    """sha256 over the sources, headers, flags and this file: what the built library must correspond to.
+    (mtimes do not survive a copy of the tree to another box; contents do.)"""
+    import hashlib
+    h = hashlib.sha256(" ".join(NVCC_FLAGS).encode())
+    for d in sorted(DEPS):
+        with open(os.path.join(CSRC, d), "rb") as f:
+            h.update(d.encode() + b"\0" + f.read())
+    return h.hexdigest()
+
+
 def stale() -> bool:
-    if not os.path.exists(LIB):
+    """True if libkvpool.so is missing or was not built from the sources that are in the tree now."""
+    if not os.path.exists(LIB) or not os.path.exists(STAMP):
         return True
-    t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPS + [os.path.join("..", "build.py")])
+    with open(STAMP) as f:
+        return f.read().strip() != source_hash()
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -41,6 +56,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if r.returncode != 0:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
         os.replace(tmp, LIB)
+        with open(STAMP, "w") as f:
+            f.write(source_hash() + "\n")
     return LIB
 
 

@@ -50,6 +50,7 @@ class BlockAllocator {
     return b;
   }
   void push(int32_t b) { free_.push_back(b); }
+  void set_high_water(int64_t v) { high_water_ = v; }
 
  private:
   std::vector<int32_t> free_;
@@ -94,6 +95,8 @@ struct DecodePlan {
   int32_t n_partials = 0;
 };
 
+constexpr int32_t kMaxBlocksPerRequest = 131072;
+
 class HostState {
  public:
   kv_pool_config_t cfg{};
@@ -109,7 +112,9 @@ class HostState {
     if (c.kv_dtype != KV_DTYPE_BF16 && c.kv_dtype != KV_DTYPE_FP8_E4M3) return KV_ERR_INVALID;
     if (c.num_q_heads % c.num_kv_heads != 0 || c.num_q_heads / c.num_kv_heads > 8) return KV_ERR_INVALID;
     if (c.num_blocks < 1 || c.num_blocks > 0x7fffffffLL) return KV_ERR_INVALID;
-    if (c.max_requests < 1 || c.max_blocks_per_request < 1) return KV_ERR_INVALID;
+    // <= 131072 blocks (2 Mi tokens) per request: lengths stay far inside int32, the (n_chunks, chunk) pair fits its
+    // 16:16 packing, and one request's descriptor (48 B + 8 B per block for a transfer) fits an ingest blob
+    if (c.max_requests < 1 || c.max_blocks_per_request < 1 || c.max_blocks_per_request > kMaxBlocksPerRequest) return KV_ERR_INVALID;
     if (static_cast<int64_t>(c.max_requests) * c.max_blocks_per_request > (1LL << 31)) return KV_ERR_INVALID;
     return KV_OK;
   }
@@ -152,15 +157,19 @@ class HostState {
     }
     if (fresh_.size() > free_slots.size()) return KV_ERR_TOO_MANY_REQUESTS;
     if (need_blocks > alloc.free_count()) return KV_ERR_NO_BLOCKS;
+    undo_.clear();
+    undo_high_water_ = alloc.high_water();
     for (int32_t i = 0; i < n_req; ++i) {
       auto it = reqs.find(ids[i]);
-      if (it == reqs.end()) {
+      const bool created = it == reqs.end();
+      if (created) {
         Request r;
         r.slot = free_slots.back();
         free_slots.pop_back();
         it = reqs.emplace(ids[i], std::move(r)).first;
       }
       Request& r = it->second;
+      undo_.push_back({ids[i], r.last_n, n_tokens[i], created});
       int32_t want = blocks_for(static_cast<int64_t>(r.len) + n_tokens[i]);
       while (static_cast<int32_t>(r.blocks.size()) < want) r.blocks.push_back(alloc.pop());
       r.len += n_tokens[i];
@@ -168,6 +177,24 @@ class HostState {
     }
     ++epoch;
     return KV_OK;
+  }
+
+  // Undo the LAST successful reserve() exactly (a call that reserved and then could not launch must leave the
+  // pool as it found it): blocks go back in reverse order of their pops, so the free list, the slot list and the
+  // high-water mark are what they were; requests the reservation created are dropped.
+  void rollback_last_reserve() {
+    for (auto u = undo_.rbegin(); u != undo_.rend(); ++u) {
+      auto it = reqs.find(u->id);
+      Request& r = it->second;
+      r.len -= u->n_tokens;
+      r.last_n = u->prev_last_n;
+      const int32_t want = blocks_for(r.len);
+      while (static_cast<int32_t>(r.blocks.size()) > want) { alloc.push(r.blocks.back()); r.blocks.pop_back(); }
+      if (u->created) { free_slots.push_back(r.slot); reqs.erase(it); }
+    }
+    alloc.set_high_water(undo_high_water_);
+    undo_.clear();
+    ++epoch;
   }
 
   // a6.  Atomic: unknown or duplicate id => nothing freed.
@@ -368,6 +395,9 @@ class HostState {
   mutable std::vector<WorkItem> unsorted_;
   mutable std::vector<int32_t> count_, order_;
   std::vector<int64_t> fresh_;
+  struct Undo { int64_t id; int32_t prev_last_n, n_tokens; bool created; };
+  std::vector<Undo> undo_;
+  int64_t undo_high_water_ = 0;
   mutable uint64_t plan_stamp_ = 0;
 };
 

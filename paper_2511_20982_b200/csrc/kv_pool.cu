@@ -1,6 +1,6 @@
-// kv_pool.cu — the C-ABI of include/kv_pool.h: argument checking, host bookkeeping
-// (kv_host.h), staging of small descriptor blobs, and kernel launches (kv_kernels.cuh).
-// Every step of the data path runs in the kernels; nothing here touches KV bytes on the host.
+// kv_pool.cu — the C-ABI of include/kv_pool.h: argument checking, host bookkeeping (kv_host.h), staging of small
+// descriptor blobs, and kernel launches (kv_copy.cuh, kv_attn.cuh).  Every step of the data path runs in the
+// kernels; nothing here touches KV bytes on the host.
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -11,9 +11,9 @@
 
 #include "../../include/kv_pool.h"
 #include "kv_host.h"
-#include "kv_kernels.cuh"
-#include "kv_fp8.cuh"
-#include "kv_attn_ring.cuh"
+#include "kv_common.cuh"
+#include "kv_copy.cuh"
+#include "kv_attn.cuh"
 
 namespace {
 
@@ -21,9 +21,11 @@ using namespace kvp;
 
 constexpr int64_t kAlign = 256;
 constexpr int kRing = 4;                       // plan staging slots
-constexpr int64_t kIngestBlobBytes = 1 << 20;  // per ingest launch; larger calls are sub-batched
+constexpr int64_t kIngestBlobBytes = 2 << 20;  // per ingest launch; larger calls are sub-batched.  One request's
+                                               // descriptor (48 B + <= 8 B x kMaxBlocksPerRequest) always fits.
 constexpr int64_t kIngestRingBytes = 16 << 20; // descriptor staging ring: ~1000 decode appends in flight
 constexpr int32_t kMaxPartials = 32768;        // split-KV partial slots in the workspace
+static_assert(48 + 8LL * kvp::kMaxBlocksPerRequest <= kIngestBlobBytes, "a request's descriptor must fit one blob");
 
 inline int64_t align_up(int64_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
@@ -32,12 +34,14 @@ struct Layout {  // byte offsets inside the caller's slab
   int64_t plan_blob_bytes;
 };
 
+int64_t tile_bytes(const kv_pool_config_t& c) {
+  return c.kv_dtype == KV_DTYPE_FP8_E4M3 ? 32LL * c.head_dim + 128 : 2LL * c.block_size * c.head_dim * 2;
+}
+
 Layout make_layout(const kv_pool_config_t& c) {
   Layout L{};
   const int64_t G = c.num_q_heads / c.num_kv_heads;
-  L.kv_bytes = c.kv_dtype == KV_DTYPE_FP8_E4M3
-                   ? static_cast<int64_t>(c.num_layers) * c.num_blocks * c.num_kv_heads * (32LL * c.head_dim + 128)
-                   : static_cast<int64_t>(c.num_layers) * c.num_blocks * c.num_kv_heads * 2 * c.block_size * c.head_dim * 2;
+  L.kv_bytes = static_cast<int64_t>(c.num_layers) * c.num_blocks * c.num_kv_heads * tile_bytes(c);
   int64_t off = align_up(L.kv_bytes);
   L.block_table = off;
   off = align_up(off + static_cast<int64_t>(c.max_requests) * c.max_blocks_per_request * 4);
@@ -129,10 +133,11 @@ struct ByteRing {
   }
 };
 
-// Event pairs around the launches of one kernel kind (kv_profile_read).
+// Event pairs around the launches of one kernel kind (kv_profile_read).  A pair may bracket a group of
+// back-to-back launches (paged_decode_step_layers): the group's time is attributed to `count` launches.
 struct ProfRing {
   std::vector<cudaEvent_t> a, b;
-  std::vector<char> live;
+  std::vector<int32_t> live;        // launches bracketed by pair i (0: free)
   int next = 0;
   int64_t launches = 0;
   double ms = 0.0;
@@ -142,7 +147,7 @@ struct ProfRing {
     cudaError_t e = cudaEventSynchronize(b[static_cast<size_t>(i)]);
     float t = 0.f;
     if (e == cudaSuccess) e = cudaEventElapsedTime(&t, a[static_cast<size_t>(i)], b[static_cast<size_t>(i)]);
-    if (e == cudaSuccess) { ms += t; ++launches; }
+    if (e == cudaSuccess) { ms += t; launches += live[static_cast<size_t>(i)]; }
     live[static_cast<size_t>(i)] = 0;
     return e;
   }
@@ -159,9 +164,9 @@ struct ProfRing {
     if (e != cudaSuccess) return e;
     return cudaEventRecord(a[static_cast<size_t>(next)], st);
   }
-  cudaError_t end(cudaStream_t st) {
+  cudaError_t end(cudaStream_t st, int32_t count = 1) {
     cudaError_t e = cudaEventRecord(b[static_cast<size_t>(next)], st);
-    live[static_cast<size_t>(next)] = 1;
+    live[static_cast<size_t>(next)] = count;
     next = (next + 1) % KV_PROFILE_RING;
     return e;
   }
@@ -186,20 +191,21 @@ struct kv_pool {
   Layout lay{};
   bool has_device = false;
   char* base = nullptr;
+  int device = 0;                  // the device the slab lives on (cudaPointerGetAttributes at create)
   int num_sms = 148;
   int32_t last_cuda = 0;
   int64_t launches = 0;
   // tuning
   int32_t min_chunk_blocks = 64;   // smallest split-KV chunk: 64 blocks = 512 KiB of KV per unit at d = 128 (bf16);
   bool min_chunk_set = false;      //   FP8 pools default to 32 blocks (tiles are half the bytes) unless the caller chose
-  int32_t ctas_per_sm = 2;
+  int32_t ctas_per_sm = 0;         // 0: what the kernel variant runs with (2 or 3); else the planner sizes for this many
   int32_t items_per_slot = 2;     // guided chunking: first chunk = remaining work / (2 x resident warps)
-  bool items_per_slot_set = false;  // FP8 ring kernel (12 warps per SM): 1 measured best unless the caller chose
+  bool items_per_slot_set = false;  // FP8 kernel (12 warps per SM): 1 measured best unless the caller chose
   bool fuse_combine = true;
   int32_t src_kv_heads = 0;       // KV-head sharding: heads of the contiguous side of ingest / gather (0: this pool's own)
   int32_t src_head_begin = 0;     //                   this pool's head 0 is that side's head src_head_begin
-  int32_t ring = 3;               // bf16 pool: 3 (default) / 2: attn_ring_kernel with that many slots per warp (2 / 3 CTAs per SM); 0: register-tile attn_splitkv_kernel
-  bool fp8_ring = true;           // FP8 pool: attn_fp8_ring_kernel (shared-memory tile ring) vs attn_fp8_kernel (register tiles)
+  int32_t ring = 3;               // bf16 pool: ring slots per warp, 3 (2 CTAs per SM, default) or 2 (3 CTAs per SM)
+  bool pdl = true;                // attention launches carry the programmatic-dependent-launch attribute
   bool profile = false;
   ProfRing prof[KV_KERNEL_KINDS];
   // staging
@@ -217,23 +223,25 @@ struct kv_pool {
   int32_t plan_append_ok = -1;  // -1 unknown, 0 / 1: every request's last reservation is one token
   int64_t plan_combine_off = 0;
   kvp::DecodePlan plan;
+  std::vector<int32_t> ones;
+  // ordering of attention launches (they share the pool's device workspace): the stream of the last one and an
+  // event behind it (the staged plan slot's), and what a following launch may assume about its predecessor
+  bool attn_any = false;
+  cudaStream_t attn_stream = nullptr;
+  cudaEvent_t attn_ev = nullptr;
+  int chain_slot = -1;          // plan slot of the pool's LAST launch if that was an attention launch, else -1
+  int chain_kind = 0;           // 0 decode, 1 decode + append, 2 variable-q
 
   int32_t cuda_fail(cudaError_t e) {
     last_cuda = static_cast<int32_t>(e);
     return KV_ERR_CUDA;
   }
-  int32_t slots() const {
-    const int32_t ctas = (hs.cfg.kv_dtype == KV_DTYPE_FP8_E4M3 && fp8_ring) ? 3
-                         : (hs.cfg.kv_dtype == KV_DTYPE_BF16 && ring == 2) ? 3 : ctas_per_sm;
-    return num_sms * ctas * kvp::kAttnWarps;
-  }
+  bool fp8() const { return hs.cfg.kv_dtype == KV_DTYPE_FP8_E4M3; }
+  int32_t kernel_ctas() const { return fp8() ? 3 : (ring == 2 ? 3 : 2); }
+  int32_t slots() const { return num_sms * (ctas_per_sm > 0 ? ctas_per_sm : kernel_ctas()) * kvp::kAttnWarps; }
   int32_t src_heads() const { return src_kv_heads > 0 ? src_kv_heads : hs.cfg.num_kv_heads; }
-  int32_t min_chunk() const {
-    return (hs.cfg.kv_dtype == KV_DTYPE_FP8_E4M3 && !min_chunk_set) ? 32 : min_chunk_blocks;
-  }
-  int32_t ips() const {
-    return (hs.cfg.kv_dtype == KV_DTYPE_FP8_E4M3 && fp8_ring && !items_per_slot_set) ? 1 : items_per_slot;
-  }
+  int32_t min_chunk() const { return (fp8() && !min_chunk_set) ? 32 : min_chunk_blocks; }
+  int32_t ips() const { return (fp8() && !items_per_slot_set) ? 1 : items_per_slot; }
 };
 
 namespace {
@@ -244,9 +252,27 @@ namespace {
     if (e_ != cudaSuccess) return (pool)->cuda_fail(e_);      \
   } while (0)
 
-int32_t acquire(kv_pool* pool, StageSlot* ring, int* next, StageSlot** out, int avoid = -1) {
-  int idx = *next;
-  if (idx == avoid) idx = (idx + 1) % kRing;
+// Calls run on the pool's device whatever device is current, and leave the caller's current device as it was.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  cudaError_t err = cudaSuccess;
+  explicit DeviceGuard(const kv_pool* pool) {
+    if (!pool->has_device) return;
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != pool->device) {
+      err = cudaSetDevice(pool->device);
+      switched = err == cudaSuccess;
+    }
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+#define KV_ON_DEVICE(pool)                                    \
+  DeviceGuard guard_(pool);                                   \
+  if (guard_.err != cudaSuccess) return (pool)->cuda_fail(guard_.err)
+
+int32_t acquire(kv_pool* pool, StageSlot* ring, int* next, StageSlot** out) {
+  const int idx = *next;
   *next = (idx + 1) % kRing;
   StageSlot& s = ring[idx];
   if (s.in_flight) {
@@ -259,9 +285,12 @@ int32_t acquire(kv_pool* pool, StageSlot* ring, int* next, StageSlot** out, int 
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-template <bool kGather>
-int32_t launch_ingest(kv_pool* pool, const std::vector<IngestReq>& reqs, const std::vector<int32_t>& ids,
-                      int64_t total_units, int32_t layer_begin, int32_t layer_count, cudaStream_t stream) {
+enum class CopyKind { kScatter, kGather, kTransfer };
+
+// One launch of a relocation kernel over the serialised requests `reqs` / block ids `ids`.
+int32_t launch_copy(kv_pool* pool, CopyKind kind, const kv_pool* src_pool, const std::vector<IngestReq>& reqs,
+                    const std::vector<int32_t>& ids, int64_t total_units, int32_t layer_begin, int32_t layer_count,
+                    cudaStream_t stream) {
   if (total_units == 0) return KV_OK;
   const size_t req_bytes = reqs.size() * sizeof(IngestReq);
   const size_t id_bytes = ids.size() * sizeof(int32_t);
@@ -288,38 +317,46 @@ int32_t launch_ingest(kv_pool* pool, const std::vector<IngestReq>& reqs, const s
   p.num_blocks = c.num_blocks;
   p.src_kv_heads = pool->src_heads();
   p.src_head_begin = pool->src_head_begin;
+  if (src_pool) {
+    p.src_kv = reinterpret_cast<const uint16_t*>(src_pool->base);
+    p.src_num_blocks = src_pool->hs.cfg.num_blocks;
+  }
+  const bool fp8 = pool->fp8(), d128 = c.head_dim == 128;
   const unsigned grid = static_cast<unsigned>((total_units + kIngestWarps - 1) / kIngestWarps);
-  ProfRing& pr = pool->prof[kGather ? KV_KERNEL_GATHER : KV_KERNEL_INGEST];
+  const int prof_kind = kind == CopyKind::kScatter ? KV_KERNEL_INGEST : kind == CopyKind::kGather ? KV_KERNEL_GATHER : KV_KERNEL_TRANSFER;
+  ProfRing& pr = pool->prof[prof_kind];
   if (pool->profile) KV_CUDA(pool, pr.begin(stream));
-  if (c.kv_dtype == KV_DTYPE_FP8_E4M3) {
-    if (kGather) return KV_ERR_UNSUPPORTED;
+  if (kind == CopyKind::kTransfer) {
+    if (fp8) { if (d128) transfer_kernel<128, true><<<grid, kIngestThreads, 0, stream>>>(p); else transfer_kernel<64, true><<<grid, kIngestThreads, 0, stream>>>(p); }
+    else     { if (d128) transfer_kernel<128, false><<<grid, kIngestThreads, 0, stream>>>(p); else transfer_kernel<64, false><<<grid, kIngestThreads, 0, stream>>>(p); }
+  } else if (kind == CopyKind::kGather) {
+    if (fp8) { if (d128) gather_fp8_kernel<128><<<grid, kIngestThreads, 0, stream>>>(p); else gather_fp8_kernel<64><<<grid, kIngestThreads, 0, stream>>>(p); }
+    else     { if (d128) ingest_kernel<128, true><<<grid, kIngestThreads, 0, stream>>>(p); else ingest_kernel<64, true><<<grid, kIngestThreads, 0, stream>>>(p); }
+  } else if (fp8) {
     const unsigned grid8 = static_cast<unsigned>((2 * total_units + kIngest8Warps - 1) / kIngest8Warps);   // a warp per (unit, K|V)
-    if (c.head_dim == 128)
-      ingest_fp8_kernel<128><<<grid8, kIngest8Threads, 0, stream>>>(p);
-    else
-      ingest_fp8_kernel<64><<<grid8, kIngest8Threads, 0, stream>>>(p);
-  } else if (c.head_dim == 128)
-    ingest_kernel<128, kGather><<<grid, kIngestThreads, 0, stream>>>(p);
-  else
-    ingest_kernel<64, kGather><<<grid, kIngestThreads, 0, stream>>>(p);
+    if (d128) ingest_fp8_kernel<128><<<grid8, kIngest8Threads, 0, stream>>>(p); else ingest_fp8_kernel<64><<<grid8, kIngest8Threads, 0, stream>>>(p);
+  } else {
+    if (d128) ingest_kernel<128, false><<<grid, kIngestThreads, 0, stream>>>(p); else ingest_kernel<64, false><<<grid, kIngestThreads, 0, stream>>>(p);
+  }
   KV_CUDA(pool, cudaGetLastError());
   if (pool->profile) KV_CUDA(pool, pr.end(stream));
   ++pool->launches;
+  pool->chain_slot = -1;   // the pool's last launch is no longer an attention launch
   KV_CUDA(pool, ring.commit(off, static_cast<int64_t>(req_bytes + id_bytes), stream));
   return KV_OK;
 }
 
-// Serialise requests into ingest launches, sub-batching so each blob fits its staging slot.
-template <bool kGather>
-int32_t run_ingest(kv_pool* pool, int32_t n_req, const int64_t* req_ids, const int32_t* n_tokens,
-                   const void* const* k_ptrs, const void* const* v_ptrs, const int32_t* start_pos,
-                   int32_t layer_begin, int32_t layer_count, cudaStream_t stream) {
+// Serialise requests into copy launches, sub-batching so each blob fits its staging segment.  For a transfer
+// src_pool / src_ids name the producer's pool and request ids; its block ids follow the consumer's per request.
+int32_t run_copy(kv_pool* pool, CopyKind kind, const kv_pool* src_pool, const int64_t* src_ids, int32_t n_req,
+                 const int64_t* req_ids, const int32_t* n_tokens, const void* const* k_ptrs, const void* const* v_ptrs,
+                 const int32_t* start_pos, int32_t layer_begin, int32_t layer_count, cudaStream_t stream) {
   const kv_pool_config_t& c = pool->hs.cfg;
   std::vector<IngestReq> reqs;
   std::vector<int32_t> ids;
   int64_t units = 0;
   auto flush = [&]() -> int32_t {
-    int32_t rc = launch_ingest<kGather>(pool, reqs, ids, units, layer_begin, layer_count, stream);
+    int32_t rc = launch_copy(pool, kind, src_pool, reqs, ids, units, layer_begin, layer_count, stream);
     reqs.clear();
     ids.clear();
     units = 0;
@@ -332,16 +369,15 @@ int32_t run_ingest(kv_pool* pool, int32_t n_req, const int64_t* req_ids, const i
     const int32_t b0 = sp / c.block_size;
     const int32_t b1 = (sp + n_tokens[i] - 1) / c.block_size;
     const int32_t touched = b1 - b0 + 1;
-    const int64_t need = static_cast<int64_t>(sizeof(IngestReq)) + 4LL * touched;
+    const int64_t need = static_cast<int64_t>(sizeof(IngestReq)) + (src_pool ? 8LL : 4LL) * touched;
     const int64_t used = static_cast<int64_t>(reqs.size() * sizeof(IngestReq) + ids.size() * 4);
-    if (need > kIngestBlobBytes) return KV_ERR_TOO_LONG;
-    if (used + need > kIngestBlobBytes) {
+    if (used + need > kIngestBlobBytes) {   // need alone always fits (kMaxBlocksPerRequest)
       int32_t rc = flush();
       if (rc != KV_OK) return rc;
     }
     IngestReq q{};
-    q.k_src = reinterpret_cast<uint64_t>(k_ptrs[i]);
-    q.v_src = reinterpret_cast<uint64_t>(v_ptrs[i]);
+    q.k_src = k_ptrs ? reinterpret_cast<uint64_t>(k_ptrs[i]) : 0;
+    q.v_src = v_ptrs ? reinterpret_cast<uint64_t>(v_ptrs[i]) : 0;
     q.unit_begin = units;
     q.n_tokens = n_tokens[i];
     q.start_pos = sp;
@@ -351,58 +387,88 @@ int32_t run_ingest(kv_pool* pool, int32_t n_req, const int64_t* req_ids, const i
     q.blk_off = static_cast<int32_t>(ids.size());
     reqs.push_back(q);
     ids.insert(ids.end(), r.blocks.begin() + b0, r.blocks.begin() + b1 + 1);
+    if (src_pool) {
+      const Request& sr = src_pool->hs.reqs.find(src_ids[i])->second;
+      ids.insert(ids.end(), sr.blocks.begin() + b0, sr.blocks.begin() + b1 + 1);
+    }
     units += static_cast<int64_t>(touched) * layer_count * c.num_kv_heads;
   }
   return flush();
 }
 
-// attn_fp8_ring_kernel launch: 4 ring slots per warp, 3 CTAs per SM.
-constexpr int kFp8RingSlots = 4;
-template <int D, bool kAppend, bool kVarQ>
-static cudaError_t launch_fp8_ring(const AttnParams& p, int num_sms, int want, cudaStream_t stream) {
-  static bool ready_dev[64] = {};                               // the opt-in is per device
-  int dev = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess) return cudaGetLastError();
-  bool& ready = ready_dev[dev & 63];
-  constexpr size_t smem = static_cast<size_t>(kAttnWarps) * kFp8RingSlots * (32 * D + 128);
-  if (!ready) {
-    cudaError_t e = cudaFuncSetAttribute(attn_fp8_ring_kernel<D, kFp8RingSlots, kAppend, kVarQ>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
-    if (e != cudaSuccess) return e;
-    ready = true;
-  }
-  const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, num_sms * 3)));
-  attn_fp8_ring_kernel<D, kFp8RingSlots, kAppend, kVarQ><<<grid, kAttnThreads, smem, stream>>>(p);
-  return cudaGetLastError();
+// ---- attention kernel variants ---------------------------------------------------------------
+
+using AttnFn = void (*)(const AttnParams);
+struct AttnVariant {
+  AttnFn fn;
+  size_t smem;
+  int ctas;
+};
+
+constexpr int kFp8RingSlots = 4;   // FP8 pools: 4 ring slots per warp, 3 CTAs per SM
+
+template <class TP, bool kAppend, bool kVarQ, int R, int kCtas>
+AttnVariant variant() {
+  return {attn_kernel<TP, kAppend, kVarQ, R, kCtas>, static_cast<size_t>(kAttnWarps) * R * TP::kSlotBytes, kCtas};
+}
+template <class TP, int R, int kCtas>
+AttnVariant variant_of(bool append, bool varq) {
+  if (varq) return variant<TP, false, true, R, kCtas>();
+  return append ? variant<TP, true, false, R, kCtas>() : variant<TP, false, false, R, kCtas>();
+}
+AttnVariant pick_variant(const kv_pool* pool, bool append, bool varq) {
+  const bool d128 = pool->hs.cfg.head_dim == 128;
+  if (pool->fp8())
+    return d128 ? variant_of<Fp8Tiles<128>, kFp8RingSlots, 3>(append, varq) : variant_of<Fp8Tiles<64>, kFp8RingSlots, 3>(append, varq);
+  if (pool->ring == 2)
+    return d128 ? variant_of<Bf16Tiles<128>, 2, 3>(append, varq) : variant_of<Bf16Tiles<64>, 2, 3>(append, varq);
+  return d128 ? variant_of<Bf16Tiles<128>, 3, 2>(append, varq) : variant_of<Bf16Tiles<64>, 3, 2>(append, varq);
 }
 
-// attn_ring_kernel launch: R slots per warp, kCtas CTAs per SM; dynamic shared memory above 48 KiB needs the opt-in.
-template <int D, bool kAppend, bool kVarQ, int R, int kCtas>
-static cudaError_t launch_ring(const AttnParams& p, int num_sms, int want, cudaStream_t stream) {
-  static bool ready_dev[64] = {};                               // the opt-in is per device
-  int dev = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess) return cudaGetLastError();
-  bool& ready = ready_dev[dev & 63];
-  constexpr size_t smem = static_cast<size_t>(kAttnWarps) * R * (2 * kBlockSize * D * 2);
-  if (!ready) {
-    cudaError_t e = cudaFuncSetAttribute(attn_ring_kernel<D, kAppend, kVarQ, R, kCtas>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
-    if (e != cudaSuccess) return e;
-    ready = true;
-  }
-  const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, num_sms * kCtas)));
-  attn_ring_kernel<D, kAppend, kVarQ, R, kCtas><<<grid, kAttnThreads, smem, stream>>>(p);
-  return cudaGetLastError();
+// Dynamic shared memory above 48 KiB needs an opt-in per (kernel, device).
+cudaError_t ensure_smem_optin(const AttnVariant& v, int device) {
+  struct Key { AttnFn fn; int dev; };
+  static std::vector<Key> done;
+  for (const Key& k : done) if (k.fn == v.fn && k.dev == device) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void*>(v.fn), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       static_cast<int>(v.smem));
+  if (e == cudaSuccess) done.push_back({v.fn, device});
+  return e;
 }
 
-template <bool kAppend, bool kVarQ>
-static cudaError_t launch_ring_any(int head_dim, int ring, const AttnParams& p, int num_sms, int want, cudaStream_t stream) {
-  if (head_dim == 128) {
-    if (ring == 2) return launch_ring<128, kAppend, kVarQ, 2, 3>(p, num_sms, want, stream);
-    return launch_ring<128, kAppend, kVarQ, 3, 2>(p, num_sms, want, stream);
+cudaError_t launch_attn_kernel(const kv_pool* pool, const AttnVariant& v, const AttnParams& p, cudaStream_t stream) {
+  cudaError_t e = ensure_smem_optin(v, pool->device);
+  if (e != cudaSuccess) return e;
+  const int32_t want = (p.n_units + kAttnWarps - 1) / kAttnWarps;
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * v.ctas))));
+  cfg.blockDim = dim3(kAttnThreads);
+  cfg.dynamicSmemBytes = v.smem;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = pool->pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, v.fn, p);
+}
+
+// Attention launches of one pool must not overlap (shared workspace): a call on another stream than the
+// previous one is ordered behind it.
+int32_t order_attention(kv_pool* pool, cudaStream_t stream) {
+  if (pool->attn_any && stream != pool->attn_stream) {
+    KV_CUDA(pool, cudaStreamWaitEvent(stream, pool->attn_ev, 0));
+    pool->chain_slot = -1;
   }
-  if (ring == 2) return launch_ring<64, kAppend, kVarQ, 2, 3>(p, num_sms, want, stream);
-  return launch_ring<64, kAppend, kVarQ, 3, 2>(p, num_sms, want, stream);
+  return KV_OK;
+}
+
+void attention_launched(kv_pool* pool, cudaStream_t stream, const StageSlot& s, int kind) {
+  pool->attn_any = true;
+  pool->attn_stream = stream;
+  pool->attn_ev = s.ev;
+  pool->chain_slot = pool->plan_slot;
+  pool->chain_kind = kind;
 }
 
 }  // namespace
@@ -438,11 +504,19 @@ int32_t kv_pool_create(const kv_pool_config_t* cfg, kv_pool_t** out_pool) {
   pool->hs.init(*cfg);
   pool->lay = lay;
   if (cfg->device_base) {
-    pool->has_device = true;
     pool->base = static_cast<char*>(cfg->device_base);
-    int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&pool->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    // the pool lives where its slab lives, whatever device happens to be current
+    cudaPointerAttributes pa{};
+    cudaError_t e = cudaPointerGetAttributes(&pa, cfg->device_base);
+    if (e == cudaSuccess && pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) {
+      delete pool;
+      return KV_ERR_INVALID;
+    }
+    if (e == cudaSuccess) pool->device = pa.device;
+    pool->has_device = true;
+    DeviceGuard guard(pool);
+    if (e == cudaSuccess) e = guard.err;
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&pool->num_sms, cudaDevAttrMultiProcessorCount, pool->device);
     if (e == cudaSuccess) e = cudaHostAlloc(reinterpret_cast<void**>(&pool->ingest_ring.host), kIngestRingBytes, cudaHostAllocDefault);
     pool->ingest_ring.dev = pool->base + lay.ingest_blobs;
     pool->ingest_ring.cap = kIngestRingBytes;
@@ -465,12 +539,15 @@ int32_t kv_pool_create(const kv_pool_config_t* cfg, kv_pool_t** out_pool) {
 
 int32_t kv_pool_destroy(kv_pool_t* pool) {
   if (!pool) return KV_ERR_INVALID;
-  pool->ingest_ring.destroy();
-  for (int i = 0; i < kRing; ++i) {
-    if (pool->plan_ring[i].host) cudaFreeHost(pool->plan_ring[i].host);
-    if (pool->plan_ring[i].ev) cudaEventDestroy(pool->plan_ring[i].ev);
+  {
+    DeviceGuard guard(pool);
+    pool->ingest_ring.destroy();
+    for (int i = 0; i < kRing; ++i) {
+      if (pool->plan_ring[i].host) cudaFreeHost(pool->plan_ring[i].host);
+      if (pool->plan_ring[i].ev) cudaEventDestroy(pool->plan_ring[i].ev);
+    }
+    for (ProfRing& r : pool->prof) r.destroy();
   }
-  for (ProfRing& r : pool->prof) r.destroy();
   delete pool;
   return KV_OK;
 }
@@ -480,9 +557,21 @@ int32_t kv_reserve(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const
   return pool->hs.reserve(n_req, req_ids, n_tokens);
 }
 
-int32_t kv_ingest(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const int32_t* n_tokens,
-                  const void* const* k_src, const void* const* v_src, int32_t layer_begin, int32_t layer_count,
-                  void* cuda_stream) {
+// a1 (reserve or continuation check) + a2/a3 launch, atomic: any failure after the reservation rolls it back.
+static int32_t ingest_reserved(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const int32_t* n_tokens,
+                               const void* const* k_dev, const void* const* v_dev, int32_t layer_begin,
+                               int32_t layer_count, cudaStream_t stream) {
+  std::vector<int32_t> start(static_cast<size_t>(n_req));
+  for (int32_t i = 0; i < n_req; ++i) start[static_cast<size_t>(i)] = pool->hs.reqs.find(req_ids[i])->second.len - n_tokens[i];
+  int32_t rc = run_copy(pool, CopyKind::kScatter, nullptr, nullptr, n_req, req_ids, n_tokens, k_dev, v_dev, start.data(),
+                        layer_begin, layer_count, stream);
+  if (rc != KV_OK && layer_begin == 0) pool->hs.rollback_last_reserve();
+  return rc;
+}
+
+static int32_t ingest_args_ok(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const int32_t* n_tokens,
+                              const void* const* k_src, const void* const* v_src, int32_t layer_begin, int32_t layer_count,
+                              bool need_aligned) {
   if (!pool || n_req < 0) return KV_ERR_INVALID;
   if (n_req > 0 && (!req_ids || !n_tokens || !k_src || !v_src)) return KV_ERR_INVALID;
   const kv_pool_config_t& c = pool->hs.cfg;
@@ -490,32 +579,78 @@ int32_t kv_ingest(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const 
   if (!pool->has_device) return KV_ERR_NO_DEVICE;
   for (int32_t i = 0; i < n_req; ++i) {
     if (n_tokens[i] < 0) return KV_ERR_INVALID;
-    if (n_tokens[i] > 0 && (!k_src[i] || !v_src[i] || !aligned16(k_src[i]) || !aligned16(v_src[i]))) return KV_ERR_INVALID;
+    if (n_tokens[i] > 0 && (!k_src[i] || !v_src[i])) return KV_ERR_INVALID;
+    if (n_tokens[i] > 0 && need_aligned && (!aligned16(k_src[i]) || !aligned16(v_src[i]))) return KV_ERR_INVALID;
   }
-  if (layer_begin == 0) {
-    int32_t rc = pool->hs.reserve(n_req, req_ids, n_tokens);
-    if (rc != KV_OK) return rc;
-  } else {  // continuation of the last reservation
-    int32_t rc = pool->hs.check_batch(n_req, req_ids, n_tokens);
-    if (rc != KV_OK) return rc;
-  }
-  std::vector<int32_t> start(static_cast<size_t>(n_req));
-  for (int32_t i = 0; i < n_req; ++i) start[static_cast<size_t>(i)] = pool->hs.reqs.find(req_ids[i])->second.len - n_tokens[i];
-  return run_ingest<false>(pool, n_req, req_ids, n_tokens, k_src, v_src, start.data(), layer_begin, layer_count,
-                           static_cast<cudaStream_t>(cuda_stream));
+  return KV_OK;
+}
+
+int32_t kv_ingest(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const int32_t* n_tokens,
+                  const void* const* k_src, const void* const* v_src, int32_t layer_begin, int32_t layer_count,
+                  void* cuda_stream) {
+  int32_t rc = ingest_args_ok(pool, n_req, req_ids, n_tokens, k_src, v_src, layer_begin, layer_count, true);
+  if (rc != KV_OK) return rc;
+  KV_ON_DEVICE(pool);
+  rc = layer_begin == 0 ? pool->hs.reserve(n_req, req_ids, n_tokens)      // a1
+                        : pool->hs.check_batch(n_req, req_ids, n_tokens); // continuation of the last reservation
+  if (rc != KV_OK) return rc;
+  return ingest_reserved(pool, n_req, req_ids, n_tokens, k_src, v_src, layer_begin, layer_count,
+                         static_cast<cudaStream_t>(cuda_stream));
+}
+
+int64_t kv_gather_bytes(const kv_pool_config_t* cfg, int32_t n_tokens) {
+  if (!cfg || n_tokens < 0) return KV_ERR_INVALID;
+  int32_t rc = HostState::validate(*cfg);
+  if (rc != KV_OK) return rc;
+  const int64_t rows = static_cast<int64_t>(cfg->num_layers) * cfg->num_kv_heads * n_tokens;
+  if (cfg->kv_dtype == KV_DTYPE_FP8_E4M3) return (rows * cfg->head_dim + 15) / 16 * 16 + rows * 4;
+  return rows * cfg->head_dim * 2;
 }
 
 int32_t kv_gather(kv_pool_t* pool, int64_t req_id, void* k_dst, void* v_dst, void* cuda_stream) {
   if (!pool || !k_dst || !v_dst || !aligned16(k_dst) || !aligned16(v_dst)) return KV_ERR_INVALID;
-  if (pool->hs.cfg.kv_dtype != KV_DTYPE_BF16) return KV_ERR_UNSUPPORTED;
   if (!pool->has_device) return KV_ERR_NO_DEVICE;
   auto it = pool->hs.reqs.find(req_id);
   if (it == pool->hs.reqs.end()) return KV_ERR_UNKNOWN_REQUEST;
+  KV_ON_DEVICE(pool);
   const int32_t n = it->second.len, zero = 0;
   const void* kp = k_dst;
   const void* vp = v_dst;
-  return run_ingest<true>(pool, 1, &req_id, &n, &kp, &vp, &zero, 0, pool->hs.cfg.num_layers,
-                          static_cast<cudaStream_t>(cuda_stream));
+  return run_copy(pool, CopyKind::kGather, nullptr, nullptr, 1, &req_id, &n, &kp, &vp, &zero, 0, pool->hs.cfg.num_layers,
+                  static_cast<cudaStream_t>(cuda_stream));
+}
+
+int32_t kv_transfer(kv_pool_t* dst, const kv_pool_t* src, int32_t n_req, const int64_t* dst_req_ids,
+                    const int64_t* src_req_ids, int32_t layer_begin, int32_t layer_count, void* cuda_stream) {
+  if (!dst || !src || dst == src || n_req < 0) return KV_ERR_INVALID;
+  if (n_req > 0 && (!dst_req_ids || !src_req_ids)) return KV_ERR_INVALID;
+  const kv_pool_config_t& a = src->hs.cfg;
+  const kv_pool_config_t& b = dst->hs.cfg;
+  if (a.num_layers != b.num_layers || a.num_kv_heads != b.num_kv_heads || a.head_dim != b.head_dim ||
+      a.block_size != b.block_size || a.kv_dtype != b.kv_dtype)
+    return KV_ERR_INVALID;
+  if (layer_begin < 0 || layer_count < 1 || layer_begin + layer_count > b.num_layers) return KV_ERR_INVALID;
+  if (!dst->has_device || !src->has_device) return KV_ERR_NO_DEVICE;
+  std::vector<int32_t> lens(static_cast<size_t>(n_req)), zeros(static_cast<size_t>(n_req), 0);
+  {
+    int32_t rc = src->hs.check_batch(n_req, src_req_ids, nullptr);   // every producer id live, none repeated
+    if (rc != KV_OK) return rc;
+  }
+  for (int32_t i = 0; i < n_req; ++i) {
+    lens[static_cast<size_t>(i)] = src->hs.reqs.find(src_req_ids[i])->second.len;
+    if (layer_begin == 0 && dst->hs.reqs.count(dst_req_ids[i])) return KV_ERR_INVALID;   // must be new on the consumer
+  }
+  KV_ON_DEVICE(dst);
+  int32_t rc = layer_begin == 0 ? dst->hs.reserve(n_req, dst_req_ids, lens.data())
+                                : dst->hs.check_batch(n_req, dst_req_ids, lens.data());
+  if (rc != KV_OK) return rc;
+  if (layer_begin > 0)
+    for (int32_t i = 0; i < n_req; ++i)
+      if (dst->hs.reqs.find(dst_req_ids[i])->second.len != lens[static_cast<size_t>(i)]) return KV_ERR_INVALID;
+  rc = run_copy(dst, CopyKind::kTransfer, src, src_req_ids, n_req, dst_req_ids, lens.data(), nullptr, nullptr, zeros.data(),
+                layer_begin, layer_count, static_cast<cudaStream_t>(cuda_stream));
+  if (rc != KV_OK && layer_begin == 0) dst->hs.rollback_last_reserve();
+  return rc;
 }
 
 int32_t kv_free(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids) {
@@ -594,15 +729,31 @@ static AttnParams attn_params(kv_pool_t* pool, int32_t layer, const void* q, voi
   return p;
 }
 
-// a4 + a5 (and a3 when k_new / v_new are given): plan (cached across the layers of a step), upload, launch.
-static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const void* q,
-                                const void* k_new, const void* v_new, void* out, float sm_scale, void* cuda_stream) {
+// a4 + a5 (and a3 when k_new / v_new are given) for layers [layer_begin, layer_begin + layer_count):
+// (reserve,) plan (cached across the layers of a step), upload, one launch per layer.
+static int32_t launch_attention(kv_pool_t* pool, int32_t layer_begin, int32_t layer_count, int32_t batch,
+                                const int64_t* req_ids, const void* q, const void* k_new, const void* v_new, void* out,
+                                int64_t q_stride, int64_t kv_stride, float sm_scale, bool reserve, void* cuda_stream) {
   if (!pool || !req_ids || !q || !out || !aligned16(q) || !aligned16(out)) return KV_ERR_INVALID;
   const kv_pool_config_t& c = pool->hs.cfg;
-  if (layer < 0 || layer >= c.num_layers || batch < 1) return KV_ERR_INVALID;
-  if (k_new && c.kv_dtype != KV_DTYPE_BF16 && !pool->fp8_ring) return KV_ERR_UNSUPPORTED;   // register-tile FP8 kernel: no fused append
+  if (layer_begin < 0 || layer_count < 1 || layer_begin + layer_count > c.num_layers || batch < 1) return KV_ERR_INVALID;
+  if ((k_new == nullptr) != (v_new == nullptr)) return KV_ERR_INVALID;
+  if (k_new && (!aligned16(k_new) || !aligned16(v_new))) return KV_ERR_INVALID;
+  if (layer_count > 1 && ((q_stride & 15) != 0 || (k_new && (kv_stride & 15) != 0))) return KV_ERR_INVALID;
+  if (reserve && (layer_begin != 0 || !k_new)) return KV_ERR_INVALID;
   if (!pool->has_device) return KV_ERR_NO_DEVICE;
+  KV_ON_DEVICE(pool);
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+
+  if (reserve) {   // a1 for the step's token of every request
+    if (static_cast<int32_t>(pool->ones.size()) < batch) pool->ones.assign(static_cast<size_t>(batch), 1);
+    int32_t rc = pool->hs.reserve(batch, req_ids, pool->ones.data());
+    if (rc != KV_OK) return rc;
+  }
+  auto fail = [&](int32_t rc) {
+    if (reserve) pool->hs.rollback_last_reserve();
+    return rc;
+  };
 
   // plan: reuse across the layers of a step (same ids, no reserve/free since)
   const bool cached = pool->plan_slot >= 0 && pool->plan_kind == 0 && pool->plan_epoch == pool->hs.epoch &&
@@ -611,112 +762,122 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer, int32_t batch, c
   if (!cached) {
     int32_t rc = pool->hs.plan_decode(batch, req_ids, pool->slots(), pool->ips(), pool->min_chunk(),
                                       kMaxPartials, &pool->plan);
-    if (rc != KV_OK) return rc;
-    StageSlot* s = nullptr;
-    int idx = acquire(pool, pool->plan_ring, &pool->plan_next, &s);
-    if (idx < 0) return idx;
+    pool->plan_slot = -1;   // pool->plan no longer is what is staged
+    if (rc != KV_OK) return fail(rc);
     const size_t item_bytes = pool->plan.items.size() * sizeof(WorkItem);
     const size_t comb_bytes = pool->plan.combines.size() * sizeof(CombineEntry);
-    if (static_cast<int64_t>(item_bytes + comb_bytes) > pool->lay.plan_blob_bytes) return KV_ERR_INVALID;
+    if (static_cast<int64_t>(item_bytes + comb_bytes) > pool->lay.plan_blob_bytes) return fail(KV_ERR_INVALID);
+    pool->plan_append_ok = -1;
+  }
+  if (k_new) {  // fused append: every request's last reservation must be the one token being appended
+    if (pool->plan_append_ok != 1) {
+      pool->plan_append_ok = 1;
+      for (int32_t i = 0; i < batch; ++i)
+        if (pool->hs.reqs.find(req_ids[i])->second.last_n != 1) { pool->plan_append_ok = 0; break; }
+    }
+    if (!pool->plan_append_ok) return fail(KV_ERR_INVALID);
+  }
+  if (int32_t rc = order_attention(pool, stream); rc != KV_OK) return fail(rc);
+  if (!cached) {
+    StageSlot* s = nullptr;
+    const int idx = acquire(pool, pool->plan_ring, &pool->plan_next, &s);
+    if (idx < 0) return fail(idx);
+    const size_t item_bytes = pool->plan.items.size() * sizeof(WorkItem);
+    const size_t comb_bytes = pool->plan.combines.size() * sizeof(CombineEntry);
     std::memcpy(s->host, pool->plan.items.data(), item_bytes);
     std::memcpy(s->host + item_bytes, pool->plan.combines.data(), comb_bytes);
     pool->plan_slot = -1;
-    KV_CUDA(pool, cudaMemcpyAsync(s->dev, s->host, item_bytes + comb_bytes, cudaMemcpyHostToDevice, stream));
+    pool->chain_slot = -1;
+    const cudaError_t e = cudaMemcpyAsync(s->dev, s->host, item_bytes + comb_bytes, cudaMemcpyHostToDevice, stream);
+    if (e != cudaSuccess) return fail(pool->cuda_fail(e));
     pool->plan_slot = idx;
     pool->plan_kind = 0;
-    pool->plan_append_ok = -1;
     pool->plan_epoch = pool->hs.epoch;
     pool->plan_ids.assign(req_ids, req_ids + batch);
     pool->plan_n_items = static_cast<int32_t>(pool->plan.items.size());
     pool->plan_n_combines = static_cast<int32_t>(pool->plan.combines.size());
     pool->plan_combine_off = static_cast<int64_t>(item_bytes);
   }
-  if (k_new) {  // fused append: every request's last reservation must be the one token being appended
-    if (!cached || pool->plan_append_ok != 1) {
-      pool->plan_append_ok = 1;
-      for (int32_t i = 0; i < batch; ++i)
-        if (pool->hs.reqs.find(req_ids[i])->second.last_n != 1) { pool->plan_append_ok = 0; break; }
-    }
-    if (!pool->plan_append_ok) return KV_ERR_INVALID;
-  }
   StageSlot& s = pool->plan_ring[pool->plan_slot];
   const int32_t G = c.num_q_heads / c.num_kv_heads;
-  AttnParams p = attn_params(pool, layer, q, out, sm_scale, s);
-  p.k_new = static_cast<const uint16_t*>(k_new);
-  p.v_new = static_cast<const uint16_t*>(v_new);
-  const int32_t want = (p.n_units + kAttnWarps - 1) / kAttnWarps;
-  const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * pool->ctas_per_sm)));
+  const int kind = k_new ? 1 : 0;
+  const AttnVariant v = pick_variant(pool, k_new != nullptr, false);
+  const bool separate_combine = pool->plan_n_combines > 0 && !pool->fuse_combine;
+  // From here on kernels are enqueued: an error is a CUDA error and leaves the stream in an undefined state
+  // (KV_ERR_CUDA is sticky); the reservation stays, as the launches already issued refer to it.
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_ATTN].begin(stream));
-  if (c.kv_dtype == KV_DTYPE_FP8_E4M3 && pool->fp8_ring) {
-    const cudaError_t re = c.head_dim == 128
-                               ? (k_new ? launch_fp8_ring<128, true, false>(p, pool->num_sms, want, stream)
-                                        : launch_fp8_ring<128, false, false>(p, pool->num_sms, want, stream))
-                               : (k_new ? launch_fp8_ring<64, true, false>(p, pool->num_sms, want, stream)
-                                        : launch_fp8_ring<64, false, false>(p, pool->num_sms, want, stream));
-    KV_CUDA(pool, re);
-  } else if (c.kv_dtype == KV_DTYPE_FP8_E4M3) {
-    if (c.head_dim == 128) attn_fp8_kernel<128><<<grid, kAttnThreads, 0, stream>>>(p);
-    else attn_fp8_kernel<64><<<grid, kAttnThreads, 0, stream>>>(p);
-  } else if (pool->ring) {
-    const cudaError_t re = k_new ? launch_ring_any<true, false>(c.head_dim, pool->ring, p, pool->num_sms, want, stream)
-                                 : launch_ring_any<false, false>(c.head_dim, pool->ring, p, pool->num_sms, want, stream);
-    KV_CUDA(pool, re);
-  } else if (c.head_dim == 128) {
-    if (k_new) attn_splitkv_kernel<128, true><<<grid, kAttnThreads, 0, stream>>>(p);
-    else attn_splitkv_kernel<128, false><<<grid, kAttnThreads, 0, stream>>>(p);
-  } else {
-    if (k_new) attn_splitkv_kernel<64, true><<<grid, kAttnThreads, 0, stream>>>(p);
-    else attn_splitkv_kernel<64, false><<<grid, kAttnThreads, 0, stream>>>(p);
-  }
-  KV_CUDA(pool, cudaGetLastError());
-  if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_ATTN].end(stream));
-  ++pool->launches;
-
-  if (pool->plan_n_combines > 0 && !pool->fuse_combine) {
-    CombineParams cp{};
-    cp.entries = reinterpret_cast<const CombineEntryDev*>(s.dev + pool->plan_combine_off);
-    cp.n_entries = pool->plan_n_combines;
-    cp.part_o = p.part_o;
-    cp.part_ml = p.part_ml;
-    cp.out = p.out;
-    cp.num_q_heads = c.num_q_heads;
-    cp.group = G;
-    cp.num_kv_heads = c.num_kv_heads;
-    const unsigned cgrid = static_cast<unsigned>((static_cast<int64_t>(cp.n_entries) * c.num_q_heads + 3) / 4);
-    if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_COMBINE].begin(stream));
-    if (c.head_dim == 128)
-      combine_kernel<128><<<cgrid, 128, 0, stream>>>(cp);
-    else
-      combine_kernel<64><<<cgrid, 128, 0, stream>>>(cp);
-    KV_CUDA(pool, cudaGetLastError());
-    if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_COMBINE].end(stream));
+  for (int32_t ll = 0; ll < layer_count; ++ll) {
+    AttnParams p = attn_params(pool, layer_begin + ll, static_cast<const char*>(q) + ll * q_stride,
+                               static_cast<char*>(out) + ll * q_stride, sm_scale, s);
+    if (k_new) {
+      p.k_new = reinterpret_cast<const uint16_t*>(static_cast<const char*>(k_new) + ll * kv_stride);
+      p.v_new = reinterpret_cast<const uint16_t*>(static_cast<const char*>(v_new) + ll * kv_stride);
+    }
+    // the stream's previous kernel is an attention launch of this very plan and kind: its CTAs may read the work
+    // items and block ids before griddepcontrol.wait
+    p.chained = pool->pdl && pool->chain_slot == pool->plan_slot && pool->chain_kind == kind ? 1 : 0;
+    KV_CUDA(pool, launch_attn_kernel(pool, v, p, stream));
     ++pool->launches;
+    pool->chain_slot = separate_combine ? -1 : pool->plan_slot;
+    pool->chain_kind = kind;
+    if (separate_combine) {
+      CombineParams cp{};
+      cp.entries = reinterpret_cast<const CombineEntryDev*>(s.dev + pool->plan_combine_off);
+      cp.n_entries = pool->plan_n_combines;
+      cp.part_o = p.part_o;
+      cp.part_ml = p.part_ml;
+      cp.out = p.out;
+      cp.num_q_heads = c.num_q_heads;
+      cp.group = G;
+      cp.num_kv_heads = c.num_kv_heads;
+      const unsigned cgrid = static_cast<unsigned>((static_cast<int64_t>(cp.n_entries) * c.num_q_heads + 3) / 4);
+      if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_COMBINE].begin(stream));
+      if (c.head_dim == 128)
+        combine_kernel<128><<<cgrid, 128, 0, stream>>>(cp);
+      else
+        combine_kernel<64><<<cgrid, 128, 0, stream>>>(cp);
+      KV_CUDA(pool, cudaGetLastError());
+      if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_COMBINE].end(stream));
+      ++pool->launches;
+    }
   }
+  if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_ATTN].end(stream, layer_count));
   KV_CUDA(pool, cudaEventRecord(s.ev, stream));
   s.in_flight = true;
+  attention_launched(pool, stream, s, kind);
+  if (separate_combine) pool->chain_slot = -1;
   return KV_OK;
 }
 
 int32_t paged_decode_attention(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const void* q,
                                void* out, float sm_scale, void* cuda_stream) {
-  return launch_attention(pool, layer, batch, req_ids, q, nullptr, nullptr, out, sm_scale, cuda_stream);
+  return launch_attention(pool, layer, 1, batch, req_ids, q, nullptr, nullptr, out, 0, 0, sm_scale, false, cuda_stream);
 }
 
 int32_t paged_decode_step(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const void* q,
                           const void* k_new, const void* v_new, void* out, float sm_scale, void* cuda_stream) {
-  if (!k_new || !v_new || !aligned16(k_new) || !aligned16(v_new)) return KV_ERR_INVALID;
-  return launch_attention(pool, layer, batch, req_ids, q, k_new, v_new, out, sm_scale, cuda_stream);
+  if (!k_new || !v_new) return KV_ERR_INVALID;
+  return launch_attention(pool, layer, 1, batch, req_ids, q, k_new, v_new, out, 0, 0, sm_scale, false, cuda_stream);
+}
+
+int32_t paged_decode_step_layers(kv_pool_t* pool, int32_t layer_begin, int32_t layer_count, int32_t batch,
+                                 const int64_t* req_ids, const void* q, const void* k_new, const void* v_new, void* out,
+                                 int64_t q_layer_stride_bytes, int64_t kv_layer_stride_bytes, float sm_scale,
+                                 int32_t flags, void* cuda_stream) {
+  if (flags & ~KV_STEP_RESERVE) return KV_ERR_INVALID;
+  return launch_attention(pool, layer_begin, layer_count, batch, req_ids, q, k_new, v_new, out, q_layer_stride_bytes,
+                          kv_layer_stride_bytes, sm_scale, (flags & KV_STEP_RESERVE) != 0, cuda_stream);
 }
 
 // NEXT-1: plan query tiles (cached while ids, q_lens and the pool epoch are unchanged, i.e. across
-// the layers of a step), stage 48-byte items, one launch of attn_splitkv_kernel<D, false, true>.
+// the layers of a step), stage 48-byte items, one launch of attn_kernel<.., kVarQ = true>.
 int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids,
                                const int32_t* q_lens, const void* q, void* out, float sm_scale, void* cuda_stream) {
   if (!pool || !req_ids || !q_lens || !q || !out || !aligned16(q) || !aligned16(out)) return KV_ERR_INVALID;
   const kv_pool_config_t& c = pool->hs.cfg;
   if (layer < 0 || layer >= c.num_layers || batch < 1) return KV_ERR_INVALID;
-  if (c.kv_dtype != KV_DTYPE_BF16 && !pool->fp8_ring) return KV_ERR_UNSUPPORTED;   // register-tile FP8 kernel: decode only
   if (!pool->has_device) return KV_ERR_NO_DEVICE;
+  KV_ON_DEVICE(pool);
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const int32_t G = c.num_q_heads / c.num_kv_heads;
 
@@ -729,11 +890,15 @@ int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
     const int32_t max_partials = static_cast<int32_t>(static_cast<int64_t>(kMaxPartials) * G / 8);
     int32_t rc = pool->hs.plan_varq(batch, req_ids, q_lens, pool->slots(), pool->ips(), pool->min_chunk(),
                                     max_partials, &pool->plan, &pool->plan_tiles);
+    pool->plan_slot = -1;   // pool->plan no longer matches what is staged
     if (rc != KV_OK) return rc;
+    if (static_cast<int64_t>(pool->plan.items.size()) * 48 > pool->lay.plan_blob_bytes) return KV_ERR_TOO_LONG;
+  }
+  if (int32_t rc = order_attention(pool, stream); rc != KV_OK) return rc;
+  if (!cached) {
     const size_t n_items = pool->plan.items.size();
-    if (static_cast<int64_t>(n_items) * 48 > pool->lay.plan_blob_bytes) return KV_ERR_TOO_LONG;
     StageSlot* s = nullptr;
-    int idx = acquire(pool, pool->plan_ring, &pool->plan_next, &s);
+    const int idx = acquire(pool, pool->plan_ring, &pool->plan_next, &s);
     if (idx < 0) return idx;
     for (size_t k = 0; k < n_items; ++k) {
       char* dst = s->host + k * 48;
@@ -741,7 +906,7 @@ int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
       const int32_t extra[4] = {pool->plan_tiles[k].pos0, pool->plan_tiles[k].n_qtok, 0, 0};
       std::memcpy(dst + sizeof(WorkItem), extra, sizeof extra);
     }
-    pool->plan_slot = -1;
+    pool->chain_slot = -1;
     KV_CUDA(pool, cudaMemcpyAsync(s->dev, s->host, n_items * 48, cudaMemcpyHostToDevice, stream));
     pool->plan_slot = idx;
     pool->plan_kind = 1;
@@ -754,51 +919,39 @@ int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
   }
   StageSlot& s = pool->plan_ring[pool->plan_slot];
   AttnParams p = attn_params(pool, layer, q, out, sm_scale, s);
-  const int32_t want = (p.n_units + kAttnWarps - 1) / kAttnWarps;
-  const unsigned grid = static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * pool->ctas_per_sm)));
+  p.chained = pool->pdl && pool->chain_slot == pool->plan_slot && pool->chain_kind == 2 ? 1 : 0;
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_VARQ].begin(stream));
-  if (c.kv_dtype == KV_DTYPE_FP8_E4M3) {
-    const cudaError_t re = c.head_dim == 128 ? launch_fp8_ring<128, false, true>(p, pool->num_sms, want, stream)
-                                             : launch_fp8_ring<64, false, true>(p, pool->num_sms, want, stream);
-    KV_CUDA(pool, re);
-  } else if (pool->ring) {
-    const cudaError_t re = launch_ring_any<false, true>(c.head_dim, pool->ring, p, pool->num_sms, want, stream);
-    KV_CUDA(pool, re);
-  } else if (c.head_dim == 128)
-    attn_splitkv_kernel<128, false, true><<<grid, kAttnThreads, 0, stream>>>(p);
-  else
-    attn_splitkv_kernel<64, false, true><<<grid, kAttnThreads, 0, stream>>>(p);
-  KV_CUDA(pool, cudaGetLastError());
+  KV_CUDA(pool, launch_attn_kernel(pool, pick_variant(pool, false, true), p, stream));
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_VARQ].end(stream));
   ++pool->launches;
   KV_CUDA(pool, cudaEventRecord(s.ev, stream));
   s.in_flight = true;
+  attention_launched(pool, stream, s, 2);
   return KV_OK;
 }
 
 int32_t kv_ingest_host(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const int32_t* n_tokens,
                        const void* const* k_src, const void* const* v_src, int32_t layer_begin, int32_t layer_count,
                        void* staging, int64_t staging_bytes, void* cuda_stream) {
-  if (!pool || n_req < 0) return KV_ERR_INVALID;
-  if (n_req > 0 && (!req_ids || !n_tokens || !k_src || !v_src)) return KV_ERR_INVALID;
+  int32_t rc = ingest_args_ok(pool, n_req, req_ids, n_tokens, k_src, v_src, layer_begin, layer_count, false);
+  if (rc != KV_OK) return rc;
   const kv_pool_config_t& c = pool->hs.cfg;
-  if (layer_begin < 0 || layer_count < 1 || layer_begin + layer_count > c.num_layers) return KV_ERR_INVALID;
-  if (!pool->has_device) return KV_ERR_NO_DEVICE;
   if (n_req > 0 && (!staging || (reinterpret_cast<uintptr_t>(staging) & (kAlign - 1)) != 0)) return KV_ERR_INVALID;
   const int64_t row_bytes = static_cast<int64_t>(layer_count) * pool->src_heads() * c.head_dim * 2;   // full-width source rows
   int64_t need = 0;
-  for (int32_t i = 0; i < n_req; ++i) {
-    if (n_tokens[i] < 0) return KV_ERR_INVALID;
-    if (n_tokens[i] > 0 && (!k_src[i] || !v_src[i])) return KV_ERR_INVALID;
-    need += 2 * align_up(row_bytes * n_tokens[i]);
-  }
+  for (int32_t i = 0; i < n_req; ++i) need += 2 * align_up(row_bytes * n_tokens[i]);
   if (need > staging_bytes) return KV_ERR_INVALID;
+  KV_ON_DEVICE(pool);
+  // a1 first: a call that cannot get its blocks must not have touched the stream
+  rc = layer_begin == 0 ? pool->hs.reserve(n_req, req_ids, n_tokens) : pool->hs.check_batch(n_req, req_ids, n_tokens);
+  if (rc != KV_OK) return rc;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   // K tensors first, then V tensors; each at a 256-byte aligned offset.  A run of requests whose
   // host ranges and staging ranges are both back to back moves with one copy.
   std::vector<const void*> kd(static_cast<size_t>(n_req)), vd(static_cast<size_t>(n_req));
   char* dst = static_cast<char*>(staging);
-  for (int pass = 0; pass < 2; ++pass) {
+  cudaError_t ce = cudaSuccess;
+  for (int pass = 0; pass < 2 && ce == cudaSuccess; ++pass) {
     const void* const* src = pass ? v_src : k_src;
     std::vector<const void*>& dev = pass ? vd : kd;
     const char* run_src = nullptr;
@@ -810,7 +963,7 @@ int32_t kv_ingest_host(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, c
       run_len = 0;
       return e;
     };
-    for (int32_t i = 0; i < n_req; ++i) {
+    for (int32_t i = 0; i < n_req && ce == cudaSuccess; ++i) {
       const int64_t bytes = row_bytes * n_tokens[i];
       dev[static_cast<size_t>(i)] = dst;
       if (bytes == 0) continue;
@@ -818,15 +971,19 @@ int32_t kv_ingest_host(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, c
       if (run_len && sp == run_src + run_len && dst == run_dst + run_len) {
         run_len += bytes;
       } else {
-        KV_CUDA(pool, flush());
+        ce = flush();
         run_src = sp; run_dst = dst; run_len = bytes;
       }
       dst += (bytes % kAlign == 0) ? bytes : align_up(bytes);
     }
-    KV_CUDA(pool, flush());
+    if (ce == cudaSuccess) ce = flush();
     dst = static_cast<char*>(staging) + align_up(dst - static_cast<char*>(staging));
   }
-  return kv_ingest(pool, n_req, req_ids, n_tokens, kd.data(), vd.data(), layer_begin, layer_count, cuda_stream);
+  if (ce != cudaSuccess) {
+    if (layer_begin == 0) pool->hs.rollback_last_reserve();
+    return pool->cuda_fail(ce);
+  }
+  return ingest_reserved(pool, n_req, req_ids, n_tokens, kd.data(), vd.data(), layer_begin, layer_count, stream);
 }
 
 static int32_t attention_host(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const void* q,
@@ -847,6 +1004,7 @@ static int32_t attention_host(kv_pool_t* pool, int32_t layer, int32_t batch, con
       if (r.len < 1 || (k_new && r.last_n != 1)) return KV_ERR_INVALID;
     }
   }
+  KV_ON_DEVICE(pool);
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   char* dq = static_cast<char*>(staging);
   char* dout = dq + align_up(qb);
@@ -857,10 +1015,11 @@ static int32_t attention_host(kv_pool_t* pool, int32_t layer, int32_t batch, con
     KV_CUDA(pool, cudaMemcpyAsync(dk, k_new, static_cast<size_t>(kb), cudaMemcpyHostToDevice, stream));
     KV_CUDA(pool, cudaMemcpyAsync(dv, v_new, static_cast<size_t>(kb), cudaMemcpyHostToDevice, stream));
   }
-  int32_t rc = launch_attention(pool, layer, batch, req_ids, dq, k_new ? dk : nullptr, k_new ? dv : nullptr, dout,
-                                sm_scale, cuda_stream);
+  int32_t rc = launch_attention(pool, layer, 1, batch, req_ids, dq, k_new ? dk : nullptr, k_new ? dv : nullptr, dout, 0, 0,
+                                sm_scale, false, cuda_stream);
   if (rc != KV_OK) return rc;
   KV_CUDA(pool, cudaMemcpyAsync(out, dout, static_cast<size_t>(qb), cudaMemcpyDeviceToHost, stream));
+  pool->chain_slot = -1;   // a copy now sits between this launch and the next
   return KV_OK;
 }
 
@@ -904,7 +1063,8 @@ int64_t kv_token_bytes(const kv_pool_config_t* cfg) {
   if (!cfg) return KV_ERR_INVALID;
   int32_t rc = HostState::validate(*cfg);
   if (rc != KV_OK) return rc;
-  return 2LL * cfg->num_layers * cfg->num_kv_heads * cfg->head_dim * 2;
+  const int64_t per_head = cfg->kv_dtype == KV_DTYPE_FP8_E4M3 ? 2LL * cfg->head_dim + 8 : 2LL * cfg->head_dim * 2;
+  return static_cast<int64_t>(cfg->num_layers) * cfg->num_kv_heads * per_head;
 }
 
 int64_t kv_launch_count(const kv_pool_t* pool) { return pool ? pool->launches : KV_ERR_INVALID; }
@@ -912,12 +1072,14 @@ int64_t kv_launch_count(const kv_pool_t* pool) { return pool ? pool->launches : 
 int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
   if (!pool || !key) return KV_ERR_INVALID;
   pool->plan_slot = -1;  // any option may change the plan
+  pool->chain_slot = -1;
   if (!std::strcmp(key, "min_chunk_blocks") && value >= 1 && value <= 65536) { pool->min_chunk_blocks = static_cast<int32_t>(value); pool->min_chunk_set = true; return KV_OK; }
-  if (!std::strcmp(key, "ctas_per_sm") && value >= 1 && value <= 8) { pool->ctas_per_sm = static_cast<int32_t>(value); return KV_OK; }
+  if (!std::strcmp(key, "ctas_per_sm") && value >= 0 && value <= 8) { pool->ctas_per_sm = static_cast<int32_t>(value); return KV_OK; }
   if (!std::strcmp(key, "items_per_slot") && value >= 1 && value <= 1024) { pool->items_per_slot = static_cast<int32_t>(value); pool->items_per_slot_set = true; return KV_OK; }
   if (!std::strcmp(key, "profile") && (value == 0 || value == 1)) { pool->profile = value != 0; return KV_OK; }
   if (!std::strcmp(key, "fuse_combine") && (value == 0 || value == 1)) { pool->fuse_combine = value != 0; return KV_OK; }
-  if (!std::strcmp(key, "ring") && (value == 0 || value == 2 || value == 3)) { pool->ring = static_cast<int32_t>(value); return KV_OK; }
+  if (!std::strcmp(key, "pdl") && (value == 0 || value == 1)) { pool->pdl = value != 0; return KV_OK; }
+  if (!std::strcmp(key, "ring") && (value == 2 || value == 3)) { pool->ring = static_cast<int32_t>(value); return KV_OK; }
   if (!std::strcmp(key, "src_kv_heads") && (value == 0 || (value >= pool->hs.cfg.num_kv_heads + pool->src_head_begin && value <= 65536))) {
     pool->src_kv_heads = static_cast<int32_t>(value);
     if (value == 0) pool->src_head_begin = 0;
@@ -927,12 +1089,12 @@ int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
     pool->src_head_begin = static_cast<int32_t>(value);
     return KV_OK;
   }
-  if (!std::strcmp(key, "fp8_ring") && (value == 0 || value == 1)) { pool->fp8_ring = value != 0; return KV_OK; }
   return KV_ERR_INVALID;
 }
 
 int32_t kv_profile_read(kv_pool_t* pool, int32_t kind, int64_t* out_launches, double* out_ms) {
   if (!pool || kind < 0 || kind >= KV_KERNEL_KINDS) return KV_ERR_INVALID;
+  KV_ON_DEVICE(pool);
   ProfRing& r = pool->prof[kind];
   KV_CUDA(pool, r.drain());
   if (out_launches) *out_launches = r.launches;
@@ -942,6 +1104,7 @@ int32_t kv_profile_read(kv_pool_t* pool, int32_t kind, int64_t* out_launches, do
 
 int32_t kv_profile_reset(kv_pool_t* pool) {
   if (!pool) return KV_ERR_INVALID;
+  KV_ON_DEVICE(pool);
   for (ProfRing& r : pool->prof) {
     KV_CUDA(pool, r.drain());
     r.launches = 0;
@@ -967,6 +1130,6 @@ const char* kv_strerror(int32_t status) {
   }
 }
 
-const char* kv_version(void) { return "0.1.0"; }
+const char* kv_version(void) { return "0.2.0"; }
 
 }  // extern "C"

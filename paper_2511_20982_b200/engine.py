@@ -9,9 +9,11 @@ One step (SURVEY §8(a), rows a1-a6; PAPER.md:200, :219-223 producer/consumer ba
     host      retire `ingest_per_step` finished requests           kv_free        (a6)
     stream B  ingest `ingest_per_step` prefill-completed requests  kv_ingest      (a1, a2)
               (they join the decode batch at the NEXT step, so the copy overlaps attention)
-    stream A  reserve the step's token for every request          kv_reserve     (a1, host)
-              for each layer l:  append + attention over len+1     paged_decode_step (a3, a4, a5: one launch)
-              (``fused=False``: kv_ingest n=1 then paged_decode_attention, two or three launches)
+    stream A  reserve the step's token for every request and, for each layer, append + attention over len+1:
+              ONE host call, paged_decode_step_layers(KV_STEP_RESERVE) — a1 on the host, then one launch per
+              layer (a3, a4, a5 fused), issued back to back with programmatic dependent launch
+              (``layered=False``: kv_reserve + one paged_decode_step call per layer;
+               ``fused=False``: kv_ingest n=1 then paged_decode_attention, two or three launches per layer)
 The decode batch keeps its size: the requests retired at step s are replaced by the ones
 ingested during step s-1.  With ``streams=1`` everything runs on stream A in program order.
 
@@ -66,20 +68,8 @@ class Schedule:
     peak_blocks: int = 0
 
 
-def kv_token_bytes_layer(w: W.Workload, fp8: bool = False) -> int:
-    """Pool bytes of one token in one layer: K and V rows of every kv head — bf16, or e4m3 codes plus the
-    two fp32 row scales (FP8 pool, NEXT-2)."""
-    return w.num_kv_heads * ((2 * w.head_dim + 8) if fp8 else (2 * w.head_dim * 2))
-
-
-def attention_bytes(w: W.Workload, lens, fp8: bool = False) -> int:
-    """Algorithmic bytes of one layer's decode attention: every resident K and V element once, q in and
-    out once, the block_table once per request, seq_lens."""
-    lens = np.asarray(lens, dtype=np.int64)
-    kv = int(lens.sum()) * kv_token_bytes_layer(w, fp8)
-    qo = 2 * len(lens) * w.num_q_heads * w.head_dim * 2
-    bt = 4 * int(((lens + w.block_size - 1) // w.block_size).sum()) + 4 * len(lens)
-    return kv + qo + bt
+kv_token_bytes_layer = W.kv_token_bytes_layer
+attention_bytes = W.attention_bytes
 
 
 def build_schedule(w: W.Workload, n_steps: int, bank_steps: int, salt: int = 0, host_from: int | None = None,
@@ -161,11 +151,12 @@ class DecodeLoop:
 
     def __init__(self, w: W.Workload, n_steps: int, n_host_steps: int = 0, device="cuda:0", streams: int = 2,
                  salt: int = 0, bank_bytes: int = 24 << 30, profile: bool = True, options: dict | None = None,
-                 sentinel: int | None = None, fused: bool = True, kv_dtype: int = B.KV_DTYPE_BF16):
+                 sentinel: int | None = None, fused: bool = True, kv_dtype: int = B.KV_DTYPE_BF16, layered: bool = True):
         """Steps [0, n_steps) take their inputs from device memory; steps [n_steps, n_steps + n_host_steps)
         take them from pinned host memory through the *_host entry points."""
         self.fp8 = kv_dtype == B.KV_DTYPE_FP8_E4M3
         self.w, self.dev, self.salt, self.fused = w, torch.device(device), salt, fused
+        self.layered = layered and fused
         self.host_from, self.n_steps = n_steps, n_steps + n_host_steps
         self.two_streams = streams >= 2 and w.ingest_per_step > 0
         L, Hkv, Hq, d, k = w.num_layers, w.num_kv_heads, w.num_q_heads, w.head_dim, w.ingest_per_step
@@ -340,7 +331,11 @@ class DecodeLoop:
         a = A.cuda_stream
         lay_kv = self.w.batch * self.row_new
         qb = self.q_layer_bytes
-        if self.fused:
+        if self.layered and not host:                                                              # a1 + L x (a3 + a4 + a5)
+            B.paged_decode_step_layers(h, 0, L, sp.batch, q.data_ptr(), kn.data_ptr(), vn.data_ptr(), out.data_ptr(),
+                                       qb, lay_kv, 0.0, B.KV_STEP_RESERVE, a)
+            L = 0
+        elif self.fused:
             B.kv_reserve(h, sp.batch, self._ones)                                                  # a1 (host)
         for l in range(L):
             kl, vl = kn.data_ptr() + l * lay_kv, vn.data_ptr() + l * lay_kv

@@ -206,6 +206,27 @@ class Workload:
         return replace(self, **kw)
 
 
+# ---------------------------------------------------------------------------------------------
+# byte accounting (SURVEY §8(d) "algorithmic bytes") — counting only, shared by bench.py's CUDA arm, its
+# oracle-timing arm and the engine; lives here so that the oracle arm never imports the CUDA binding
+# ---------------------------------------------------------------------------------------------
+
+def kv_token_bytes_layer(w: Workload, fp8: bool = False) -> int:
+    """Pool bytes of one token in one layer: K and V rows of every kv head — bf16, or e4m3 codes plus the
+    two fp32 row scales (FP8 pool, NEXT-2)."""
+    return w.num_kv_heads * ((2 * w.head_dim + 8) if fp8 else (2 * w.head_dim * 2))
+
+
+def attention_bytes(w: Workload, lens, fp8: bool = False) -> int:
+    """Algorithmic bytes of one layer's decode attention: every resident K and V element once, q in and
+    out once, the block_table once per request, seq_lens."""
+    lens = np.asarray(lens, dtype=np.int64)
+    kv = int(lens.sum()) * kv_token_bytes_layer(w, fp8)
+    qo = 2 * len(lens) * w.num_q_heads * w.head_dim * 2
+    bt = 4 * int(((lens + w.block_size - 1) // w.block_size).sum()) + 4 * len(lens)
+    return kv + qo + bt
+
+
 CONFIGS: dict[str, Workload] = {
     # configs[0] tiny correctness case
     "cfg1_tiny": Workload("cfg1_tiny", 1, 8, 2, 64, 4, lengths_fixed([17, 64, 130, 255]), 2098201,

@@ -97,3 +97,7 @@ def test_library_argument_checks():
     cfg = kv.PoolConfig(num_layers=32, num_q_heads=32, num_kv_heads=8, head_dim=128, num_blocks=8, max_requests=4,
                         max_blocks_per_request=4)
     assert B.kv_token_bytes(cfg) == 131072           # config 3, 131 072 B per token
+    # an FP8 pool: codes + the two fp32 row scales per (layer, kv head) — M_token of Eq. 13 shrinks by 1.94
+    cfg8 = kv.PoolConfig(**{**cfg.__dict__, "kv_dtype": B.KV_DTYPE_FP8_E4M3})
+    assert B.kv_token_bytes(cfg8) == 32 * 8 * (2 * 128 + 8) == 67584
+    assert B.kv_token_bytes(cfg8) * cfg8.block_size * cfg8.num_blocks == B.kv_pool_kv_bytes(cfg8)

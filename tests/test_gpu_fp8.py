@@ -20,7 +20,7 @@ pytestmark = pytest.mark.gpu
 
 MODES = [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=1024),
          dict(min_chunk_blocks=2, items_per_slot=2, fuse_combine=0), dict(min_chunk_blocks=5, items_per_slot=1, ctas_per_sm=1),
-         dict(fp8_ring=0), dict(fp8_ring=0, min_chunk_blocks=2, items_per_slot=1024)]
+         dict(pdl=0), dict(pdl=0, min_chunk_blocks=2, items_per_slot=1024)]
 SENT = 0xFF   # e4m3 NaN code / NaN scale bytes: an unmasked read poisons the output
 
 
@@ -163,24 +163,27 @@ def test_decode_loop_appends_with_ingest():
     assert np.array_equal(pool_bytes(pool), slab)
 
 
-def test_unsupported_calls():
-    pool = make_fp8_pool(1, 8, 2, 64, 16)
-    w = W.Workload("fp8u", 1, 8, 2, 64, 1, None, 5, max_len=256)
-    k, v = kv_src(w, 1, 0, 20, DEV)
-    pool.ingest([1], [k], [v])
-    q = torch.zeros((1, 8, 64), dtype=torch.bfloat16, device=DEV)
-    with pytest.raises(B.KVError) as e:
-        pool.gather(1)
-    assert e.value.status == B.KV_ERR_UNSUPPORTED
-    pool.set_option("fp8_ring", 0)                                 # the register-tile variant: decode attention only
-    with pytest.raises(B.KVError) as e:
-        pool.varlen_attention(0, [1], [1], q)
-    assert e.value.status == B.KV_ERR_UNSUPPORTED
-    pool.reserve([1], [1])
-    with pytest.raises(B.KVError) as e:
-        pool.decode_step(0, [1], q, torch.zeros((1, 2, 64), dtype=torch.bfloat16, device=DEV),
-                         torch.zeros((1, 2, 64), dtype=torch.bfloat16, device=DEV))
-    assert e.value.status == B.KV_ERR_UNSUPPORTED
+@pytest.mark.parametrize("Hkv,d", [(2, 64), (8, 128)])
+def test_gather_fp8_returns_stored_codes_and_scales(Hkv, d):
+    """kv_gather on an FP8 pool: the stored codes and row scales, contiguous, byte for byte == oracle.gather_fp8
+    (the inverse of ingest's relocation, not of its quantisation); the pool is not modified."""
+    L, lens = 2, [1, 16, 45, 300]
+    pool = make_fp8_pool(L, Hkv * 4, Hkv, d, 40)
+    w = W.Workload("fp8g", L, Hkv * 4, Hkv, d, len(lens), None, 5, max_len=512)
+    ids = [11, 12, 13, 14]
+    srcs = [kv_src(w, u, 0, n, DEV) for u, n in zip(ids, lens)]
+    pool.ingest(ids, [x[0] for x in srcs], [x[1] for x in srcs])
+    torch.cuda.synchronize()
+    before = pool_bytes(pool).copy()
+    for u, n in zip(ids, lens):
+        assert B.kv_gather_bytes(pool.cfg, n) == (L * Hkv * n * d + 15) // 16 * 16 + 4 * L * Hkv * n
+        kc, ks, vc, vs = pool.gather(u)
+        torch.cuda.synchronize()
+        wkc, wks, wvc, wvs = oracle.gather_fp8(before, dims_of(pool), pool.block_table(u)[0], n)
+        assert np.array_equal(kc.cpu().numpy(), wkc) and np.array_equal(vc.cpu().numpy(), wvc)
+        assert np.array_equal(ks.cpu().numpy().view(np.uint32), wks.view(np.uint32))
+        assert np.array_equal(vs.cpu().numpy().view(np.uint32), wvs.view(np.uint32))
+    assert np.array_equal(pool_bytes(pool), before)
 
 
 @pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=2)])

@@ -17,7 +17,7 @@ from helpers import bf16_bits, bits_of, bits_to_f64
 pytestmark = pytest.mark.gpu
 
 MODES = [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=1024),
-         dict(min_chunk_blocks=2, items_per_slot=2, ctas_per_sm=1), dict(ring=2), dict(ring=0), dict(ring=0, min_chunk_blocks=1, items_per_slot=1024)]
+         dict(min_chunk_blocks=2, items_per_slot=2, ctas_per_sm=1), dict(ring=2), dict(pdl=0), dict(pdl=0, min_chunk_blocks=1, items_per_slot=1024)]
 SHAPES = [(8, 2, 64), (32, 32, 128), (64, 8, 128), (6, 2, 64), (5, 1, 128), (4, 2, 128)]   # G = 4, 1, 8, 3, 5, 2
 
 

@@ -256,3 +256,53 @@ def test_kv_head_shards_take_identical_allocator_decisions():
         shards[0].set_option("src_head_begin", 7)            # heads [7, 9) do not exist in an 8-head source
     with pytest.raises(kv.KVError):
         full.set_option("src_kv_heads", 4)                   # narrower than the pool itself
+
+
+def test_round2_entry_points_check_their_arguments_on_the_host():
+    """kv_transfer / paged_decode_step_layers / kv_gather_bytes / config caps: refusals that need no GPU."""
+    a, b = host_pool(), host_pool(num_blocks=64)
+    a.reserve([1], [40])
+    for dst, src, ids, status in [(a, a, ([2], [1]), B.KV_ERR_INVALID),                      # a pool cannot feed itself
+                                  (b, host_pool(head_dim=128), ([2], [1]), B.KV_ERR_INVALID),  # geometry mismatch
+                                  (b, host_pool(kv_dtype=B.KV_DTYPE_FP8_E4M3), ([2], [1]), B.KV_ERR_INVALID),
+                                  (b, a, ([2], [1]), B.KV_ERR_NO_DEVICE)]:                   # host-only pools launch nothing
+        with pytest.raises(kv.KVError) as e:
+            B.kv_transfer(dst.handle, src.handle, ids[0], ids[1], 0, 2)
+        assert e.value.status == status
+    assert b.stats()["live_requests"] == 0 and a.block_table(1)[1] == 40
+    with pytest.raises(kv.KVError) as e:
+        B.paged_decode_step_layers(a.handle, 0, 2, [1], 256, 512, 768, 1024, 4096, 1024, 0.0, B.KV_STEP_RESERVE, 0)
+    assert e.value.status == B.KV_ERR_NO_DEVICE and a.block_table(1)[1] == 40                 # nothing was reserved
+    cfg = kv.PoolConfig(num_layers=2, num_q_heads=8, num_kv_heads=2, head_dim=64, num_blocks=8, max_requests=4,
+                        max_blocks_per_request=4)
+    assert B.kv_gather_bytes(cfg, 10) == 2 * 2 * 10 * 64 * 2
+    cfg8 = kv.PoolConfig(**{**cfg.__dict__, "kv_dtype": B.KV_DTYPE_FP8_E4M3})
+    assert B.kv_gather_bytes(cfg8, 10) == 2 * 2 * 10 * 64 + 4 * 2 * 2 * 10                    # codes (16-byte multiple) + scales
+    assert B.kv_gather_bytes(cfg8, 3) == (2 * 2 * 3 * 64 + 15) // 16 * 16 + 4 * 2 * 2 * 3
+    # a request may not exceed 131072 blocks: lengths stay inside int32 and the plan's 16:16 packing holds
+    big = kv.PoolConfig(**{**cfg.__dict__, "max_requests": 1, "max_blocks_per_request": 131073})
+    with pytest.raises(kv.KVError) as e:
+        kv.kv_pool_required_bytes(big)
+    assert e.value.status == B.KV_ERR_INVALID
+    assert kv.kv_pool_required_bytes(kv.PoolConfig(**{**cfg.__dict__, "max_requests": 1, "max_blocks_per_request": 131072})) > 0
+    # removed tuning values are refused, new ones accepted
+    for key, val, ok in [("ring", 0, False), ("fp8_ring", 0, False), ("ring", 2, True), ("pdl", 0, True), ("pdl", 2, False)]:
+        if ok:
+            a.set_option(key, val)
+        else:
+            with pytest.raises(kv.KVError):
+                a.set_option(key, val)
+
+
+def test_library_is_the_one_built_from_this_tree():
+    """binding refuses a libkvpool.so whose source hash differs from the sources in the tree (a stale binary
+    would make every GPU test meaningless); the check is by content, so it survives a copy to another box."""
+    from paper_2511_20982_b200 import build
+    assert not build.stale()
+    assert open(build.STAMP).read().strip() == build.source_hash()
+    deps = list(build.DEPS)
+    try:
+        build.DEPS.append(os.path.join("..", "binding.py"))              # any change to what is hashed flips it
+        assert build.stale()
+    finally:
+        build.DEPS[:] = deps
