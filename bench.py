@@ -451,6 +451,7 @@ def measure(args, rep, sampler, wname: str, K: int, Wm: int, headline: bool):
                "decode_tokens_per_s": sum_over_ranks(float(eb["tokens"])) / (ems * 1e-3),
                "pcie_gbs": sum_over_ranks(float(h2d + d2h)) / (ems * 1e-3) / 1e9,
                "api": "kv_ingest_host + paged_decode_step_host (pinned host q / K / V in, out back)"}
+    host_call_us = host_cost_per_step(loop) if not args.unfused else None
     stats = pool.stats()
     kv_gb_layer = by["attn"] / K / w.num_layers / 1e9
     res = {
@@ -470,6 +471,9 @@ def measure(args, rep, sampler, wname: str, K: int, Wm: int, headline: bool):
         "decode_tokens_per_s": total_tokens / (ms * 1e-3),
         "bytes_per_step": {"attention": by["attn"] // K, "ingest": by["ingest"] // K, "append": by["append"] // K},
         "host_enqueue_ms_per_step": host_s / K * 1e3,
+        "host_enqueue_note": "wall time of the enqueue loop / K: once the host is 16 plan uploads ahead it waits for the GPU, so this "
+                             "approaches ms_per_step whenever the host is faster; host_call_us_per_step is the CPU cost of one step's call",
+        "host_call_us_per_step": host_call_us,
         "gpu_launches": launches, "kernels": kernels, "roofline": roofline, "isolated": isolated,
         "cpu_baseline": cpu_base, "parity_sample": check, "e2e": e2e,
     }
@@ -528,6 +532,36 @@ def run_cuda(args):
     rep.close()
     if rank == 0 and failed:
         sys.exit(1)
+
+
+def host_cost_per_step(loop, reps: int = 12):
+    """CPU time of enqueueing ONE decode step (a1 reservation, split-KV plan, plan upload, L launches) through
+    paged_decode_step_layers, measured with the GPU idle so that no queue back-pressure is included: median wall
+    time of the call.  Runs extra steps on the pool after everything else has been measured and checked (the
+    appended rows are the last step's k_new / v_new again; nothing reads them)."""
+    import numpy as np
+    import torch
+    from paper_2511_20982_b200 import binding as B
+    last = min(loop.step_idx, loop.host_from) - 1              # the last device-resident step that ran
+    if last < 0:
+        return None
+    sp = loop.sched.steps[last]
+    if loop.step_idx > loop.host_from:                         # host-buffer steps followed: that batch is what is live now
+        sp = loop.sched.steps[loop.step_idx - 1]
+    q, kn, vn, out = loop.q[last], loop.k_new[last], loop.v_new[last], loop.out[last]
+    L, a = loop.w.num_layers, loop.sA.cuda_stream
+    times = []
+    try:
+        for _ in range(reps):
+            torch.cuda.synchronize(loop.dev)
+            t = time.perf_counter()
+            B.paged_decode_step_layers(loop.pool.handle, 0, L, sp.batch, q.data_ptr(), kn.data_ptr(), vn.data_ptr(), out.data_ptr(),
+                                       loop.q_layer_bytes, loop.w.batch * loop.row_new, 0.0, B.KV_STEP_RESERVE, a)
+            times.append(time.perf_counter() - t)
+    except B.KVError:
+        pass
+    torch.cuda.synchronize(loop.dev)
+    return float(np.median(times[2:]) * 1e6) if len(times) > 2 else None
 
 
 def isolated_legs(loop, last_step: int, peak: float, reps: int = 5, with_varlen: bool = True, with_transfer: bool = True):

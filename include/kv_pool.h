@@ -331,7 +331,10 @@ int32_t kv_plan_decode(kv_pool_t* pool, int32_t batch, const int64_t* req_ids /*
  * "together with KV-cache" handed from P to D) and the step's queries arriving in HOST
  * memory.  Same semantics and errors as kv_ingest / paged_decode_attention, except that
  * k_src[i] / v_src[i] / q / out are HOST pointers (pinned memory for true asynchrony;
- * pageable memory works but the copy is synchronous for the host).  The copies are issued
+ * pageable memory works but the copy is synchronous for the host).  kv_ingest_host reads sources
+ * that are pinned, device-addressable (cudaHostAlloc / cudaHostRegister) and 16-byte aligned IN PLACE:
+ * the scatter kernel pulls them over PCIe straight into their blocks and `staging` is not touched
+ * (option "host_zero_copy", default 1).  Otherwise the copies are issued
  * on `cuda_stream` through the caller-owned device staging buffer `staging` (device,
  * 256-byte aligned): ingest needs sum_i 2 * layer_count*Hkv*n_tokens[i]*d*2 bytes (each
  * tensor rounded up to 256 B), attention needs 2 * batch*Hq*d*2 bytes (rounded likewise);
@@ -411,6 +414,14 @@ int64_t kv_token_bytes(const kv_pool_config_t* cfg);
 /* Number of kernels this pool has launched since creation (bench `gpu_launches`).         */
 int64_t kv_launch_count(const kv_pool_t* pool);
 
+/* Event counters of this pool since creation, by name (>= 0; KV_ERR_INVALID for an unknown name):
+ *   "launches" (= kv_launch_count), "plans_uploaded" (split-KV plans staged; a step's layers share one),
+ *   "attn_chained_launches" (attention launches whose predecessor on the stream was an attention launch of the same
+ *   plan: their CTAs read work items and block ids before griddepcontrol.wait), "attn_stream_switches" (attention
+ *   calls that arrived on another stream and were ordered behind the previous one), "host_ingest_zero_copy" /
+ *   "host_ingest_staged" (kv_ingest_host calls that read pinned sources in place / went through `staging`).  */
+int64_t kv_pool_counter(const kv_pool_t* pool, const char* name);
+
 /*
  * Per-kernel device timing (bench `roofline`).  With option "profile" = 1 every kernel
  * launch (paged_decode_step_layers: every group of layer_count launches, counted as layer_count) is
@@ -437,7 +448,7 @@ int32_t kv_profile_reset(kv_pool_t* pool);
  * (1, default: the split-KV merge runs inside the attention kernel; 0: separate combine
  * kernel), "ring" (bf16 pools: 3, default, or 2 = shared-memory tile ring with that many slots per warp and
  * 2 / 3 CTAs per SM), "pdl" (1, default: attention launches carry the programmatic-dependent-launch attribute;
- * 0: plain launches), "profile" (0/1, see kv_profile_read);
+ * 0: plain launches), "host_zero_copy" (1, default: see kv_ingest_host), "profile" (0/1, see kv_profile_read);
  * KV-head sharding of a TP-sharded D-instance: "src_kv_heads" = H (0 = off) then
  * "src_head_begin" = h0 declare that the contiguous side of kv_ingest(_host) / kv_gather is the FULL-width tensor
  * [layer_count][H][n_tokens][head_dim] of which this pool holds heads [h0, h0 + num_kv_heads): every GPU of the

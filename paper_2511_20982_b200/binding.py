@@ -74,6 +74,7 @@ _SIGS = {
     "kv_optimal_pd_ratio": (_i32, [ctypes.c_double] * 4 + [ctypes.POINTER(ctypes.c_double)]),
     "kv_token_bytes": (_i64, [_CFG]),
     "kv_launch_count": (_i64, [_P]),
+    "kv_pool_counter": (_i64, [_P, ctypes.c_char_p]),
     "kv_profile_read": (_i32, [_P, _i32, ctypes.POINTER(_i64), ctypes.POINTER(ctypes.c_double)]),
     "kv_profile_reset": (_i32, [_P]),
     "kv_pool_set_option": (_i32, [_P, ctypes.c_char_p, _i64]),
@@ -355,6 +356,13 @@ def kv_launch_count(handle: int) -> int:
     return int(lib.kv_launch_count(handle))
 
 
+def kv_pool_counter(handle: int, name: str) -> int:
+    n = int(lib.kv_pool_counter(handle, name.encode()))
+    if n < 0:
+        raise KVError(n, f"kv_pool_counter({name})")
+    return n
+
+
 def kv_pool_set_option(handle: int, key: str, value: int) -> None:
     _check(lib.kv_pool_set_option(handle, key.encode(), value), f"kv_pool_set_option({key})")
 
@@ -492,6 +500,9 @@ class KVPool:
     @property
     def launches(self) -> int:
         return kv_launch_count(self.handle)
+
+    def counter(self, name: str) -> int:
+        return kv_pool_counter(self.handle, name)
 
     def close(self):
         if getattr(self, "handle", None):

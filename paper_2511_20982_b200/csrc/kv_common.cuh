@@ -343,6 +343,16 @@ __device__ __forceinline__ void combine_cols(const float* part_o, const float* p
     combine_heads<D, 1>(part_o, part_ml, pb, n_chunks, stride, col0 + head, out_row0 + head * D, lane);
 }
 
+// Plan upload as a KERNEL (pinned host staging, read in place over PCIe -> the plan slot in the slab), so that the
+// stream holds only kernels and programmatic dependent launch chains straight through a decode step's boundary: its
+// copy overlaps the tail of the previous attention launch (a different plan slot), and it completes only after that
+// launch has (griddepcontrol.wait), so the attention launch behind it inherits the ordering.
+__global__ void __launch_bounds__(256) plan_upload_kernel(const uint4* __restrict__ host_src, uint4* __restrict__ dst, int n16) {
+  pdl_launch_dependents();
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += gridDim.x * blockDim.x) dst[i] = host_src[i];
+  pdl_wait();
+}
+
 struct CombineEntryDev { int32_t batch_idx, partial_begin, n_chunks, pad; };  // == kvp::CombineEntry
 
 struct CombineParams {

@@ -28,7 +28,9 @@ struct IngestUnit {
 };
 
 // Request of unit u: last i with unit_begin <= u.  The lanes test 32 candidates at a time (independent loads, one
-// ballot each) rather than walk a binary search of dependent loads.
+// ballot each) rather than walk a binary search of dependent loads.  kRun > 1: a unit is a RUN of up to kRun
+// consecutive touched blocks of one (request, layer, kv head) — the returned fields describe the run's first block.
+template <int kRun = 1>
 __device__ __forceinline__ IngestUnit locate_unit(const IngestParams& p, int64_t u, int lane) {
   int lo = -1;
   for (int base = 0; base < p.n_req; base += 32) {
@@ -39,8 +41,9 @@ __device__ __forceinline__ IngestUnit locate_unit(const IngestParams& p, int64_t
   IngestUnit x;
   x.r = p.reqs[lo];
   const int64_t local = u - x.r.unit_begin;
-  x.jj = static_cast<int>(local % x.r.n_touched);
-  const int rest = static_cast<int>(local / x.r.n_touched);
+  const int runs = (x.r.n_touched + kRun - 1) / kRun;
+  x.jj = static_cast<int>(local % runs) * kRun;
+  const int rest = static_cast<int>(local / runs);
   x.h = rest % p.num_kv_heads;
   x.ll = rest / p.num_kv_heads;
   x.lb = x.r.blk0 + x.jj;
@@ -91,52 +94,117 @@ __global__ void __launch_bounds__(kIngestThreads) ingest_kernel(const IngestPara
 }
 
 // ---------------------------------------------------------------------------------------------
-// quantising scatter (NEXT-2): same units, same descriptors as ingest_kernel (IngestParams::kv = the FP8 region),
-// but one warp per (unit, K|V): the quantisation arithmetic sits between a warp's loads and its stores,
-// so the kernel wants many light warps (4 KiB in flight each, ~50 registers) rather than few heavy ones.
-// Launch with 2 * total_units warps.
+// quantising scatter (NEXT-2): same descriptors as ingest_kernel (IngestParams::kv = the FP8 region).  Unlike the
+// plain copies this kernel has arithmetic between its loads and its stores, and the first version (one warp per
+// (block, K|V), every lane dividing for every piece) was ISSUE-bound: 74 % issue slots, 990 instructions per 4 KiB of
+// source (profiles/r02).  This one
+//   * gives a warp a RUN of kIngest8Run consecutive blocks of one (request, layer, kv head, K|V): one descriptor
+//     lookup per run, 16 KiB of contiguous source per warp, the next block's loads issued before the current
+//     block is quantised (two register buffers);
+//   * finds the 16 row maxima of a block with a halving butterfly (8 shuffles per lane instead of 32): after it
+//     every lane OWNS one row, computes that row's scale and inverse once (two IEEE divisions per lane instead of
+//     sixteen), stores the scale, and hands the inverse to the lanes holding the row's pieces (one shuffle each).
+// The arithmetic that decides a code is unchanged (C3): amax exact, fl32 divisions, fl32 product, RNE
+// e4m3 saturating — byte-exact against oracle_scatter_fp8.  Launch with 2 * total_units warps (unit = run).
 // ---------------------------------------------------------------------------------------------
-constexpr int kIngest8Threads = 64;   // small CTAs: an SM slot frees as soon as two warps are done (one-shot warps of uneven length)
+constexpr int kIngest8Threads = 64;
 constexpr int kIngest8Warps = kIngest8Threads / 32;
+constexpr int kIngest8Run = 4;
 template <int D>
 __global__ void __launch_bounds__(kIngest8Threads) ingest_fp8_kernel(const IngestParams p) {
   constexpr int kPiecesPerRow = D / 8;                          // 16-byte source pieces (8 bf16) per token row
-  constexpr int kMaxPerLane = kBlockSize * kPiecesPerRow / 32;  // 8 at D=128, 4 at D=64
+  constexpr int NV = kBlockSize * kPiecesPerRow / 32;           // pieces per lane and block: 8 at D=128, 4 at D=64
+  static_assert(kPiecesPerRow == 2 * NV, "a row's pieces sit on 2 * NV neighbouring lanes");
   const int lane = threadIdx.x & 31;
   const int64_t u2 = static_cast<int64_t>(blockIdx.x) * kIngest8Warps + (threadIdx.x >> 5);
   const int64_t u = u2 >> 1;
-  const int c = static_cast<int>(u2 & 1);                        // 0: the K rows of the unit, 1: the V rows
+  const int c = static_cast<int>(u2 & 1);                        // 0: the K rows of the run, 1: the V rows
   if (u >= p.total_units) return;
-  const IngestUnit x = locate_unit(p, u, lane);
-  const int blk = __ldg(&p.blk_ids[x.r.blk_off + x.jj]);
-  const int pieces = (x.row1 - x.row0) * kPiecesPerRow;
+  const IngestUnit x = locate_unit<kIngest8Run>(p, u, lane);
+  const int n_run = min(kIngest8Run, x.r.n_touched - x.jj);
+  const int32_t blk_id = lane < n_run ? __ldg(&p.blk_ids[x.r.blk_off + x.jj + lane]) : 0;
+  const int grp = lane / kPiecesPerRow;                          // which of the 32 / kPiecesPerRow rows a piece index step covers
+  const int own = (lane >> 1) & (NV - 1);                        // the value index this lane owns after the butterfly
+  const uint16_t* src = reinterpret_cast<const uint16_t*>(c ? x.r.v_src : x.r.k_src) +
+                        (static_cast<int64_t>(x.ll) * p.src_kv_heads + p.src_head_begin + x.h) * x.r.n_tokens * D;
+  uint8_t* const layer_head = reinterpret_cast<uint8_t*>(p.kv) +
+                              (static_cast<int64_t>(p.layer_begin + x.ll) * p.num_blocks * p.num_kv_heads + x.h) * fp8_tile_bytes<D>();
 
-  const int64_t src_off = ((static_cast<int64_t>(x.ll) * p.src_kv_heads + p.src_head_begin + x.h) * x.r.n_tokens + x.t0) * D;
-  const uint4* lin = reinterpret_cast<const uint4*>(reinterpret_cast<const uint16_t*>(c ? x.r.v_src : x.r.k_src) + src_off);
-  uint8_t* tile = reinterpret_cast<uint8_t*>(p.kv) +
-                  ((static_cast<int64_t>(p.layer_begin + x.ll) * p.num_blocks + blk) * p.num_kv_heads + x.h) * fp8_tile_bytes<D>();
+  // rows [row0, row1) of run block b and its first source token
+  auto rows_of = [&](int b, int& row0, int& row1, int& t0) {
+    const int lb = x.lb + b;
+    row0 = (x.jj + b == 0) ? (x.r.start_pos & (kBlockSize - 1)) : 0;
+    row1 = min(kBlockSize, x.r.start_pos + x.r.n_tokens - lb * kBlockSize);
+    t0 = lb * kBlockSize + row0 - x.r.start_pos;
+  };
+  auto load = [&](uint4 (&buf)[NV], int b) {
+    int row0, row1, t0;
+    rows_of(b, row0, row1, t0);
+    const uint4* lin = reinterpret_cast<const uint4*>(src + static_cast<int64_t>(t0) * D);
+    const int pieces = (row1 - row0) * kPiecesPerRow;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) buf[i] = ldg_copy_pred(lin + lane + 32 * i, lane + 32 * i < pieces);
+  };
+  auto quantise_store = [&](const uint4 (&buf)[NV], int b) {
+    int row0, row1, t0;
+    rows_of(b, row0, row1, t0);
+    const int rows = row1 - row0;
+    const int32_t blk = __shfl_sync(kFull, blk_id, b);
+    uint8_t* tile = layer_head + static_cast<int64_t>(blk) * p.num_kv_heads * fp8_tile_bytes<D>();
+    // packed |x| maxima of the lane's NV pieces (piece i belongs to row (32 / kPiecesPerRow) * i + grp of the block's rows)
+    uint32_t m[NV];
+#pragma unroll
+    for (int i = 0; i < NV; ++i)
+      m[i] = __vmaxu2(__vmaxu2(buf[i].x & 0x7fff7fffu, buf[i].y & 0x7fff7fffu), __vmaxu2(buf[i].z & 0x7fff7fffu, buf[i].w & 0x7fff7fffu));
+    // halving butterfly over the 2 * NV lanes that share rows: each step keeps half of the values and swaps the other half
+#pragma unroll
+    for (int n = NV, off = NV; n > 1; n >>= 1, off >>= 1) {
+      const bool up = (lane & off) != 0;
+#pragma unroll
+      for (int k = 0; k < n / 2; ++k) {
+        const uint32_t send = up ? m[k] : m[k + n / 2];
+        const uint32_t keep = up ? m[k + n / 2] : m[k];
+        m[k] = __vmaxu2(keep, __shfl_xor_sync(kFull, send, off));
+      }
+    }
+    m[0] = __vmaxu2(m[0], __shfl_xor_sync(kFull, m[0], 1));
+    const uint32_t mx = max(m[0] & 0xffffu, m[0] >> 16);          // row maximum of the row this lane owns (bf16 bits)
+    const float amax = __uint_as_float(mx << 16);
+    const float scale = mx == 0 ? 1.f : __fdiv_rn(amax, 448.f);
+    const float inv = mx == 0 ? 1.f : __fdiv_rn(448.f, amax);
+    const int own_row = (32 / kPiecesPerRow) * own + grp;          // relative to row0
+    if ((lane & 1) == 0 && own_row < rows)
+      *reinterpret_cast<float*>(tile + 2 * kBlockSize * D + (row0 + own_row) * 8 + c * 4) = scale;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      const float inv_i = __shfl_sync(kFull, inv, (lane & ~(2 * NV - 1)) | (i << 1));
+      const int idx = lane + 32 * i;
+      uint32_t w[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const uint32_t e = u4_get(buf[i], k);
+        w[k] = f32x2_to_e4m3x2(__fmul_rn(__uint_as_float(e << 16), inv_i), __fmul_rn(__uint_as_float(e & 0xffff0000u), inv_i));
+      }
+      if (idx < rows * kPiecesPerRow)
+        *reinterpret_cast<uint2*>(tile + c * (kBlockSize * D) + row0 * D + idx * 8) = make_uint2(w[0] | (w[1] << 16), w[2] | (w[3] << 16));
+    }
+    if (c == 0 && x.ll == 0 && x.h == 0 && lane == 0)             // device block_table mirror (a1, device half)
+      p.block_table[static_cast<int64_t>(x.r.slot) * p.bt_stride + x.lb + b] = blk;
+  };
 
-  uint4 buf[kMaxPerLane];
+  uint4 bufa[NV], bufb[NV];
+  load(bufa, 0);
 #pragma unroll
-  for (int i = 0; i < kMaxPerLane; ++i) buf[i] = ldg_copy_pred(lin + lane + 32 * i, lane + 32 * i < pieces);   // all loads first
-#pragma unroll
-  for (int i = 0; i < kMaxPerLane; ++i) {
-    const int idx = lane + 32 * i;
-    const bool ok = idx < pieces;
-    const int row = x.row0 + idx / kPiecesPerRow, cp = idx % kPiecesPerRow;
-    uint32_t mx = amax_bits8(buf[i]);                            // row amax: a row's pieces sit on neighbouring lanes
-#pragma unroll
-    for (int off = kPiecesPerRow / 2; off > 0; off >>= 1) mx = max(mx, __shfl_xor_sync(kFull, mx, off));
-    float scale;
-    const uint2 codes = quantise_piece(buf[i], mx, &scale);
-    if (ok) {
-      uint8_t* dst = tile + c * (kBlockSize * D) + row * D + cp * 8;
-      *reinterpret_cast<uint2*>(dst) = codes;
-      if (cp == 0) *reinterpret_cast<float*>(tile + 2 * kBlockSize * D + row * 8 + c * 4) = scale;
+  for (int b = 0; b < kIngest8Run; b += 2) {
+    if (b < n_run) {
+      if (b + 1 < n_run) load(bufb, b + 1);
+      quantise_store(bufa, b);
+    }
+    if (b + 1 < n_run) {
+      if (b + 2 < n_run) load(bufa, b + 2);
+      quantise_store(bufb, b + 1);
     }
   }
-  if (c == 0 && x.ll == 0 && x.h == 0 && lane == 0)             // device block_table mirror (a1, device half)
-    p.block_table[static_cast<int64_t>(x.r.slot) * p.bt_stride + x.lb] = blk;
 }
 
 // ---------------------------------------------------------------------------------------------

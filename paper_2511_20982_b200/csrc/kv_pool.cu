@@ -20,7 +20,7 @@ namespace {
 using namespace kvp;
 
 constexpr int64_t kAlign = 256;
-constexpr int kRing = 4;                       // plan staging slots
+constexpr int kRing = 16;                      // plan staging slots: the host may run this many plan uploads ahead of the GPU
 constexpr int64_t kIngestBlobBytes = 2 << 20;  // per ingest launch; larger calls are sub-batched.  One request's
                                                // descriptor (48 B + <= 8 B x kMaxBlocksPerRequest) always fits.
 constexpr int64_t kIngestRingBytes = 16 << 20; // descriptor staging ring: ~1000 decode appends in flight
@@ -66,6 +66,7 @@ Layout make_layout(const kv_pool_config_t& c) {
 
 struct StageSlot {
   char* host = nullptr;   // pinned
+  char* host_dev = nullptr;  // the same pinned buffer as the device addresses it (zero-copy reads by plan_upload_kernel)
   char* dev = nullptr;    // inside the slab
   cudaEvent_t ev = nullptr;
   bool in_flight = false;
@@ -206,6 +207,9 @@ struct kv_pool {
   int32_t src_head_begin = 0;     //                   this pool's head 0 is that side's head src_head_begin
   int32_t ring = 3;               // bf16 pool: ring slots per warp, 3 (2 CTAs per SM, default) or 2 (3 CTAs per SM)
   bool pdl = true;                // attention launches carry the programmatic-dependent-launch attribute
+  // event counters (kv_pool_counter)
+  int64_t n_zero_copy = 0, n_staged = 0, n_chained = 0, n_stream_switch = 0, n_plans = 0;
+  bool host_zero_copy = true;     // kv_ingest_host reads device-addressable pinned sources in place (no staging pass)
   bool profile = false;
   ProfRing prof[KV_KERNEL_KINDS];
   // staging
@@ -352,6 +356,8 @@ int32_t run_copy(kv_pool* pool, CopyKind kind, const kv_pool* src_pool, const in
                  const int64_t* req_ids, const int32_t* n_tokens, const void* const* k_ptrs, const void* const* v_ptrs,
                  const int32_t* start_pos, int32_t layer_begin, int32_t layer_count, cudaStream_t stream) {
   const kv_pool_config_t& c = pool->hs.cfg;
+  // blocks per unit: the quantising scatter gives a warp a run of consecutive blocks, the plain copies one block
+  const int32_t run = (kind == CopyKind::kScatter && pool->fp8()) ? kIngest8Run : 1;
   std::vector<IngestReq> reqs;
   std::vector<int32_t> ids;
   int64_t units = 0;
@@ -391,7 +397,7 @@ int32_t run_copy(kv_pool* pool, CopyKind kind, const kv_pool* src_pool, const in
       const Request& sr = src_pool->hs.reqs.find(src_ids[i])->second;
       ids.insert(ids.end(), sr.blocks.begin() + b0, sr.blocks.begin() + b1 + 1);
     }
-    units += static_cast<int64_t>(touched) * layer_count * c.num_kv_heads;
+    units += static_cast<int64_t>((touched + run - 1) / run) * layer_count * c.num_kv_heads;
   }
   return flush();
 }
@@ -453,12 +459,31 @@ cudaError_t launch_attn_kernel(const kv_pool* pool, const AttnVariant& v, const 
   return cudaLaunchKernelEx(&cfg, v.fn, p);
 }
 
+// Stage a plan blob: with PDL a kernel reads the pinned staging buffer in place (the stream stays kernel-only, so
+// the programmatic chain is not cut by a copy); without it a plain cudaMemcpyAsync.
+cudaError_t upload_plan(kv_pool* pool, const StageSlot& s, size_t bytes, cudaStream_t stream) {
+  ++pool->n_plans;
+  if (!pool->pdl || bytes == 0) return bytes ? cudaMemcpyAsync(s.dev, s.host, bytes, cudaMemcpyHostToDevice, stream) : cudaSuccess;
+  const int n16 = static_cast<int>((bytes + 15) / 16);
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(static_cast<unsigned>(std::max(1, std::min((n16 + 255) / 256, 32))));
+  cfg.blockDim = dim3(256);
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, plan_upload_kernel, reinterpret_cast<const uint4*>(s.host_dev), reinterpret_cast<uint4*>(s.dev), n16);
+}
+
 // Attention launches of one pool must not overlap (shared workspace): a call on another stream than the
 // previous one is ordered behind it.
 int32_t order_attention(kv_pool* pool, cudaStream_t stream) {
   if (pool->attn_any && stream != pool->attn_stream) {
     KV_CUDA(pool, cudaStreamWaitEvent(stream, pool->attn_ev, 0));
     pool->chain_slot = -1;
+    ++pool->n_stream_switch;
   }
   return KV_OK;
 }
@@ -521,7 +546,8 @@ int32_t kv_pool_create(const kv_pool_config_t* cfg, kv_pool_t** out_pool) {
     pool->ingest_ring.dev = pool->base + lay.ingest_blobs;
     pool->ingest_ring.cap = kIngestRingBytes;
     for (int i = 0; e == cudaSuccess && i < kRing; ++i) {
-      e = cudaHostAlloc(reinterpret_cast<void**>(&pool->plan_ring[i].host), lay.plan_blob_bytes, cudaHostAllocDefault);
+      e = cudaHostAlloc(reinterpret_cast<void**>(&pool->plan_ring[i].host), lay.plan_blob_bytes, cudaHostAllocMapped);
+      if (e == cudaSuccess) e = cudaHostGetDevicePointer(reinterpret_cast<void**>(&pool->plan_ring[i].host_dev), pool->plan_ring[i].host, 0);
       if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pool->plan_ring[i].ev, cudaEventDisableTiming);
       pool->plan_ring[i].dev = pool->base + lay.plan_blobs + i * lay.plan_blob_bytes;
     }
@@ -788,7 +814,7 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer_begin, int32_t la
     std::memcpy(s->host + item_bytes, pool->plan.combines.data(), comb_bytes);
     pool->plan_slot = -1;
     pool->chain_slot = -1;
-    const cudaError_t e = cudaMemcpyAsync(s->dev, s->host, item_bytes + comb_bytes, cudaMemcpyHostToDevice, stream);
+    const cudaError_t e = upload_plan(pool, *s, item_bytes + comb_bytes, stream);
     if (e != cudaSuccess) return fail(pool->cuda_fail(e));
     pool->plan_slot = idx;
     pool->plan_kind = 0;
@@ -816,6 +842,7 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer_begin, int32_t la
     // the stream's previous kernel is an attention launch of this very plan and kind: its CTAs may read the work
     // items and block ids before griddepcontrol.wait
     p.chained = pool->pdl && pool->chain_slot == pool->plan_slot && pool->chain_kind == kind ? 1 : 0;
+    pool->n_chained += p.chained;
     KV_CUDA(pool, launch_attn_kernel(pool, v, p, stream));
     ++pool->launches;
     pool->chain_slot = separate_combine ? -1 : pool->plan_slot;
@@ -907,7 +934,7 @@ int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
       std::memcpy(dst + sizeof(WorkItem), extra, sizeof extra);
     }
     pool->chain_slot = -1;
-    KV_CUDA(pool, cudaMemcpyAsync(s->dev, s->host, n_items * 48, cudaMemcpyHostToDevice, stream));
+    KV_CUDA(pool, upload_plan(pool, *s, n_items * 48, stream));
     pool->plan_slot = idx;
     pool->plan_kind = 1;
     pool->plan_append_ok = -1;
@@ -920,6 +947,7 @@ int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
   StageSlot& s = pool->plan_ring[pool->plan_slot];
   AttnParams p = attn_params(pool, layer, q, out, sm_scale, s);
   p.chained = pool->pdl && pool->chain_slot == pool->plan_slot && pool->chain_kind == 2 ? 1 : 0;
+  pool->n_chained += p.chained;
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_VARQ].begin(stream));
   KV_CUDA(pool, launch_attn_kernel(pool, pick_variant(pool, false, true), p, stream));
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_VARQ].end(stream));
@@ -946,9 +974,25 @@ int32_t kv_ingest_host(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, c
   rc = layer_begin == 0 ? pool->hs.reserve(n_req, req_ids, n_tokens) : pool->hs.check_batch(n_req, req_ids, n_tokens);
   if (rc != KV_OK) return rc;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-  // K tensors first, then V tensors; each at a 256-byte aligned offset.  A run of requests whose
-  // host ranges and staging ranges are both back to back moves with one copy.
   std::vector<const void*> kd(static_cast<size_t>(n_req)), vd(static_cast<size_t>(n_req));
+  // Zero-copy: when every source is pinned host memory the device can address (cudaHostAlloc / cudaHostRegister
+  // under unified addressing) and 16-byte aligned, the scatter kernel reads it over PCIe itself — the KV crosses the
+  // bus once, straight into its blocks, with no staging pass and no copy engine serialised in front of the kernel.
+  bool direct = pool->host_zero_copy;
+  for (int32_t i = 0; i < n_req && direct; ++i) {
+    if (n_tokens[i] == 0) { kd[static_cast<size_t>(i)] = vd[static_cast<size_t>(i)] = nullptr; continue; }
+    for (int pass = 0; pass < 2 && direct; ++pass) {
+      cudaPointerAttributes pa{};
+      const void* hp = pass ? v_src[i] : k_src[i];
+      if (cudaPointerGetAttributes(&pa, hp) != cudaSuccess) { cudaGetLastError(); direct = false; break; }
+      if (pa.type != cudaMemoryTypeHost || !pa.devicePointer || !aligned16(pa.devicePointer)) { direct = false; break; }
+      (pass ? vd : kd)[static_cast<size_t>(i)] = pa.devicePointer;
+    }
+  }
+  ++(direct ? pool->n_zero_copy : pool->n_staged);
+  if (direct) return ingest_reserved(pool, n_req, req_ids, n_tokens, kd.data(), vd.data(), layer_begin, layer_count, stream);
+  // Staged: K tensors first, then V tensors; each at a 256-byte aligned offset.  A run of requests whose
+  // host ranges and staging ranges are both back to back moves with one copy.
   char* dst = static_cast<char*>(staging);
   cudaError_t ce = cudaSuccess;
   for (int pass = 0; pass < 2 && ce == cudaSuccess; ++pass) {
@@ -1069,6 +1113,17 @@ int64_t kv_token_bytes(const kv_pool_config_t* cfg) {
 
 int64_t kv_launch_count(const kv_pool_t* pool) { return pool ? pool->launches : KV_ERR_INVALID; }
 
+int64_t kv_pool_counter(const kv_pool_t* pool, const char* name) {
+  if (!pool || !name) return KV_ERR_INVALID;
+  if (!std::strcmp(name, "launches")) return pool->launches;
+  if (!std::strcmp(name, "plans_uploaded")) return pool->n_plans;
+  if (!std::strcmp(name, "attn_chained_launches")) return pool->n_chained;
+  if (!std::strcmp(name, "attn_stream_switches")) return pool->n_stream_switch;
+  if (!std::strcmp(name, "host_ingest_zero_copy")) return pool->n_zero_copy;
+  if (!std::strcmp(name, "host_ingest_staged")) return pool->n_staged;
+  return KV_ERR_INVALID;
+}
+
 int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
   if (!pool || !key) return KV_ERR_INVALID;
   pool->plan_slot = -1;  // any option may change the plan
@@ -1079,6 +1134,7 @@ int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
   if (!std::strcmp(key, "profile") && (value == 0 || value == 1)) { pool->profile = value != 0; return KV_OK; }
   if (!std::strcmp(key, "fuse_combine") && (value == 0 || value == 1)) { pool->fuse_combine = value != 0; return KV_OK; }
   if (!std::strcmp(key, "pdl") && (value == 0 || value == 1)) { pool->pdl = value != 0; return KV_OK; }
+  if (!std::strcmp(key, "host_zero_copy") && (value == 0 || value == 1)) { pool->host_zero_copy = value != 0; return KV_OK; }
   if (!std::strcmp(key, "ring") && (value == 2 || value == 3)) { pool->ring = static_cast<int32_t>(value); return KV_OK; }
   if (!std::strcmp(key, "src_kv_heads") && (value == 0 || (value >= pool->hs.cfg.num_kv_heads + pool->src_head_begin && value <= 65536))) {
     pool->src_kv_heads = static_cast<int32_t>(value);

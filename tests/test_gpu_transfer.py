@@ -208,6 +208,10 @@ def test_step_layers_equals_per_layer_calls_and_oracle(opts, fp8):
             compare_attention(out_a[l], want)
     assert np.array_equal(raw(pools[0]) if fp8 else pool_bits(pools[0]), slab)
     assert pools[0].profile()["attn"][0] == 3 * L                       # a group of L launches counts as L
+    if opts.get("pdl", 1) and opts.get("fuse_combine", 1):              # layers 1..L-1 of every step chain behind layer 0
+        assert pools[0].counter("attn_chained_launches") == 3 * (L - 1) and pools[0].counter("plans_uploaded") == 3
+    else:
+        assert pools[0].counter("attn_chained_launches") == 0
     # attention only (no append) over several layers in one call == per-layer paged_decode_attention
     out_c, out_d = torch.empty_like(q), torch.empty_like(q)
     B.paged_decode_step_layers(pools[0].handle, 1, L - 1, ids, q[1].data_ptr(), 0, 0, out_c[1].data_ptr(), q[0].numel() * 2, 0, 0.0, 0, s)
@@ -276,6 +280,7 @@ def test_attention_on_two_streams_is_ordered_by_the_library():
         torch.cuda.current_stream().synchronize()
         outs.append((batch, rep % L, q, pool.attention(rep % L, batch, q, stream=st)))
     torch.cuda.synchronize()
+    assert pool.counter("attn_stream_switches") == 5                     # every call after the first changed stream
     for batch, layer, q, out in outs:
         compare_attention(out, oracle_attention(slab, pool, layer, batch, q))
 
@@ -308,9 +313,18 @@ def test_failed_ingest_changes_nothing():
         with pytest.raises(B.KVError):
             pool.block_table(2)
         assert np.array_equal(pool_bits(pool), bits)
-    # the host-buffer form refuses before touching the stream, then works once there is room
+    # the host-buffer form refuses before touching the stream, then works once there is room: pinned sources are read in
+    # place by the scatter kernel (zero-copy), pageable ones go through the staging buffer — same bytes either way
     pool.free([1])
     B.kv_ingest_host(pool.handle, [2], [70], [kh.data_ptr()], [vh.data_ptr()], 0, L, stage.data_ptr(), stage.numel(), 0)
     torch.cuda.synchronize()
+    assert pool.counter("host_ingest_zero_copy") == 1 and pool.counter("host_ingest_staged") == 0
     gk, gv = pool.gather(2)
+    assert torch.equal(gk, kb) and torch.equal(gv, vb)
+    pool.free([2])
+    kp, vp = kb.cpu(), vb.cpu()                                          # pageable host memory
+    B.kv_ingest_host(pool.handle, [3], [70], [kp.data_ptr()], [vp.data_ptr()], 0, L, stage.data_ptr(), stage.numel(), 0)
+    torch.cuda.synchronize()
+    assert pool.counter("host_ingest_staged") == 1
+    gk, gv = pool.gather(3)
     assert torch.equal(gk, kb) and torch.equal(gv, vb)
