@@ -29,13 +29,26 @@ namespace kvp {
 // =============================================================================================
 // bf16 tiles: K[16][D] | V[16][D] bf16, 4 D bytes per token... 64 D bytes per tile (8 KiB at D = 128)
 // =============================================================================================
-template <int D_>
+// kTmaL = true (D = 128 only): the ring slot has the layout the TMA unit writes for a [64 rows][128 B] box with
+// CU_TENSOR_MAP_SWIZZLE_128B — 128-byte row rho of the tile (token t's K row = rows 2t, 2t+1; V rows follow at 32 + ...)
+// at rho * 128 with its 16-byte chunks XORed with rho & 7 — so that full tiles can be fetched by ONE
+// cp.async.bulk.tensor instruction (SASS UTMALDG) issued by one lane, completion on an mbarrier.  That swizzle is not
+// the one this kernel would choose (the fragment reads of MMA rows g, g+1 would collide), so the TOKENS are permuted
+// over the MMA rows instead: row r of S^T holds token tok(r) — an online softmax does not care — which makes both
+// fragment read patterns conflict-free again.  Ragged and fused-append tiles still go through LDGSTS (same layout).
+template <int D_, bool kTmaL = false>
 struct Bf16Tiles {
   static constexpr int D = D_;
+  static_assert(!kTmaL || D_ == 128, "the TMA layout is built for 256-byte rows");
+  static constexpr bool kTma = kTmaL;
   static constexpr int KJ = D / 32;                             // K vectors per row per lane
   static constexpr int KS = D / 16, MT = D / 16, NE = D / 8;
   static constexpr uint32_t kSlotBytes = 2 * kBlockSize * D * 2;
   static constexpr int64_t kPoolTileBytes = kSlotBytes;
+  static constexpr int kTmaRows = kSlotBytes / 128;             // 128-byte rows of a tile (the TMA box height)
+
+  // token held by MMA row r (r in [0, 8); rows r + 8 hold token tok(r) + 8)
+  static __device__ __forceinline__ int tok(int r) { return kTmaL ? static_cast<int>((0x57463120u >> (4 * r)) & 7u) : r; }
   static constexpr bool kVScaled = false;                       // no per-token V scale in the softmax reference
   static constexpr bool kLazyRescale = false;
   static constexpr bool kPatchNewRow = false;                   // the fused append sources the new row in copy_tile
@@ -50,7 +63,12 @@ struct Bf16Tiles {
   // byte offset of 16-byte chunk `chunk` of row `row` inside a K or V half of a slot:
   // chunk' = chunk ^ (row bit 1) << 1 ^ (row bit 2 ^ row bit 0) << 2
   static __device__ __forceinline__ uint32_t chunk_off(int row, int chunk) {
-    return row * (D * 2) + ((chunk ^ (((row >> 1) & 1) << 1) ^ ((((row >> 2) ^ row) & 1) << 2)) << 4);
+    if constexpr (kTmaL) {
+      const int rho = 2 * row + (chunk >> 3);
+      return rho * 128 + (((chunk & 7) ^ (rho & 7)) << 4);
+    } else {
+      return row * (D * 2) + ((chunk ^ (((row >> 1) & 1) << 1) ^ ((((row >> 2) ^ row) & 1) << 2)) << 4);
+    }
   }
 
   // q^T as B fragments: lane (g, c) holds MMA column g, d columns of chunk c + 4j (zero if !ok)
@@ -95,12 +113,12 @@ struct Bf16Tiles {
 #pragma unroll
     for (int rs = 0; rs < 2; ++rs)
 #pragma unroll
-      for (int j = 0; j < KJ; ++j) T.k[rs][j] = lds128(slot_addr + chunk_off(g + 8 * rs, c + 4 * j));
+      for (int j = 0; j < KJ; ++j) T.k[rs][j] = lds128(slot_addr + chunk_off(tok(g) + 8 * rs, c + 4 * j));
 #pragma unroll
     for (int i = 0; i < 4; ++i)
 #pragma unroll
       for (int cs = 0; cs < D / 64; ++cs)
-        T.v[i][cs] = lds128(slot_addr + kBlockSize * D * 2 + chunk_off(2 * c + (i & 1) + 8 * (i >> 1), g + 8 * cs));
+        T.v[i][cs] = lds128(slot_addr + kBlockSize * D * 2 + chunk_off(tok(2 * c + (i & 1)) + 8 * (i >> 1), g + 8 * cs));
   }
 
   // s[0], s[1]: token g, MMA columns 2c, 2c+1;  s[2], s[3]: token g+8   (log2 units)
@@ -173,6 +191,8 @@ struct Fp8Tiles {
   static constexpr int KS = D / 16, MT = D / 16, NE = D / 8;
   static constexpr uint32_t kSlotBytes = 32 * D + 128;
   static constexpr int64_t kPoolTileBytes = kSlotBytes;
+  static constexpr bool kTma = false;
+  static __device__ __forceinline__ int tok(int r) { return r; }
   static constexpr bool kVScaled = true;
   static constexpr bool kLazyRescale = true;                    // rescale O only when some running maximum moved
   static constexpr bool kPatchNewRow = true;                    // the quantised new row is patched into the slot after it landed
@@ -292,13 +312,13 @@ struct Fp8Tiles {
                                                 float (&vs)[2]) {
     float sa[4] = {0.f, 0.f, 0.f, 0.f}, sb[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-    for (int j = 0; j < D / 64; ++j)
+      for (int j = 0; j < D / 64; ++j)
 #pragma unroll
-      for (int w = 0; w < 4; ++w) {
-        const uint32_t r0 = u4_get(T.k[0][j], w), r1 = u4_get(T.k[1][j], w);
-        mma_f16_m16n8k16((w & 1) ? sb : sa, e4m3x2_lo_to_f16x2(r0), e4m3x2_lo_to_f16x2(r1), e4m3x2_hi_to_f16x2(r0),
-                         e4m3x2_hi_to_f16x2(r1), Q.f[4 * j + w][0], Q.f[4 * j + w][1]);
-      }
+        for (int w = 0; w < 4; ++w) {
+          const uint32_t r0 = u4_get(T.k[0][j], w), r1 = u4_get(T.k[1][j], w);
+          mma_f16_m16n8k16((w & 1) ? sb : sa, e4m3x2_lo_to_f16x2(r0), e4m3x2_lo_to_f16x2(r1), e4m3x2_hi_to_f16x2(r0),
+                           e4m3x2_hi_to_f16x2(r1), Q.f[4 * j + w][0], Q.f[4 * j + w][1]);
+        }
     s[0] = (sa[0] + sb[0]) * (T.sc[0].x * cs0);
     s[1] = (sa[1] + sb[1]) * (T.sc[0].x * cs1);
     s[2] = (sa[2] + sb[2]) * (T.sc[1].x * cs0);
@@ -347,12 +367,26 @@ struct Fp8Tiles {
 // (unless p.chained) the work items and the block table are all accessed after it.
 // =============================================================================================
 template <class TP, bool kAppend, bool kVarQ, int R, int kCtas>
-__global__ void __launch_bounds__(kAttnThreads, kCtas) attn_kernel(const AttnParams p) {
+__global__ void __launch_bounds__(kAttnThreads, kCtas) attn_kernel(const __grid_constant__ AttnParams p) {
   extern __shared__ __align__(128) unsigned char ring_smem[];
   constexpr int D = TP::D, MT = TP::MT, NE = TP::NE;
-  const uint32_t ring = static_cast<uint32_t>(__cvta_generic_to_shared(ring_smem)) + (threadIdx.x >> 5) * (R * TP::kSlotBytes);
   const int lane = threadIdx.x & 31;
+  uint32_t smem0 = static_cast<uint32_t>(__cvta_generic_to_shared(ring_smem));
+  if constexpr (TP::kTma) smem0 = (smem0 + 1023u) & ~1023u;     // the 128-byte swizzle is a function of the address
+  const uint32_t ring = smem0 + (threadIdx.x >> 5) * (R * TP::kSlotBytes);
+  // TMA variants: one mbarrier per ring slot of this warp (behind the rings), and the parity each is next waited on
+  const uint32_t bars = smem0 + kAttnWarps * (R * TP::kSlotBytes) + (threadIdx.x >> 5) * (R * 8);
+  uint32_t bar_parity = 0;
+  if constexpr (TP::kTma) {
+    if (lane == 0) {
+#pragma unroll
+      for (int s = 0; s < R; ++s) mbar_init(bars + s * 8, 1);
+      mbar_init_fence();
+    }
+    __syncwarp();
+  }
   const int g = lane >> 2, c = lane & 3;
+  const int tg = TP::tok(g);                                     // the token (of a block's first 8) on MMA row g
   const int G = p.group;
   const int64_t blk_stride = static_cast<int64_t>(p.num_kv_heads) * TP::kPoolTileBytes;
   unsigned char* const kv = reinterpret_cast<unsigned char*>(p.kv_layer);
@@ -432,8 +466,20 @@ __global__ void __launch_bounds__(kAttnThreads, kCtas) attn_kernel(const AttnPar
           tile = kvh + __shfl_sync(kFull, ids, t & 31) * blk_stride;
         }
         const int nv = n_tokens - t * kBlockSize;
-        TP::template copy_tile<kAppend>(ring + (v % R) * TP::kSlotBytes, tile, nv, lane, first_special ? nv - 1 : -1,
-                                        p.k_new + new_row, p.v_new + new_row);
+        bool by_tma = false;
+        if constexpr (TP::kTma) by_tma = nv >= kBlockSize && !first_special;   // full tiles: one bulk tensor copy
+        if (by_tma) {
+          if (lane == 0) {
+            const uint32_t bar = bars + (v % R) * 8;
+            fence_proxy_async();                                 // the slot's last readers used the generic proxy
+            mbar_arrive_expect_tx(bar, TP::kSlotBytes);
+            tma_load_2d(ring + (v % R) * TP::kSlotBytes, p.tmap, bar, 0,
+                        static_cast<int32_t>(p.tma_row0 + (tile - kv) / 128));
+          }
+        } else {
+          TP::template copy_tile<kAppend>(ring + (v % R) * TP::kSlotBytes, tile, nv, lane, first_special ? nv - 1 : -1,
+                                          p.k_new + new_row, p.v_new + new_row);
+        }
         if constexpr (kAppend) {
           if (first_special) {                                   // a3: the new row goes into the pool
             TP::append_row(last_tile, nv - 1, p.k_new + new_row, p.v_new + new_row, lane, nr);
@@ -441,13 +487,23 @@ __global__ void __launch_bounds__(kAttnThreads, kCtas) attn_kernel(const AttnPar
           }
         }
       }
-      cp_async_commit();
+      if constexpr (!TP::kTma) cp_async_commit();
     };
 
     auto consume = [&](int v) {
       const int t = (special && v == 0) ? n_blocks - 1 : v - sp;
       const int nv = n_tokens - t * kBlockSize;
       const uint32_t slot_addr = ring + (v % R) * TP::kSlotBytes;
+      if constexpr (TP::kTma) {                                  // wait for the tile: mbarrier (TMA) or this warp's LDGSTS
+        if (nv >= kBlockSize && !(special && v == 0)) {
+          mbar_wait(bars + (v % R) * 8, (bar_parity >> (v % R)) & 1u);
+          bar_parity ^= 1u << (v % R);
+        } else {
+          cp_async_commit();
+          cp_async_wait<0>();
+          __syncwarp();
+        }
+      }
       if constexpr (kAppend && TP::kPatchNewRow) {
         if (special && v == 0) {
           TP::patch_slot(slot_addr, nv - 1, lane, nr);
@@ -460,17 +516,17 @@ __global__ void __launch_bounds__(kAttnThreads, kCtas) attn_kernel(const AttnPar
       TP::scores(T, Q, cs0, cs1, s, vs);
       float iv0 = 1.f, iv1 = 1.f;
       if constexpr (TP::kVScaled) {                              // t = s + log2(vs); ragged last block masked by index
-        const bool ok0 = g < nv, ok1 = g + 8 < nv;
+        const bool ok0 = tg < nv, ok1 = tg + 8 < nv;
         const float lv0 = ok0 ? fast_log2(vs[0]) : -INFINITY, lv1 = ok1 ? fast_log2(vs[1]) : -INFINITY;
-        iv0 = ok0 ? __frcp_rn(vs[0]) : 0.f;
-        iv1 = ok1 ? __frcp_rn(vs[1]) : 0.f;
+        iv0 = ok0 ? fast_rcp(vs[0]) : 0.f;
+        iv1 = ok1 ? fast_rcp(vs[1]) : 0.f;
         s[0] += lv0; s[1] += lv0; s[2] += lv1; s[3] += lv1;
       } else if (nv < kBlockSize) {                              // ragged last block: mask by index, not value
-        if (g >= nv) s[0] = s[1] = -INFINITY;
-        if (g + 8 >= nv) s[2] = s[3] = -INFINITY;
+        if (tg >= nv) s[0] = s[1] = -INFINITY;
+        if (tg + 8 >= nv) s[2] = s[3] = -INFINITY;
       }
       if constexpr (kVarQ) {                                    // causal: column sees tokens <= its own position
-        const int tok = t * kBlockSize + g;
+        const int tok = t * kBlockSize + tg;
         if (tok > rel0) s[0] = -INFINITY;
         if (tok > rel1) s[1] = -INFINITY;
         if (tok + 8 > rel0) s[2] = -INFINITY;
@@ -511,12 +567,12 @@ __global__ void __launch_bounds__(kAttnThreads, kCtas) attn_kernel(const AttnPar
 #pragma unroll
     for (int v = 0; v < R - 1; ++v) issue(v);                    // R - 1 tiles ahead
     for (int v = 0; v < n_blocks; ++v) {
-      cp_async_wait<R - 2>();                                    // tile v has landed (this lane's copies)
+      if constexpr (!TP::kTma) cp_async_wait<R - 2>();           // tile v has landed (this lane's copies)
       __syncwarp();                                              // ... everyone's; and slot (v - 1) % R is free
       issue(v + R - 1);
       consume(v);
     }
-    cp_async_wait<0>();
+    if constexpr (!TP::kTma) cp_async_wait<0>();
     __syncwarp();
 
     // ---- epilogue: finish l over the token lanes, then store ----

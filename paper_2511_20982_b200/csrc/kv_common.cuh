@@ -100,6 +100,36 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// ---- TMA (cp.async.bulk.tensor, SASS UTMALDG) + mbarrier --------------------------------------------------
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+// make freshly initialised barriers visible to the async proxy (the TMA unit completes transactions on them)
+__device__ __forceinline__ void mbar_init_fence() {
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+// order this thread's earlier generic-proxy accesses to shared memory before later async-proxy (TMA) writes
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+               : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  while (!mbar_try_wait(bar, parity)) {}
+}
+// 2-D tiled tensor copy global -> shared; completion (bytes) is signalled on `bar`.  `tmap` is the generic address of a
+// CUtensorMap living in kernel parameter space (__grid_constant__).
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const void* tmap, uint32_t bar, int32_t c0, int32_t c1) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+               ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+
 // Programmatic dependent launch (PDL).  wait: block until every grid this launch depends on has completed and its
 // memory is visible (a no-op for a launch without the programmatic attribute).  launch_dependents: allow the next
 // launch of the stream, if it carries the attribute, to start its CTAs as SM resources free up.
@@ -148,6 +178,13 @@ __device__ __forceinline__ uint32_t pack_f16x2(float lo, float hi) {
 __device__ __forceinline__ float fast_exp2(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+// 1 / x to ~1 ulp, subnormal inputs handled (not flushed)
+__device__ __forceinline__ float fast_rcp(float x) {
+  float y;
+  asm("rcp.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
 
@@ -265,6 +302,8 @@ struct AttnParams {
   int32_t chained;             // 1: the stream's previous kernel is an attention launch of the same plan, so work items,
                                //    block ids and this layer's KV may be read before griddepcontrol.wait
   float scale_log2;            // sm_scale * log2(e)
+  int64_t tma_row0;            // TMA variants: first 128-byte row of this layer's KV inside the tensor map
+  alignas(64) unsigned char tmap[128];   // CUtensorMap over the KV region as [rows][128 B] (TMA variants; else unused)
 };
 
 // ---------------------------------------------------------------------------------------------

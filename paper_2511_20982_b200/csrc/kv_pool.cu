@@ -1,6 +1,7 @@
 // kv_pool.cu — the C-ABI of include/kv_pool.h: argument checking, host bookkeeping (kv_host.h), staging of small
 // descriptor blobs, and kernel launches (kv_copy.cuh, kv_attn.cuh).  Every step of the data path runs in the
 // kernels; nothing here touches KV bytes on the host.
+#include <cuda.h>           // CUtensorMap and its enums only; the encoder is fetched through the runtime (no -lcuda)
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -25,6 +26,7 @@ constexpr int64_t kIngestBlobBytes = 2 << 20;  // per ingest launch; larger call
                                                // descriptor (48 B + <= 8 B x kMaxBlocksPerRequest) always fits.
 constexpr int64_t kIngestRingBytes = 16 << 20; // descriptor staging ring: ~1000 decode appends in flight
 constexpr int32_t kMaxPartials = 32768;        // split-KV partial slots in the workspace
+static_assert(sizeof(CUtensorMap) == 128, "AttnParams::tmap carries a CUtensorMap");
 static_assert(48 + 8LL * kvp::kMaxBlocksPerRequest <= kIngestBlobBytes, "a request's descriptor must fit one blob");
 
 inline int64_t align_up(int64_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
@@ -207,6 +209,9 @@ struct kv_pool {
   int32_t src_head_begin = 0;     //                   this pool's head 0 is that side's head src_head_begin
   int32_t ring = 3;               // bf16 pool: ring slots per warp, 3 (2 CTAs per SM, default) or 2 (3 CTAs per SM)
   bool pdl = true;                // attention launches carry the programmatic-dependent-launch attribute
+  bool tma = false;               // bf16 pools, head_dim 128: full tiles by cp.async.bulk.tensor (UTMALDG) instead of LDGSTS
+  bool tmap_ok = false;
+  alignas(64) CUtensorMap tmap;   // the KV region as [rows][128 B], box 64 rows, 128-byte swizzle
   // event counters (kv_pool_counter)
   int64_t n_zero_copy = 0, n_staged = 0, n_chained = 0, n_stream_switch = 0, n_plans = 0;
   bool host_zero_copy = true;     // kv_ingest_host reads device-addressable pinned sources in place (no staging pass)
@@ -415,7 +420,9 @@ constexpr int kFp8RingSlots = 4;   // FP8 pools: 4 ring slots per warp, 3 CTAs p
 
 template <class TP, bool kAppend, bool kVarQ, int R, int kCtas>
 AttnVariant variant() {
-  return {attn_kernel<TP, kAppend, kVarQ, R, kCtas>, static_cast<size_t>(kAttnWarps) * R * TP::kSlotBytes, kCtas};
+  // TMA variants: + 1 KiB so the rings can start on a 1 KiB boundary, + one mbarrier per slot and warp
+  const size_t extra = TP::kTma ? 1024 + static_cast<size_t>(kAttnWarps) * R * 8 : 0;
+  return {attn_kernel<TP, kAppend, kVarQ, R, kCtas>, static_cast<size_t>(kAttnWarps) * R * TP::kSlotBytes + extra, kCtas};
 }
 template <class TP, int R, int kCtas>
 AttnVariant variant_of(bool append, bool varq) {
@@ -426,9 +433,37 @@ AttnVariant pick_variant(const kv_pool* pool, bool append, bool varq) {
   const bool d128 = pool->hs.cfg.head_dim == 128;
   if (pool->fp8())
     return d128 ? variant_of<Fp8Tiles<128>, kFp8RingSlots, 3>(append, varq) : variant_of<Fp8Tiles<64>, kFp8RingSlots, 3>(append, varq);
+  if (pool->tma && pool->tmap_ok && d128) return variant_of<Bf16Tiles<128, true>, 3, 2>(append, varq);
   if (pool->ring == 2)
     return d128 ? variant_of<Bf16Tiles<128>, 2, 3>(append, varq) : variant_of<Bf16Tiles<64>, 2, 3>(append, varq);
   return d128 ? variant_of<Bf16Tiles<128>, 3, 2>(append, varq) : variant_of<Bf16Tiles<64>, 3, 2>(append, varq);
+}
+
+// The KV region of a bf16 pool as a 2-D tensor of 128-byte rows; a (block, kv head) tile is 64 consecutive rows
+// (head_dim 128).  CU_TENSOR_MAP_SWIZZLE_128B is the layout Bf16Tiles<128, true> reads.
+bool make_tensor_map(kv_pool* pool) {
+  const kv_pool_config_t& c = pool->hs.cfg;
+  if (pool->fp8() || c.head_dim != 128 || pool->lay.kv_bytes % 128 != 0) return false;
+  using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres{};
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  const cuuint64_t rows = static_cast<cuuint64_t>(pool->lay.kv_bytes / 128);
+  if (rows >= (1ull << 31)) return false;                       // tile coordinates are int32
+  const cuuint64_t gdim[2] = {128, rows};
+  const cuuint64_t gstride[1] = {128};                           // bytes between rows (dimension 1)
+  const cuuint32_t box[2] = {128, 64};
+  const cuuint32_t estride[2] = {1, 1};
+  const CUresult r = reinterpret_cast<EncodeFn>(fn)(&pool->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, pool->base, gdim, gstride, box,
+                                                    estride, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                                    CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
 }
 
 // Dynamic shared memory above 48 KiB needs an opt-in per (kernel, device).
@@ -552,6 +587,7 @@ int32_t kv_pool_create(const kv_pool_config_t* cfg, kv_pool_t** out_pool) {
       pool->plan_ring[i].dev = pool->base + lay.plan_blobs + i * lay.plan_blob_bytes;
     }
     // work counters start at zero; the attention kernel rewinds them itself afterwards
+    if (e == cudaSuccess) pool->tmap_ok = make_tensor_map(pool);
     if (e == cudaSuccess) e = cudaMemset(pool->base + lay.counters, 0, 256);
     if (e == cudaSuccess) e = cudaMemset(pool->base + lay.arrive, 0, static_cast<size_t>(kMaxPartials) * 4);
     if (e != cudaSuccess) {
@@ -751,6 +787,10 @@ static AttnParams attn_params(kv_pool_t* pool, int32_t layer, const void* q, voi
   p.num_kv_heads = c.num_kv_heads;
   p.group = c.num_q_heads / c.num_kv_heads;
   p.scale_log2 = scale * 1.4426950408889634f;
+  if (pool->tma && pool->tmap_ok) {
+    p.tma_row0 = static_cast<int64_t>(layer) * (layer_bytes / 128);
+    std::memcpy(p.tmap, &pool->tmap, sizeof(CUtensorMap));
+  }
   p.n_units = p.n_items * c.num_kv_heads;
   return p;
 }
@@ -1134,6 +1174,11 @@ int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
   if (!std::strcmp(key, "profile") && (value == 0 || value == 1)) { pool->profile = value != 0; return KV_OK; }
   if (!std::strcmp(key, "fuse_combine") && (value == 0 || value == 1)) { pool->fuse_combine = value != 0; return KV_OK; }
   if (!std::strcmp(key, "pdl") && (value == 0 || value == 1)) { pool->pdl = value != 0; return KV_OK; }
+  if (!std::strcmp(key, "tma") && (value == 0 || value == 1)) {   // bf16, head_dim 128 pools with a device slab only
+    if (value == 1 && !pool->tmap_ok) return KV_ERR_UNSUPPORTED;
+    pool->tma = value != 0;
+    return KV_OK;
+  }
   if (!std::strcmp(key, "host_zero_copy") && (value == 0 || value == 1)) { pool->host_zero_copy = value != 0; return KV_OK; }
   if (!std::strcmp(key, "ring") && (value == 2 || value == 3)) { pool->ring = static_cast<int32_t>(value); return KV_OK; }
   if (!std::strcmp(key, "src_kv_heads") && (value == 0 || (value >= pool->hs.cfg.num_kv_heads + pool->src_head_begin && value <= 65536))) {

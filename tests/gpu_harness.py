@@ -31,6 +31,18 @@ def make_pool(w: W.Workload, num_blocks, max_requests=None, alloc_seed=1, sentin
     return pool
 
 
+def apply_options(pool, opts):
+    """set_option for every (key, value); a pool that cannot run the TMA variant (head_dim 64, FP8) skips that mode."""
+    import pytest
+    for k_, v_ in (opts or {}).items():
+        try:
+            pool.set_option(k_, v_)
+        except kv.KVError as e:
+            if k_ == "tma" and e.status == kv.binding.KV_ERR_UNSUPPORTED:
+                pytest.skip("tma=1 needs a bf16 pool with head_dim 128")
+            raise
+
+
 def dims_of(pool) -> oracle.Dims:
     c = pool.cfg
     return oracle.Dims(c.num_layers, c.num_kv_heads, c.head_dim, c.block_size, c.num_blocks)

@@ -8,7 +8,7 @@ import oracle
 import paper_2511_20982_b200 as kv
 from paper_2511_20982_b200 import binding as B
 from paper_2511_20982_b200 import workloads as W
-from gpu_harness import (DEV, compare_attention, dims_of, kv_src, make_pool, oracle_attention, oracle_ingest,
+from gpu_harness import (apply_options, DEV, compare_attention, dims_of, kv_src, make_pool, oracle_attention, oracle_ingest,
                          oracle_slab, pool_bits)
 from helpers import bits_of
 
@@ -17,7 +17,8 @@ pytestmark = pytest.mark.gpu
 MODES = [dict(), dict(fuse_combine=0), dict(min_chunk_blocks=1, items_per_slot=1024),
          dict(min_chunk_blocks=3, items_per_slot=1024, fuse_combine=0),
          dict(min_chunk_blocks=1, items_per_slot=2), dict(min_chunk_blocks=5, items_per_slot=1),
-         dict(ring=2), dict(pdl=0), dict(pdl=0, min_chunk_blocks=1, items_per_slot=1024), dict(ring=2, min_chunk_blocks=3, items_per_slot=1024)]
+         dict(ring=2), dict(pdl=0), dict(pdl=0, min_chunk_blocks=1, items_per_slot=1024), dict(ring=2, min_chunk_blocks=3, items_per_slot=1024),
+         dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024), dict(tma=1, min_chunk_blocks=3, items_per_slot=2, fuse_combine=0)]
 SHAPES = [(8, 2, 64), (32, 32, 128), (64, 8, 128)]
 # lengths BEFORE the first step: fill a block (15 -> 16), open a new one (16 -> 17), mid-block, one token,
 # empty (0 -> 1), exact multiples, and contexts long enough to be split into several chunks
@@ -46,8 +47,7 @@ def test_fused_step_matches_oracle_and_leaves_pool_bit_exact(Hq, Hkv, d, opts):
     ids = list(range(300, 300 + len(LENS)))
     lens = list(LENS)
     pool = make_pool(w, sum((n + 15) // 16 + 1 for n in lens) + 8, alloc_seed=11)
-    for k_, v_ in opts.items():
-        pool.set_option(k_, v_)
+    apply_options(pool, opts)
     slab = oracle_slab(pool)
     have = [(u, n) for u, n in zip(ids, lens) if n > 0]
     srcs = [kv_src(w, u, 0, n, DEV) for u, n in have]

@@ -13,7 +13,7 @@ import torch
 import oracle
 import paper_2511_20982_b200 as kv
 from paper_2511_20982_b200 import workloads as W
-from gpu_harness import (DEV, NAN_BITS, compare_attention, dims_of, kv_src, make_pool, oracle_attention,
+from gpu_harness import (apply_options, DEV, NAN_BITS, compare_attention, dims_of, kv_src, make_pool, oracle_attention,
                          oracle_ingest, oracle_slab, pool_bits)
 from helpers import bf16_bits, bits_of, bits_to_f64
 
@@ -23,7 +23,8 @@ SPLIT_MODES = [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_c
                dict(min_chunk_blocks=2, items_per_slot=1024, fuse_combine=0),
                dict(min_chunk_blocks=1, items_per_slot=2), dict(min_chunk_blocks=5, items_per_slot=1),
                dict(min_chunk_blocks=1, items_per_slot=1024, ctas_per_sm=1),
-               dict(ring=2), dict(pdl=0), dict(pdl=0, min_chunk_blocks=1, items_per_slot=1024), dict(ring=2, min_chunk_blocks=3, items_per_slot=1024)]
+               dict(ring=2), dict(pdl=0), dict(pdl=0, min_chunk_blocks=1, items_per_slot=1024), dict(ring=2, min_chunk_blocks=3, items_per_slot=1024),
+               dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024), dict(tma=1, min_chunk_blocks=3, items_per_slot=2, pdl=0)]
 
 
 def from_bits(bits: np.ndarray) -> torch.Tensor:
@@ -35,8 +36,7 @@ def run_structured(Hq, Hkv, d, lens, K, V, q, scale=None, num_blocks=None, optio
     w = W.Workload("structured", L, Hq, Hkv, d, len(lens), None, 0, max_len=max(lens) + 16)
     nb = num_blocks or sum((n + 15) // 16 for n in lens) + 8
     pool = make_pool(w, nb, alloc_seed=alloc_seed)
-    for k_, v_ in (options or {}).items():
-        pool.set_option(k_, v_)
+    apply_options(pool, options)
     slab = oracle_slab(pool)
     ids = list(range(500, 500 + len(lens)))
     kb = [bf16_bits(k) for k in K]
@@ -63,8 +63,7 @@ def test_cfg1_tiny_full(opts):
     assert lens == [17, 64, 130, 255]
     ids = [10, 11, 12, 13]
     pool = make_pool(w, 128, alloc_seed=w.seed)
-    for k_, v_ in opts.items():
-        pool.set_option(k_, v_)
+    apply_options(pool, opts)
     slab = oracle_slab(pool)
     srcs = [kv_src(w, uid, 0, n, DEV) for uid, n in zip(ids, lens)]
     pool.ingest(ids, [s[0] for s in srcs], [s[1] for s in srcs])
@@ -88,8 +87,7 @@ def test_cfg1_tiny_full(opts):
 
     # one-by-one ingest gives the same slab (and P4: another placement gives the same output)
     pool_b = make_pool(w, 128, alloc_seed=w.seed + 1)
-    for k_, v_ in opts.items():
-        pool_b.set_option(k_, v_)
+    apply_options(pool_b, opts)
     for uid, (k, v) in zip(ids, srcs):
         pool_b.ingest([uid], [k], [v])
     slab_b = oracle_slab(pool_b)
@@ -229,7 +227,7 @@ def test_p2_p5_p8_closed_forms(d, opts):
         assert np.all(np.abs(got[:, h, 0] - 1.0) <= 2 ** -7)
 
 
-@pytest.mark.parametrize("opts", SPLIT_MODES[:2])
+@pytest.mark.parametrize("opts", SPLIT_MODES[:2] + [dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024)])
 def test_p3_needle_every_boundary(opts):
     d, n = 128, 1040
     rng = np.random.default_rng(3)
@@ -286,7 +284,7 @@ def append_one(pool, w, ids, lens, slab):
         oracle_ingest(slab, pool, w, uid, n, n + 1)
 
 
-@pytest.mark.parametrize("opts", SPLIT_MODES[:2])
+@pytest.mark.parametrize("opts", SPLIT_MODES[:2] + [dict(tma=1)])
 def test_cfg2_scaled_decode_steps(opts):
     """7B-MHA shape (G = 1): ingest, then decode steps = append one token per request + attend."""
     w = W.CONFIGS["cfg2_7b_mha"].scaled(batch=12)
@@ -294,8 +292,7 @@ def test_cfg2_scaled_decode_steps(opts):
     lens[:4] = [511, 527, 1024, 2047]                          # block-boundary crossings within the steps
     ids = list(range(12))
     pool = make_pool(w, sum((n + 24) // 16 + 1 for n in lens), alloc_seed=w.seed)
-    for k_, v_ in opts.items():
-        pool.set_option(k_, v_)
+    apply_options(pool, opts)
     slab = oracle_slab(pool)
     ingest_all(pool, w, ids, lens, slab)
     for step in range(4):
@@ -360,9 +357,8 @@ def test_cfg4_scaled_fragmented_long_context():
     assert np.mean(np.abs(np.diff(bt)) == 1) < 0.05             # consecutive logical blocks are not adjacent
     torch.cuda.synchronize()
     assert np.array_equal(pool_bits(pool), slab)
-    for opts in SPLIT_MODES[:2] + [dict(min_chunk_blocks=64, items_per_slot=1)]:
-        for k_, v_ in opts.items():
-            pool.set_option(k_, v_)
+    for opts in SPLIT_MODES[:2] + [dict(min_chunk_blocks=64, items_per_slot=1), dict(tma=1)]:
+        apply_options(pool, opts)
         q = W.q_values(w.seed, 0, 0, len(ids), w.num_q_heads, w.head_dim, DEV)
         out = pool.attention(0, ids, q)
         compare_attention(out, oracle_attention(slab, pool, 0, ids, q))

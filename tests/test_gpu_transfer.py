@@ -16,7 +16,7 @@ import oracle
 import paper_2511_20982_b200 as kv
 from paper_2511_20982_b200 import binding as B
 from paper_2511_20982_b200 import workloads as W
-from gpu_harness import (DEV, NAN_BITS, compare_attention, dims_of, kv_src, make_pool, oracle_attention, oracle_ingest,
+from gpu_harness import (apply_options, DEV, NAN_BITS, compare_attention, dims_of, kv_src, make_pool, oracle_attention, oracle_ingest,
                          oracle_slab, pool_bits)
 from helpers import bits_of
 
@@ -170,8 +170,7 @@ def test_step_layers_equals_per_layer_calls_and_oracle(opts, fp8):
     nb = sum((n + 15) // 16 + 1 for n in lens0) + 8
     pools = [fp8_pool(w, nb, 11) if fp8 else make_pool(w, nb, alloc_seed=11, max_requests=32) for _ in range(2)]
     for p in pools:
-        for k_, v_ in opts.items():
-            p.set_option(k_, v_)
+        apply_options(p, opts)
         p.set_option("profile", 1)
     have = [(u, n) for u, n in zip(ids, lens0) if n > 0]
     srcs = [kv_src(w, u, 0, n, DEV) for u, n in have]

@@ -11,13 +11,14 @@ import torch
 import oracle
 from paper_2511_20982_b200 import binding as B
 from paper_2511_20982_b200 import workloads as W
-from gpu_harness import DEV, compare_attention, dims_of, kv_src, make_pool, oracle_ingest, oracle_slab, pool_bits
+from gpu_harness import DEV, apply_options, compare_attention, dims_of, kv_src, make_pool, oracle_ingest, oracle_slab, pool_bits
 from helpers import bf16_bits, bits_of, bits_to_f64
 
 pytestmark = pytest.mark.gpu
 
 MODES = [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=1024),
-         dict(min_chunk_blocks=2, items_per_slot=2, ctas_per_sm=1), dict(ring=2), dict(pdl=0), dict(pdl=0, min_chunk_blocks=1, items_per_slot=1024)]
+         dict(min_chunk_blocks=2, items_per_slot=2, ctas_per_sm=1), dict(ring=2), dict(pdl=0), dict(pdl=0, min_chunk_blocks=1, items_per_slot=1024),
+         dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024)]
 SHAPES = [(8, 2, 64), (32, 32, 128), (64, 8, 128), (6, 2, 64), (5, 1, 128), (4, 2, 128)]   # G = 4, 1, 8, 3, 5, 2
 
 
@@ -30,8 +31,7 @@ def oracle_varq(slab, pool, layer, ids, q_lens, q, scale=None):
 def build(Hq, Hkv, d, lens, opts, L=1, seed=4242, alloc_seed=9):
     w = W.Workload("varq", L, Hq, Hkv, d, len(lens), None, seed, max_len=max(lens) + 16)
     pool = make_pool(w, sum((n + 15) // 16 for n in lens) + 8, max_requests=len(lens) + 4, alloc_seed=alloc_seed)
-    for k_, v_ in opts.items():
-        pool.set_option(k_, v_)
+    apply_options(pool, opts)
     slab = oracle_slab(pool)
     ids = list(range(900, 900 + len(lens)))
     srcs = [kv_src(w, uid, 0, n, DEV) for uid, n in zip(ids, lens)]
@@ -76,8 +76,7 @@ def test_structured_running_mean_and_first_token():
     w = W.Workload("varq_s", 1, Hq, Hkv, d, 2, None, 1, max_len=n + 16)
     for opts in MODES:
         pool = make_pool(w, 40, alloc_seed=3)
-        for k_, v_ in opts.items():
-            pool.set_option(k_, v_)
+        apply_options(pool, opts)
         v = np.zeros((1, Hkv, n, d)); v[..., 0] = 1.0
         v[0, :, :, 1] = (np.arange(n) % 256)[None, :]
         k = np.random.default_rng(0).standard_normal((1, Hkv, n, d))
