@@ -445,12 +445,25 @@ def measure(args, rep, sampler, wname: str, K: int, Wm: int, headline: bool):
         eb = loop.bytes_of_steps(lo, lo + e2e_steps)
         h2d, d2h = loop.io_bytes(lo, lo + e2e_steps)
         etotal = sum_over_ranks(float(eb["attn"] + eb["append"] + eb["ingest"]))
+        # the bus itself, for scale: a plain pinned host -> device copy of 512 MiB on the same stream (best of 3)
+        hbuf = torch.empty(512 << 20, dtype=torch.uint8, pin_memory=True)
+        dbuf = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+        best = 0.0
+        with torch.cuda.stream(A):
+            for _ in range(3):
+                g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                g0.record(A); dbuf.copy_(hbuf, non_blocking=True); g1.record(A); A.synchronize()
+                best = max(best, hbuf.numel() / (g0.elapsed_time(g1) * 1e-3) / 1e9)
+        del hbuf, dbuf
         e2e = {"value": etotal / (ems * 1e-3) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": h2d // e2e_steps,
+               "pcie_h2d_memcpy_gbs": best,
+               "host_ingest": {"zero_copy_calls": pool.counter("host_ingest_zero_copy"), "staged_calls": pool.counter("host_ingest_staged")},
                "d2h_bytes_per_step": d2h // e2e_steps, "steps": e2e_steps, "warmup": e2e_w,
                "ms_per_step": ems / e2e_steps,
                "decode_tokens_per_s": sum_over_ranks(float(eb["tokens"])) / (ems * 1e-3),
                "pcie_gbs": sum_over_ranks(float(h2d + d2h)) / (ems * 1e-3) / 1e9,
-               "api": "kv_ingest_host + paged_decode_step_host (pinned host q / K / V in, out back)"}
+               "api": "kv_ingest_host (pinned sources read in place by the scatter kernel) + paged_decode_step_host "
+                      "(pinned host q / K / V in, out back)"}
     host_call_us = host_cost_per_step(loop) if not args.unfused else None
     stats = pool.stats()
     kv_gb_layer = by["attn"] / K / w.num_layers / 1e9

@@ -448,9 +448,10 @@ int32_t kv_profile_reset(kv_pool_t* pool);
  * (1, default: the split-KV merge runs inside the attention kernel; 0: separate combine
  * kernel), "ring" (bf16 pools: 3, default, or 2 = shared-memory tile ring with that many slots per warp and
  * 2 / 3 CTAs per SM), "pdl" (1, default: attention launches carry the programmatic-dependent-launch attribute;
- * 0: plain launches), "tma" (0, default; 1: bf16 pools with head_dim 128 fetch full KV tiles with one
- * cp.async.bulk.tensor per tile instead of 16-byte cp.async — the measured alternative of DESIGN.md §5;
- * KV_ERR_UNSUPPORTED for other pools), "host_zero_copy" (1, default: see kv_ingest_host), "profile" (0/1, see kv_profile_read);
+ * 0: plain launches), "tma" (0, default; 1: pools with head_dim 128 fetch full KV tiles with one
+ * cp.async.bulk.tensor per tile (FP8: plus one bulk copy of the tile's scales) instead of 16-byte cp.async — the
+ * measured alternative of DESIGN.md §5; KV_ERR_UNSUPPORTED for head_dim 64), "side_upload" (1, default: plan uploads run on a stream the pool owns, beside whatever the
+ * caller's stream is executing, and the caller's stream waits for them by event; 0: uploads on the caller's stream), "host_zero_copy" (1, default: see kv_ingest_host), "profile" (0/1, see kv_profile_read);
  * KV-head sharding of a TP-sharded D-instance: "src_kv_heads" = H (0 = off) then
  * "src_head_begin" = h0 declare that the contiguous side of kv_ingest(_host) / kv_gather is the FULL-width tensor
  * [layer_count][H][n_tokens][head_dim] of which this pool holds heads [h0, h0 + num_kv_heads): every GPU of the

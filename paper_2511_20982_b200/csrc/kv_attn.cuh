@@ -45,7 +45,15 @@ struct Bf16Tiles {
   static constexpr int KS = D / 16, MT = D / 16, NE = D / 8;
   static constexpr uint32_t kSlotBytes = 2 * kBlockSize * D * 2;
   static constexpr int64_t kPoolTileBytes = kSlotBytes;
-  static constexpr int kTmaRows = kSlotBytes / 128;             // 128-byte rows of a tile (the TMA box height)
+  static constexpr uint32_t kSlotStride = kSlotBytes;           // ring slot pitch (a multiple of 1 KiB at D = 128)
+  template <int R> static __host__ __device__ constexpr uint32_t warp_ring_bytes() { return R * kSlotStride; }
+  template <int R> static __device__ __forceinline__ uint32_t scales_addr(uint32_t, int) { return 0; }
+  // TMA: one tensor copy per tile
+  static __device__ __forceinline__ void tma_tile(uint32_t slot_addr, uint32_t, const void* tmap, uint32_t bar, int64_t row,
+                                                  const unsigned char*) {
+    mbar_arrive_expect_tx(bar, kSlotBytes);
+    tma_load_2d(slot_addr, tmap, bar, 0, static_cast<int32_t>(row));
+  }
 
   // token held by MMA row r (r in [0, 8); rows r + 8 hold token tok(r) + 8)
   static __device__ __forceinline__ int tok(int r) { return kTmaL ? static_cast<int>((0x57463120u >> (4 * r)) & 7u) : r; }
@@ -85,7 +93,7 @@ struct Bf16Tiles {
   // start the copies of one tile into a ring slot; row r_new (>= 0 only for the fused append's tile) comes from
   // the new token's rows instead of the pool
   template <bool kAppend>
-  static __device__ __forceinline__ void copy_tile(uint32_t slot_addr, const unsigned char* tile, int nv, int lane, int r_new,
+  static __device__ __forceinline__ void copy_tile(uint32_t slot_addr, uint32_t, const unsigned char* tile, int nv, int lane, int r_new,
                                                    const uint16_t* knew_row, const uint16_t* vnew_row) {
     constexpr int kCh = D / 8;                                  // 16-byte chunks per row
 #pragma unroll
@@ -107,9 +115,9 @@ struct Bf16Tiles {
       *reinterpret_cast<uint4*>(tile + cc * (kBlockSize * D * 2) + r_new * (D * 2) + ch * 16) = x;
     }
   }
-  static __device__ __forceinline__ void patch_slot(uint32_t, int, int, const NewRow&) {}
+  static __device__ __forceinline__ void patch_slot(uint32_t, uint32_t, int, int, const NewRow&) {}
 
-  static __device__ __forceinline__ void load_frags(Frag& T, uint32_t slot_addr, int g, int c) {
+  static __device__ __forceinline__ void load_frags(Frag& T, uint32_t slot_addr, uint32_t, int g, int c) {
 #pragma unroll
     for (int rs = 0; rs < 2; ++rs)
 #pragma unroll
@@ -185,14 +193,34 @@ struct Bf16Tiles {
 //     overflow or underflow to manage — while l accumulates p'_t / vs_t.  O and l share the reference m', so O / l
 //     and the LSE merge are unchanged.
 // =============================================================================================
-template <int D_>
+// kTmaL = true (D = 128): the codes of a tile (32 rows of 128 B) arrive by one cp.async.bulk.tensor into a 1 KiB-aligned
+// 4 KiB slot in the hardware's 128-byte swizzle, the 128 bytes of scales by a second (1-D) bulk copy into a small ring
+// behind the code slots, both completing on the slot's mbarrier; tokens are permuted over the MMA rows (tok) so that the
+// fragment reads stay conflict-free under that swizzle.  This is where TMA pays: the FP8 loop spends 9 LDGSTS + ~45
+// integer instructions per 4 KiB tile on copies, on a warp that is issue-limited.
+template <int D_, bool kTmaL = false>
 struct Fp8Tiles {
   static constexpr int D = D_;
+  static_assert(!kTmaL || D_ == 128, "the TMA layout is built for 128-byte code rows");
   static constexpr int KS = D / 16, MT = D / 16, NE = D / 8;
-  static constexpr uint32_t kSlotBytes = 32 * D + 128;
+  static constexpr uint32_t kSlotBytes = 32 * D + 128;          // bytes of a tile (what a copy moves)
   static constexpr int64_t kPoolTileBytes = kSlotBytes;
-  static constexpr bool kTma = false;
-  static __device__ __forceinline__ int tok(int r) { return r; }
+  static constexpr bool kTma = kTmaL;
+  static constexpr uint32_t kSlotStride = kTmaL ? 32 * D : kSlotBytes;
+  // per-warp ring: R slots (+ R x 128 B of scales behind them in the TMA layout), padded to a multiple of 1 KiB
+  template <int R> static __host__ __device__ constexpr uint32_t warp_ring_bytes() {
+    return kTmaL ? (R * kSlotStride + R * 128 + 1023u) / 1024u * 1024u : R * kSlotStride;
+  }
+  template <int R> static __device__ __forceinline__ uint32_t scales_addr(uint32_t ring, int s) {
+    return kTmaL ? ring + R * kSlotStride + s * 128 : ring + s * kSlotStride + 2 * kBlockSize * D;
+  }
+  static __device__ __forceinline__ int tok(int r) { return kTmaL ? static_cast<int>((0x37156240u >> (4 * r)) & 7u) : r; }
+  static __device__ __forceinline__ void tma_tile(uint32_t slot_addr, uint32_t sc_addr, const void* tmap, uint32_t bar, int64_t row,
+                                                  const unsigned char* tile) {
+    mbar_arrive_expect_tx(bar, kSlotBytes);
+    tma_load_2d(slot_addr, tmap, bar, 0, static_cast<int32_t>(row));
+    bulk_load_1d(sc_addr, tile + 2 * kBlockSize * D, 128, bar);
+  }
   static constexpr bool kVScaled = true;
   static constexpr bool kLazyRescale = true;                    // rescale O only when some running maximum moved
   static constexpr bool kPatchNewRow = true;                    // the quantised new row is patched into the slot after it landed
@@ -206,7 +234,8 @@ struct Fp8Tiles {
   };
 
   static __device__ __forceinline__ uint32_t chunk_off(int row, int chunk) {   // byte offset of a 16-byte chunk of a code row
-    if constexpr (D == 128) return row * 128 + ((chunk ^ (((row >> 1) & 1) << 1) ^ ((((row >> 2) ^ row) & 1) << 2)) << 4);
+    if constexpr (kTmaL) return row * 128 + ((chunk ^ (row & 7)) << 4);
+    else if constexpr (D == 128) return row * 128 + ((chunk ^ (((row >> 1) & 1) << 1) ^ ((((row >> 2) ^ row) & 1) << 2)) << 4);
     else return row * 64 + ((chunk ^ ((row >> 1) & 3)) << 4);                 // 4 chunks per row: rows pair up per 128 bytes
   }
 
@@ -242,7 +271,7 @@ struct Fp8Tiles {
   }
 
   template <bool kAppend>
-  static __device__ __forceinline__ void copy_tile(uint32_t slot_addr, const unsigned char* tile, int nv, int lane, int,
+  static __device__ __forceinline__ void copy_tile(uint32_t slot_addr, uint32_t sc_addr, const unsigned char* tile, int nv, int lane, int,
                                                    const uint16_t*, const uint16_t*) {
     constexpr int kChunksPerRow = D / 16;
 #pragma unroll
@@ -253,7 +282,7 @@ struct Fp8Tiles {
     }
     if (lane < 8) {                                                           // sc[16] {ks, vs}: 8 chunks of 2 rows
       const int sz = 2 * lane < nv ? (2 * lane + 1 < nv ? 16 : 8) : 0;
-      asm volatile("cp.async.ca.shared.global [%0], [%1], 16, %2;" ::"r"(slot_addr + 2 * kBlockSize * D + lane * 16),
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 16, %2;" ::"r"(sc_addr + lane * 16),
                    "l"(tile + 2 * kBlockSize * D + lane * 16), "r"(sz) : "memory");
     }
   }
@@ -276,27 +305,27 @@ struct Fp8Tiles {
     }
   }
   // ... and, once the tile's stale bytes have landed in the slot, the same row goes on top of them
-  static __device__ __forceinline__ void patch_slot(uint32_t slot_addr, int r_new, int lane, const NewRow& nr) {
+  static __device__ __forceinline__ void patch_slot(uint32_t slot_addr, uint32_t sc_addr, int r_new, int lane, const NewRow& nr) {
     constexpr int kP = D / 8;
     const int cc = lane / kP, cp = lane % kP;
     if (lane < 2 * kP) {
       asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(slot_addr + cc * (kBlockSize * D) + chunk_off(r_new, cp >> 1) + (cp & 1) * 8),
                    "r"(nr.codes.x), "r"(nr.codes.y) : "memory");
-      if (cp == 0) asm volatile("st.shared.f32 [%0], %1;" ::"r"(slot_addr + 2 * kBlockSize * D + r_new * 8 + cc * 4), "f"(nr.scale) : "memory");
+      if (cp == 0) asm volatile("st.shared.f32 [%0], %1;" ::"r"(sc_addr + r_new * 8 + cc * 4), "f"(nr.scale) : "memory");
     }
   }
 
-  static __device__ __forceinline__ void load_frags(Frag& T, uint32_t slot, int g, int c) {
+  static __device__ __forceinline__ void load_frags(Frag& T, uint32_t slot, uint32_t sc_addr, int g, int c) {
 #pragma unroll
     for (int rs = 0; rs < 2; ++rs) {
-      const int row = g + 8 * rs;
+      const int row = tok(g) + 8 * rs;
 #pragma unroll
       for (int j = 0; j < D / 64; ++j) T.k[rs][j] = lds128(slot + chunk_off(row, c + 4 * j));
-      asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(T.sc[rs].x), "=f"(T.sc[rs].y) : "r"(slot + 2 * kBlockSize * D + row * 8));
+      asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(T.sc[rs].x), "=f"(T.sc[rs].y) : "r"(sc_addr + row * 8));
     }
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      const int row = 2 * c + (i & 1) + 8 * (i >> 1);
+      const int row = tok(2 * c + (i & 1)) + 8 * (i >> 1);
       if constexpr (D == 128) {
         const uint4 x = lds128(slot + kBlockSize * D + chunk_off(row, g));
         T.v[i][0] = x.x; T.v[i][1] = x.y; T.v[i][2] = x.z; T.v[i][3] = x.w;
@@ -373,9 +402,9 @@ __global__ void __launch_bounds__(kAttnThreads, kCtas) attn_kernel(const __grid_
   const int lane = threadIdx.x & 31;
   uint32_t smem0 = static_cast<uint32_t>(__cvta_generic_to_shared(ring_smem));
   if constexpr (TP::kTma) smem0 = (smem0 + 1023u) & ~1023u;     // the 128-byte swizzle is a function of the address
-  const uint32_t ring = smem0 + (threadIdx.x >> 5) * (R * TP::kSlotBytes);
+  const uint32_t ring = smem0 + (threadIdx.x >> 5) * TP::template warp_ring_bytes<R>();
   // TMA variants: one mbarrier per ring slot of this warp (behind the rings), and the parity each is next waited on
-  const uint32_t bars = smem0 + kAttnWarps * (R * TP::kSlotBytes) + (threadIdx.x >> 5) * (R * 8);
+  const uint32_t bars = smem0 + kAttnWarps * TP::template warp_ring_bytes<R>() + (threadIdx.x >> 5) * (R * 8);
   uint32_t bar_parity = 0;
   if constexpr (TP::kTma) {
     if (lane == 0) {
@@ -468,16 +497,14 @@ __global__ void __launch_bounds__(kAttnThreads, kCtas) attn_kernel(const __grid_
         const int nv = n_tokens - t * kBlockSize;
         bool by_tma = false;
         if constexpr (TP::kTma) by_tma = nv >= kBlockSize && !first_special;   // full tiles: one bulk tensor copy
+        const uint32_t dst = ring + (v % R) * TP::kSlotStride, dst_sc = TP::template scales_addr<R>(ring, v % R);
         if (by_tma) {
           if (lane == 0) {
-            const uint32_t bar = bars + (v % R) * 8;
             fence_proxy_async();                                 // the slot's last readers used the generic proxy
-            mbar_arrive_expect_tx(bar, TP::kSlotBytes);
-            tma_load_2d(ring + (v % R) * TP::kSlotBytes, p.tmap, bar, 0,
-                        static_cast<int32_t>(p.tma_row0 + (tile - kv) / 128));
+            TP::tma_tile(dst, dst_sc, p.tmap, bars + (v % R) * 8, p.tma_row0 + (tile - kv) / 128, tile);
           }
         } else {
-          TP::template copy_tile<kAppend>(ring + (v % R) * TP::kSlotBytes, tile, nv, lane, first_special ? nv - 1 : -1,
+          TP::template copy_tile<kAppend>(dst, dst_sc, tile, nv, lane, first_special ? nv - 1 : -1,
                                           p.k_new + new_row, p.v_new + new_row);
         }
         if constexpr (kAppend) {
@@ -493,7 +520,7 @@ __global__ void __launch_bounds__(kAttnThreads, kCtas) attn_kernel(const __grid_
     auto consume = [&](int v) {
       const int t = (special && v == 0) ? n_blocks - 1 : v - sp;
       const int nv = n_tokens - t * kBlockSize;
-      const uint32_t slot_addr = ring + (v % R) * TP::kSlotBytes;
+      const uint32_t slot_addr = ring + (v % R) * TP::kSlotStride, sc_addr = TP::template scales_addr<R>(ring, v % R);
       if constexpr (TP::kTma) {                                  // wait for the tile: mbarrier (TMA) or this warp's LDGSTS
         if (nv >= kBlockSize && !(special && v == 0)) {
           mbar_wait(bars + (v % R) * 8, (bar_parity >> (v % R)) & 1u);
@@ -506,12 +533,12 @@ __global__ void __launch_bounds__(kAttnThreads, kCtas) attn_kernel(const __grid_
       }
       if constexpr (kAppend && TP::kPatchNewRow) {
         if (special && v == 0) {
-          TP::patch_slot(slot_addr, nv - 1, lane, nr);
+          TP::patch_slot(slot_addr, sc_addr, nv - 1, lane, nr);
           __syncwarp();
         }
       }
       typename TP::Frag T;
-      TP::load_frags(T, slot_addr, g, c);
+      TP::load_frags(T, slot_addr, sc_addr, g, c);
       float s[4], vs[2];
       TP::scores(T, Q, cs0, cs1, s, vs);
       float iv0 = 1.f, iv1 = 1.f;

@@ -130,6 +130,12 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const void* tmap, uint
                ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(bar), "r"(c0), "r"(c1) : "memory");
 }
 
+// 1-D bulk copy global -> shared (SASS UBLKCP), 16-byte aligned, size a multiple of 16; completion on `bar`
+__device__ __forceinline__ void bulk_load_1d(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
 // Programmatic dependent launch (PDL).  wait: block until every grid this launch depends on has completed and its
 // memory is visible (a no-op for a launch without the programmatic attribute).  launch_dependents: allow the next
 // launch of the stream, if it carries the attribute, to start its CTAs as SM resources free up.

@@ -71,6 +71,7 @@ struct StageSlot {
   char* host_dev = nullptr;  // the same pinned buffer as the device addresses it (zero-copy reads by plan_upload_kernel)
   char* dev = nullptr;    // inside the slab
   cudaEvent_t ev = nullptr;
+  cudaEvent_t up_ev = nullptr;  // side-stream upload of this slot's plan has completed
   bool in_flight = false;
 };
 
@@ -209,6 +210,8 @@ struct kv_pool {
   int32_t src_head_begin = 0;     //                   this pool's head 0 is that side's head src_head_begin
   int32_t ring = 3;               // bf16 pool: ring slots per warp, 3 (2 CTAs per SM, default) or 2 (3 CTAs per SM)
   bool pdl = true;                // attention launches carry the programmatic-dependent-launch attribute
+  bool side_upload = true;        // plan uploads on the pool's own stream (overlapping the caller's stream), joined by an event
+  cudaStream_t up_stream = nullptr;
   bool tma = false;               // bf16 pools, head_dim 128: full tiles by cp.async.bulk.tensor (UTMALDG) instead of LDGSTS
   bool tmap_ok = false;
   alignas(64) CUtensorMap tmap;   // the KV region as [rows][128 B], box 64 rows, 128-byte swizzle
@@ -422,7 +425,7 @@ template <class TP, bool kAppend, bool kVarQ, int R, int kCtas>
 AttnVariant variant() {
   // TMA variants: + 1 KiB so the rings can start on a 1 KiB boundary, + one mbarrier per slot and warp
   const size_t extra = TP::kTma ? 1024 + static_cast<size_t>(kAttnWarps) * R * 8 : 0;
-  return {attn_kernel<TP, kAppend, kVarQ, R, kCtas>, static_cast<size_t>(kAttnWarps) * R * TP::kSlotBytes + extra, kCtas};
+  return {attn_kernel<TP, kAppend, kVarQ, R, kCtas>, static_cast<size_t>(kAttnWarps) * TP::template warp_ring_bytes<R>() + extra, kCtas};
 }
 template <class TP, int R, int kCtas>
 AttnVariant variant_of(bool append, bool varq) {
@@ -431,6 +434,7 @@ AttnVariant variant_of(bool append, bool varq) {
 }
 AttnVariant pick_variant(const kv_pool* pool, bool append, bool varq) {
   const bool d128 = pool->hs.cfg.head_dim == 128;
+  if (pool->fp8() && pool->tma && pool->tmap_ok && d128) return variant_of<Fp8Tiles<128, true>, kFp8RingSlots, 3>(append, varq);
   if (pool->fp8())
     return d128 ? variant_of<Fp8Tiles<128>, kFp8RingSlots, 3>(append, varq) : variant_of<Fp8Tiles<64>, kFp8RingSlots, 3>(append, varq);
   if (pool->tma && pool->tmap_ok && d128) return variant_of<Bf16Tiles<128, true>, 3, 2>(append, varq);
@@ -439,11 +443,11 @@ AttnVariant pick_variant(const kv_pool* pool, bool append, bool varq) {
   return d128 ? variant_of<Bf16Tiles<128>, 3, 2>(append, varq) : variant_of<Bf16Tiles<64>, 3, 2>(append, varq);
 }
 
-// The KV region of a bf16 pool as a 2-D tensor of 128-byte rows; a (block, kv head) tile is 64 consecutive rows
-// (head_dim 128).  CU_TENSOR_MAP_SWIZZLE_128B is the layout Bf16Tiles<128, true> reads.
+// The KV region as a 2-D tensor of 128-byte rows (head_dim 128): a bf16 (block, kv head) tile is 64 consecutive rows,
+// an FP8 tile 33 (32 code rows + the scales row).  CU_TENSOR_MAP_SWIZZLE_128B is the layout the <.., true> providers read.
 bool make_tensor_map(kv_pool* pool) {
   const kv_pool_config_t& c = pool->hs.cfg;
-  if (pool->fp8() || c.head_dim != 128 || pool->lay.kv_bytes % 128 != 0) return false;
+  if (c.head_dim != 128 || pool->lay.kv_bytes % 128 != 0) return false;
   using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -458,7 +462,7 @@ bool make_tensor_map(kv_pool* pool) {
   if (rows >= (1ull << 31)) return false;                       // tile coordinates are int32
   const cuuint64_t gdim[2] = {128, rows};
   const cuuint64_t gstride[1] = {128};                           // bytes between rows (dimension 1)
-  const cuuint32_t box[2] = {128, 64};
+  const cuuint32_t box[2] = {128, pool->fp8() ? 32u : 64u};    // FP8: the 32 code rows of a tile (its scales row follows them)
   const cuuint32_t estride[2] = {1, 1};
   const CUresult r = reinterpret_cast<EncodeFn>(fn)(&pool->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, pool->base, gdim, gstride, box,
                                                     estride, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
@@ -500,8 +504,18 @@ cudaError_t upload_plan(kv_pool* pool, const StageSlot& s, size_t bytes, cudaStr
   ++pool->n_plans;
   if (!pool->pdl || bytes == 0) return bytes ? cudaMemcpyAsync(s.dev, s.host, bytes, cudaMemcpyHostToDevice, stream) : cudaSuccess;
   const int n16 = static_cast<int>((bytes + 15) / 16);
+  const unsigned grid = static_cast<unsigned>(std::max(1, std::min((n16 + 255) / 256, 32)));
+  if (pool->side_upload && pool->up_stream) {
+    // The slot is free (acquire waited for its last reader) and nothing else touches it: the copy may run beside
+    // whatever the caller's stream is executing; the caller's stream only waits for its completion.
+    plan_upload_kernel<<<grid, 256, 0, pool->up_stream>>>(reinterpret_cast<const uint4*>(s.host_dev), reinterpret_cast<uint4*>(s.dev), n16);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaEventRecord(s.up_ev, pool->up_stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, s.up_ev, 0);
+    return e;
+  }
   cudaLaunchConfig_t cfg{};
-  cfg.gridDim = dim3(static_cast<unsigned>(std::max(1, std::min((n16 + 255) / 256, 32))));
+  cfg.gridDim = dim3(grid);
   cfg.blockDim = dim3(256);
   cfg.stream = stream;
   cudaLaunchAttribute attr[1];
@@ -584,8 +598,10 @@ int32_t kv_pool_create(const kv_pool_config_t* cfg, kv_pool_t** out_pool) {
       e = cudaHostAlloc(reinterpret_cast<void**>(&pool->plan_ring[i].host), lay.plan_blob_bytes, cudaHostAllocMapped);
       if (e == cudaSuccess) e = cudaHostGetDevicePointer(reinterpret_cast<void**>(&pool->plan_ring[i].host_dev), pool->plan_ring[i].host, 0);
       if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pool->plan_ring[i].ev, cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pool->plan_ring[i].up_ev, cudaEventDisableTiming);
       pool->plan_ring[i].dev = pool->base + lay.plan_blobs + i * lay.plan_blob_bytes;
     }
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&pool->up_stream, cudaStreamNonBlocking);
     // work counters start at zero; the attention kernel rewinds them itself afterwards
     if (e == cudaSuccess) pool->tmap_ok = make_tensor_map(pool);
     if (e == cudaSuccess) e = cudaMemset(pool->base + lay.counters, 0, 256);
@@ -607,8 +623,10 @@ int32_t kv_pool_destroy(kv_pool_t* pool) {
     for (int i = 0; i < kRing; ++i) {
       if (pool->plan_ring[i].host) cudaFreeHost(pool->plan_ring[i].host);
       if (pool->plan_ring[i].ev) cudaEventDestroy(pool->plan_ring[i].ev);
+      if (pool->plan_ring[i].up_ev) cudaEventDestroy(pool->plan_ring[i].up_ev);
     }
     for (ProfRing& r : pool->prof) r.destroy();
+    if (pool->up_stream) { cudaStreamSynchronize(pool->up_stream); cudaStreamDestroy(pool->up_stream); }
   }
   delete pool;
   return KV_OK;
@@ -1174,6 +1192,7 @@ int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
   if (!std::strcmp(key, "profile") && (value == 0 || value == 1)) { pool->profile = value != 0; return KV_OK; }
   if (!std::strcmp(key, "fuse_combine") && (value == 0 || value == 1)) { pool->fuse_combine = value != 0; return KV_OK; }
   if (!std::strcmp(key, "pdl") && (value == 0 || value == 1)) { pool->pdl = value != 0; return KV_OK; }
+  if (!std::strcmp(key, "side_upload") && (value == 0 || value == 1)) { pool->side_upload = value != 0; return KV_OK; }
   if (!std::strcmp(key, "tma") && (value == 0 || value == 1)) {   // bf16, head_dim 128 pools with a device slab only
     if (value == 1 && !pool->tmap_ok) return KV_ERR_UNSUPPORTED;
     pool->tma = value != 0;

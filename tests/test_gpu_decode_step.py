@@ -18,7 +18,7 @@ MODES = [dict(), dict(fuse_combine=0), dict(min_chunk_blocks=1, items_per_slot=1
          dict(min_chunk_blocks=3, items_per_slot=1024, fuse_combine=0),
          dict(min_chunk_blocks=1, items_per_slot=2), dict(min_chunk_blocks=5, items_per_slot=1),
          dict(ring=2), dict(pdl=0), dict(pdl=0, min_chunk_blocks=1, items_per_slot=1024), dict(ring=2, min_chunk_blocks=3, items_per_slot=1024),
-         dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024), dict(tma=1, min_chunk_blocks=3, items_per_slot=2, fuse_combine=0)]
+         dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024), dict(tma=1, min_chunk_blocks=3, items_per_slot=2, fuse_combine=0), dict(side_upload=0), dict(side_upload=0, min_chunk_blocks=1, items_per_slot=1024)]
 SHAPES = [(8, 2, 64), (32, 32, 128), (64, 8, 128)]
 # lengths BEFORE the first step: fill a block (15 -> 16), open a new one (16 -> 17), mid-block, one token,
 # empty (0 -> 1), exact multiples, and contexts long enough to be split into several chunks

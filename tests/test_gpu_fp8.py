@@ -13,14 +13,15 @@ import oracle
 import paper_2511_20982_b200 as kv
 from paper_2511_20982_b200 import binding as B
 from paper_2511_20982_b200 import workloads as W
-from gpu_harness import DEV, compare_attention, dims_of, kv_src
+from gpu_harness import DEV, apply_options, compare_attention, dims_of, kv_src
 from helpers import bf16_bits, bits_of, bits_to_f64
 
 pytestmark = pytest.mark.gpu
 
 MODES = [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=1024),
          dict(min_chunk_blocks=2, items_per_slot=2, fuse_combine=0), dict(min_chunk_blocks=5, items_per_slot=1, ctas_per_sm=1),
-         dict(pdl=0), dict(pdl=0, min_chunk_blocks=2, items_per_slot=1024)]
+         dict(pdl=0), dict(pdl=0, min_chunk_blocks=2, items_per_slot=1024),
+         dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024), dict(tma=1, min_chunk_blocks=3, items_per_slot=2, fuse_combine=0)]
 SENT = 0xFF   # e4m3 NaN code / NaN scale bytes: an unmasked read poisons the output
 
 
@@ -84,8 +85,7 @@ def test_attention_matches_oracle(Hq, Hkv, d, opts):
     lens = [17, 64, 130, 255, 1, 16, 33, 700, 1900, 5]
     ids = list(range(300, 300 + len(lens)))
     pool = make_fp8_pool(1, Hq, Hkv, d, sum((n + 15) // 16 for n in lens) + 8)
-    for k_, v_ in opts.items():
-        pool.set_option(k_, v_)
+    apply_options(pool, opts)
     w = W.Workload("fp8", 1, Hq, Hkv, d, len(lens), None, 99, max_len=4096)
     srcs = [kv_src(w, uid, 0, n, DEV) for uid, n in zip(ids, lens)]
     pool.ingest(ids, [s[0] for s in srcs], [s[1] for s in srcs])
@@ -107,7 +107,7 @@ def test_attention_matches_oracle(Hq, Hkv, d, opts):
     assert np.abs(want - exact).max() < 0.15 and np.abs(want - exact).mean() < 0.01
 
 
-@pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=2, items_per_slot=1024)])
+@pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=2, items_per_slot=1024), dict(tma=1)])
 def test_attention_wide_dynamic_range(opts):
     """Row magnitudes from e^-6 to e^6 in K and V, scaled-up queries, a zero row and an outlier element."""
     rng = np.random.default_rng(8)
@@ -115,8 +115,7 @@ def test_attention_wide_dynamic_range(opts):
     lens = [40, 333, 1000]
     ids = [1, 2, 3]
     pool = make_fp8_pool(1, Hq, Hkv, d, 100)
-    for k_, v_ in opts.items():
-        pool.set_option(k_, v_)
+    apply_options(pool, opts)
     K = [bf16_bits(rng.standard_normal((1, Hkv, n, d)) * 0.3) for n in lens]      # keep the scores moderate
     V = [wide_rows(rng, 1, Hkv, n, d) for n in lens]
     pool.ingest(ids, [tb(k) for k in K], [tb(v) for v in V])
@@ -186,7 +185,8 @@ def test_gather_fp8_returns_stored_codes_and_scales(Hkv, d):
     assert np.array_equal(pool_bytes(pool), before)
 
 
-@pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=2)])
+@pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=2),
+                                  dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024)])
 @pytest.mark.parametrize("Hq,Hkv,d", [(32, 8, 128), (8, 2, 64), (32, 32, 128)])
 def test_fused_decode_step_quantises_like_ingest(Hq, Hkv, d, opts):
     """paged_decode_step on an FP8 pool: the appended row's codes and scales are the bytes kv_ingest would have
@@ -196,8 +196,7 @@ def test_fused_decode_step_quantises_like_ingest(Hq, Hkv, d, opts):
     ids = list(range(len(lens)))
     w = W.Workload("fp8s", L, Hq, Hkv, d, len(lens), None, 6, max_len=2048)
     pool = make_fp8_pool(L, Hq, Hkv, d, 160)
-    for k_, v_ in opts.items():
-        pool.set_option(k_, v_)
+    apply_options(pool, opts)
     slab = oracle.new_slab_fp8(dims_of(pool), SENT)
     live = [(u, n) for u, n in zip(ids, lens) if n]
     srcs = [kv_src(w, u, 0, n, DEV) for u, n in live]
@@ -223,7 +222,8 @@ def test_fused_decode_step_quantises_like_ingest(Hq, Hkv, d, opts):
         assert np.array_equal(pool_bytes(pool), slab), f"step {step}: fused FP8 append is not byte-exact"
 
 
-@pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=2)])
+@pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=2),
+                                  dict(tma=1), dict(tma=1, min_chunk_blocks=2, items_per_slot=1024)])
 @pytest.mark.parametrize("Hq,Hkv,d", [(8, 2, 64), (32, 32, 128), (64, 8, 128), (6, 2, 64)])
 def test_varlen_attention_on_fp8_pool(Hq, Hkv, d, opts):
     """In-place prefill rows + decode rows over an FP8 pool == oracle.attention_varq_fp8."""
@@ -231,8 +231,7 @@ def test_varlen_attention_on_fp8_pool(Hq, Hkv, d, opts):
     q_lens = [17, 1, 130, 7, 1, 16, 1, 1, 300, 5, 31, 100]
     ids = list(range(700, 700 + len(lens)))
     pool = make_fp8_pool(1, Hq, Hkv, d, sum((n + 15) // 16 for n in lens) + 8)
-    for k_, v_ in opts.items():
-        pool.set_option(k_, v_)
+    apply_options(pool, opts)
     w = W.Workload("fp8v", 1, Hq, Hkv, d, len(lens), None, 98, max_len=4096)
     srcs = [kv_src(w, uid, 0, n, DEV) for uid, n in zip(ids, lens)]
     pool.ingest(ids, [s[0] for s in srcs], [s[1] for s in srcs])

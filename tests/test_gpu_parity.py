@@ -24,7 +24,7 @@ SPLIT_MODES = [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_c
                dict(min_chunk_blocks=1, items_per_slot=2), dict(min_chunk_blocks=5, items_per_slot=1),
                dict(min_chunk_blocks=1, items_per_slot=1024, ctas_per_sm=1),
                dict(ring=2), dict(pdl=0), dict(pdl=0, min_chunk_blocks=1, items_per_slot=1024), dict(ring=2, min_chunk_blocks=3, items_per_slot=1024),
-               dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024), dict(tma=1, min_chunk_blocks=3, items_per_slot=2, pdl=0)]
+               dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024), dict(tma=1, min_chunk_blocks=3, items_per_slot=2, pdl=0), dict(side_upload=0), dict(side_upload=0, min_chunk_blocks=1, items_per_slot=1024)]
 
 
 def from_bits(bits: np.ndarray) -> torch.Tensor:
