@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libkvpool.so")
 SOURCES = ["kv_pool.cu"]
-DEPS = SOURCES + ["kv_common.cuh", "kv_copy.cuh", "kv_attn.cuh", "kv_host.h", os.path.join("..", "..", "include", "kv_pool.h")]
+DEPS = SOURCES + ["kv_common.cuh", "kv_copy.cuh", "kv_attn.cuh", "kv_attn_tc.cuh", "kv_host.h", os.path.join("..", "..", "include", "kv_pool.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

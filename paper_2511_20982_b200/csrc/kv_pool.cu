@@ -15,6 +15,7 @@
 #include "kv_common.cuh"
 #include "kv_copy.cuh"
 #include "kv_attn.cuh"
+#include "kv_attn_tc.cuh"
 
 namespace {
 
@@ -214,6 +215,9 @@ struct kv_pool {
   cudaStream_t up_stream = nullptr;
   bool tma = false;               // bf16 pools, head_dim 128: full tiles by cp.async.bulk.tensor (UTMALDG) instead of LDGSTS
   bool tmap_ok = false;
+  bool tc = false;                // FP8 pools, head_dim 128: decode attention on tcgen05 / TMEM (attn_tc_kernel)
+  bool tmap16_ok = false;
+  alignas(64) CUtensorMap tmap16; // the same region, box 16 rows: the K codes or the V codes of one (block, kv head) tile
   alignas(64) CUtensorMap tmap;   // the KV region as [rows][128 B], box 64 rows, 128-byte swizzle
   // event counters (kv_pool_counter)
   int64_t n_zero_copy = 0, n_staged = 0, n_chained = 0, n_stream_switch = 0, n_plans = 0;
@@ -250,7 +254,13 @@ struct kv_pool {
   }
   bool fp8() const { return hs.cfg.kv_dtype == KV_DTYPE_FP8_E4M3; }
   int32_t kernel_ctas() const { return fp8() ? 3 : (ring == 2 ? 3 : 2); }
-  int32_t slots() const { return num_sms * (ctas_per_sm > 0 ? ctas_per_sm : kernel_ctas()) * kvp::kAttnWarps; }
+  bool tc_decode() const { return tc && tmap16_ok; }
+  // work units the attention kernel of a decode (or variable-q) launch processes at a time: resident warps of the
+  // mma.sync kernels, resident CTAs of the tcgen05 kernel
+  int32_t slots(bool varq = false) const {
+    if (!varq && tc_decode()) return num_sms * (ctas_per_sm > 0 ? ctas_per_sm : 2);
+    return num_sms * (ctas_per_sm > 0 ? ctas_per_sm : kernel_ctas()) * kvp::kAttnWarps;
+  }
   int32_t src_heads() const { return src_kv_heads > 0 ? src_kv_heads : hs.cfg.num_kv_heads; }
   int32_t min_chunk() const { return (fp8() && !min_chunk_set) ? 32 : min_chunk_blocks; }
   int32_t ips() const { return (fp8() && !items_per_slot_set) ? 1 : items_per_slot; }
@@ -417,6 +427,8 @@ struct AttnVariant {
   AttnFn fn;
   size_t smem;
   int ctas;
+  int threads = kAttnThreads;
+  int units_per_cta = kAttnWarps;   // work units a CTA processes at a time
 };
 
 constexpr int kFp8RingSlots = 4;   // FP8 pools: 4 ring slots per warp, 3 CTAs per SM
@@ -434,6 +446,8 @@ AttnVariant variant_of(bool append, bool varq) {
 }
 AttnVariant pick_variant(const kv_pool* pool, bool append, bool varq) {
   const bool d128 = pool->hs.cfg.head_dim == 128;
+  if (!varq && pool->tc_decode())
+    return {append ? attn_tc_kernel<true> : attn_tc_kernel<false>, kTcSmemBytes, 2, kTcThreads, 1};
   if (pool->fp8() && pool->tma && pool->tmap_ok && d128) return variant_of<Fp8Tiles<128, true>, kFp8RingSlots, 3>(append, varq);
   if (pool->fp8())
     return d128 ? variant_of<Fp8Tiles<128>, kFp8RingSlots, 3>(append, varq) : variant_of<Fp8Tiles<64>, kFp8RingSlots, 3>(append, varq);
@@ -445,7 +459,7 @@ AttnVariant pick_variant(const kv_pool* pool, bool append, bool varq) {
 
 // The KV region as a 2-D tensor of 128-byte rows (head_dim 128): a bf16 (block, kv head) tile is 64 consecutive rows,
 // an FP8 tile 33 (32 code rows + the scales row).  CU_TENSOR_MAP_SWIZZLE_128B is the layout the <.., true> providers read.
-bool make_tensor_map(kv_pool* pool) {
+bool make_tensor_map(kv_pool* pool, CUtensorMap* out, uint32_t box_rows) {
   const kv_pool_config_t& c = pool->hs.cfg;
   if (c.head_dim != 128 || pool->lay.kv_bytes % 128 != 0) return false;
   using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -462,9 +476,9 @@ bool make_tensor_map(kv_pool* pool) {
   if (rows >= (1ull << 31)) return false;                       // tile coordinates are int32
   const cuuint64_t gdim[2] = {128, rows};
   const cuuint64_t gstride[1] = {128};                           // bytes between rows (dimension 1)
-  const cuuint32_t box[2] = {128, pool->fp8() ? 32u : 64u};    // FP8: the 32 code rows of a tile (its scales row follows them)
+  const cuuint32_t box[2] = {128, box_rows};
   const cuuint32_t estride[2] = {1, 1};
-  const CUresult r = reinterpret_cast<EncodeFn>(fn)(&pool->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, pool->base, gdim, gstride, box,
+  const CUresult r = reinterpret_cast<EncodeFn>(fn)(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, pool->base, gdim, gstride, box,
                                                     estride, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                                                     CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS;
@@ -484,10 +498,10 @@ cudaError_t ensure_smem_optin(const AttnVariant& v, int device) {
 cudaError_t launch_attn_kernel(const kv_pool* pool, const AttnVariant& v, const AttnParams& p, cudaStream_t stream) {
   cudaError_t e = ensure_smem_optin(v, pool->device);
   if (e != cudaSuccess) return e;
-  const int32_t want = (p.n_units + kAttnWarps - 1) / kAttnWarps;
+  const int32_t want = (p.n_units + v.units_per_cta - 1) / v.units_per_cta;
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(static_cast<unsigned>(std::max(1, std::min(want, pool->num_sms * v.ctas))));
-  cfg.blockDim = dim3(kAttnThreads);
+  cfg.blockDim = dim3(static_cast<unsigned>(v.threads));
   cfg.dynamicSmemBytes = v.smem;
   cfg.stream = stream;
   cudaLaunchAttribute attr[1];
@@ -603,7 +617,9 @@ int32_t kv_pool_create(const kv_pool_config_t* cfg, kv_pool_t** out_pool) {
     }
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&pool->up_stream, cudaStreamNonBlocking);
     // work counters start at zero; the attention kernel rewinds them itself afterwards
-    if (e == cudaSuccess) pool->tmap_ok = make_tensor_map(pool);
+    // FP8: the 32 code rows of a tile in one box (its scales row follows them); bf16: the tile's 64 rows
+    if (e == cudaSuccess) pool->tmap_ok = make_tensor_map(pool, &pool->tmap, pool->fp8() ? 32u : 64u);
+    if (e == cudaSuccess && pool->fp8()) pool->tmap16_ok = make_tensor_map(pool, &pool->tmap16, 16u);
     if (e == cudaSuccess) e = cudaMemset(pool->base + lay.counters, 0, 256);
     if (e == cudaSuccess) e = cudaMemset(pool->base + lay.arrive, 0, static_cast<size_t>(kMaxPartials) * 4);
     if (e != cudaSuccess) {
@@ -784,7 +800,7 @@ int32_t kv_plan_decode(kv_pool_t* pool, int32_t batch, const int64_t* req_ids, i
 
 // Launch parameters common to the decode and the variable-q calls (plan staged in `s`).
 static AttnParams attn_params(kv_pool_t* pool, int32_t layer, const void* q, void* out, float sm_scale,
-                              const StageSlot& s) {
+                              const StageSlot& s, bool tc = false) {
   const kv_pool_config_t& c = pool->hs.cfg;
   const float scale = sm_scale > 0.f ? sm_scale : 1.0f / std::sqrt(static_cast<float>(c.head_dim));
   AttnParams p{};
@@ -808,6 +824,10 @@ static AttnParams attn_params(kv_pool_t* pool, int32_t layer, const void* q, voi
   if (pool->tma && pool->tmap_ok) {
     p.tma_row0 = static_cast<int64_t>(layer) * (layer_bytes / 128);
     std::memcpy(p.tmap, &pool->tmap, sizeof(CUtensorMap));
+  }
+  if (tc) {
+    p.tma_row0 = static_cast<int64_t>(layer) * (layer_bytes / 128);
+    std::memcpy(p.tmap, &pool->tmap16, sizeof(CUtensorMap));
   }
   p.n_units = p.n_items * c.num_kv_heads;
   return p;
@@ -892,7 +912,7 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer_begin, int32_t la
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_ATTN].begin(stream));
   for (int32_t ll = 0; ll < layer_count; ++ll) {
     AttnParams p = attn_params(pool, layer_begin + ll, static_cast<const char*>(q) + ll * q_stride,
-                               static_cast<char*>(out) + ll * q_stride, sm_scale, s);
+                               static_cast<char*>(out) + ll * q_stride, sm_scale, s, pool->tc_decode());
     if (k_new) {
       p.k_new = reinterpret_cast<const uint16_t*>(static_cast<const char*>(k_new) + ll * kv_stride);
       p.v_new = reinterpret_cast<const uint16_t*>(static_cast<const char*>(v_new) + ll * kv_stride);
@@ -973,7 +993,7 @@ int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
   if (!cached) {
     // a partial slot of this kernel is 8 columns wide; the workspace is sized in G-column slots
     const int32_t max_partials = static_cast<int32_t>(static_cast<int64_t>(kMaxPartials) * G / 8);
-    int32_t rc = pool->hs.plan_varq(batch, req_ids, q_lens, pool->slots(), pool->ips(), pool->min_chunk(),
+    int32_t rc = pool->hs.plan_varq(batch, req_ids, q_lens, pool->slots(true), pool->ips(), pool->min_chunk(),
                                     max_partials, &pool->plan, &pool->plan_tiles);
     pool->plan_slot = -1;   // pool->plan no longer matches what is staged
     if (rc != KV_OK) return rc;
@@ -1193,6 +1213,12 @@ int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
   if (!std::strcmp(key, "fuse_combine") && (value == 0 || value == 1)) { pool->fuse_combine = value != 0; return KV_OK; }
   if (!std::strcmp(key, "pdl") && (value == 0 || value == 1)) { pool->pdl = value != 0; return KV_OK; }
   if (!std::strcmp(key, "side_upload") && (value == 0 || value == 1)) { pool->side_upload = value != 0; return KV_OK; }
+  if (!std::strcmp(key, "tc") && (value == 0 || value == 1)) {   // FP8, head_dim 128 pools with a device slab only
+    if (value == 1 && !pool->tmap16_ok) return KV_ERR_UNSUPPORTED;
+    pool->tc = value != 0;
+    pool->plan_slot = -1;                                         // the planner sizes chunks for the kernel that runs
+    return KV_OK;
+  }
   if (!std::strcmp(key, "tma") && (value == 0 || value == 1)) {   // bf16, head_dim 128 pools with a device slab only
     if (value == 1 && !pool->tmap_ok) return KV_ERR_UNSUPPORTED;
     pool->tma = value != 0;
