@@ -288,21 +288,28 @@ struct Fp8Tiles {
   }
 
   // a3 inside a4: quantise the new token's K and V rows exactly as ingest_fp8_kernel does (same fp32 roundings, same
-  // codes) and write codes and scales into the pool tile: lanes [0, D/8) hold the K pieces, [D/8, D/4) the V pieces
-  static __device__ __forceinline__ void append_row(unsigned char* tile, int r_new, const uint16_t* knew_row,
-                                                    const uint16_t* vnew_row, int lane, NewRow& nr) {
+  // codes) and write codes and scales into the pool tile: lanes [0, D/8) hold the K pieces, [D/8, D/4) the V pieces.
+  // Two halves, so that a caller may issue the load early: append_load (the lane's 16-byte piece of the new rows) and
+  // append_store (quantise + store).
+  static __device__ __forceinline__ uint4 append_load(const uint16_t* knew_row, const uint16_t* vnew_row, int lane) {
+    constexpr int kP = D / 8;
+    return ldg_stream_pred((lane / kP ? vnew_row : knew_row) + (lane % kP) * 8, lane < 2 * kP);
+  }
+  static __device__ __forceinline__ void append_store(unsigned char* tile, int r_new, const uint4& x, int lane, NewRow& nr) {
     constexpr int kP = D / 8;
     const int cc = lane / kP, cp = lane % kP;
-    const bool on = lane < 2 * kP;
-    const uint4 x = ldg_stream_pred((cc ? vnew_row : knew_row) + cp * 8, on);
     uint32_t mx = amax_bits8(x);
 #pragma unroll
     for (int off = kP / 2; off > 0; off >>= 1) mx = max(mx, __shfl_xor_sync(kFull, mx, off));
     nr.codes = quantise_piece(x, mx, &nr.scale);
-    if (on) {
+    if (lane < 2 * kP) {
       *reinterpret_cast<uint2*>(tile + cc * (kBlockSize * D) + r_new * D + cp * 8) = nr.codes;
       if (cp == 0) *reinterpret_cast<float*>(tile + 2 * kBlockSize * D + r_new * 8 + cc * 4) = nr.scale;
     }
+  }
+  static __device__ __forceinline__ void append_row(unsigned char* tile, int r_new, const uint16_t* knew_row,
+                                                    const uint16_t* vnew_row, int lane, NewRow& nr) {
+    append_store(tile, r_new, append_load(knew_row, vnew_row, lane), lane, nr);
   }
   // ... and, once the tile's stale bytes have landed in the slot, the same row goes on top of them
   static __device__ __forceinline__ void patch_slot(uint32_t slot_addr, uint32_t sc_addr, int r_new, int lane, const NewRow& nr) {

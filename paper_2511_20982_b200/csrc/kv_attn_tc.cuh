@@ -21,8 +21,8 @@
 //     EXACTLY into four e5m2 terms by masking its top byte three times (f16 and e5m2 share sign and exponent, and
 //     x - (x & 0xff00) is exact), written as bytes P^T[term][head][token] into the K-major B operand of GEMM2; the
 //     four column groups of O^T are summed after the TMEM load.  Numerics are those of the mma.sync kernel.
-//   * m_ref is a LAZY reference: it moves only when some score of a tile exceeds it by more than 2^8 (p' <= 256 fits
-//     f16 and e5m2 with room), so the rescale of O^T in TMEM (tcgen05.ld / st) runs a handful of times per unit.
+//   * m_ref is a LAZY reference: it moves only when some score of a tile exceeds it by more than 2^8 (p' <= 256; times the
+//     bias 2^7 below, 2^15 fits f16 and e5m2), so the rescale of O^T in TMEM (tcgen05.ld / st) runs a handful of times per unit.
 //
 // Roles (192 threads, 2 CTAs per SM, 112 KiB of shared memory each):
 //   warps 0-3  softmax + epilogue: thread i owns token i of a tile (TMEM lane i of S^T) and column d = i of O^T
@@ -48,6 +48,11 @@ constexpr uint32_t kTcMiscOff = kTcStages * kTcStageBytes + 2 * kTcQBytes + 2 * 
 constexpr uint32_t kTcSmemBytes = kTcMiscOff + 1024;                              // 114688 = 112 KiB
 constexpr uint32_t kTcTmemCols = 128;       // S^T: 2 x 16 columns, O^T: 2 x 32 columns
 constexpr float kTcLazyLog2 = 8.f;          // m_ref moves when a score exceeds it by more than this (log2 units)
+// The weights are fed as 2^(s - m_ref + kTcWeightBias): the four e5m2 terms of a weight bottom out at e5m2's smallest
+// subnormal, 2^-16, whereas the f16 they split has 2^-24 — so the weights sit as high as the formats allow (<= 2^15 with the
+// lazy reference, below e5m2's 57344 and f16's 65504) and keep all 11 bits down to 2^-13 of the reference.  O and l
+// carry the same factor; it cancels in O / l and in the merge of partials.
+constexpr float kTcWeightBias = 7.f;
 
 // ---- tcgen05 / TMEM wrappers ---------------------------------------------------------------------------------
 __device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
@@ -194,126 +199,190 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
 
   if (warp == 4) {
     // ===================================== producer =====================================
+    // A unit costs a chain of dependent global loads before its first tile can be asked for (claim -> work item ->
+    // block ids; q and the new rows hang off the work item).  With two CTAs per SM there are no other warps to hide
+    // that chain behind, so it is software-pipelined: while the last three tiles of unit u are being issued the warp
+    // claims unit u + 1, fetches its work item, then its block ids, its q rows and its new K / V row — one link per
+    // tile, each link's loads in flight while the warp waits for a free stage anyway.  At the unit switch the first
+    // tile goes out before anything else; Q8 is staged and the new row appended while it is in flight.
     bool waited = !p.chained;
     if (waited) pdl_wait();
     unsigned char* const kv = reinterpret_cast<unsigned char*>(p.kv_layer);
     const int64_t blk_stride = static_cast<int64_t>(p.num_kv_heads) * TP::kPoolTileBytes;
+    const int32_t row_blk = 33 * p.num_kv_heads;
+    const int b = lane & (kTcTileBlocks - 1);
+    const int qhead = lane >> 2, quarter = lane & 3;                 // Q8 staging: head of the group, 32 d columns
+    const bool qok = qhead < G;
     uint32_t g_tile = 0, u_seq = 0;
-    for (int unit = blockIdx.x;; ++u_seq) {
+
+    // what is known of a unit before it starts
+    struct Desc { int32_t unit; int4 w0, w1; int32_t ids; uint4 q[4]; uint4 nrow; };
+    auto fetch_item = [&](Desc& d) {                                 // link 2: the work item
+      if (d.unit < p.n_units) {
+        const int4* wi = reinterpret_cast<const int4*>(p.items) + (d.unit / p.num_kv_heads) * 2;
+        d.w0 = __ldg(wi);
+        d.w1 = __ldg(wi + 1);
+      }
+    };
+    auto fetch_rows = [&](Desc& d, bool with_inputs) {               // link 3: block ids (+ q rows, new K / V row)
+      if (d.unit >= p.n_units) return;
+      const int h = d.unit % p.num_kv_heads;
+      const int batch_idx = d.w0.x, slot = d.w0.y, blk_begin = d.w0.z, n_blocks = d.w0.w;
+      const int32_t* bt = p.block_table + static_cast<int64_t>(slot) * p.bt_stride + blk_begin;
+      d.ids = lane < n_blocks ? __ldg(bt + lane) : 0;                // physical ids of blocks [0, 32) of the chunk
+      if (with_inputs) {
+        const uint16_t* qrow = p.q + (static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G + (qok ? qhead : 0)) * D + quarter * 32;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) d.q[k] = ldg_stream_pred(qrow + k * 8, qok);
+        if constexpr (kAppend) {
+          const int n_chunks = static_cast<int>(static_cast<uint32_t>(d.w1.z) >> 16), chunk_idx = d.w1.z & 0xffff;
+          if (chunk_idx == n_chunks - 1) {
+            const int64_t new_row = (static_cast<int64_t>(batch_idx) * p.num_kv_heads + h) * D;
+            d.nrow = TP::append_load(p.k_new + new_row, p.v_new + new_row, lane);
+          }
+        }
+      }
+    };
+
+    Desc cur{};
+    cur.unit = blockIdx.x;
+    fetch_item(cur);
+    fetch_rows(cur, waited);                                         // q, k_new, v_new only after griddepcontrol.wait
+    if (!waited) {
+      pdl_wait();
+      waited = true;
+      if (cur.unit < p.n_units) {                                    // (the block ids are re-read: harmless)
+        fetch_rows(cur, true);
+      }
+    }
+
+    for (;; ++u_seq) {
       const int e = u_seq & 1;
-      mbar_wait(b_u_empty + 8 * e, ((u_seq >> 1) & 1u) ^ 1u);
       TcUnit* const U = units + e;
-      if (unit >= p.n_units) {
+      if (cur.unit >= p.n_units) {
+        mbar_wait(b_u_empty + 8 * e, ((u_seq >> 1) & 1u) ^ 1u);
         if (lane == 0) {
           U->n_tiles = 0;
           mbar_arrive(b_u_full + 8 * e);
         }
         break;
       }
-      const int h = unit % p.num_kv_heads;
-      const int4* wi = reinterpret_cast<const int4*>(p.items) + (unit / p.num_kv_heads) * 2;
-      const int4 w0 = __ldg(wi);
-      const int4 w1 = __ldg(wi + 1);
-      const int batch_idx = w0.x, slot = w0.y, blk_begin = w0.z, n_blocks = w0.w;
-      const int n_tokens = w1.x;
-      const int n_chunks = static_cast<int>(static_cast<uint32_t>(w1.z) >> 16), chunk_idx = w1.z & 0xffff, last_blk = w1.w;
-      const int pbase = w1.y < 0 ? -1 : w1.y + h * n_chunks;
+      const int h = cur.unit % p.num_kv_heads;
+      const int batch_idx = cur.w0.x, slot = cur.w0.y, blk_begin = cur.w0.z, n_blocks = cur.w0.w;
+      const int n_tokens = cur.w1.x;
+      const int n_chunks = static_cast<int>(static_cast<uint32_t>(cur.w1.z) >> 16), chunk_idx = cur.w1.z & 0xffff, last_blk = cur.w1.w;
+      const int pbase = cur.w1.y < 0 ? -1 : cur.w1.y + h * n_chunks;
       const int n_tiles = (n_blocks + kTcTileBlocks - 1) / kTcTileBlocks;
+      const bool owns_last = chunk_idx == n_chunks - 1;
       const int32_t* bt = p.block_table + static_cast<int64_t>(slot) * p.bt_stride + blk_begin;
-      int32_t ids = lane < n_blocks ? __ldg(bt + lane) : 0;     // physical ids of blocks [32k, 32k+32)
-      int32_t ids_next = 0;
-      if (!waited) { pdl_wait(); waited = true; }
-
-      // ---- Q8: head = lane / 4 of the group, this lane's 32 d columns; two e4m3 terms, rows term * 8 + head ----
-      {
-        const int head = lane >> 2, quarter = lane & 3;
-        const bool ok = head < G;
-        const uint16_t* qrow = p.q + (static_cast<int64_t>(batch_idx) * p.num_q_heads + h * G + (ok ? head : 0)) * D + quarter * 32;
-        uint4 raw[4];
-        uint32_t mx = 0;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          raw[k] = ldg_stream_pred(qrow + k * 8, ok);
-          mx = max(mx, amax_bits8(raw[k]));
-        }
-        mx = max(mx, __shfl_xor_sync(kFull, mx, 1));
-        mx = max(mx, __shfl_xor_sync(kFull, mx, 2));
-        const uint32_t eb = min(max(mx >> 7, 8u), 253u);          // biased exponent of the row maximum
-        const float sf = __uint_as_float((261u - eb) << 23);       // 2^(134 - eb): row maximum -> [128, 256)
-        if (quarter == 0) U->qs[head] = ok ? __uint_as_float((eb - 7u) << 23) * p.scale_log2 : 0.f;
-        uint32_t t1[8], t2[8];                                     // 32 codes per term = 8 words
-#pragma unroll
-        for (int k = 0; k < 4; ++k)
-#pragma unroll
-          for (int w = 0; w < 4; w += 2) {
-            uint32_t c1[2], c2[2];
-#pragma unroll
-            for (int ww = 0; ww < 2; ++ww) {
-              const uint32_t e2 = u4_get(raw[k], w + ww);
-              const float x0 = __uint_as_float(e2 << 16) * sf, x1 = __uint_as_float(e2 & 0xffff0000u) * sf;
-              c1[ww] = f32x2_to_e4m3x2(x0, x1);
-              const uint32_t hb = e4m3x2_lo_to_f16x2(c1[ww]);       // what the first term holds, exactly
-              const float2 back = __half22float2(*reinterpret_cast<const __half2*>(&hb));
-              c2[ww] = f32x2_to_e4m3x2(x0 - back.x, x1 - back.y);
-            }
-            t1[2 * k + w / 2] = c1[0] | (c1[1] << 16);
-            t2[2 * k + w / 2] = c2[0] | (c2[1] << 16);
-          }
-        const uint32_t qb = q_smem + e * kTcQBytes;
-#pragma unroll
-        for (int half = 0; half < 2; ++half) {
-          const int chunk = quarter * 2 + half;
-          sts128(qb + head * 128 + ((chunk ^ head) << 4), make_uint4(t1[4 * half], t1[4 * half + 1], t1[4 * half + 2], t1[4 * half + 3]));
-          sts128(qb + (8 + head) * 128 + ((chunk ^ head) << 4), make_uint4(t2[4 * half], t2[4 * half + 1], t2[4 * half + 2], t2[4 * half + 3]));
-        }
-      }
-      // ---- a3 inside a4: the unit that owns the request's last block quantises the new row into the pool; the tile
-      //      is fetched afterwards, so the TMA copy below already sees it ----
-      if constexpr (kAppend) {
-        if (chunk_idx == n_chunks - 1) {
-          const int64_t new_row = (static_cast<int64_t>(batch_idx) * p.num_kv_heads + h) * D;
-          unsigned char* const last_tile = kv + static_cast<int64_t>(h) * TP::kPoolTileBytes + last_blk * blk_stride;
-          typename TP::NewRow nr;
-          TP::append_row(last_tile, n_tokens - (n_blocks - 1) * kBlockSize - 1, p.k_new + new_row, p.v_new + new_row, lane, nr);
-          if (h == 0 && lane == 0) p.block_table[static_cast<int64_t>(slot) * p.bt_stride + blk_begin + n_blocks - 1] = last_blk;
-          __threadfence();
-          asm volatile("fence.proxy.async;" ::: "memory");         // generic-proxy global writes before async-proxy (TMA) reads
-        }
-      }
-      fence_proxy_async();                                          // Q8 in shared memory -> visible to the tensor core
-      __syncwarp();
-      if (lane == 0) {
-        U->n_tiles = n_tiles; U->n_tokens = n_tokens; U->batch_idx = batch_idx; U->h = h;
-        U->pidx = w1.y < 0 ? -1 : pbase + chunk_idx; U->pbase = pbase; U->n_chunks = n_chunks;
-        mbar_arrive(b_u_full + 8 * e);
-      }
-      // ---- tiles: lane b < 8 owns block b of the tile (its id, its three copies); the warp issues them one lane
-      //      after the other, but every address is computed by all lanes at once ----
-      const int32_t row_h = static_cast<int32_t>(p.tma_row0) + h * 33, row_blk = 33 * p.num_kv_heads;
+      int32_t ids = cur.ids, ids_next = 0;
+      const int32_t row_h = static_cast<int32_t>(p.tma_row0) + h * 33;
       const unsigned char* const sc_h = kv + static_cast<int64_t>(h) * TP::kPoolTileBytes + 4096;
-      const int b = lane & (kTcTileBlocks - 1);
+      bool append_pending = kAppend && owns_last;
+
+      Desc nxt{};
+      nxt.unit = p.n_units;
+      int link = 0;                                                  // links of the next unit's chain already started
       for (int t = 0; t < n_tiles; ++t, ++g_tile) {
-        const uint32_t s = g_tile % kTcStages;
-        const int blk0 = t * kTcTileBlocks;
-        if ((blk0 & 31) == 0 && blk0 > 0) ids = ids_next;
-        if ((blk0 & 31) == 8 && blk0 + 24 + lane < n_blocks) ids_next = __ldg(bt + blk0 + 24 + lane);
-        const int32_t id = __shfl_sync(kFull, ids, (blk0 + b) & 31);
-        const int nb = min(kTcTileBlocks, n_blocks - blk0);
-        const uint32_t st = smem0 + s * kTcStageBytes, bar = b_full + 8 * s;
-        mbar_wait(b_empty + 8 * s, ((g_tile / kTcStages) & 1u) ^ 1u);
-        if (lane == 0) mbar_arrive_expect_tx(bar, static_cast<uint32_t>(nb) * static_cast<uint32_t>(TP::kPoolTileBytes));
-        __syncwarp();
-        if (lane < nb) {
-          const int32_t row = row_h + id * row_blk;
-          tma_load_2d(st + b * 2048, p.tmap, bar, 0, row);
-          tma_load_2d(st + 16384 + b * 2048, p.tmap, bar, 0, row + 16);
-          bulk_load_1d(st + 32768 + b * 128, sc_h + id * blk_stride, 128, bar);
+        const int left = n_tiles - t;                                // tiles of this unit not yet issued
+        if (left <= 3 && link == 0) {                                // link 1: claim
+          int32_t c = 0;
+          if (lane == 0) c = gridDim.x + atomicAdd(&p.counters[0], 1);
+          nxt.unit = c;
+          link = 1;
+        }
+        if (left <= 2 && link == 1) {
+          nxt.unit = __shfl_sync(kFull, nxt.unit, 0);
+          fetch_item(nxt);
+          link = 2;
+        }
+        if (left <= 1 && link == 2) {
+          fetch_rows(nxt, true);
+          link = 3;
+        }
+        // a3 inside a4: the unit that owns the request's last block quantises the new row into the pool before the
+        // tile holding that block (the unit's last tile) is asked for, so the TMA copy already sees it
+        if constexpr (kAppend) {
+          if (append_pending && t == n_tiles - 1) {
+            unsigned char* const last_tile = kv + static_cast<int64_t>(h) * TP::kPoolTileBytes + last_blk * blk_stride;
+            typename TP::NewRow nr;
+            TP::append_store(last_tile, n_tokens - (n_blocks - 1) * kBlockSize - 1, cur.nrow, lane, nr);
+            if (h == 0 && lane == 0) p.block_table[static_cast<int64_t>(slot) * p.bt_stride + blk_begin + n_blocks - 1] = last_blk;
+            __threadfence();
+            asm volatile("fence.proxy.async;" ::: "memory");         // generic-proxy global writes before async-proxy (TMA) reads
+            __syncwarp();
+            append_pending = false;
+          }
+        }
+        // ---- tile t: lane b < 8 owns block b of the tile (its id, its three copies) ----
+        {
+          const uint32_t s = g_tile % kTcStages;
+          const int blk0 = t * kTcTileBlocks;
+          if ((blk0 & 31) == 0 && blk0 > 0) ids = ids_next;
+          if ((blk0 & 31) == 8 && blk0 + 24 + lane < n_blocks) ids_next = __ldg(bt + blk0 + 24 + lane);
+          int32_t id = __shfl_sync(kFull, ids, (blk0 + b) & 31);
+          // the request's last block may have been opened by this very step (a1 on the host): the device block table
+          // does not hold it before layer 0's append has run, the work item does
+          if (owns_last && blk0 + b == n_blocks - 1) id = last_blk;
+          const int nb = min(kTcTileBlocks, n_blocks - blk0);
+          const uint32_t st = smem0 + s * kTcStageBytes, bar = b_full + 8 * s;
+          mbar_wait(b_empty + 8 * s, ((g_tile / kTcStages) & 1u) ^ 1u);
+          if (lane == 0) mbar_arrive_expect_tx(bar, static_cast<uint32_t>(nb) * static_cast<uint32_t>(TP::kPoolTileBytes));
+          __syncwarp();
+          if (lane < nb) {
+            const int32_t row = row_h + id * row_blk;
+            tma_load_2d(st + b * 2048, p.tmap, bar, 0, row);
+            tma_load_2d(st + 16384 + b * 2048, p.tmap, bar, 0, row + 16);
+            bulk_load_1d(st + 32768 + b * 128, sc_h + id * blk_stride, 128, bar);
+          }
+        }
+        if (t == 0) {
+          // ---- Q8 (while tile 0 is in flight): two e4m3 terms of this lane's 32 d columns, rows term * 8 + head ----
+          mbar_wait(b_u_empty + 8 * e, ((u_seq >> 1) & 1u) ^ 1u);
+          uint32_t mx = 0;
+#pragma unroll
+          for (int k = 0; k < 4; ++k) mx = max(mx, amax_bits8(cur.q[k]));
+          mx = max(mx, __shfl_xor_sync(kFull, mx, 1));
+          mx = max(mx, __shfl_xor_sync(kFull, mx, 2));
+          const uint32_t eb = min(max(mx >> 7, 8u), 253u);          // biased exponent of the row maximum
+          const float sf = __uint_as_float((261u - eb) << 23);       // 2^(134 - eb): row maximum -> [128, 256)
+          if (quarter == 0) U->qs[qhead] = qok ? __uint_as_float((eb - 7u) << 23) * p.scale_log2 : 0.f;
+          uint32_t t1[8], t2[8];                                     // 32 codes per term = 8 words
+#pragma unroll
+          for (int k = 0; k < 4; ++k)
+#pragma unroll
+            for (int w = 0; w < 4; w += 2) {
+              uint32_t c1[2], c2[2];
+#pragma unroll
+              for (int ww = 0; ww < 2; ++ww) {
+                const uint32_t e2 = u4_get(cur.q[k], w + ww);
+                const float x0 = __uint_as_float(e2 << 16) * sf, x1 = __uint_as_float(e2 & 0xffff0000u) * sf;
+                c1[ww] = f32x2_to_e4m3x2(x0, x1);
+                const uint32_t hb = e4m3x2_lo_to_f16x2(c1[ww]);     // what the first term holds, exactly
+                const float2 back = __half22float2(*reinterpret_cast<const __half2*>(&hb));
+                c2[ww] = f32x2_to_e4m3x2(x0 - back.x, x1 - back.y);
+              }
+              t1[2 * k + w / 2] = c1[0] | (c1[1] << 16);
+              t2[2 * k + w / 2] = c2[0] | (c2[1] << 16);
+            }
+          const uint32_t qb = q_smem + e * kTcQBytes;
+#pragma unroll
+          for (int half = 0; half < 2; ++half) {
+            const int chunk = quarter * 2 + half;
+            sts128(qb + qhead * 128 + ((chunk ^ qhead) << 4), make_uint4(t1[4 * half], t1[4 * half + 1], t1[4 * half + 2], t1[4 * half + 3]));
+            sts128(qb + (8 + qhead) * 128 + ((chunk ^ qhead) << 4), make_uint4(t2[4 * half], t2[4 * half + 1], t2[4 * half + 2], t2[4 * half + 3]));
+          }
+          fence_proxy_async();                                        // Q8 in shared memory -> visible to the tensor core
+          __syncwarp();
+          if (lane == 0) {
+            U->n_tiles = n_tiles; U->n_tokens = n_tokens; U->batch_idx = batch_idx; U->h = h;
+            U->pidx = cur.w1.y < 0 ? -1 : pbase + chunk_idx; U->pbase = pbase; U->n_chunks = n_chunks;
+            mbar_arrive(b_u_full + 8 * e);
+          }
         }
       }
-      if (lane == 0) unit = gridDim.x + atomicAdd(&p.counters[0], 1);
-      unit = __shfl_sync(kFull, unit, 0);
+      cur = nxt;
     }
-    if (!waited) pdl_wait();
   } else if (warp == 5) {
     // ===================================== MMA issuer: one thread =====================================
     if (lane == 0) {
@@ -467,7 +536,7 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
         const uint32_t pbuf = p_smem + pb * kTcPBytes;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-          const float p0 = fast_exp2(sc[2 * j] - m_ref[2 * j]), p1 = fast_exp2(sc[2 * j + 1] - m_ref[2 * j + 1]);
+          const float p0 = fast_exp2(sc[2 * j] - m_ref[2 * j] + kTcWeightBias), p1 = fast_exp2(sc[2 * j + 1] - m_ref[2 * j + 1] + kTcWeightBias);
           l[2 * j] += p0 * iv;
           l[2 * j + 1] += p1 * iv;
           uint32_t x = pack_f16x2(p0, p1);

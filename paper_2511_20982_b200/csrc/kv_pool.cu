@@ -375,6 +375,7 @@ int32_t run_copy(kv_pool* pool, CopyKind kind, const kv_pool* src_pool, const in
                  const int32_t* start_pos, int32_t layer_begin, int32_t layer_count, cudaStream_t stream) {
   const kv_pool_config_t& c = pool->hs.cfg;
   // blocks per unit: the quantising scatter gives a warp a run of consecutive blocks, the plain copies one block
+  // (a run of two FP8 tiles per warp in the transfer was measured: 0.951 -> 0.928 of the copy ceiling, not kept)
   const int32_t run = (kind == CopyKind::kScatter && pool->fp8()) ? kIngest8Run : 1;
   std::vector<IngestReq> reqs;
   std::vector<int32_t> ids;

@@ -32,14 +32,14 @@ def make_pool(w: W.Workload, num_blocks, max_requests=None, alloc_seed=1, sentin
 
 
 def apply_options(pool, opts):
-    """set_option for every (key, value); a pool that cannot run the TMA variant (head_dim 64) skips that mode."""
+    """set_option for every (key, value); a pool that cannot run the TMA / tcgen05 variants (head_dim 64) skips that mode."""
     import pytest
     for k_, v_ in (opts or {}).items():
         try:
             pool.set_option(k_, v_)
         except kv.KVError as e:
-            if k_ == "tma" and e.status == kv.binding.KV_ERR_UNSUPPORTED:
-                pytest.skip("tma=1 needs head_dim 128")
+            if k_ in ("tma", "tc") and e.status == kv.binding.KV_ERR_UNSUPPORTED:
+                pytest.skip(f"{k_}=1 needs head_dim 128")
             raise
 
 

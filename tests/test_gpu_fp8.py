@@ -21,7 +21,10 @@ pytestmark = pytest.mark.gpu
 MODES = [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=1024),
          dict(min_chunk_blocks=2, items_per_slot=2, fuse_combine=0), dict(min_chunk_blocks=5, items_per_slot=1, ctas_per_sm=1),
          dict(pdl=0), dict(pdl=0, min_chunk_blocks=2, items_per_slot=1024),
-         dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024), dict(tma=1, min_chunk_blocks=3, items_per_slot=2, fuse_combine=0)]
+         dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024), dict(tma=1, min_chunk_blocks=3, items_per_slot=2, fuse_combine=0),
+         # tc=1: attn_tc_kernel (tcgen05 / TMEM / TMA, 128-token tiles): single tile, many tiles per unit, one block per chunk
+         dict(tc=1), dict(tc=1, min_chunk_blocks=1, items_per_slot=1024), dict(tc=1, min_chunk_blocks=9, items_per_slot=1024),
+         dict(tc=1, min_chunk_blocks=3, items_per_slot=2, fuse_combine=0), dict(tc=1, pdl=0, min_chunk_blocks=17, items_per_slot=1)]
 SENT = 0xFF   # e4m3 NaN code / NaN scale bytes: an unmasked read poisons the output
 
 
@@ -107,7 +110,8 @@ def test_attention_matches_oracle(Hq, Hkv, d, opts):
     assert np.abs(want - exact).max() < 0.15 and np.abs(want - exact).mean() < 0.01
 
 
-@pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=2, items_per_slot=1024), dict(tma=1)])
+@pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=2, items_per_slot=1024), dict(tma=1), dict(tc=1),
+                                  dict(tc=1, min_chunk_blocks=2, items_per_slot=1024)])
 def test_attention_wide_dynamic_range(opts):
     """Row magnitudes from e^-6 to e^6 in K and V, scaled-up queries, a zero row and an outlier element."""
     rng = np.random.default_rng(8)
@@ -186,7 +190,8 @@ def test_gather_fp8_returns_stored_codes_and_scales(Hkv, d):
 
 
 @pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=2),
-                                  dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024)])
+                                  dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024),
+                                  dict(tc=1), dict(tc=1, min_chunk_blocks=1, items_per_slot=1024), dict(tc=1, min_chunk_blocks=9, items_per_slot=2)])
 @pytest.mark.parametrize("Hq,Hkv,d", [(32, 8, 128), (8, 2, 64), (32, 32, 128)])
 def test_fused_decode_step_quantises_like_ingest(Hq, Hkv, d, opts):
     """paged_decode_step on an FP8 pool: the appended row's codes and scales are the bytes kv_ingest would have
