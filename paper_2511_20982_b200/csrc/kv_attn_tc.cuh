@@ -24,11 +24,15 @@
 //   * m_ref is a LAZY reference: it moves only when some score of a tile exceeds it by more than 2^8 (p' <= 256; times the
 //     bias 2^7 below, 2^15 fits f16 and e5m2), so the rescale of O^T in TMEM (tcgen05.ld / st) runs a handful of times per unit.
 //
-// Roles (192 threads, 2 CTAs per SM, 112 KiB of shared memory each):
+// Roles (256 threads, 2 CTAs per SM, 112.5 KiB of shared memory each):
 //   warps 0-3  softmax + epilogue: thread i owns token i of a tile (TMEM lane i of S^T) and column d = i of O^T
-//   warp 4     producer: claims units, stages Q8, appends the new row (a3), issues the TMA copies of a 3-stage tile
-//              ring — and keeps running ahead ACROSS unit boundaries (it owns no registers worth mentioning)
+//   warp 4     lead producer: claims units, stages Q8, appends the new row (a3), publishes each unit's descriptor to
+//              the two helper warps, issues the scale copies of the 3-stage tile ring
 //   warp 5     MMA issuer (one lane) + TMEM allocation
+//   warp 6, 7  helper producers: the K-code and the V-code copies of every tile.  A tile is 24 bulk copies (8 blocks x
+//              {K codes, V codes, scales}) and ONE warp issues a copy every ~45 ns: 1.1 us per tile, at which point the
+//              producer, not HBM, paces the CTA (profiles/README.md r02) — so the issue is spread over three warps.
+//   The producers run ahead ACROSS unit boundaries (they own no registers worth mentioning).
 // All hand-offs are mbarriers; the only block-wide barrier is at start-up and tear-down.
 #pragma once
 
@@ -38,14 +42,14 @@
 
 namespace kvp {
 
-constexpr int kTcThreads = 192;
+constexpr int kTcThreads = 256;
 constexpr int kTcSoftmaxThreads = 128;
 constexpr int kTcStages = 3;
 constexpr int kTcTileBlocks = 8, kTcTileTokens = kTcTileBlocks * kBlockSize;
 constexpr uint32_t kTcStageBytes = 2 * kTcTileTokens * 128 + kTcTileTokens * 8;   // 33792 = 33 KiB
 constexpr uint32_t kTcQBytes = 16 * 128, kTcPBytes = 32 * 128;
 constexpr uint32_t kTcMiscOff = kTcStages * kTcStageBytes + 2 * kTcQBytes + 2 * kTcPBytes;
-constexpr uint32_t kTcSmemBytes = kTcMiscOff + 1024;                              // 114688 = 112 KiB
+constexpr uint32_t kTcSmemBytes = kTcMiscOff + 1536;                              // 115200 = 112.5 KiB
 constexpr uint32_t kTcTmemCols = 128;       // S^T: 2 x 16 columns, O^T: 2 x 32 columns
 constexpr float kTcLazyLog2 = 8.f;          // m_ref moves when a score exceeds it by more than this (log2 units)
 // The weights are fed as 2^(s - m_ref + kTcWeightBias): the four e5m2 terms of a weight bottom out at e5m2's smallest
@@ -155,6 +159,18 @@ struct TcUnit {            // what the producer hands to the MMA and softmax war
 };
 static_assert(sizeof(TcUnit) == 64, "TcUnit");
 
+struct TcDesc {            // what the lead producer hands to the helper producers for one unit (shared memory, 160 bytes)
+  int32_t n_blocks;        // 0: no more work
+  int32_t row_h;           // first 128-byte row of (layer, block 0, this kv head) in the tensor map
+  int32_t slot, blk_begin; // where the chunk's block ids continue in the device block table
+  int32_t owns_last;       // the chunk ends with the request's last block ...
+  int32_t last_blk;        // ... whose physical id is this (the device block table may not hold it yet)
+  int32_t append;          // the lead appends the new row to that block: wait for it before the unit's last tile
+  int32_t pad;
+  int32_t ids[32];         // physical ids of the chunk's first 32 blocks
+};
+static_assert(sizeof(TcDesc) == 160, "TcDesc");
+
 template <bool kAppend>
 __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_constant__ AttnParams p) {
   extern __shared__ __align__(1024) unsigned char tc_smem[];
@@ -167,21 +183,26 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
   const uint32_t misc = smem0 + kTcMiscOff;
   // mbarriers
   const uint32_t b_full = misc, b_empty = misc + 24, b_d1_full = misc + 48, b_d1_empty = misc + 64, b_p_full = misc + 80,
-                 b_p_free = misc + 96, b_o_full = misc + 112, b_o_empty = misc + 128, b_u_full = misc + 144, b_u_empty = misc + 160;
+                 b_p_free = misc + 96, b_o_full = misc + 112, b_o_empty = misc + 128, b_u_full = misc + 144, b_u_empty = misc + 160,
+                 b_dsc_full = misc + 192, b_dsc_empty = misc + 208;
   const uint32_t tmem_slot = misc + 176, merge_flag = misc + 180;
-  TcUnit* const units = reinterpret_cast<TcUnit*>(tc_smem + kTcMiscOff + 192);
-  const uint32_t flags_smem = misc + 320;   // [2][4] int
-  const uint32_t wmax_smem = misc + 352;    // [2][4][8] float
-  const uint32_t lsum_smem = misc + 608;    // [4][8] float
+  const uint32_t app_ctr = misc + 184;      // appends completed by the lead producer (monotonic; polled by the helpers)
+  TcUnit* const units = reinterpret_cast<TcUnit*>(tc_smem + kTcMiscOff + 256);
+  const uint32_t flags_smem = misc + 384;   // [2][4] int
+  const uint32_t wmax_smem = misc + 416;    // [2][4][8] float
+  const uint32_t lsum_smem = misc + 672;    // [4][8] float
+  const uint32_t desc_smem = misc + 800;    // [2] TcDesc
 
   if (threadIdx.x == 0) {
     if (smem0 & 1023u) __trap();            // the 128-byte swizzle is a function of the shared-memory address
-    for (int s = 0; s < kTcStages; ++s) { mbar_init(b_full + 8 * s, 1); mbar_init(b_empty + 8 * s, 1); }
+    sts32(app_ctr, 0u);
+    for (int s = 0; s < kTcStages; ++s) { mbar_init(b_full + 8 * s, 3); mbar_init(b_empty + 8 * s, 1); }   // three issuing warps
     for (int i = 0; i < 2; ++i) {
       mbar_init(b_d1_full + 8 * i, 1); mbar_init(b_d1_empty + 8 * i, kTcSoftmaxThreads);
       mbar_init(b_p_full + 8 * i, kTcSoftmaxThreads); mbar_init(b_p_free + 8 * i, 1);
       mbar_init(b_o_full + 8 * i, 1); mbar_init(b_o_empty + 8 * i, kTcSoftmaxThreads);
       mbar_init(b_u_full + 8 * i, 1); mbar_init(b_u_empty + 8 * i, kTcSoftmaxThreads);
+      mbar_init(b_dsc_full + 8 * i, 1); mbar_init(b_dsc_empty + 8 * i, 2);
     }
     mbar_init_fence();
   }
@@ -209,11 +230,10 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
     if (waited) pdl_wait();
     unsigned char* const kv = reinterpret_cast<unsigned char*>(p.kv_layer);
     const int64_t blk_stride = static_cast<int64_t>(p.num_kv_heads) * TP::kPoolTileBytes;
-    const int32_t row_blk = 33 * p.num_kv_heads;
     const int b = lane & (kTcTileBlocks - 1);
     const int qhead = lane >> 2, quarter = lane & 3;                 // Q8 staging: head of the group, 32 d columns
     const bool qok = qhead < G;
-    uint32_t g_tile = 0, u_seq = 0;
+    uint32_t g_tile = 0, u_seq = 0, n_appends = 0;
 
     // what is known of a unit before it starts
     struct Desc { int32_t unit; int4 w0, w1; int32_t ids; uint4 q[4]; uint4 nrow; };
@@ -259,11 +279,15 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
     for (;; ++u_seq) {
       const int e = u_seq & 1;
       TcUnit* const U = units + e;
+      TcDesc* const Dsc = reinterpret_cast<TcDesc*>(tc_smem + kTcMiscOff + 800) + e;
+      mbar_wait(b_dsc_empty + 8 * e, ((u_seq >> 1) & 1u) ^ 1u);       // both helpers have read the descriptor two units back
       if (cur.unit >= p.n_units) {
         mbar_wait(b_u_empty + 8 * e, ((u_seq >> 1) & 1u) ^ 1u);
         if (lane == 0) {
           U->n_tiles = 0;
+          Dsc->n_blocks = 0;
           mbar_arrive(b_u_full + 8 * e);
+          mbar_arrive(b_dsc_full + 8 * e);
         }
         break;
       }
@@ -276,9 +300,16 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
       const bool owns_last = chunk_idx == n_chunks - 1;
       const int32_t* bt = p.block_table + static_cast<int64_t>(slot) * p.bt_stride + blk_begin;
       int32_t ids = cur.ids, ids_next = 0;
-      const int32_t row_h = static_cast<int32_t>(p.tma_row0) + h * 33;
       const unsigned char* const sc_h = kv + static_cast<int64_t>(h) * TP::kPoolTileBytes + 4096;
       bool append_pending = kAppend && owns_last;
+      // ---- the unit's descriptor goes to the helper producers before anything else ----
+      Dsc->ids[lane] = ids;
+      if (lane == 0) {
+        Dsc->n_blocks = n_blocks; Dsc->row_h = static_cast<int32_t>(p.tma_row0) + h * 33; Dsc->slot = slot; Dsc->blk_begin = blk_begin;
+        Dsc->owns_last = owns_last ? 1 : 0; Dsc->last_blk = last_blk; Dsc->append = append_pending ? 1 : 0;
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(b_dsc_full + 8 * e);
 
       Desc nxt{};
       nxt.unit = p.n_units;
@@ -296,12 +327,9 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
           fetch_item(nxt);
           link = 2;
         }
-        if (left <= 1 && link == 2) {
-          fetch_rows(nxt, true);
-          link = 3;
-        }
         // a3 inside a4: the unit that owns the request's last block quantises the new row into the pool before the
-        // tile holding that block (the unit's last tile) is asked for, so the TMA copy already sees it
+        // tile holding that block (the unit's last tile) is asked for, so the TMA copies already see it
+        // (doing it right after tile 0 instead was measured: equal to slightly slower)
         if constexpr (kAppend) {
           if (append_pending && t == n_tiles - 1) {
             unsigned char* const last_tile = kv + static_cast<int64_t>(h) * TP::kPoolTileBytes + last_blk * blk_stride;
@@ -311,30 +339,25 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
             __threadfence();
             asm volatile("fence.proxy.async;" ::: "memory");         // generic-proxy global writes before async-proxy (TMA) reads
             __syncwarp();
+            if (lane == 0)                                              // the helpers may fetch the unit's last tile
+              asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(app_ctr), "r"(++n_appends) : "memory");
             append_pending = false;
           }
         }
-        // ---- tile t: lane b < 8 owns block b of the tile (its id, its three copies) ----
+        // ---- tile t, this warp's share: the scales of its (up to) 8 blocks, lane b < 8 owns block b ----
         {
           const uint32_t s = g_tile % kTcStages;
           const int blk0 = t * kTcTileBlocks;
           if ((blk0 & 31) == 0 && blk0 > 0) ids = ids_next;
           if ((blk0 & 31) == 8 && blk0 + 24 + lane < n_blocks) ids_next = __ldg(bt + blk0 + 24 + lane);
           int32_t id = __shfl_sync(kFull, ids, (blk0 + b) & 31);
-          // the request's last block may have been opened by this very step (a1 on the host): the device block table
-          // does not hold it before layer 0's append has run, the work item does
-          if (owns_last && blk0 + b == n_blocks - 1) id = last_blk;
+          if (owns_last && blk0 + b == n_blocks - 1) id = last_blk;   // see TcDesc::last_blk
           const int nb = min(kTcTileBlocks, n_blocks - blk0);
           const uint32_t st = smem0 + s * kTcStageBytes, bar = b_full + 8 * s;
           mbar_wait(b_empty + 8 * s, ((g_tile / kTcStages) & 1u) ^ 1u);
-          if (lane == 0) mbar_arrive_expect_tx(bar, static_cast<uint32_t>(nb) * static_cast<uint32_t>(TP::kPoolTileBytes));
+          if (lane == 0) mbar_arrive_expect_tx(bar, static_cast<uint32_t>(nb) * 128u);
           __syncwarp();
-          if (lane < nb) {
-            const int32_t row = row_h + id * row_blk;
-            tma_load_2d(st + b * 2048, p.tmap, bar, 0, row);
-            tma_load_2d(st + 16384 + b * 2048, p.tmap, bar, 0, row + 16);
-            bulk_load_1d(st + 32768 + b * 128, sc_h + id * blk_stride, 128, bar);
-          }
+          if (lane < nb) bulk_load_1d(st + 32768 + b * 128, sc_h + id * blk_stride, 128, bar);
         }
         if (t == 0) {
           // ---- Q8 (while tile 0 is in flight): two e4m3 terms of this lane's 32 d columns, rows term * 8 + head ----
@@ -380,8 +403,59 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
             mbar_arrive(b_u_full + 8 * e);
           }
         }
+        if (left <= 1 && link == 2) {                                // link 3 (after this unit's q registers are dead)
+          fetch_rows(nxt, true);
+          link = 3;
+        }
       }
       cur = nxt;
+    }
+  } else if (warp >= 6) {
+    // ===================================== helper producers: K codes (warp 6), V codes (warp 7) =====================================
+    if (!p.chained) pdl_wait();                                      // they read the block table beyond a chunk's first 32 ids
+    const int b = lane & (kTcTileBlocks - 1);
+    const uint32_t part = warp == 6 ? 0u : 16384u;                   // offset of this warp's codes inside a stage ...
+    const int32_t part_row = warp == 6 ? 0 : 16;                     // ... and inside a pool tile (128-byte rows)
+    const int32_t row_blk = 33 * p.num_kv_heads;
+    uint32_t g_tile = 0, u_seq = 0, n_appends = 0;                  // appends of the units seen so far
+    for (;; ++u_seq) {
+      const int e = u_seq & 1;
+      mbar_wait(b_dsc_full + 8 * e, (u_seq >> 1) & 1u);
+      const uint32_t da = desc_smem + e * static_cast<uint32_t>(sizeof(TcDesc));
+      const uint4 d0 = lds128(da), d1 = lds128(da + 16);
+      int32_t ids = static_cast<int32_t>(lds32(da + 32 + lane * 4)), ids_next = 0;
+      __syncwarp();
+      if (lane == 0) mbar_arrive(b_dsc_empty + 8 * e);
+      const int n_blocks = static_cast<int>(d0.x);
+      if (n_blocks == 0) break;
+      const int32_t row_h = static_cast<int32_t>(d0.y) + part_row;
+      const int32_t* bt = p.block_table + static_cast<int64_t>(static_cast<int32_t>(d0.z)) * p.bt_stride + static_cast<int32_t>(d0.w);
+      const bool owns_last = d1.x != 0;
+      const int32_t last_blk = static_cast<int32_t>(d1.y);
+      const bool wait_append = kAppend && d1.z != 0;
+      const int n_tiles = (n_blocks + kTcTileBlocks - 1) / kTcTileBlocks;
+      for (int t = 0; t < n_tiles; ++t, ++g_tile) {
+        const uint32_t s = g_tile % kTcStages;
+        const int blk0 = t * kTcTileBlocks;
+        if ((blk0 & 31) == 0 && blk0 > 0) ids = ids_next;
+        if ((blk0 & 31) == 8 && blk0 + 24 + lane < n_blocks) ids_next = __ldg(bt + blk0 + 24 + lane);
+        int32_t id = __shfl_sync(kFull, ids, (blk0 + b) & 31);
+        if (owns_last && blk0 + b == n_blocks - 1) id = last_blk;
+        const int nb = min(kTcTileBlocks, n_blocks - blk0);
+        const uint32_t st = smem0 + s * kTcStageBytes + part, bar = b_full + 8 * s;
+        if (wait_append && t == n_tiles - 1) {                       // the new row is in the pool (and visible to TMA)
+          ++n_appends;
+          uint32_t done;
+          do {
+            asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(done) : "r"(app_ctr) : "memory");
+          } while (static_cast<int32_t>(done - n_appends) < 0);
+          asm volatile("fence.proxy.async;" ::: "memory");
+        }
+        mbar_wait(b_empty + 8 * s, ((g_tile / kTcStages) & 1u) ^ 1u);
+        if (lane == 0) mbar_arrive_expect_tx(bar, static_cast<uint32_t>(nb) * 2048u);
+        __syncwarp();
+        if (lane < nb) tma_load_2d(st + b * 2048, p.tmap, bar, 0, row_h + id * row_blk);
+      }
     }
   } else if (warp == 5) {
     // ===================================== MMA issuer: one thread =====================================
@@ -390,7 +464,7 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
       for (;; ++u_seq) {
         const int e = u_seq & 1;
         mbar_wait(b_u_full + 8 * e, (u_seq >> 1) & 1u);
-        const int n_tiles = static_cast<int>(lds32(misc + 192 + e * 64));
+        const int n_tiles = static_cast<int>(lds32(misc + 256 + e * 64));
         if (n_tiles == 0) break;
         mbar_wait(b_o_empty + 8 * e, ((u_seq >> 1) & 1u) ^ 1u);    // O^T buffer e: the unit two back has been read out
         const uint64_t qdesc = tc_smem_desc(q_smem + e * kTcQBytes);
@@ -451,7 +525,7 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
       mbar_wait(b_u_full + 8 * e, (u_seq >> 1) & 1u);
       TcUnit U;
       {
-        const uint32_t ua = misc + 192 + e * 64;
+        const uint32_t ua = misc + 256 + e * 64;
         const uint4 a = lds128(ua), b = lds128(ua + 16), c = lds128(ua + 32), d = lds128(ua + 48);
         U.n_tiles = static_cast<int32_t>(a.x); U.n_tokens = static_cast<int32_t>(a.y);
         U.batch_idx = static_cast<int32_t>(a.z); U.h = static_cast<int32_t>(a.w);
