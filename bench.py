@@ -13,8 +13,9 @@ every layer append the new token's K/V and run paged decode attention + LSE comb
   e2e       the same metric through the host-buffer C-ABI calls (kv_ingest_host,
             paged_decode_attention_host): every step's q, appended K/V and arriving requests' K/V
             come from pinned host memory and the outputs go back to it, inside the timed region
-  roofline  the attention kernel (attn_ring_kernel): algorithmic bytes per launch / mean launch duration (CUDA event
-            pairs recorded by the library around every launch of the timed region)
+  roofline  the attention kernel (attn_kernel<TileProvider, append=1>): algorithmic bytes per launch / mean launch
+            duration (CUDA event pairs recorded by the library around every group of layer launches of the timed region)
+  per_config  the same measurement for the other large BASELINE.json configs (2, 4, 5), in the same run
   cpu_baseline  the fp64 oracle timed on this box's host cores on a bounded sample
 
 Multi-GPU: the path shards by request with no exchange step: N independent
@@ -382,8 +383,10 @@ def measure(args, rep, sampler, wname: str, K: int, Wm: int, headline: bool):
     ing_n, ing_ms = prof["ingest"]
     attn_bytes_per_launch = by["attn"] / max(attn_n, 1)
     achieved = attn_bytes_per_launch / (attn_ms / max(attn_n, 1) * 1e-3) / 1e9 if attn_ms > 0 else None
-    tp = ("Fp8Tiles" if fp8 else "Bf16Tiles") + f"<{w.head_dim}>"
+    tp = ("Fp8Tiles" if fp8 else "Bf16Tiles") + f"<{w.head_dim}{', tma' if opts.get('tma') else ''}>"
     attn_kernel = f"attn_kernel<{tp}, append={0 if args.unfused else 1}>"
+    if fp8 and opts.get("tc") and w.head_dim == 128:
+        attn_kernel = f"attn_tc_kernel<append={0 if args.unfused else 1}> (tcgen05 / TMEM / TMA)"
     roofline = {"kernel": attn_kernel, "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak if achieved else None, "peak_source": peak_src,
                 "frac_of_nominal_8000": achieved / NOMINAL_HBM_GBS if achieved else None,

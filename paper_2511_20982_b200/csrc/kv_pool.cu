@@ -213,6 +213,13 @@ struct kv_pool {
   bool pdl = true;                // attention launches carry the programmatic-dependent-launch attribute
   bool side_upload = true;        // plan uploads on the pool's own stream (overlapping the caller's stream), joined by an event
   cudaStream_t up_stream = nullptr;
+  // kv_ingest_host, staged form: the copy engine fills the caller's staging buffer on this stream, group of requests
+  // by group, while the scatter of the previous group runs on the caller's stream
+  cudaStream_t copy_stream = nullptr;
+  static constexpr int kStageGroups = 16;
+  cudaEvent_t grp_ev[kStageGroups] = {};
+  cudaEvent_t stage_ev = nullptr;   // behind the last scatter that read the staging buffer
+  bool stage_busy = false;
   bool tma = false;               // bf16 pools, head_dim 128: full tiles by cp.async.bulk.tensor (UTMALDG) instead of LDGSTS
   bool tmap_ok = false;
   bool tc = false;                // FP8 pools, head_dim 128: decode attention on tcgen05 / TMEM (attn_tc_kernel)
@@ -617,6 +624,9 @@ int32_t kv_pool_create(const kv_pool_config_t* cfg, kv_pool_t** out_pool) {
       pool->plan_ring[i].dev = pool->base + lay.plan_blobs + i * lay.plan_blob_bytes;
     }
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&pool->up_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&pool->copy_stream, cudaStreamNonBlocking);
+    for (int i = 0; e == cudaSuccess && i < kv_pool::kStageGroups; ++i) e = cudaEventCreateWithFlags(&pool->grp_ev[i], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pool->stage_ev, cudaEventDisableTiming);
     // work counters start at zero; the attention kernel rewinds them itself afterwards
     // FP8: the 32 code rows of a tile in one box (its scales row follows them); bf16: the tile's 64 rows
     if (e == cudaSuccess) pool->tmap_ok = make_tensor_map(pool, &pool->tmap, pool->fp8() ? 32u : 64u);
@@ -644,6 +654,9 @@ int32_t kv_pool_destroy(kv_pool_t* pool) {
     }
     for (ProfRing& r : pool->prof) r.destroy();
     if (pool->up_stream) { cudaStreamSynchronize(pool->up_stream); cudaStreamDestroy(pool->up_stream); }
+    if (pool->copy_stream) { cudaStreamSynchronize(pool->copy_stream); cudaStreamDestroy(pool->copy_stream); }
+    for (cudaEvent_t ev : pool->grp_ev) if (ev) cudaEventDestroy(ev);
+    if (pool->stage_ev) cudaEventDestroy(pool->stage_ev);
   }
   delete pool;
   return KV_OK;
@@ -1070,43 +1083,72 @@ int32_t kv_ingest_host(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, c
   }
   ++(direct ? pool->n_zero_copy : pool->n_staged);
   if (direct) return ingest_reserved(pool, n_req, req_ids, n_tokens, kd.data(), vd.data(), layer_begin, layer_count, stream);
-  // Staged: K tensors first, then V tensors; each at a 256-byte aligned offset.  A run of requests whose
-  // host ranges and staging ranges are both back to back moves with one copy.
-  char* dst = static_cast<char*>(staging);
+  // Staged: the copy engine brings the sources into the caller's staging buffer (request after request, K then V,
+  // each at a 256-byte aligned offset) on a stream the pool owns, in groups of requests; the scatter of a group is
+  // enqueued on the caller's stream behind that group's copies, so it runs while the next group crosses the bus.
+  // (A copy-engine transfer moves ~55 GB/s over PCIe 5 x16 where SM loads of pinned memory reach ~48: option
+  // host_zero_copy = 0 selects this form for pinned sources too.)
+  char* const stage0 = static_cast<char*>(staging);
+  std::vector<int64_t> off(static_cast<size_t>(n_req) + 1, 0);
+  for (int32_t i = 0; i < n_req; ++i) off[static_cast<size_t>(i) + 1] = off[static_cast<size_t>(i)] + 2 * align_up(row_bytes * n_tokens[i]);
+  const int64_t total = off[static_cast<size_t>(n_req)];
+  const int64_t group_bytes = std::max<int64_t>(64LL << 20, (total + kv_pool::kStageGroups - 1) / kv_pool::kStageGroups);
+  cudaStream_t cs = pool->copy_stream;
   cudaError_t ce = cudaSuccess;
-  for (int pass = 0; pass < 2 && ce == cudaSuccess; ++pass) {
-    const void* const* src = pass ? v_src : k_src;
-    std::vector<const void*>& dev = pass ? vd : kd;
-    const char* run_src = nullptr;
-    char* run_dst = nullptr;
-    int64_t run_len = 0;
-    auto flush = [&]() -> cudaError_t {
-      cudaError_t e = run_len ? cudaMemcpyAsync(run_dst, run_src, static_cast<size_t>(run_len), cudaMemcpyHostToDevice, stream)
-                              : cudaSuccess;
-      run_len = 0;
-      return e;
-    };
-    for (int32_t i = 0; i < n_req && ce == cudaSuccess; ++i) {
+  if (pool->stage_busy) ce = cudaStreamWaitEvent(cs, pool->stage_ev, 0);   // the previous call's scatters have read the buffer
+  // what precedes this call on the caller's stream may be what made `staging` available: order the copies behind it
+  if (ce == cudaSuccess) ce = cudaEventRecord(pool->grp_ev[0], stream);
+  if (ce == cudaSuccess) ce = cudaStreamWaitEvent(cs, pool->grp_ev[0], 0);
+  int32_t launched = 0;
+  int g = 0;
+  for (int32_t i0 = 0; i0 < n_req && ce == cudaSuccess;) {
+    int32_t i1 = i0;
+    while (i1 < n_req && (i1 == i0 || off[static_cast<size_t>(i1) + 1] - off[static_cast<size_t>(i0)] <= group_bytes)) ++i1;
+    for (int32_t i = i0; i < i1 && ce == cudaSuccess; ++i) {
       const int64_t bytes = row_bytes * n_tokens[i];
-      dev[static_cast<size_t>(i)] = dst;
+      char* kdst = stage0 + off[static_cast<size_t>(i)];
+      char* vdst = kdst + align_up(bytes);
+      kd[static_cast<size_t>(i)] = kdst;
+      vd[static_cast<size_t>(i)] = vdst;
       if (bytes == 0) continue;
-      const char* sp = static_cast<const char*>(src[i]);
-      if (run_len && sp == run_src + run_len && dst == run_dst + run_len) {
-        run_len += bytes;
-      } else {
-        ce = flush();
-        run_src = sp; run_dst = dst; run_len = bytes;
+      // pieces of 8 MiB: a small copy another stream hands to the same copy engine (a decode step's q) waits for
+      // ~150 us at most, not for a whole request
+      constexpr int64_t kPiece = 8LL << 20;
+      for (int pass = 0; pass < 2 && ce == cudaSuccess; ++pass) {
+        char* dstp = pass ? vdst : kdst;
+        const char* srcp = static_cast<const char*>(pass ? v_src[i] : k_src[i]);
+        for (int64_t o = 0; o < bytes && ce == cudaSuccess; o += kPiece)
+          ce = cudaMemcpyAsync(dstp + o, srcp + o, static_cast<size_t>(std::min(kPiece, bytes - o)), cudaMemcpyHostToDevice, cs);
       }
-      dst += (bytes % kAlign == 0) ? bytes : align_up(bytes);
     }
-    if (ce == cudaSuccess) ce = flush();
-    dst = static_cast<char*>(staging) + align_up(dst - static_cast<char*>(staging));
+    if (ce == cudaSuccess) ce = cudaEventRecord(pool->grp_ev[g], cs);
+    if (ce == cudaSuccess) ce = cudaStreamWaitEvent(stream, pool->grp_ev[g], 0);
+    if (ce != cudaSuccess) break;
+    const int32_t n = i1 - i0;
+    const size_t o = static_cast<size_t>(i0);
+    std::vector<int32_t> start(static_cast<size_t>(n));
+    for (int32_t i = 0; i < n; ++i) start[static_cast<size_t>(i)] = pool->hs.reqs.find(req_ids[o + i])->second.len - n_tokens[o + i];
+    rc = run_copy(pool, CopyKind::kScatter, nullptr, nullptr, n, req_ids + o, n_tokens + o, kd.data() + o, vd.data() + o, start.data(),
+                  layer_begin, layer_count, stream);
+    if (rc != KV_OK) {
+      // nothing of this call has been launched yet: the reservation can go back; otherwise the error is a CUDA error
+      // on a stream that already carries part of the call (KV_ERR_CUDA is sticky)
+      if (launched == 0 && layer_begin == 0) pool->hs.rollback_last_reserve();
+      return rc;
+    }
+    ++launched;
+    g = (g + 1) % kv_pool::kStageGroups;
+    i0 = i1;
+  }
+  if (ce == cudaSuccess && n_req > 0) {
+    ce = cudaEventRecord(pool->stage_ev, stream);
+    pool->stage_busy = ce == cudaSuccess;
   }
   if (ce != cudaSuccess) {
-    if (layer_begin == 0) pool->hs.rollback_last_reserve();
+    if (launched == 0 && layer_begin == 0) pool->hs.rollback_last_reserve();
     return pool->cuda_fail(ce);
   }
-  return ingest_reserved(pool, n_req, req_ids, n_tokens, kd.data(), vd.data(), layer_begin, layer_count, stream);
+  return KV_OK;
 }
 
 static int32_t attention_host(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const void* q,

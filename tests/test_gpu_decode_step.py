@@ -196,6 +196,35 @@ def test_host_buffer_entry_points():
     assert e.value.status == B.KV_ERR_INVALID
 
 
+def test_host_ingest_staged_in_groups():
+    """kv_ingest_host with host_zero_copy = 0: the copy engine fills the staging buffer group of requests by group of
+    requests on the pool's own stream while the previous group is scattered; two calls back to back reuse the
+    staging buffer (the second call's copies wait for the first call's scatters).  Whole slab == oracle."""
+    L, Hkv, d = 2, 8, 128
+    w = W.Workload("stage", L, 32, Hkv, d, 10, None, 91, max_len=8192)
+    lens_a, ids_a = [4000, 3000, 4100, 17, 3900, 4200], [1, 2, 3, 4, 5, 6]      # ~150 MB of K + V: three groups
+    lens_b, ids_b = [3500, 4500, 1, 2600], [11, 12, 13, 14]
+    pool = make_pool(w, sum((n + 15) // 16 for n in lens_a + lens_b) + 8, alloc_seed=3, max_requests=16, max_len=8192)
+    pool.set_option("host_zero_copy", 0)
+    slab = oracle_slab(pool)
+    tok = L * Hkv * d * 2
+    need = max(sum(2 * ((n * tok + 255) // 256 * 256) for n in ls) for ls in (lens_a, lens_b))
+    staging = torch.empty(need, dtype=torch.uint8, device=DEV)
+    s = torch.cuda.current_stream().cuda_stream
+    keep = []
+    for ids, lens in ((ids_a, lens_a), (ids_b, lens_b)):
+        src = [tuple(t.pin_memory() for t in kv_src(w, u, 0, n, "cpu")) for u, n in zip(ids, lens)]
+        keep.append(src)
+        B.kv_ingest_host(pool.handle, ids, lens, [k.data_ptr() for k, _ in src], [v.data_ptr() for _, v in src], 0, L,
+                         staging.data_ptr(), need, s)
+    for ids, lens in ((ids_a, lens_a), (ids_b, lens_b)):
+        for u, n in zip(ids, lens):
+            oracle_ingest(slab, pool, w, u, 0, n)
+    torch.cuda.synchronize()
+    assert pool.counter("host_ingest_staged") == 2 and pool.counter("host_ingest_zero_copy") == 0
+    assert np.array_equal(pool_bits(pool), slab)
+
+
 def test_profile_counts_every_launch():
     w = W.Workload("prof", 1, 8, 2, 64, 4, None, 3, max_len=4096)
     pool = make_pool(w, 600)
