@@ -395,7 +395,7 @@ def measure(args, rep, sampler, wname: str, K: int, Wm: int, headline: bool):
                           "back-to-back layer launches of the timed region (kv_profile_read); duration / launches",
                 "algorithmic_bytes_per_launch": attn_bytes_per_launch, "traffic": None}
     traffic, traffic_path = load_traffic()
-    ent = traffic.get(wname, {}).get(args.kv_dtype)
+    ent = traffic.get(wname, {}).get("fp8_tc" if (fp8 and opts.get("tc") and w.head_dim == 128) else args.kv_dtype)
     if ent:
         roofline.update({"traffic": attn_bytes_per_launch * ent["dram_bytes_per_algorithmic_byte"],
                          "traffic_source": f"modelled: {traffic_path} ({ent['source']}): DRAM read+write bytes of one ncu --set full "

@@ -110,6 +110,30 @@ def test_attention_matches_oracle(Hq, Hkv, d, opts):
     assert np.abs(want - exact).max() < 0.15 and np.abs(want - exact).mean() < 0.01
 
 
+@pytest.mark.parametrize("opts", [dict(), dict(tc=1), dict(tc=1, min_chunk_blocks=9, items_per_slot=1024)])
+@pytest.mark.parametrize("G", [2, 3, 5, 6, 7])
+def test_attention_every_group_size(G, opts):
+    """GQA groups that do not fill the 8 MMA columns (mma.sync kernel) / the 8 head rows of Q8 and P (tcgen05 kernel)."""
+    Hkv, d = 2, 128
+    Hq = G * Hkv
+    lens = [1, 16, 17, 129, 1000, 2049]
+    ids = list(range(40, 40 + len(lens)))
+    pool = make_fp8_pool(1, Hq, Hkv, d, sum((n + 15) // 16 for n in lens) + 4)
+    apply_options(pool, opts)
+    w = W.Workload("fp8g", 1, Hq, Hkv, d, len(lens), None, 100 + G, max_len=4096)
+    srcs = [kv_src(w, uid, 0, n, DEV) for uid, n in zip(ids, lens)]
+    pool.ingest(ids, [s[0] for s in srcs], [s[1] for s in srcs])
+    slab = oracle.new_slab_fp8(dims_of(pool), SENT)
+    for uid, n, (k, v) in zip(ids, lens, srcs):
+        oracle.scatter_fp8(slab, dims_of(pool), pool.block_table(uid)[0], 0, bits_of(k), bits_of(v))
+    q = W.q_values(w.seed, 1, 0, len(lens), Hq, d, DEV)
+    out = pool.attention(0, ids, q)
+    torch.cuda.synchronize()
+    assert np.array_equal(pool_bytes(pool), slab)
+    lists = [pool.block_table(u)[0] for u in ids]
+    compare_attention(out, oracle.attention_fp8(slab, dims_of(pool), 0, Hq, lists, lens, bits_of(q)))
+
+
 @pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=2, items_per_slot=1024), dict(tma=1), dict(tc=1),
                                   dict(tc=1, min_chunk_blocks=2, items_per_slot=1024)])
 def test_attention_wide_dynamic_range(opts):
