@@ -83,12 +83,12 @@ def check_rows(loop, name, step, layer, rows, fp8, gen_device):
     return float(err.max())
 
 
-def run_config(name, n_short, n_long, kv_dtype=B.KV_DTYPE_BF16, fused=True, all_rows=False):
+def run_config(name, n_short, n_long, kv_dtype=B.KV_DTYPE_BF16, fused=True, all_rows=False, options=None):
     w = W.CONFIGS[name]
     free, total = torch.cuda.mem_get_info()
     try:
         loop = DecodeLoop(w, STEPS, device=DEV, sentinel=int(np.uint16(NAN_BITS).astype(np.int16)), profile=False,
-                          kv_dtype=kv_dtype, fused=fused)
+                          kv_dtype=kv_dtype, fused=fused, options=options)
     except (torch.cuda.OutOfMemoryError, AssertionError) as e:
         pytest.skip(f"{name} does not fit this device ({free / 1e9:.0f} GB free of {total / 1e9:.0f}): {e}")
     fp8 = kv_dtype == B.KV_DTYPE_FP8_E4M3
@@ -181,6 +181,16 @@ def test_cfg5_stress_full():
 
 def test_cfg3_8b_gqa_full_fp8_pool():
     run_config("cfg3_8b_gqa", n_short=12, n_long=6, kv_dtype=B.KV_DTYPE_FP8_E4M3)
+
+
+def test_cfg3_8b_gqa_full_fp8_pool_tcgen05():
+    """The same through attn_tc_kernel (option tc=1): 32 PDL-chained launches per step, fused append, concurrent ingest."""
+    run_config("cfg3_8b_gqa", n_short=12, n_long=6, kv_dtype=B.KV_DTYPE_FP8_E4M3, options=dict(tc=1))
+
+
+def test_cfg2_7b_mha_full_fp8_pool_tcgen05():
+    """G = 1, 32 kv heads, every unit owns its request's last block (fused append in every unit)."""
+    run_config("cfg2_7b_mha", n_short=8, n_long=8, kv_dtype=B.KV_DTYPE_FP8_E4M3, options=dict(tc=1))
 
 
 def test_cfg2_7b_mha_full_unfused():
