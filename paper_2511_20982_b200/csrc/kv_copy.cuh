@@ -137,17 +137,19 @@ __global__ void __launch_bounds__(kIngest8Threads) ingest_fp8_kernel(const Inges
     row1 = min(kBlockSize, x.r.start_pos + x.r.n_tokens - lb * kBlockSize);
     t0 = lb * kBlockSize + row0 - x.r.start_pos;
   };
-  auto load = [&](uint4 (&buf)[NV], int b) {
-    int row0, row1, t0;
-    rows_of(b, row0, row1, t0);
+  // kWhole (a literal at every call site, folded after inlining): the block is known to hold 16 of this call's rows —
+  // no per-piece predicates (the common case: the run lies inside the request; the kernel is issue-bound)
+  auto load = [&](uint4 (&buf)[NV], int b, const bool kWhole) {
+    int row0 = 0, row1 = kBlockSize, t0 = (x.lb + b) * kBlockSize - x.r.start_pos;
+    if (!kWhole) rows_of(b, row0, row1, t0);
     const uint4* lin = reinterpret_cast<const uint4*>(src + static_cast<int64_t>(t0) * D);
     const int pieces = (row1 - row0) * kPiecesPerRow;
 #pragma unroll
-    for (int i = 0; i < NV; ++i) buf[i] = ldg_copy_pred(lin + lane + 32 * i, lane + 32 * i < pieces);
+    for (int i = 0; i < NV; ++i) buf[i] = ldg_copy_pred(lin + lane + 32 * i, kWhole || lane + 32 * i < pieces);
   };
-  auto quantise_store = [&](const uint4 (&buf)[NV], int b) {
-    int row0, row1, t0;
-    rows_of(b, row0, row1, t0);
+  auto quantise_store = [&](const uint4 (&buf)[NV], int b, const bool kWhole) {
+    int row0 = 0, row1 = kBlockSize, t0 = 0;
+    if (!kWhole) rows_of(b, row0, row1, t0);
     const int rows = row1 - row0;
     const int32_t blk = __shfl_sync(kFull, blk_id, b);
     uint8_t* tile = layer_head + static_cast<int64_t>(blk) * p.num_kv_heads * fp8_tile_bytes<D>();
@@ -173,7 +175,7 @@ __global__ void __launch_bounds__(kIngest8Threads) ingest_fp8_kernel(const Inges
     const float scale = mx == 0 ? 1.f : __fdiv_rn(amax, 448.f);
     const float inv = mx == 0 ? 1.f : __fdiv_rn(448.f, amax);
     const int own_row = (32 / kPiecesPerRow) * own + grp;          // relative to row0
-    if ((lane & 1) == 0 && own_row < rows)
+    if ((lane & 1) == 0 && (kWhole || own_row < rows))
       *reinterpret_cast<float*>(tile + 2 * kBlockSize * D + (row0 + own_row) * 8 + c * 4) = scale;
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
@@ -185,7 +187,7 @@ __global__ void __launch_bounds__(kIngest8Threads) ingest_fp8_kernel(const Inges
         const uint32_t e = u4_get(buf[i], k);
         w[k] = f32x2_to_e4m3x2(__fmul_rn(__uint_as_float(e << 16), inv_i), __fmul_rn(__uint_as_float(e & 0xffff0000u), inv_i));
       }
-      if (idx < rows * kPiecesPerRow)
+      if (kWhole || idx < rows * kPiecesPerRow)
         *reinterpret_cast<uint2*>(tile + c * (kBlockSize * D) + row0 * D + idx * 8) = make_uint2(w[0] | (w[1] << 16), w[2] | (w[3] << 16));
     }
     if (c == 0 && x.ll == 0 && x.h == 0 && lane == 0)             // device block_table mirror (a1, device half)
@@ -193,16 +195,30 @@ __global__ void __launch_bounds__(kIngest8Threads) ingest_fp8_kernel(const Inges
   };
 
   uint4 bufa[NV], bufb[NV];
-  load(bufa, 0);
+  // the whole run lies inside this call's rows: four full blocks, no predicates
+  const bool run_full = n_run == kIngest8Run && (x.jj > 0 || (x.r.start_pos & (kBlockSize - 1)) == 0) &&
+                        x.r.start_pos + x.r.n_tokens >= (x.lb + kIngest8Run) * kBlockSize;
+  if (run_full) {
+    load(bufa, 0, true);
+#pragma unroll
+    for (int b = 0; b < kIngest8Run; b += 2) {
+      load(bufb, b + 1, true);
+      quantise_store(bufa, b, true);
+      if (b + 2 < kIngest8Run) load(bufa, b + 2, true);
+      quantise_store(bufb, b + 1, true);
+    }
+    return;
+  }
+  load(bufa, 0, false);
 #pragma unroll
   for (int b = 0; b < kIngest8Run; b += 2) {
     if (b < n_run) {
-      if (b + 1 < n_run) load(bufb, b + 1);
-      quantise_store(bufa, b);
+      if (b + 1 < n_run) load(bufb, b + 1, false);
+      quantise_store(bufa, b, false);
     }
     if (b + 1 < n_run) {
-      if (b + 2 < n_run) load(bufa, b + 2);
-      quantise_store(bufb, b + 1);
+      if (b + 2 < n_run) load(bufa, b + 2, false);
+      quantise_store(bufb, b + 1, false);
     }
   }
 }
