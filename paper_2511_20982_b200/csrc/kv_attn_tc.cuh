@@ -33,6 +33,9 @@
 //              {K codes, V codes, scales}) and ONE warp issues a copy every ~45 ns: 1.1 us per tile, at which point the
 //              producer, not HBM, paces the CTA (profiles/README.md r02) — so the issue is spread over three warps.
 //   The producers run ahead ACROSS unit boundaries (they own no registers worth mentioning).
+//   The fused append never waits for a global store to reach the TMA unit: the lead producer writes the quantised row to
+//   the pool AND to shared memory, the tile holding its slot is fetched like any other, and the MMA warp patches the
+//   row into the stage before that tile's GEMM1 (the softmax thread of that token takes its two scales from the copy).
 // All hand-offs are mbarriers; the only block-wide barrier is at start-up and tear-down.
 #pragma once
 
@@ -49,7 +52,7 @@ constexpr int kTcTileBlocks = 8, kTcTileTokens = kTcTileBlocks * kBlockSize;
 constexpr uint32_t kTcStageBytes = 2 * kTcTileTokens * 128 + kTcTileTokens * 8;   // 33792 = 33 KiB
 constexpr uint32_t kTcQBytes = 16 * 128, kTcPBytes = 32 * 128;
 constexpr uint32_t kTcMiscOff = kTcStages * kTcStageBytes + 2 * kTcQBytes + 2 * kTcPBytes;
-constexpr uint32_t kTcSmemBytes = kTcMiscOff + 1536;                              // 115200 = 112.5 KiB
+constexpr uint32_t kTcSmemBytes = kTcMiscOff + 1664;                              // 115328 = 112.6 KiB
 constexpr uint32_t kTcTmemCols = 128;       // S^T: 2 x 16 columns, O^T: 2 x 32 columns
 constexpr float kTcLazyLog2 = 8.f;          // m_ref moves when a score exceeds it by more than this (log2 units)
 // The weights are fed as 2^(s - m_ref + kTcWeightBias): the four e5m2 terms of a weight bottom out at e5m2's smallest
@@ -154,7 +157,8 @@ struct TcUnit {            // what the producer hands to the MMA and softmax war
   int32_t n_tiles;         // 0: no more work
   int32_t n_tokens;        // valid tokens of the chunk
   int32_t batch_idx, h;
-  int32_t pidx, pbase, n_chunks, pad;
+  int32_t pidx, pbase, n_chunks;
+  int32_t new_row;         // fused append: row of the unit's LAST tile that holds the token being appended, else -1
   float qs[8];             // per head: 2^(eb - 134) * sm_scale * log2(e), the factor that turns K8 . q8 * ks into log2 scores
 };
 static_assert(sizeof(TcUnit) == 64, "TcUnit");
@@ -165,8 +169,7 @@ struct TcDesc {            // what the lead producer hands to the helper produce
   int32_t slot, blk_begin; // where the chunk's block ids continue in the device block table
   int32_t owns_last;       // the chunk ends with the request's last block ...
   int32_t last_blk;        // ... whose physical id is this (the device block table may not hold it yet)
-  int32_t append;          // the lead appends the new row to that block: wait for it before the unit's last tile
-  int32_t pad;
+  int32_t pad[2];
   int32_t ids[32];         // physical ids of the chunk's first 32 blocks
 };
 static_assert(sizeof(TcDesc) == 160, "TcDesc");
@@ -186,16 +189,15 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
                  b_p_free = misc + 96, b_o_full = misc + 112, b_o_empty = misc + 128, b_u_full = misc + 144, b_u_empty = misc + 160,
                  b_dsc_full = misc + 192, b_dsc_empty = misc + 208;
   const uint32_t tmem_slot = misc + 176, merge_flag = misc + 180;
-  const uint32_t app_ctr = misc + 184;      // appends completed by the lead producer (monotonic; polled by the helpers)
   TcUnit* const units = reinterpret_cast<TcUnit*>(tc_smem + kTcMiscOff + 256);
   const uint32_t flags_smem = misc + 384;   // [2][4] int
   const uint32_t wmax_smem = misc + 416;    // [2][4][8] float
   const uint32_t lsum_smem = misc + 672;    // [4][8] float
   const uint32_t desc_smem = misc + 800;    // [2] TcDesc
+  const uint32_t stash_smem = misc + 1120;  // [2] the appended row as the pool stores it: K codes[128] | V codes[128] | ks, vs | pad (272 B)
 
   if (threadIdx.x == 0) {
     if (smem0 & 1023u) __trap();            // the 128-byte swizzle is a function of the shared-memory address
-    sts32(app_ctr, 0u);
     for (int s = 0; s < kTcStages; ++s) { mbar_init(b_full + 8 * s, 3); mbar_init(b_empty + 8 * s, 1); }   // three issuing warps
     for (int i = 0; i < 2; ++i) {
       mbar_init(b_d1_full + 8 * i, 1); mbar_init(b_d1_empty + 8 * i, kTcSoftmaxThreads);
@@ -233,7 +235,7 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
     const int b = lane & (kTcTileBlocks - 1);
     const int qhead = lane >> 2, quarter = lane & 3;                 // Q8 staging: head of the group, 32 d columns
     const bool qok = qhead < G;
-    uint32_t g_tile = 0, u_seq = 0, n_appends = 0;
+    uint32_t g_tile = 0, u_seq = 0;
 
     // what is known of a unit before it starts
     struct Desc { int32_t unit; int4 w0, w1; int32_t ids; uint4 q[4]; uint4 nrow; };
@@ -301,12 +303,12 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
       const int32_t* bt = p.block_table + static_cast<int64_t>(slot) * p.bt_stride + blk_begin;
       int32_t ids = cur.ids, ids_next = 0;
       const unsigned char* const sc_h = kv + static_cast<int64_t>(h) * TP::kPoolTileBytes + 4096;
-      bool append_pending = kAppend && owns_last;
+      const bool append = kAppend && owns_last;
       // ---- the unit's descriptor goes to the helper producers before anything else ----
       Dsc->ids[lane] = ids;
       if (lane == 0) {
         Dsc->n_blocks = n_blocks; Dsc->row_h = static_cast<int32_t>(p.tma_row0) + h * 33; Dsc->slot = slot; Dsc->blk_begin = blk_begin;
-        Dsc->owns_last = owns_last ? 1 : 0; Dsc->last_blk = last_blk; Dsc->append = append_pending ? 1 : 0;
+        Dsc->owns_last = owns_last ? 1 : 0; Dsc->last_blk = last_blk;
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(b_dsc_full + 8 * e);
@@ -326,23 +328,6 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
           nxt.unit = __shfl_sync(kFull, nxt.unit, 0);
           fetch_item(nxt);
           link = 2;
-        }
-        // a3 inside a4: the unit that owns the request's last block quantises the new row into the pool before the
-        // tile holding that block (the unit's last tile) is asked for, so the TMA copies already see it
-        // (doing it right after tile 0 instead was measured: equal to slightly slower)
-        if constexpr (kAppend) {
-          if (append_pending && t == n_tiles - 1) {
-            unsigned char* const last_tile = kv + static_cast<int64_t>(h) * TP::kPoolTileBytes + last_blk * blk_stride;
-            typename TP::NewRow nr;
-            TP::append_store(last_tile, n_tokens - (n_blocks - 1) * kBlockSize - 1, cur.nrow, lane, nr);
-            if (h == 0 && lane == 0) p.block_table[static_cast<int64_t>(slot) * p.bt_stride + blk_begin + n_blocks - 1] = last_blk;
-            __threadfence();
-            asm volatile("fence.proxy.async;" ::: "memory");         // generic-proxy global writes before async-proxy (TMA) reads
-            __syncwarp();
-            if (lane == 0)                                              // the helpers may fetch the unit's last tile
-              asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(app_ctr), "r"(++n_appends) : "memory");
-            append_pending = false;
-          }
         }
         // ---- tile t, this warp's share: the scales of its (up to) 8 blocks, lane b < 8 owns block b ----
         {
@@ -395,11 +380,27 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
             sts128(qb + qhead * 128 + ((chunk ^ qhead) << 4), make_uint4(t1[4 * half], t1[4 * half + 1], t1[4 * half + 2], t1[4 * half + 3]));
             sts128(qb + (8 + qhead) * 128 + ((chunk ^ qhead) << 4), make_uint4(t2[4 * half], t2[4 * half + 1], t2[4 * half + 2], t2[4 * half + 3]));
           }
+          // a3 inside a4: the unit that owns the request's last block quantises the new row (ingest's arithmetic, ingest's
+          // bytes), writes it to the pool for the steps to come, and leaves a copy in shared memory: the tile that holds
+          // its slot is fetched like any other (stale bytes in that row) and the MMA warp patches the row in before it
+          // issues the tile's GEMM1.  Nothing waits for a global store to become visible to the TMA unit.
+          if constexpr (kAppend) {
+            if (append) {
+              unsigned char* const last_tile = kv + static_cast<int64_t>(h) * TP::kPoolTileBytes + last_blk * blk_stride;
+              typename TP::NewRow nr;
+              TP::append_store(last_tile, n_tokens - (n_blocks - 1) * kBlockSize - 1, cur.nrow, lane, nr);
+              if (h == 0 && lane == 0) p.block_table[static_cast<int64_t>(slot) * p.bt_stride + blk_begin + n_blocks - 1] = last_blk;
+              const uint32_t sa = stash_smem + e * 272u;
+              asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(sa + lane * 8), "r"(nr.codes.x), "r"(nr.codes.y) : "memory");
+              if ((lane & 15) == 0) sts32(sa + 256 + (lane >> 4) * 4, __float_as_uint(nr.scale));
+            }
+          }
           fence_proxy_async();                                        // Q8 in shared memory -> visible to the tensor core
           __syncwarp();
           if (lane == 0) {
             U->n_tiles = n_tiles; U->n_tokens = n_tokens; U->batch_idx = batch_idx; U->h = h;
             U->pidx = cur.w1.y < 0 ? -1 : pbase + chunk_idx; U->pbase = pbase; U->n_chunks = n_chunks;
+            U->new_row = append ? n_tokens - 1 - (n_tiles - 1) * kTcTileTokens : -1;
             mbar_arrive(b_u_full + 8 * e);
           }
         }
@@ -417,7 +418,7 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
     const uint32_t part = warp == 6 ? 0u : 16384u;                   // offset of this warp's codes inside a stage ...
     const int32_t part_row = warp == 6 ? 0 : 16;                     // ... and inside a pool tile (128-byte rows)
     const int32_t row_blk = 33 * p.num_kv_heads;
-    uint32_t g_tile = 0, u_seq = 0, n_appends = 0;                  // appends of the units seen so far
+    uint32_t g_tile = 0, u_seq = 0;
     for (;; ++u_seq) {
       const int e = u_seq & 1;
       mbar_wait(b_dsc_full + 8 * e, (u_seq >> 1) & 1u);
@@ -432,7 +433,6 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
       const int32_t* bt = p.block_table + static_cast<int64_t>(static_cast<int32_t>(d0.z)) * p.bt_stride + static_cast<int32_t>(d0.w);
       const bool owns_last = d1.x != 0;
       const int32_t last_blk = static_cast<int32_t>(d1.y);
-      const bool wait_append = kAppend && d1.z != 0;
       const int n_tiles = (n_blocks + kTcTileBlocks - 1) / kTcTileBlocks;
       for (int t = 0; t < n_tiles; ++t, ++g_tile) {
         const uint32_t s = g_tile % kTcStages;
@@ -443,14 +443,6 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
         if (owns_last && blk0 + b == n_blocks - 1) id = last_blk;
         const int nb = min(kTcTileBlocks, n_blocks - blk0);
         const uint32_t st = smem0 + s * kTcStageBytes + part, bar = b_full + 8 * s;
-        if (wait_append && t == n_tiles - 1) {                       // the new row is in the pool (and visible to TMA)
-          ++n_appends;
-          uint32_t done;
-          do {
-            asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(done) : "r"(app_ctr) : "memory");
-          } while (static_cast<int32_t>(done - n_appends) < 0);
-          asm volatile("fence.proxy.async;" ::: "memory");
-        }
         mbar_wait(b_empty + 8 * s, ((g_tile / kTcStages) & 1u) ^ 1u);
         if (lane == 0) mbar_arrive_expect_tx(bar, static_cast<uint32_t>(nb) * 2048u);
         __syncwarp();
@@ -466,6 +458,7 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
         mbar_wait(b_u_full + 8 * e, (u_seq >> 1) & 1u);
         const int n_tiles = static_cast<int>(lds32(misc + 256 + e * 64));
         if (n_tiles == 0) break;
+        const int new_row = kAppend ? static_cast<int>(lds32(misc + 256 + e * 64 + 28)) : -1;
         mbar_wait(b_o_empty + 8 * e, ((u_seq >> 1) & 1u) ^ 1u);    // O^T buffer e: the unit two back has been read out
         const uint64_t qdesc = tc_smem_desc(q_smem + e * kTcQBytes);
         const uint32_t o_tmem = tmem + 32 + e * 32;
@@ -485,6 +478,18 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
             if (must || (mbar_try_wait(b_full + 8 * s1, (g1 / kTcStages) & 1u) &&
                          mbar_try_wait(b_d1_empty + 8 * db, ((g1 >> 1) & 1u) ^ 1u))) {
               tc_fence_after();
+              if (kAppend && new_row >= 0 && t1 == n_tiles - 1) {
+                // a3 inside a4: the appended row goes on top of the stale bytes the tile brought for its slot (row
+                // `new_row` of the K and of the V codes, 16-byte chunks in the 128-byte swizzle, and its two scales)
+                const uint32_t st = smem0 + s1 * kTcStageBytes, sa = stash_smem + e * 272u;
+                const uint32_t row = static_cast<uint32_t>(new_row);
+#pragma unroll
+                for (uint32_t c = 0; c < 8; ++c) {
+                  sts128(st + row * 128 + ((c ^ (row & 7u)) << 4), lds128(sa + c * 16));
+                  sts128(st + 16384 + row * 128 + ((c ^ (row & 7u)) << 4), lds128(sa + 128 + c * 16));
+                }
+                fence_proxy_async();                               // ... before the tensor core reads them
+              }
               const uint64_t kdesc = tc_smem_desc(smem0 + s1 * kTcStageBytes);
 #pragma unroll
               for (int k = 0; k < 4; ++k) tc_mma_f8(tmem + db * 16, kdesc + 2 * k, qdesc + 2 * k, kTcIdescQK, k > 0);
@@ -530,6 +535,7 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
         U.n_tiles = static_cast<int32_t>(a.x); U.n_tokens = static_cast<int32_t>(a.y);
         U.batch_idx = static_cast<int32_t>(a.z); U.h = static_cast<int32_t>(a.w);
         U.pidx = static_cast<int32_t>(b.x); U.pbase = static_cast<int32_t>(b.y); U.n_chunks = static_cast<int32_t>(b.z);
+        U.new_row = static_cast<int32_t>(b.w);
         U.qs[0] = __uint_as_float(c.x); U.qs[1] = __uint_as_float(c.y); U.qs[2] = __uint_as_float(c.z); U.qs[3] = __uint_as_float(c.w);
         U.qs[4] = __uint_as_float(d.x); U.qs[5] = __uint_as_float(d.y); U.qs[6] = __uint_as_float(d.z); U.qs[7] = __uint_as_float(d.w);
       }
@@ -545,6 +551,8 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
         mbar_wait(b_full + 8 * s, (g / kTcStages) & 1u);           // the tile's scales (and V rows, below) are readable
         float ks, vs;
         asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(ks), "=f"(vs) : "r"(st + 32768 + tid * 8) : "memory");
+        if (kAppend && t == U.n_tiles - 1 && tid == U.new_row)       // the appended row's scales: the tile brought stale ones
+          asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(ks), "=f"(vs) : "r"(stash_smem + e * 272u + 256u) : "memory");
         const bool valid = t * kTcTileTokens + tid < U.n_tokens;
         if (t == U.n_tiles - 1 && !valid) {                        // rows past the chunk's end: no stale V byte reaches GEMM2
           const uint4 z = make_uint4(0u, 0u, 0u, 0u);
