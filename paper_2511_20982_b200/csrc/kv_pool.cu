@@ -222,7 +222,7 @@ struct kv_pool {
   bool stage_busy = false;
   bool tma = false;               // bf16 pools, head_dim 128: full tiles by cp.async.bulk.tensor (UTMALDG) instead of LDGSTS
   bool tmap_ok = false;
-  bool tc = false;                // FP8 pools, head_dim 128: decode attention on tcgen05 / TMEM (attn_tc_kernel)
+  bool tc = true;                 // FP8 pools, head_dim 128: decode attention on tcgen05 / TMEM (attn_tc_kernel); 0: mma.sync kernel
   bool tmap16_ok = false;
   alignas(64) CUtensorMap tmap16; // the same region, box 16 rows: the K codes or the V codes of one (block, kv head) tile
   alignas(64) CUtensorMap tmap;   // the KV region as [rows][128 B], box 64 rows, 128-byte swizzle

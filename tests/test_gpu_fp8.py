@@ -18,10 +18,11 @@ from helpers import bf16_bits, bits_of, bits_to_f64
 
 pytestmark = pytest.mark.gpu
 
-MODES = [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=1024),
-         dict(min_chunk_blocks=2, items_per_slot=2, fuse_combine=0), dict(min_chunk_blocks=5, items_per_slot=1, ctas_per_sm=1),
-         dict(pdl=0), dict(pdl=0, min_chunk_blocks=2, items_per_slot=1024),
-         dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024), dict(tma=1, min_chunk_blocks=3, items_per_slot=2, fuse_combine=0),
+# tc=0: the mma.sync kernel (attn_kernel<Fp8Tiles>), which head_dim-64 pools run whatever the option says
+MODES = [dict(), dict(tc=0), dict(tc=0, min_chunk_blocks=1, items_per_slot=1024), dict(tc=0, min_chunk_blocks=3, items_per_slot=1024),
+         dict(tc=0, min_chunk_blocks=2, items_per_slot=2, fuse_combine=0), dict(tc=0, min_chunk_blocks=5, items_per_slot=1, ctas_per_sm=1),
+         dict(tc=0, pdl=0), dict(tc=0, pdl=0, min_chunk_blocks=2, items_per_slot=1024),
+         dict(tc=0, tma=1), dict(tc=0, tma=1, min_chunk_blocks=1, items_per_slot=1024), dict(tc=0, tma=1, min_chunk_blocks=3, items_per_slot=2, fuse_combine=0),
          # tc=1: attn_tc_kernel (tcgen05 / TMEM / TMA, 128-token tiles): single tile, many tiles per unit, one block per chunk
          dict(tc=1), dict(tc=1, min_chunk_blocks=1, items_per_slot=1024), dict(tc=1, min_chunk_blocks=9, items_per_slot=1024),
          dict(tc=1, min_chunk_blocks=3, items_per_slot=2, fuse_combine=0), dict(tc=1, pdl=0, min_chunk_blocks=17, items_per_slot=1)]
@@ -110,7 +111,7 @@ def test_attention_matches_oracle(Hq, Hkv, d, opts):
     assert np.abs(want - exact).max() < 0.15 and np.abs(want - exact).mean() < 0.01
 
 
-@pytest.mark.parametrize("opts", [dict(), dict(tc=1), dict(tc=1, min_chunk_blocks=9, items_per_slot=1024)])
+@pytest.mark.parametrize("opts", [dict(tc=0), dict(tc=1), dict(tc=1, min_chunk_blocks=9, items_per_slot=1024)])
 @pytest.mark.parametrize("G", [2, 3, 5, 6, 7])
 def test_attention_every_group_size(G, opts):
     """GQA groups that do not fill the 8 MMA columns (mma.sync kernel) / the 8 head rows of Q8 and P (tcgen05 kernel)."""
@@ -134,7 +135,7 @@ def test_attention_every_group_size(G, opts):
     compare_attention(out, oracle.attention_fp8(slab, dims_of(pool), 0, Hq, lists, lens, bits_of(q)))
 
 
-@pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=2, items_per_slot=1024), dict(tma=1), dict(tc=1),
+@pytest.mark.parametrize("opts", [dict(tc=0), dict(tc=0, min_chunk_blocks=2, items_per_slot=1024), dict(tc=0, tma=1), dict(tc=1),
                                   dict(tc=1, min_chunk_blocks=2, items_per_slot=1024)])
 def test_attention_wide_dynamic_range(opts):
     """Row magnitudes from e^-6 to e^6 in K and V, scaled-up queries, a zero row and an outlier element."""
@@ -213,8 +214,8 @@ def test_gather_fp8_returns_stored_codes_and_scales(Hkv, d):
     assert np.array_equal(pool_bytes(pool), before)
 
 
-@pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(min_chunk_blocks=3, items_per_slot=2),
-                                  dict(tma=1), dict(tma=1, min_chunk_blocks=1, items_per_slot=1024),
+@pytest.mark.parametrize("opts", [dict(), dict(tc=0), dict(tc=0, min_chunk_blocks=1, items_per_slot=1024), dict(tc=0, min_chunk_blocks=3, items_per_slot=2),
+                                  dict(tc=0, tma=1), dict(tc=0, tma=1, min_chunk_blocks=1, items_per_slot=1024),
                                   dict(tc=1), dict(tc=1, min_chunk_blocks=1, items_per_slot=1024), dict(tc=1, min_chunk_blocks=9, items_per_slot=2)])
 @pytest.mark.parametrize("Hq,Hkv,d", [(32, 8, 128), (8, 2, 64), (32, 32, 128)])
 def test_fused_decode_step_quantises_like_ingest(Hq, Hkv, d, opts):

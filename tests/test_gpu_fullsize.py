@@ -180,17 +180,19 @@ def test_cfg5_stress_full():
 
 
 def test_cfg3_8b_gqa_full_fp8_pool():
+    """FP8 pool, default kernel = attn_tc_kernel (tcgen05 / TMEM / TMA): 32 PDL-chained launches per step, fused append,
+    concurrent ingest."""
     run_config("cfg3_8b_gqa", n_short=12, n_long=6, kv_dtype=B.KV_DTYPE_FP8_E4M3)
 
 
-def test_cfg3_8b_gqa_full_fp8_pool_tcgen05():
-    """The same through attn_tc_kernel (option tc=1): 32 PDL-chained launches per step, fused append, concurrent ingest."""
-    run_config("cfg3_8b_gqa", n_short=12, n_long=6, kv_dtype=B.KV_DTYPE_FP8_E4M3, options=dict(tc=1))
+def test_cfg3_8b_gqa_full_fp8_pool_mma_sync():
+    """The same through attn_kernel<Fp8Tiles<128>> (option tc=0)."""
+    run_config("cfg3_8b_gqa", n_short=12, n_long=6, kv_dtype=B.KV_DTYPE_FP8_E4M3, options=dict(tc=0))
 
 
-def test_cfg2_7b_mha_full_fp8_pool_tcgen05():
-    """G = 1, 32 kv heads, every unit owns its request's last block (fused append in every unit)."""
-    run_config("cfg2_7b_mha", n_short=8, n_long=8, kv_dtype=B.KV_DTYPE_FP8_E4M3, options=dict(tc=1))
+def test_cfg2_7b_mha_full_fp8_pool():
+    """G = 1, 32 kv heads, every unit owns its request's last block (fused append in every unit); tcgen05 kernel."""
+    run_config("cfg2_7b_mha", n_short=8, n_long=8, kv_dtype=B.KV_DTYPE_FP8_E4M3)
 
 
 def test_cfg2_7b_mha_full_unfused():

@@ -161,7 +161,8 @@ def test_transfer_fp8_codes_and_scales_verbatim(Hq, Hkv, d):
 # ---------------------------------------------------------------------------------------------
 
 @pytest.mark.parametrize("fp8", [False, True])
-@pytest.mark.parametrize("opts", [dict(), dict(pdl=0), dict(min_chunk_blocks=1, items_per_slot=1024), dict(fuse_combine=0), dict(tc=1)])
+@pytest.mark.parametrize("opts", [dict(), dict(pdl=0), dict(min_chunk_blocks=1, items_per_slot=1024), dict(fuse_combine=0), dict(tc=0),
+                                  dict(tc=0, min_chunk_blocks=1, items_per_slot=1024)])
 def test_step_layers_equals_per_layer_calls_and_oracle(opts, fp8):
     L, Hq, Hkv, d = 4, 32, 8, 128
     lens0 = [15, 16, 17, 1, 0, 31, 255, 1039, 2047, 700]
