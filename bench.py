@@ -356,6 +356,7 @@ def measure(args, rep, sampler, wname: str, K: int, Wm: int, headline: bool):
     barrier()
     pool.profile_reset()
     launches0 = pool.launches
+    tc0 = pool.counter("attn_tc_launches")
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     wall0 = time.time()
@@ -371,6 +372,7 @@ def measure(args, rep, sampler, wname: str, K: int, Wm: int, headline: bool):
         sampler.window(wall0, wall1, wname)
     ms = max_over_ranks(ev0.elapsed_time(ev1))
     launches = pool.launches - launches0
+    ran_tc = pool.counter("attn_tc_launches") - tc0 > 0        # FP8, head_dim 128: the pool picks the kernel per batch (option tc)
     prof = pool.profile()
     by = loop.bytes_of_steps(first, first + K)
     total_bytes = sum_over_ranks(float(by["attn"] + by["append"] + by["ingest"]))
@@ -385,7 +387,7 @@ def measure(args, rep, sampler, wname: str, K: int, Wm: int, headline: bool):
     achieved = attn_bytes_per_launch / (attn_ms / max(attn_n, 1) * 1e-3) / 1e9 if attn_ms > 0 else None
     tp = ("Fp8Tiles" if fp8 else "Bf16Tiles") + f"<{w.head_dim}{', tma' if opts.get('tma') else ''}>"
     attn_kernel = f"attn_kernel<{tp}, append={0 if args.unfused else 1}>"
-    if fp8 and opts.get("tc", 1) and w.head_dim == 128:
+    if ran_tc:
         attn_kernel = f"attn_tc_kernel<append={0 if args.unfused else 1}> (tcgen05 / TMEM / TMA)"
     roofline = {"kernel": attn_kernel, "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak if achieved else None, "peak_source": peak_src,
@@ -395,7 +397,7 @@ def measure(args, rep, sampler, wname: str, K: int, Wm: int, headline: bool):
                           "back-to-back layer launches of the timed region (kv_profile_read); duration / launches",
                 "algorithmic_bytes_per_launch": attn_bytes_per_launch, "traffic": None}
     traffic, traffic_path = load_traffic()
-    ent = traffic.get(wname, {}).get("fp8_tc" if (fp8 and opts.get("tc", 1) and w.head_dim == 128) else args.kv_dtype)
+    ent = traffic.get(wname, {}).get("fp8_tc" if ran_tc else args.kv_dtype)
     if ent:
         roofline.update({"traffic": attn_bytes_per_launch * ent["dram_bytes_per_algorithmic_byte"],
                          "traffic_source": f"modelled: {traffic_path} ({ent['source']}): DRAM read+write bytes of one ncu --set full "

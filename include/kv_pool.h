@@ -452,12 +452,13 @@ int32_t kv_profile_reset(kv_pool_t* pool);
  * 2 / 3 CTAs per SM), "pdl" (1, default: attention launches carry the programmatic-dependent-launch attribute;
  * 0: plain launches), "tma" (0, default; 1: pools with head_dim 128 fetch full KV tiles with one
  * cp.async.bulk.tensor per tile (FP8: plus one bulk copy of the tile's scales) instead of 16-byte cp.async — the
- * measured alternative of DESIGN.md §5; KV_ERR_UNSUPPORTED for head_dim 64), "tc" (1, default on FP8 pools with
- * head_dim 128: decode attention (paged_decode_attention / _step / _step_layers) runs on the tcgen05 tensor cores —
- * attn_tc_kernel: 128-token tiles staged by TMA, e4m3 operands fed to tcgen05.mma straight from shared memory,
- * accumulators in TMEM; 0: the mma.sync kernel, which also serves paged_varlen_attention, head_dim 64 and bf16 pools
- * whatever the option says; same results within the stated tolerance, same bytes appended; setting 1 on a pool that
- * cannot run it => KV_ERR_UNSUPPORTED), "side_upload" (1, default: plan uploads run on a stream the pool owns, beside whatever the
+ * measured alternative of DESIGN.md §5; KV_ERR_UNSUPPORTED for head_dim 64), "tc" (FP8 pools with head_dim 128: which kernel runs
+ * decode attention (paged_decode_attention / _step / _step_layers).  1: attn_tc_kernel on the tcgen05 tensor cores —
+ * 128-token tiles staged by TMA, e4m3 operands fed to tcgen05.mma straight from shared memory, accumulators in TMEM;
+ * 0: the mma.sync kernel, which also serves paged_varlen_attention, head_dim 64 and bf16 pools whatever the option says;
+ * 2 (default): attn_tc_kernel unless more than half of the batch's requests are at most 256 tokens long (it runs one
+ * work unit per CTA at a time and pays a pipeline fill per unit; counter "attn_tc_launches" says what ran).  Same
+ * results within the stated tolerance, same bytes appended; 1 on a pool that cannot run it => KV_ERR_UNSUPPORTED), "side_upload" (1, default: plan uploads run on a stream the pool owns, beside whatever the
  * caller's stream is executing, and the caller's stream waits for them by event; 0: uploads on the caller's stream), "host_zero_copy" (1, default: see kv_ingest_host), "profile" (0/1, see kv_profile_read);
  * KV-head sharding of a TP-sharded D-instance: "src_kv_heads" = H (0 = off) then
  * "src_head_begin" = h0 declare that the contiguous side of kv_ingest(_host) / kv_gather is the FULL-width tensor

@@ -222,12 +222,13 @@ struct kv_pool {
   bool stage_busy = false;
   bool tma = false;               // bf16 pools, head_dim 128: full tiles by cp.async.bulk.tensor (UTMALDG) instead of LDGSTS
   bool tmap_ok = false;
-  bool tc = true;                 // FP8 pools, head_dim 128: decode attention on tcgen05 / TMEM (attn_tc_kernel); 0: mma.sync kernel
+  int32_t tc = 2;                 // FP8 pools, head_dim 128: decode attention on tcgen05 / TMEM (attn_tc_kernel): 0 never (mma.sync
+                                  //   kernel), 1 always, 2 (default) unless most of the batch's requests are one or two tiles long
   bool tmap16_ok = false;
   alignas(64) CUtensorMap tmap16; // the same region, box 16 rows: the K codes or the V codes of one (block, kv head) tile
   alignas(64) CUtensorMap tmap;   // the KV region as [rows][128 B], box 64 rows, 128-byte swizzle
   // event counters (kv_pool_counter)
-  int64_t n_zero_copy = 0, n_staged = 0, n_chained = 0, n_stream_switch = 0, n_plans = 0;
+  int64_t n_zero_copy = 0, n_staged = 0, n_chained = 0, n_stream_switch = 0, n_plans = 0, n_tc_launches = 0;
   bool host_zero_copy = true;     // kv_ingest_host reads device-addressable pinned sources in place (no staging pass)
   bool profile = false;
   ProfRing prof[KV_KERNEL_KINDS];
@@ -241,6 +242,7 @@ struct kv_pool {
   int plan_slot = -1;
   int32_t plan_n_items = 0, plan_n_combines = 0;
   int32_t plan_kind = 0;        // 0: decode plan, 1: variable-q plan (48-byte items)
+  bool plan_tc = false;         // the decode plan was sized for (and runs on) attn_tc_kernel
   std::vector<int32_t> plan_qlens;
   std::vector<kvp::HostState::QueryTile> plan_tiles;
   int32_t plan_append_ok = -1;  // -1 unknown, 0 / 1: every request's last reservation is one token
@@ -261,11 +263,24 @@ struct kv_pool {
   }
   bool fp8() const { return hs.cfg.kv_dtype == KV_DTYPE_FP8_E4M3; }
   int32_t kernel_ctas() const { return fp8() ? 3 : (ring == 2 ? 3 : 2); }
-  bool tc_decode() const { return tc && tmap16_ok; }
+  bool tc_capable() const { return tc != 0 && tmap16_ok; }
+  // tcgen05 kernel for this decode batch?  It runs ONE unit at a time per CTA (two per SM): a batch made mostly of requests
+  // of one or two 128-token tiles (config 5: 80 % of the requests, 3280 of 4392 units) is better served by the mma.sync
+  // kernel's twelve independent warps per SM (measured: 1.02 vs 0.995 of the copy ceiling there; 1.05 vs 1.07 on config 4)
+  bool tc_for(int32_t batch, const int64_t* req_ids) const {
+    if (!tc_capable()) return false;
+    if (tc == 1) return true;
+    int32_t small = 0;
+    for (int32_t i = 0; i < batch; ++i) {
+      auto it = hs.reqs.find(req_ids[i]);
+      if (it != hs.reqs.end() && it->second.len <= 2 * kvp::kTcTileTokens) ++small;
+    }
+    return 2 * small <= batch;
+  }
   // work units the attention kernel of a decode (or variable-q) launch processes at a time: resident warps of the
   // mma.sync kernels, resident CTAs of the tcgen05 kernel
-  int32_t slots(bool varq = false) const {
-    if (!varq && tc_decode()) return num_sms * (ctas_per_sm > 0 ? ctas_per_sm : 2);
+  int32_t slots(bool varq = false, bool use_tc = false) const {
+    if (!varq && use_tc) return num_sms * (ctas_per_sm > 0 ? ctas_per_sm : 2);
     return num_sms * (ctas_per_sm > 0 ? ctas_per_sm : kernel_ctas()) * kvp::kAttnWarps;
   }
   int32_t src_heads() const { return src_kv_heads > 0 ? src_kv_heads : hs.cfg.num_kv_heads; }
@@ -452,9 +467,9 @@ AttnVariant variant_of(bool append, bool varq) {
   if (varq) return variant<TP, false, true, R, kCtas>();
   return append ? variant<TP, true, false, R, kCtas>() : variant<TP, false, false, R, kCtas>();
 }
-AttnVariant pick_variant(const kv_pool* pool, bool append, bool varq) {
+AttnVariant pick_variant(const kv_pool* pool, bool append, bool varq, bool use_tc = false) {
   const bool d128 = pool->hs.cfg.head_dim == 128;
-  if (!varq && pool->tc_decode())
+  if (!varq && use_tc)
     return {append ? attn_tc_kernel<true> : attn_tc_kernel<false>, kTcSmemBytes, 2, kTcThreads, 1};
   if (pool->fp8() && pool->tma && pool->tmap_ok && d128) return variant_of<Fp8Tiles<128, true>, kFp8RingSlots, 3>(append, varq);
   if (pool->fp8())
@@ -795,7 +810,8 @@ int32_t kv_plan_decode(kv_pool_t* pool, int32_t batch, const int64_t* req_ids, i
                        int32_t* out_n_items, int32_t* out_chunk_blocks) {
   if (!pool || cap_items < 0 || (cap_items > 0 && !out_items)) return KV_ERR_INVALID;
   DecodePlan plan;
-  int32_t rc = pool->hs.plan_decode(batch, req_ids, pool->slots(), pool->ips(), pool->min_chunk(),
+  const bool use_tc = req_ids && batch > 0 && pool->tc_for(batch, req_ids);
+  int32_t rc = pool->hs.plan_decode(batch, req_ids, pool->slots(false, use_tc), pool->ips(), pool->min_chunk(),
                                     kMaxPartials, &plan);
   if (rc != KV_OK) return rc;
   const int32_t Hkv = pool->hs.cfg.num_kv_heads;
@@ -878,7 +894,8 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer_begin, int32_t la
                       static_cast<int32_t>(pool->plan_ids.size()) == batch &&
                       std::memcmp(pool->plan_ids.data(), req_ids, sizeof(int64_t) * static_cast<size_t>(batch)) == 0;
   if (!cached) {
-    int32_t rc = pool->hs.plan_decode(batch, req_ids, pool->slots(), pool->ips(), pool->min_chunk(),
+    pool->plan_tc = pool->tc_for(batch, req_ids);
+    int32_t rc = pool->hs.plan_decode(batch, req_ids, pool->slots(false, pool->plan_tc), pool->ips(), pool->min_chunk(),
                                       kMaxPartials, &pool->plan);
     pool->plan_slot = -1;   // pool->plan no longer is what is staged
     if (rc != KV_OK) return fail(rc);
@@ -919,14 +936,14 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer_begin, int32_t la
   StageSlot& s = pool->plan_ring[pool->plan_slot];
   const int32_t G = c.num_q_heads / c.num_kv_heads;
   const int kind = k_new ? 1 : 0;
-  const AttnVariant v = pick_variant(pool, k_new != nullptr, false);
+  const AttnVariant v = pick_variant(pool, k_new != nullptr, false, pool->plan_tc);
   const bool separate_combine = pool->plan_n_combines > 0 && !pool->fuse_combine;
   // From here on kernels are enqueued: an error is a CUDA error and leaves the stream in an undefined state
   // (KV_ERR_CUDA is sticky); the reservation stays, as the launches already issued refer to it.
   if (pool->profile) KV_CUDA(pool, pool->prof[KV_KERNEL_ATTN].begin(stream));
   for (int32_t ll = 0; ll < layer_count; ++ll) {
     AttnParams p = attn_params(pool, layer_begin + ll, static_cast<const char*>(q) + ll * q_stride,
-                               static_cast<char*>(out) + ll * q_stride, sm_scale, s, pool->tc_decode());
+                               static_cast<char*>(out) + ll * q_stride, sm_scale, s, pool->plan_tc);
     if (k_new) {
       p.k_new = reinterpret_cast<const uint16_t*>(static_cast<const char*>(k_new) + ll * kv_stride);
       p.v_new = reinterpret_cast<const uint16_t*>(static_cast<const char*>(v_new) + ll * kv_stride);
@@ -937,6 +954,7 @@ static int32_t launch_attention(kv_pool_t* pool, int32_t layer_begin, int32_t la
     pool->n_chained += p.chained;
     KV_CUDA(pool, launch_attn_kernel(pool, v, p, stream));
     ++pool->launches;
+    pool->n_tc_launches += pool->plan_tc ? 1 : 0;
     pool->chain_slot = separate_combine ? -1 : pool->plan_slot;
     pool->chain_kind = kind;
     if (separate_combine) {
@@ -1242,6 +1260,7 @@ int64_t kv_pool_counter(const kv_pool_t* pool, const char* name) {
   if (!std::strcmp(name, "attn_stream_switches")) return pool->n_stream_switch;
   if (!std::strcmp(name, "host_ingest_zero_copy")) return pool->n_zero_copy;
   if (!std::strcmp(name, "host_ingest_staged")) return pool->n_staged;
+  if (!std::strcmp(name, "attn_tc_launches")) return pool->n_tc_launches;
   return KV_ERR_INVALID;
 }
 
@@ -1256,9 +1275,9 @@ int32_t kv_pool_set_option(kv_pool_t* pool, const char* key, int64_t value) {
   if (!std::strcmp(key, "fuse_combine") && (value == 0 || value == 1)) { pool->fuse_combine = value != 0; return KV_OK; }
   if (!std::strcmp(key, "pdl") && (value == 0 || value == 1)) { pool->pdl = value != 0; return KV_OK; }
   if (!std::strcmp(key, "side_upload") && (value == 0 || value == 1)) { pool->side_upload = value != 0; return KV_OK; }
-  if (!std::strcmp(key, "tc") && (value == 0 || value == 1)) {   // FP8, head_dim 128 pools with a device slab only
+  if (!std::strcmp(key, "tc") && value >= 0 && value <= 2) {   // FP8, head_dim 128 pools with a device slab only
     if (value == 1 && !pool->tmap16_ok) return KV_ERR_UNSUPPORTED;
-    pool->tc = value != 0;
+    pool->tc = static_cast<int32_t>(value);
     pool->plan_slot = -1;                                         // the planner sizes chunks for the kernel that runs
     return KV_OK;
   }

@@ -111,6 +111,28 @@ def test_attention_matches_oracle(Hq, Hkv, d, opts):
     assert np.abs(want - exact).max() < 0.15 and np.abs(want - exact).mean() < 0.01
 
 
+def test_default_picks_the_kernel_per_batch():
+    """Option tc = 2 (default): attn_tc_kernel unless most of the batch's requests are one or two tiles long."""
+    Hq, Hkv, d = 32, 8, 128
+    lens = [40, 100, 200, 3000, 5000, 700, 33, 256]
+    ids = list(range(len(lens)))
+    pool = make_fp8_pool(1, Hq, Hkv, d, sum((n + 15) // 16 for n in lens) + 4, max_len=8192)
+    w = W.Workload("fp8a", 1, Hq, Hkv, d, len(lens), None, 321, max_len=8192)
+    srcs = [kv_src(w, uid, 0, n, DEV) for uid, n in zip(ids, lens)]
+    pool.ingest(ids, [s[0] for s in srcs], [s[1] for s in srcs])
+    slab = oracle.new_slab_fp8(dims_of(pool), SENT)
+    for uid, n, (k, v) in zip(ids, lens, srcs):
+        oracle.scatter_fp8(slab, dims_of(pool), pool.block_table(uid)[0], 0, bits_of(k), bits_of(v))
+    q = W.q_values(w.seed, 1, 0, len(lens), Hq, d, DEV)
+    for sel, want_tc in (([0, 1, 2, 3, 6, 7], False), ([3, 4, 5, 0], True), (list(range(8)), False), ([3, 4, 5, 0, 1, 2], True)):
+        before = pool.counter("attn_tc_launches")
+        out = pool.attention(0, [ids[i] for i in sel], q[sel].contiguous())
+        torch.cuda.synchronize()
+        assert (pool.counter("attn_tc_launches") - before == 1) == want_tc, sel
+        lists = [pool.block_table(ids[i])[0] for i in sel]
+        compare_attention(out, oracle.attention_fp8(slab, dims_of(pool), 0, Hq, lists, [lens[i] for i in sel], bits_of(q[sel].contiguous())))
+
+
 @pytest.mark.parametrize("opts", [dict(tc=0), dict(tc=1), dict(tc=1, min_chunk_blocks=9, items_per_slot=1024)])
 @pytest.mark.parametrize("G", [2, 3, 5, 6, 7])
 def test_attention_every_group_size(G, opts):
