@@ -54,7 +54,11 @@ def parse_args():
     ap.add_argument("--no-per-config", action="store_true", help="headline workload only")
     ap.add_argument("--per-layer-calls", action="store_true",
                     help="one paged_decode_step call per layer instead of one paged_decode_step_layers call per step")
-    ap.add_argument("--streams", type=int, default=2, help="2: ingest on its own stream, overlapping attention")
+    ap.add_argument("--streams", type=int, default=0,
+                    help="2: the arrivals' ingest on its own stream, beside attention; 1: in line on the decode stream; 0 (default): "
+                         "2 on bf16 pools; on FP8 pools device-resident arrivals in line, host-resident ones on the second stream (measured: beside the issue-bound FP8 kernels the overlapped ingest "
+                         "starves and the step waits for it: config 3 0.948 -> 0.970, config 5 0.975 -> 1.021 of the copy ceiling "
+                         "in line; bf16: 1.043 vs 1.039 overlapped)")
     ap.add_argument("--e2e-steps", type=int, default=4, help="timed steps of the host-buffer leg (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-isolated", action="store_true", help="skip the attention-alone / ingest-alone legs")
@@ -332,7 +336,9 @@ def measure(args, rep, sampler, wname: str, K: int, Wm: int, headline: bool):
     fp8 = args.kv_dtype == "fp8"
     kvd = B.KV_DTYPE_FP8_E4M3 if fp8 else B.KV_DTYPE_BF16
     t_setup = time.time()
-    loop = DecodeLoop(w, (0 if exact else Wm) + K, n_host_steps=e2e_w + e2e_steps, device=dev, streams=args.streams,
+    streams = args.streams if args.streams > 0 else 2
+    inline = args.streams == 0 and fp8
+    loop = DecodeLoop(w, (0 if exact else Wm) + K, n_host_steps=e2e_w + e2e_steps, device=dev, streams=streams, inline_ingest=inline,
                       salt=rep.salt, options=opts, fused=not args.unfused, kv_dtype=kvd, layered=not args.per_layer_calls)
     t_setup = time.time() - t_setup
     pool, A = loop.pool, loop.sA
@@ -476,7 +482,9 @@ def measure(args, rep, sampler, wname: str, K: int, Wm: int, headline: bool):
         "value": value, "unit": "GB/s", "steps": K, "warmup": Wm, "ms_per_step": ms / K,
         "config": {"workload": wname, "kv_dtype": args.kv_dtype, "layers": w.num_layers, "q_heads": w.num_q_heads,
                    "kv_heads": w.num_kv_heads, "head_dim": w.head_dim, "block_size": w.block_size,
-                   "batch": w.batch, "ingest_per_step": w.ingest_per_step, "streams": 2 if loop.two_streams else 1,
+                   "batch": w.batch, "ingest_per_step": w.ingest_per_step,
+                   "streams": ("2 (device-resident arrivals ingested in line on the decode stream)" if loop.inline_ingest
+                               else 2 if loop.two_streams else 1),
                    "decode_call": ("paged_decode_step_layers (a1 + per layer fused a3+a4+a5, PDL-chained launches)" if loop.layered
                                    else "paged_decode_step (fused a3+a4+a5)" if loop.fused else "kv_ingest + paged_decode_attention"),
                    "pool_blocks": loop.cfg.num_blocks, "pool_gb": pool.kv_bytes / 1e9,

@@ -151,7 +151,8 @@ class DecodeLoop:
 
     def __init__(self, w: W.Workload, n_steps: int, n_host_steps: int = 0, device="cuda:0", streams: int = 2,
                  salt: int = 0, bank_bytes: int = 24 << 30, profile: bool = True, options: dict | None = None,
-                 sentinel: int | None = None, fused: bool = True, kv_dtype: int = B.KV_DTYPE_BF16, layered: bool = True):
+                 sentinel: int | None = None, fused: bool = True, kv_dtype: int = B.KV_DTYPE_BF16, layered: bool = True,
+                 inline_ingest: bool = False):
         """Steps [0, n_steps) take their inputs from device memory; steps [n_steps, n_steps + n_host_steps)
         take them from pinned host memory through the *_host entry points."""
         self.fp8 = kv_dtype == B.KV_DTYPE_FP8_E4M3
@@ -159,6 +160,9 @@ class DecodeLoop:
         self.layered = layered and fused
         self.host_from, self.n_steps = n_steps, n_steps + n_host_steps
         self.two_streams = streams >= 2 and w.ingest_per_step > 0
+        # device-resident arrivals ingested in line on the decode stream (host-resident ones stay on stream B: their copy
+        # is PCIe-bound and overlaps for free).  Worth it on FP8 pools, see bench.py --streams
+        self.inline_ingest = inline_ingest and self.two_streams
         L, Hkv, Hq, d, k = w.num_layers, w.num_kv_heads, w.num_q_heads, w.head_dim, w.ingest_per_step
         self.tok_bytes = L * Hkv * d * 2                      # one tensor (K or V), one token, all layers
         mean_len = float(np.mean(w.draw_lengths(n=4096, salt=900)))
@@ -319,12 +323,13 @@ class DecodeLoop:
         L = self.w.num_layers
         if sp.retire.size:
             B.kv_free(h, sp.retire)                                     # a6 (host)
-        if sp.arrive.size:                                               # a1 + a2 on stream B
-            if self.two_streams and s > 0:
-                Bs.wait_event(self.evA[(s - 1) % 4])                     # recycled blocks were read by step s-1
-            self._ingest_arrivals(sp, Bs, host)
+        if sp.arrive.size:                                               # a1 + a2 on stream B (or in line on A)
+            S = A if (self.inline_ingest and not host) else Bs
+            if self.two_streams and s > 0 and S is not A:
+                S.wait_event(self.evA[(s - 1) % 4])                      # recycled blocks were read by step s-1
+            self._ingest_arrivals(sp, S, host)
             if self.two_streams:
-                self.evB[s % 4].record(Bs)
+                self.evB[s % 4].record(S)
         if self.two_streams and s > 0:
             A.wait_event(self.evB[(s - 1) % 4])                          # joiners of this step were ingested at s-1
         kn, vn, q, out = self.k_new[s], self.v_new[s], self.q[s], self.out[s]
