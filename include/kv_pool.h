@@ -73,6 +73,8 @@ extern "C" {
 #define KV_ERR_CUDA               -6  /* a CUDA runtime call failed; see kv_last_cuda_error  */
 #define KV_ERR_NO_DEVICE          -7  /* pool was created without a device slab (host-only)  */
 #define KV_ERR_UNSUPPORTED        -8  /* call not available for this pool's kv_dtype         */
+#define KV_ERR_SCRATCH_LIMIT      -9  /* paged_decode_attention_static: the plan needs more split-KV
+                                         partial slots than KV_STATIC_MAX_PARTIALS; nothing changed */
 
 /* ---- KV element types ---------------------------------------------------------------- */
 #define KV_DTYPE_BF16              0  /* bf16 pool (the BASELINE.json configs)               */
@@ -235,6 +237,31 @@ int32_t paged_decode_step_layers(kv_pool_t* pool, int32_t layer_begin, int32_t l
                                  const void* k_new /*device or NULL*/, const void* v_new /*device or NULL*/,
                                  void* out /*device*/, int64_t q_layer_stride_bytes, int64_t kv_layer_stride_bytes,
                                  float sm_scale, int32_t flags, void* cuda_stream);
+
+/*
+ * a4 + a5 for callers that must not allocate — code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc.  Same operation, arguments, result and errors as paged_decode_attention (Eq. 1 in
+ * the decode form of PAPER.md:200/:219; same plan, same kernel, same merge), but the split-KV workspace — arrival
+ * counters and the (m, l, O) partials — is NOT taken from the pool's slab: it lives in a file-scope
+ * `static __device__` array of the library, KV_STATIC_MAX_PARTIALS partial slots at the widest geometry
+ * (G = 8, head_dim 128), kv_static_scratch_bytes() = 17 055 744 bytes (16.3 MiB), which every GPU that loads the
+ * library holds until the process exits.  The call itself performs no cudaMalloc, no cudaFree and no allocating
+ * library routine: it looks the array's device address up once per device (cudaGetSymbolAddress, with the pool's
+ * device current), stages the plan through the pinned slots kv_pool_create set up, clears the arrival counters it
+ * is going to use (cudaMemsetAsync on `cuda_stream`; the array keeps the last call's contents) and launches.
+ *   Limit: a batch whose split-KV plan needs more than KV_STATIC_MAX_PARTIALS partial slots (one per (split request,
+ *   kv head, chunk); kv_plan_decode shows the plan) => KV_ERR_SCRATCH_LIMIT, nothing changed.  Larger
+ *   "min_chunk_blocks" / smaller "items_per_slot" options shrink the count; paged_decode_attention has no such limit.
+ *   Sharing: ALL calls of ALL pools on a device share the one array.  Calls that may overlap on the GPU (different
+ *   streams without an ordering between them, or two pools driven from two threads) race on it and return garbage;
+ *   the caller orders them.  Calls on one stream are ordered by the stream.  Relative to the pool's other attention
+ *   calls the one-attention-stream rule above applies unchanged.
+ */
+#define KV_STATIC_MAX_PARTIALS 4096
+int64_t kv_static_scratch_bytes(void);
+int32_t paged_decode_attention_static(kv_pool_t* pool, int32_t layer, int32_t batch,
+                                      const int64_t* req_ids /*host*/, const void* q /*device*/,
+                                      void* out /*device*/, float sm_scale, void* cuda_stream);
 
 /*
  * NEXT-1 — variable-q-length causal paged attention: in-place prefill of ultra-short requests

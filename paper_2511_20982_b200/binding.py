@@ -32,6 +32,8 @@ lib = ctypes.CDLL(lib_path)
 KV_OK = 0
 KV_ERR_INVALID, KV_ERR_NO_BLOCKS, KV_ERR_UNKNOWN_REQUEST, KV_ERR_TOO_LONG = -1, -2, -3, -4
 KV_ERR_TOO_MANY_REQUESTS, KV_ERR_CUDA, KV_ERR_NO_DEVICE, KV_ERR_UNSUPPORTED = -5, -6, -7, -8
+KV_ERR_SCRATCH_LIMIT = -9
+KV_STATIC_MAX_PARTIALS = 4096
 KV_DTYPE_BF16, KV_DTYPE_FP8_E4M3 = 0, 1
 
 
@@ -56,6 +58,8 @@ _SIGS = {
     "kv_reserve": (_i32, [_P, _i32, _P, _P]),
     "kv_ingest": (_i32, [_P, _i32, _P, _P, _P, _P, _i32, _i32, _P]),
     "paged_decode_attention": (_i32, [_P, _i32, _i32, _P, _P, _P, ctypes.c_float, _P]),
+    "paged_decode_attention_static": (_i32, [_P, _i32, _i32, _P, _P, _P, ctypes.c_float, _P]),
+    "kv_static_scratch_bytes": (_i64, []),
     "paged_decode_step": (_i32, [_P, _i32, _i32, _P, _P, _P, _P, _P, ctypes.c_float, _P]),
     "paged_decode_step_host": (_i32, [_P, _i32, _i32, _P, _P, _P, _P, _P, ctypes.c_float, _P, _i64, _P]),
     "paged_decode_step_layers": (_i32, [_P, _i32, _i32, _i32, _P, _P, _P, _P, _P, _i64, _i64, ctypes.c_float, _i32, _P]),
@@ -191,6 +195,18 @@ def paged_decode_attention(handle: int, layer: int, req_ids, q_ptr: int, out_ptr
     ids = _ids(req_ids)
     _check(lib.paged_decode_attention(handle, layer, ids.size, _np(ids), q_ptr, out_ptr, sm_scale, stream or None),
            "paged_decode_attention")
+
+
+def paged_decode_attention_static(handle: int, layer: int, req_ids, q_ptr: int, out_ptr: int, sm_scale: float = 0.0,
+                                  stream: int = 0) -> None:
+    """paged_decode_attention with its split-KV workspace in the library's static device array (allocates nothing)."""
+    ids = _ids(req_ids)
+    _check(lib.paged_decode_attention_static(handle, layer, ids.size, _np(ids), q_ptr, out_ptr, sm_scale,
+                                             stream or None), "paged_decode_attention_static")
+
+
+def kv_static_scratch_bytes() -> int:
+    return int(lib.kv_static_scratch_bytes())
 
 
 def paged_decode_step(handle: int, layer: int, req_ids, q_ptr: int, k_new_ptr: int, v_new_ptr: int, out_ptr: int,
@@ -422,6 +438,19 @@ class KVPool:
         if out is None:
             out = torch.empty_like(q)
         paged_decode_attention(self.handle, layer, req_ids, q.data_ptr(), out.data_ptr(), sm_scale, self._stream(stream))
+        return out
+
+    def decode_attention_static(self, layer, req_ids, q, out=None, sm_scale=0.0, stream=None):
+        """decode_attention through paged_decode_attention_static: split-KV workspace in the library's static
+        device array, no allocation inside the call (``out`` given).  KV_ERR_SCRATCH_LIMIT beyond
+        KV_STATIC_MAX_PARTIALS partial slots."""
+        import torch
+
+        assert q.is_contiguous() and q.dtype == torch.bfloat16
+        if out is None:
+            out = torch.empty_like(q)
+        paged_decode_attention_static(self.handle, layer, req_ids, q.data_ptr(), out.data_ptr(), sm_scale,
+                                      self._stream(stream))
         return out
 
     def decode_step(self, layer, req_ids, q, k_new, v_new, out=None, sm_scale=0.0, stream=None):

@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstring>
 #include <deque>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -31,6 +32,41 @@ static_assert(sizeof(CUtensorMap) == 128, "AttnParams::tmap carries a CUtensorMa
 static_assert(48 + 8LL * kvp::kMaxBlocksPerRequest <= kIngestBlobBytes, "a request's descriptor must fit one blob");
 
 inline int64_t align_up(int64_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+// ---- static scratch of paged_decode_attention_static (the entry point that allocates nothing) -------------------
+// Split-KV workspace for at most KV_STATIC_MAX_PARTIALS partial slots at the widest geometry (G = 8, head_dim 128):
+//     arrive  int32 [P]            chunks finished per split (request, kv head) — must be zero when a launch starts
+//     part_ml float [P][8][2]      (m, l) of a partial
+//     part_o  float [P][8][128]    un-normalised partial outputs
+// One array per device that loads the library, held until the process exits; shared by every pool and every call.
+constexpr int64_t kStaticArriveBytes = static_cast<int64_t>(KV_STATIC_MAX_PARTIALS) * 4;
+constexpr int64_t kStaticMlBytes = static_cast<int64_t>(KV_STATIC_MAX_PARTIALS) * 8 * 2 * 4;
+constexpr int64_t kStaticOBytes = static_cast<int64_t>(KV_STATIC_MAX_PARTIALS) * 8 * 128 * 4;
+constexpr int64_t kStaticScratchBytes = kStaticArriveBytes + kStaticMlBytes + kStaticOBytes;
+static_assert(kStaticArriveBytes % kAlign == 0 && kStaticMlBytes % kAlign == 0, "sections stay 256-byte aligned");
+}  // namespace
+
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+namespace {
+// Device address of g_static_scratch on `device`, which must be current.  In host code the array's name is only a
+// handle for the runtime, not an address a kernel can use: the address is looked up once per device and cached.
+constexpr int kMaxStaticDevices = 64;
+cudaError_t static_scratch_address(int device, unsigned char** out) {
+  static std::mutex mu;
+  static unsigned char* ptrs[kMaxStaticDevices] = {};
+  if (device < 0 || device >= kMaxStaticDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!ptrs[device]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    ptrs[device] = static_cast<unsigned char*>(p);
+  }
+  *out = ptrs[device];
+  return cudaSuccess;
+}
 
 struct Layout {  // byte offsets inside the caller's slab
   int64_t kv_bytes, block_table, counters, arrive, ingest_blobs, plan_blobs, part_o, part_ml, total;
@@ -1006,6 +1042,84 @@ int32_t paged_decode_step_layers(kv_pool_t* pool, int32_t layer_begin, int32_t l
                           kv_layer_stride_bytes, sm_scale, (flags & KV_STEP_RESERVE) != 0, cuda_stream);
 }
 
+// a4 + a5 with the split-KV workspace in g_static_scratch: no cudaMalloc / cudaFree / allocating library call on this
+// path (the plan goes through the staging slots kv_pool_create set up).  Same plan, same kernel and same merge as
+// paged_decode_attention, so the same result; not profiled, not chained to its neighbours.
+int64_t kv_static_scratch_bytes(void) { return kStaticScratchBytes; }
+
+int32_t paged_decode_attention_static(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const void* q,
+                                      void* out, float sm_scale, void* cuda_stream) {
+  if (!pool || !req_ids || !q || !out || !aligned16(q) || !aligned16(out)) return KV_ERR_INVALID;
+  const kv_pool_config_t& c = pool->hs.cfg;
+  if (layer < 0 || layer >= c.num_layers || batch < 1) return KV_ERR_INVALID;
+  if (!pool->has_device) return KV_ERR_NO_DEVICE;
+  KV_ON_DEVICE(pool);
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  unsigned char* scratch = nullptr;
+  KV_CUDA(pool, static_scratch_address(pool->device, &scratch));   // set-up: once per device, pool's device current
+
+  const bool use_tc = pool->tc_for(batch, req_ids);
+  DecodePlan plan;
+  int32_t rc = pool->hs.plan_decode(batch, req_ids, pool->slots(false, use_tc), pool->ips(), pool->min_chunk(),
+                                    kMaxPartials, &plan);
+  if (rc != KV_OK) return rc;
+  if (plan.n_partials > KV_STATIC_MAX_PARTIALS) return KV_ERR_SCRATCH_LIMIT;
+  const size_t item_bytes = plan.items.size() * sizeof(WorkItem);
+  const size_t comb_bytes = plan.combines.size() * sizeof(CombineEntry);
+  if (static_cast<int64_t>(item_bytes + comb_bytes) > pool->lay.plan_blob_bytes) return KV_ERR_INVALID;
+  if (rc = order_attention(pool, stream); rc != KV_OK) return rc;
+
+  // the staged plan of the pool's other attention calls is dropped (they re-plan), this call stages its own
+  pool->plan_slot = -1;
+  pool->chain_slot = -1;
+  StageSlot* sp = nullptr;
+  const int idx = acquire(pool, pool->plan_ring, &pool->plan_next, &sp);
+  if (idx < 0) return idx;
+  StageSlot& s = *sp;
+  std::memcpy(s.host, plan.items.data(), item_bytes);
+  std::memcpy(s.host + item_bytes, plan.combines.data(), comb_bytes);
+  KV_CUDA(pool, upload_plan(pool, s, item_bytes + comb_bytes, stream));
+
+  AttnParams p = attn_params(pool, layer, q, out, sm_scale, s, use_tc);
+  p.n_items = static_cast<int32_t>(plan.items.size());
+  p.n_units = p.n_items * c.num_kv_heads;
+  p.arrive = reinterpret_cast<int32_t*>(scratch);
+  p.part_ml = reinterpret_cast<float*>(scratch + kStaticArriveBytes);
+  p.part_o = reinterpret_cast<float*>(scratch + kStaticArriveBytes + kStaticMlBytes);
+  p.chained = 0;
+  // the array keeps whatever the last call (of any pool) left: the arrival counters must start at zero; every
+  // partial slot that is read has been written by this launch
+  if (plan.n_partials > 0)
+    KV_CUDA(pool, cudaMemsetAsync(scratch, 0, static_cast<size_t>(plan.n_partials) * 4, stream));
+  const AttnVariant v = pick_variant(pool, false, false, use_tc);
+  KV_CUDA(pool, launch_attn_kernel(pool, v, p, stream));
+  ++pool->launches;
+  pool->n_tc_launches += use_tc ? 1 : 0;
+  if (!plan.combines.empty() && !pool->fuse_combine) {
+    CombineParams cp{};
+    cp.entries = reinterpret_cast<const CombineEntryDev*>(s.dev + item_bytes);
+    cp.n_entries = static_cast<int32_t>(plan.combines.size());
+    cp.part_o = p.part_o;
+    cp.part_ml = p.part_ml;
+    cp.out = p.out;
+    cp.num_q_heads = c.num_q_heads;
+    cp.group = c.num_q_heads / c.num_kv_heads;
+    cp.num_kv_heads = c.num_kv_heads;
+    const unsigned cgrid = static_cast<unsigned>((static_cast<int64_t>(cp.n_entries) * c.num_q_heads + 3) / 4);
+    if (c.head_dim == 128)
+      combine_kernel<128><<<cgrid, 128, 0, stream>>>(cp);
+    else
+      combine_kernel<64><<<cgrid, 128, 0, stream>>>(cp);
+    KV_CUDA(pool, cudaGetLastError());
+    ++pool->launches;
+  }
+  KV_CUDA(pool, cudaEventRecord(s.ev, stream));
+  s.in_flight = true;
+  attention_launched(pool, stream, s, 0);
+  pool->chain_slot = -1;
+  return KV_OK;
+}
+
 // NEXT-1: plan query tiles (cached while ids, q_lens and the pool epoch are unchanged, i.e. across
 // the layers of a step), stage 48-byte items, one launch of attn_kernel<.., kVarQ = true>.
 int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids,
@@ -1334,6 +1448,7 @@ const char* kv_strerror(int32_t status) {
     case KV_ERR_CUDA: return "CUDA runtime error (see kv_last_cuda_error)";
     case KV_ERR_NO_DEVICE: return "pool has no device slab (host-only)";
     case KV_ERR_UNSUPPORTED: return "call not available for this pool's kv_dtype";
+    case KV_ERR_SCRATCH_LIMIT: return "split-KV plan needs more partial slots than the static scratch holds (KV_STATIC_MAX_PARTIALS)";
     default: return "unknown status";
   }
 }
