@@ -19,8 +19,9 @@
 //     the two terms occupy 16 N-columns and are summed after the TMEM load.
 //   * the weights p' = 2^(s + log2 vs - m_ref) are rounded to f16 (as in the mma.sync kernel) and that f16 is split
 //     EXACTLY into four e5m2 terms by masking its top byte three times (f16 and e5m2 share sign and exponent, and
-//     x - (x & 0xff00) is exact), written as bytes P^T[term][head][token] into the K-major B operand of GEMM2; the
-//     four column groups of O^T are summed after the TMEM load.  Numerics are those of the mma.sync kernel.
+//     x - (x & 0xff00) is exact); a token's 32 bytes [term][head] go into the B operand of GEMM2 with two 16-byte
+//     stores (MN-major, un-swizzled: kTcPByToken below); the four column groups of O^T are summed after the TMEM
+//     load.  Numerics are those of the mma.sync kernel.
 //   * m_ref is a LAZY reference: it moves only when some score of a tile exceeds it by more than 2^8 (p' <= 256; times the
 //     bias 2^7 below, 2^15 fits f16 and e5m2), so the rescale of O^T in TMEM (tcgen05.ld / st) runs a handful of times per unit.
 //
@@ -152,6 +153,17 @@ __device__ __forceinline__ uint64_t tc_smem_desc(uint32_t addr) {
 // a_major bit 15 (1 = MN-major), b_major bit 16, N >> 3 at bits 17-22, M >> 4 at bits 24-28
 constexpr uint32_t kTcIdescQK = (1u << 4) | (0u << 7) | (0u << 10) | (0u << 15) | ((16u >> 3) << 17) | ((128u >> 4) << 24);
 constexpr uint32_t kTcIdescPV = (1u << 4) | (0u << 7) | (1u << 10) | (1u << 15) | ((32u >> 3) << 17) | ((128u >> 4) << 24);
+// P^T, the B operand of GEMM2 (N = 32 (term, head) columns, K = 128 tokens).  kTcPByToken = true: MN-major and
+// un-swizzled — core matrices of 8 tokens x 16 N-bytes (128 contiguous bytes, a token's 16 bytes per row), the two
+// N-halves 2 KiB apart (SBO), 8-token groups 128 B apart (LBO) — so that the thread that owns a token writes its 32
+// weight bytes with TWO 16-byte stores; a warp's stores are 512 contiguous bytes, no bank conflict.  false: K-major in
+// the 128-byte swizzle (rows = (term, head), a token = one byte of each of 32 rows: 32 one-byte stores per thread, four
+// lanes to a word — 2.5-8.4 M bank conflicts per launch, profiles/README.md r02).
+constexpr bool kTcPByToken = true;
+constexpr uint32_t kTcIdescPVt = kTcIdescPV | (1u << 16);
+__device__ __forceinline__ uint64_t tc_smem_desc_p(uint32_t addr) {   // layout type 0 (no swizzle), version 1
+  return static_cast<uint64_t>((addr & 0x3ffffu) >> 4) | ((128ull >> 4) << 16) | ((2048ull >> 4) << 32) | (1ull << 46);
+}
 
 struct TcUnit {            // what the producer hands to the MMA and softmax warps for one unit (shared memory, 64 bytes)
   int32_t n_tiles;         // 0: no more work
@@ -506,9 +518,15 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
           }
           tc_fence_after();
           const uint64_t vdesc = tc_smem_desc(smem0 + s * kTcStageBytes + 16384);
-          const uint64_t pdesc = tc_smem_desc(p_smem + pb * kTcPBytes);
+          if constexpr (kTcPByToken) {
+            const uint64_t pdesc = tc_smem_desc_p(p_smem + pb * kTcPBytes);
 #pragma unroll
-          for (int k = 0; k < 4; ++k) tc_mma_f8(o_tmem, vdesc + 256 * k, pdesc + 2 * k, kTcIdescPV, (t2 > 0 || k > 0) ? 1u : 0u);
+            for (int k = 0; k < 4; ++k) tc_mma_f8(o_tmem, vdesc + 256 * k, pdesc + 32 * k, kTcIdescPVt, (t2 > 0 || k > 0) ? 1u : 0u);
+          } else {
+            const uint64_t pdesc = tc_smem_desc(p_smem + pb * kTcPBytes);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) tc_mma_f8(o_tmem, vdesc + 256 * k, pdesc + 2 * k, kTcIdescPV, (t2 > 0 || k > 0) ? 1u : 0u);
+          }
           tc_commit(b_empty + 8 * s);                              // the stage goes back to the producer
           tc_commit(b_p_free + 8 * pb);
           if (t2 == n_tiles - 1) tc_commit(b_o_full + 8 * e);
@@ -616,6 +634,32 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
         // ---- weights: f16, split exactly into four e5m2 terms; bytes P^T[term][head][token] ----
         if (g >= 2) mbar_wait(b_p_free + 8 * pb, ((g >> 1) - 1) & 1u);   // GEMM2 of tile g - 2 has read this buffer
         const uint32_t pbuf = p_smem + pb * kTcPBytes;
+        if constexpr (kTcPByToken) {
+          uint32_t x[4], wt[8];                                     // x[j]: f16 weights of heads 2j, 2j+1; wt: [term][head] bytes
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const float p0 = fast_exp2(sc[2 * j] - m_ref[2 * j] + kTcWeightBias), p1 = fast_exp2(sc[2 * j + 1] - m_ref[2 * j + 1] + kTcWeightBias);
+            l[2 * j] += p0 * iv;
+            l[2 * j + 1] += p1 * iv;
+            x[j] = pack_f16x2(p0, p1);
+          }
+#pragma unroll
+          for (int term = 0; term < 4; ++term) {
+            wt[2 * term] = __byte_perm(x[0], x[1], 0x7531);         // the top bytes (e5m2 terms) of heads 0..3
+            wt[2 * term + 1] = __byte_perm(x[2], x[3], 0x7531);     //                          ... of heads 4..7
+            if (term < 3) {
+#pragma unroll
+              for (int j = 0; j < 4; ++j) {
+                const uint32_t top = x[j] & 0xff00ff00u;
+                const __half2 r = __hsub2(*reinterpret_cast<const __half2*>(&x[j]), *reinterpret_cast<const __half2*>(&top));
+                x[j] = *reinterpret_cast<const uint32_t*>(&r);
+              }
+            }
+          }
+          const uint32_t prow = pbuf + (tid >> 3) * 128 + (tid & 7) * 16;
+          sts128(prow, make_uint4(wt[0], wt[1], wt[2], wt[3]));          // N = 0..15: terms 0, 1
+          sts128(prow + 2048, make_uint4(wt[4], wt[5], wt[6], wt[7]));   // N = 16..31: terms 2, 3
+        } else {
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
           const float p0 = fast_exp2(sc[2 * j] - m_ref[2 * j] + kTcWeightBias), p1 = fast_exp2(sc[2 * j + 1] - m_ref[2 * j + 1] + kTcWeightBias);
@@ -632,6 +676,7 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
               x = *reinterpret_cast<const uint32_t*>(&r);
             }
           }
+        }
         }
         fence_proxy_async();                                       // P^T (and zeroed V rows) -> visible to the tensor core
         mbar_arrive(b_p_full + 8 * pb);

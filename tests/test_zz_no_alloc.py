@@ -23,13 +23,15 @@ def n_partials(pool, ids):
     return int(sum(1 for it in items if it[4] >= 0))
 
 
-def close_to_existing(got, ref):
-    """The tolerance the attention parity tests use (BASELINE.json north_star: max abs <= 1e-2, mean abs <= 1e-3)."""
+def close_to_existing(got, ref, same_plan=True):
+    """The tolerance the attention parity tests use (BASELINE.json north_star: max abs <= 1e-2, mean abs <= 1e-3) —
+    and, where the two calls ran the same plan (same split, same kernel, partials merged in chunk order), the same bits."""
     a, b = bits_to_f64(bits_of(got)), bits_to_f64(bits_of(ref))
     assert np.all(np.isfinite(a))
     err = np.abs(a - b)
     assert err.max() <= 1e-2 and err.mean() <= 1e-3, (float(err.max()), float(err.mean()))
-    return bool(np.array_equal(bits_of(got), bits_of(ref)))
+    if same_plan:
+        assert np.array_equal(bits_of(got), bits_of(ref)), (float(err.max()), float(err.mean()))
 
 
 def fill(pool, w, ids, lens, slab=None):
@@ -127,6 +129,6 @@ def test_second_call_allocates_no_device_memory_and_limit_is_enforced():
     assert e.value.status == B.KV_ERR_SCRATCH_LIMIT and "static scratch" in kv.kv_strerror(e.value.status)
     torch.cuda.synchronize()
     assert pool.launches == launches and torch.equal(out.view(torch.int16), before.view(torch.int16))
-    ref = pool.attention(0, ids, q)            # the existing path has no such limit
+    ref = pool.attention(0, ids, q)            # the existing path has no such limit (a finer split: other roundings)
     torch.cuda.synchronize()
-    close_to_existing(ref, before)
+    close_to_existing(ref, before, same_plan=False)
