@@ -53,7 +53,16 @@ def test_host_only_pool_refuses_kernel_calls():
     with pytest.raises(kv.KVError) as e:
         kv.paged_decode_attention(p.handle, 0, [1], 256, 512)
     assert e.value.status == B.KV_ERR_NO_DEVICE
+    with pytest.raises(kv.KVError) as e:                   # the no-allocation form: same checks before any GPU work
+        kv.paged_decode_attention_static(p.handle, 0, [1], 256, 512)
+    assert e.value.status == B.KV_ERR_NO_DEVICE
+    with pytest.raises(kv.KVError) as e:
+        kv.paged_decode_attention_static(p.handle, 0, [1], 0, 512)
+    assert e.value.status == B.KV_ERR_INVALID
     assert p.launches == 0
+    # its static scratch: KV_STATIC_MAX_PARTIALS slots of (arrival counter, (m, l) x 8 heads, O x 8 heads x 128) fp32
+    assert kv.kv_static_scratch_bytes() == B.KV_STATIC_MAX_PARTIALS * (4 + 8 * 2 * 4 + 8 * 128 * 4) == 17055744
+    assert "static scratch" in kv.kv_strerror(B.KV_ERR_SCRATCH_LIMIT)
 
 
 def test_sequential_and_seeded_free_lists():
