@@ -572,10 +572,16 @@ __global__ void __launch_bounds__(kTcThreads, 2) attn_tc_kernel(const __grid_con
         if (kAppend && t == U.n_tiles - 1 && tid == U.new_row)       // the appended row's scales: the tile brought stale ones
           asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(ks), "=f"(vs) : "r"(stash_smem + e * 272u + 256u) : "memory");
         const bool valid = t * kTcTileTokens + tid < U.n_tokens;
-        if (t == U.n_tiles - 1 && !valid) {                        // rows past the chunk's end: no stale V byte reaches GEMM2
+        if (t == U.n_tiles - 1) {                                  // rows past the chunk's end: no stale V byte reaches GEMM2
+          // the warp zeroes its invalid rows (a suffix of its 32) four rows per store: lane -> (row r + lane / 8, 16-byte
+          // chunk lane % 8), 512 contiguous bytes per instruction (a thread zeroing its own 128-byte row is a 32-way
+          // bank conflict: 0.94 M excess wavefronts per launch on config 3, ncu source page)
+          const int first = max(U.n_tokens - t * kTcTileTokens, warp * 32);   // first invalid row of the tile, within this warp's
           const uint4 z = make_uint4(0u, 0u, 0u, 0u);
-#pragma unroll
-          for (int c = 0; c < 8; ++c) sts128(st + 16384 + tid * 128 + c * 16, z);
+          for (int r = first & ~3; r < warp * 32 + 32; r += 4) {
+            const int row = r + (lane >> 3);
+            if (row >= first) sts128(st + 16384 + row * 128 + (lane & 7) * 16, z);
+          }
         }
         mbar_wait(b_d1_full + 8 * db, (g >> 1) & 1u);
         tc_fence_after();
