@@ -289,6 +289,30 @@ int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch,
                                void* cuda_stream);
 
 /*
+ * NEXT-1, the new tokens' K/V written into the pool as the step goes (§V-E: the ultra-short
+ * request's prefill runs in place on the D-instance, so its K/V are produced there, layer by layer, beside the decode
+ * rows' one new token each).  One host call per layer, equivalent to
+ *     if (flags & KV_STEP_RESERVE) kv_reserve(pool, batch, req_ids, q_lens);              (layer must be 0)
+ *     kv_ingest(pool, batch, req_ids, q_lens, k_new, v_new, layer, 1, stream)             as a continuation of that
+ *                                                                                          reservation (also for layer 0)
+ *     paged_varlen_attention(pool, layer, batch, req_ids, q_lens, q, out, sm_scale, stream)
+ *   k_new[i], v_new[i]: device, bf16, contiguous [num_kv_heads][q_lens[i]][head_dim] — THIS layer's K / V of request i's
+ *   q_lens[i] new tokens (a decode row: one token; an in-place prefill row: its prompt, or the next chunk of it);
+ *   host arrays of `batch` device pointers.  q, out: as paged_varlen_attention.  An FP8 pool quantises the rows exactly
+ *   as kv_ingest does.  Two launches on `cuda_stream` (scatter, attention); the attention's plan is made once per step
+ *   and reused by the following layers.
+ * Without KV_STEP_RESERVE every request's last reservation must be exactly q_lens[i] tokens (kv_reserve by the caller,
+ * or this call for layer 0), else KV_ERR_INVALID.  Errors: as kv_reserve / kv_ingest / paged_varlen_attention;
+ * q_lens[i] < 1 => KV_ERR_INVALID.  If the call fails before anything is enqueued — allocation, validation, a plan that
+ * does not fit — nothing changes (a reservation it made is rolled back).
+ */
+int32_t paged_varlen_step(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids /*host*/,
+                          const int32_t* q_lens /*host*/, const void* q /*device*/,
+                          const void* const* k_new /*host array of device ptrs*/,
+                          const void* const* v_new /*host array of device ptrs*/, void* out /*device*/,
+                          float sm_scale, int32_t flags, void* cuda_stream);
+
+/*
  * a6 — free (a completed request releases consumer capacity).  Host only
  * and immediate: blocks return to the free list (LIFO) and the table row is dropped.  The
  * caller must not ingest into recycled blocks on a different stream before the attention

@@ -12,7 +12,7 @@ _BINDING_NAMES = (
     "KVPool", "KVError", "PoolConfig", "lib", "lib_path",
     "kv_pool_create", "kv_pool_destroy", "kv_pool_kv_bytes", "kv_pool_required_bytes", "kv_reserve",
     "kv_ingest", "paged_decode_attention", "kv_free", "kv_block_table", "kv_pool_stats", "kv_gather",
-    "kv_plan_decode", "kv_launch_count", "paged_decode_step", "paged_decode_step_layers", "kv_transfer", "kv_gather_bytes", "kv_token_bytes", "kv_capacity", "kv_optimal_pd_ratio", "paged_varlen_attention", "paged_decode_step_host", "kv_ingest_host", "paged_decode_attention_host", "kv_profile_read", "kv_profile_reset", "kv_pool_set_option", "kv_last_cuda_error", "kv_strerror", "paged_decode_attention_static", "kv_static_scratch_bytes",
+    "kv_plan_decode", "kv_launch_count", "paged_decode_step", "paged_decode_step_layers", "kv_transfer", "kv_gather_bytes", "kv_token_bytes", "kv_capacity", "kv_optimal_pd_ratio", "paged_varlen_attention", "paged_decode_step_host", "kv_ingest_host", "paged_decode_attention_host", "kv_profile_read", "kv_profile_reset", "kv_pool_set_option", "kv_last_cuda_error", "kv_strerror", "paged_decode_attention_static", "kv_static_scratch_bytes", "paged_varlen_step",
     "kv_version",
 )
 

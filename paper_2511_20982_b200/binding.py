@@ -64,6 +64,7 @@ _SIGS = {
     "paged_decode_step_host": (_i32, [_P, _i32, _i32, _P, _P, _P, _P, _P, ctypes.c_float, _P, _i64, _P]),
     "paged_decode_step_layers": (_i32, [_P, _i32, _i32, _i32, _P, _P, _P, _P, _P, _i64, _i64, ctypes.c_float, _i32, _P]),
     "paged_varlen_attention": (_i32, [_P, _i32, _i32, _P, _P, _P, _P, ctypes.c_float, _P]),
+    "paged_varlen_step": (_i32, [_P, _i32, _i32, _P, _P, _P, _P, _P, _P, ctypes.c_float, _i32, _P]),
     "kv_free": (_i32, [_P, _i32, _P]),
     "kv_block_table": (_i32, [_P, _i64, _P, _i32, ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
     "kv_pool_stats": (_i32, [_P, ctypes.POINTER(_i64), ctypes.POINTER(_i64), ctypes.POINTER(_i32),
@@ -266,6 +267,16 @@ def paged_varlen_attention(handle: int, layer: int, req_ids, q_lens, q_ptr: int,
 
 
 KERNEL_KINDS = {"attn": 0, "combine": 1, "ingest": 2, "gather": 3, "varq": 4, "transfer": 5}
+
+
+def paged_varlen_step(handle: int, layer: int, req_ids, q_lens, q_ptr: int, k_new_ptrs, v_new_ptrs, out_ptr: int,
+                      sm_scale: float = 0.0, flags: int = 0, stream: int = 0) -> None:
+    """(a1,) a2 of this layer's new rows, then the variable-q attention; k_new_ptrs / v_new_ptrs: one device pointer
+    per request ([Hkv][q_len][d] bf16)."""
+    ids, ql, kp, vp = _ids(req_ids), _i32s(q_lens), _ptrs(k_new_ptrs), _ptrs(v_new_ptrs)
+    assert ids.size == ql.size == kp.size == vp.size
+    _check(lib.paged_varlen_step(handle, layer, ids.size, _np(ids), _np(ql), q_ptr, _np(kp), _np(vp), out_ptr, sm_scale,
+                                 flags, stream or None), "paged_varlen_step")
 
 
 def kv_profile_read(handle: int, kind: int):
@@ -474,6 +485,18 @@ class KVPool:
             out = torch.empty_like(q)
         paged_varlen_attention(self.handle, layer, req_ids, q_lens, q.data_ptr(), out.data_ptr(), sm_scale,
                                self._stream(stream))
+        return out
+
+    def varlen_step(self, layer, req_ids, q_lens, q, k_new, v_new, out=None, sm_scale=0.0, reserve=False, stream=None):
+        """k_new[i], v_new[i]: bf16 [Hkv][q_lens[i]][d] of THIS layer; q: bf16 [sum(q_lens)][Hq][d]."""
+        import torch
+
+        assert q.is_contiguous() and q.dtype == torch.bfloat16 and all(t.is_contiguous() for t in list(k_new) + list(v_new))
+        if out is None:
+            out = torch.empty_like(q)
+        paged_varlen_step(self.handle, layer, req_ids, q_lens, q.data_ptr(), [t.data_ptr() for t in k_new],
+                          [t.data_ptr() for t in v_new], out.data_ptr(), sm_scale, KV_STEP_RESERVE if reserve else 0,
+                          self._stream(stream))
         return out
 
     def gather(self, req_id, stream=None, src_kv_heads=None):

@@ -1122,20 +1122,16 @@ int32_t paged_decode_attention_static(kv_pool_t* pool, int32_t layer, int32_t ba
 
 // NEXT-1: plan query tiles (cached while ids, q_lens and the pool epoch are unchanged, i.e. across
 // the layers of a step), stage 48-byte items, one launch of attn_kernel<.., kVarQ = true>.
-int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids,
-                               const int32_t* q_lens, const void* q, void* out, float sm_scale, void* cuda_stream) {
-  if (!pool || !req_ids || !q_lens || !q || !out || !aligned16(q) || !aligned16(out)) return KV_ERR_INVALID;
+// Host half of the variable-q call: the plan for (ids, q_lens) at the pool's current epoch, reused if it is the one staged.
+// No GPU work; on error nothing is staged.
+static int32_t varlen_prepare(kv_pool_t* pool, int32_t batch, const int64_t* req_ids, const int32_t* q_lens, bool* cached_out) {
   const kv_pool_config_t& c = pool->hs.cfg;
-  if (layer < 0 || layer >= c.num_layers || batch < 1) return KV_ERR_INVALID;
-  if (!pool->has_device) return KV_ERR_NO_DEVICE;
-  KV_ON_DEVICE(pool);
-  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const int32_t G = c.num_q_heads / c.num_kv_heads;
-
   const bool cached = pool->plan_slot >= 0 && pool->plan_kind == 1 && pool->plan_epoch == pool->hs.epoch &&
                       static_cast<int32_t>(pool->plan_ids.size()) == batch &&
                       std::memcmp(pool->plan_ids.data(), req_ids, sizeof(int64_t) * static_cast<size_t>(batch)) == 0 &&
                       std::memcmp(pool->plan_qlens.data(), q_lens, sizeof(int32_t) * static_cast<size_t>(batch)) == 0;
+  *cached_out = cached;
   if (!cached) {
     // a partial slot of this kernel is 8 columns wide; the workspace is sized in G-column slots
     const int32_t max_partials = static_cast<int32_t>(static_cast<int64_t>(kMaxPartials) * G / 8);
@@ -1145,6 +1141,12 @@ int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
     if (rc != KV_OK) return rc;
     if (static_cast<int64_t>(pool->plan.items.size()) * 48 > pool->lay.plan_blob_bytes) return KV_ERR_TOO_LONG;
   }
+  return KV_OK;
+}
+
+// Device half: stage the plan (unless cached) and launch.
+static int32_t varlen_enqueue(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const int32_t* q_lens,
+                              const void* q, void* out, float sm_scale, cudaStream_t stream, bool cached) {
   if (int32_t rc = order_attention(pool, stream); rc != KV_OK) return rc;
   if (!cached) {
     const size_t n_items = pool->plan.items.size();
@@ -1180,6 +1182,49 @@ int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, co
   s.in_flight = true;
   attention_launched(pool, stream, s, 2);
   return KV_OK;
+}
+
+int32_t paged_varlen_attention(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids,
+                               const int32_t* q_lens, const void* q, void* out, float sm_scale, void* cuda_stream) {
+  if (!pool || !req_ids || !q_lens || !q || !out || !aligned16(q) || !aligned16(out)) return KV_ERR_INVALID;
+  const kv_pool_config_t& c = pool->hs.cfg;
+  if (layer < 0 || layer >= c.num_layers || batch < 1) return KV_ERR_INVALID;
+  if (!pool->has_device) return KV_ERR_NO_DEVICE;
+  KV_ON_DEVICE(pool);
+  bool cached = false;
+  if (int32_t rc = varlen_prepare(pool, batch, req_ids, q_lens, &cached); rc != KV_OK) return rc;
+  return varlen_enqueue(pool, layer, batch, req_ids, q_lens, q, out, sm_scale, static_cast<cudaStream_t>(cuda_stream), cached);
+}
+
+// NEXT-1 with the new tokens' K/V written "as it goes": (a1,) a2 of this layer's rows, then the variable-q attention.
+int32_t paged_varlen_step(kv_pool_t* pool, int32_t layer, int32_t batch, const int64_t* req_ids, const int32_t* q_lens,
+                          const void* q, const void* const* k_new, const void* const* v_new, void* out, float sm_scale,
+                          int32_t flags, void* cuda_stream) {
+  if (!pool || !req_ids || !q_lens || !q || !out || !aligned16(q) || !aligned16(out) || batch < 1) return KV_ERR_INVALID;
+  if (flags & ~KV_STEP_RESERVE) return KV_ERR_INVALID;
+  const bool reserve = (flags & KV_STEP_RESERVE) != 0;
+  if (reserve && layer != 0) return KV_ERR_INVALID;
+  int32_t rc = ingest_args_ok(pool, batch, req_ids, q_lens, k_new, v_new, layer, 1, true);
+  if (rc != KV_OK) return rc;
+  for (int32_t i = 0; i < batch; ++i)
+    if (q_lens[i] < 1) return KV_ERR_INVALID;
+  KV_ON_DEVICE(pool);
+  rc = reserve ? pool->hs.reserve(batch, req_ids, q_lens)         // a1: the q_lens[i] new tokens of every request
+               : pool->hs.check_batch(batch, req_ids, q_lens);    // reserved by the caller / by this step's layer 0
+  if (rc != KV_OK) return rc;
+  auto fail = [&](int32_t e) {
+    if (reserve) pool->hs.rollback_last_reserve();
+    return e;
+  };
+  bool cached = false;                                           // the attention's plan first: nothing is enqueued if it fails
+  if (rc = varlen_prepare(pool, batch, req_ids, q_lens, &cached); rc != KV_OK) return fail(rc);
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  std::vector<int32_t> start(static_cast<size_t>(batch));
+  for (int32_t i = 0; i < batch; ++i) start[static_cast<size_t>(i)] = pool->hs.reqs.find(req_ids[i])->second.len - q_lens[i];
+  rc = run_copy(pool, CopyKind::kScatter, nullptr, nullptr, batch, req_ids, q_lens, k_new, v_new, start.data(), layer, 1, stream);
+  if (rc != KV_OK) return fail(rc);
+  // from here on work is enqueued: the reservation stays (as in paged_decode_step_layers)
+  return varlen_enqueue(pool, layer, batch, req_ids, q_lens, q, out, sm_scale, stream, cached);
 }
 
 int32_t kv_ingest_host(kv_pool_t* pool, int32_t n_req, const int64_t* req_ids, const int32_t* n_tokens,

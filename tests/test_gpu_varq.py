@@ -139,3 +139,117 @@ def test_errors_change_nothing():
     out = pool.varlen_attention(0, ids, [20, 30], q[:50].contiguous())   # still works afterwards
     torch.cuda.synchronize()
     assert np.all(np.isfinite(bits_to_f64(bits_of(out))))
+
+
+# ---------------------------------------------------------------------------------------------
+# paged_varlen_step: the new tokens' K/V written into the pool as the step goes
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("opts", [dict(), dict(min_chunk_blocks=1, items_per_slot=1024), dict(pdl=0)])
+@pytest.mark.parametrize("Hq,Hkv,d", [(8, 2, 64), (32, 8, 128), (32, 32, 128)])
+def test_varlen_step_equals_ingest_then_attention_and_oracle(Hq, Hkv, d, opts):
+    """Two steps over three layers of a mixed batch: decode rows (one new token), fresh in-place prefills (requests that
+    do not exist before the step) and a chunked prefill on top of a stored prefix.  The fused call == layer-sliced
+    kv_ingest + paged_varlen_attention on a twin pool, bit for bit (pool and outputs), the pool == the
+    oracle's scatter over the whole slab, the outputs == oracle_attention_varq."""
+    L = 3
+    prefix = [40, 0, 255, 16, 0, 700]                 # stored before the first step (0: the request does not exist yet)
+    steps = [[1, 33, 1, 48, 130, 1], [1, 1, 1, 17, 1, 1]]
+    w = W.Workload("varq_step", L, Hq, Hkv, d, len(prefix), None, 777, max_len=1024)
+    nb = sum((p + sum(s[i] for s in steps) + 15) // 16 for i, p in enumerate(prefix)) + 8
+    pools = [make_pool(w, nb, max_requests=16, alloc_seed=13) for _ in range(2)]
+    for p in pools:
+        apply_options(p, opts)
+    ids = list(range(40, 40 + len(prefix)))
+    have = [(u, n) for u, n in zip(ids, prefix) if n > 0]
+    srcs = [kv_src(w, u, 0, n, DEV) for u, n in have]
+    for p in pools:
+        p.ingest([u for u, _ in have], [s[0] for s in srcs], [s[1] for s in srcs])
+    slab = oracle_slab(pools[0])
+    for u, n in have:
+        oracle_ingest(slab, pools[0], w, u, 0, n)
+    lens = list(prefix)
+    for step, q_lens in enumerate(steps):
+        new = [kv_src(w, u, n, n + ql, DEV) for u, n, ql in zip(ids, lens, q_lens)]       # [L][Hkv][ql][d] each
+        for layer in range(L):                         # twin pool: kv_ingest(layer 0) makes the reservation, layers 1.. continue it
+            q = W.q_values(w.seed, step, layer, sum(q_lens), Hq, d, DEV)
+            kl = [k[layer].contiguous() for k, _ in new]
+            vl = [v[layer].contiguous() for _, v in new]
+            n0 = pools[0].launches
+            out_a = pools[0].varlen_step(layer, ids, q_lens, q, kl, vl, reserve=(layer == 0))
+            assert pools[0].launches - n0 == 2                                            # scatter + attention
+            B.kv_ingest(pools[1].handle, ids, q_lens, kl, vl, layer, 1)
+            out_b = pools[1].varlen_attention(layer, ids, q_lens, q)
+            torch.cuda.synchronize()
+            assert torch.equal(out_a.view(torch.int16), out_b.view(torch.int16))
+            if layer == 0:
+                for u, n, ql in zip(ids, lens, q_lens):
+                    oracle_ingest(slab, pools[0], w, u, n, n + ql)
+            compare_attention(out_a, oracle_varq(slab, pools[0], layer, ids, q_lens, q))
+        lens = [n + ql for n, ql in zip(lens, q_lens)]
+        assert np.array_equal(pool_bits(pools[0]), slab), "the step's rows are not where the oracle puts them"
+        assert torch.equal(pools[0].slab[: pools[0].kv_bytes], pools[1].slab[: pools[1].kv_bytes])
+    assert pools[0].counter("plans_uploaded") == len(steps)                               # one plan per step, three layers each
+
+
+def test_varlen_step_errors_change_nothing():
+    w = W.Workload("varq_step_err", 2, 8, 2, 64, 2, None, 5, max_len=512)
+    pool = make_pool(w, 11, max_requests=4, alloc_seed=0)                                # 3 blocks used below, 8 free
+    ids = [900, 901]
+    srcs = [kv_src(w, u, 0, n, DEV) for u, n in zip(ids, [32, 16])]
+    pool.ingest(ids, [s_[0] for s_ in srcs], [s_[1] for s_ in srcs])
+    torch.cuda.synchronize()
+    q = torch.zeros((400, 8, 64), dtype=torch.bfloat16, device=DEV)
+    kn = [torch.zeros((2, 200, 64), dtype=torch.bfloat16, device=DEV) for _ in range(2)]
+    stats, bits = pool.stats(), pool_bits(pool).copy()
+    for a_ids, ql, layer, reserve, status in [
+            ([900, 901], [200, 200], 0, True, B.KV_ERR_NO_BLOCKS),         # 2 x 13 new blocks, 8 free
+            ([7, 900], [1, 1], 1, False, B.KV_ERR_UNKNOWN_REQUEST),
+            ([900, 901], [1, 1], 1, True, B.KV_ERR_INVALID),                # reserve needs layer 0
+            ([900, 901], [1, 1], 0, False, B.KV_ERR_INVALID),               # no one-token reservation to continue
+            ([900, 901], [0, 1], 0, True, B.KV_ERR_INVALID),
+            ([900, 900], [1, 1], 0, True, B.KV_ERR_INVALID)]:
+        with pytest.raises(B.KVError) as e:
+            pool.varlen_step(layer, a_ids, ql, q[: max(sum(ql), 1)].contiguous(), [k[:, : max(n, 1)].contiguous() for k, n in zip(kn, ql)],
+                             [k[:, : max(n, 1)].contiguous() for k, n in zip(kn, ql)], reserve=reserve)
+        assert e.value.status == status, (a_ids, ql, layer, reserve)
+        assert pool.stats() == stats and pool.block_table(900)[1] == 32 and pool.block_table(901)[1] == 16
+    torch.cuda.synchronize()
+    assert np.array_equal(pool_bits(pool), bits)
+    out = pool.varlen_step(0, ids, [1, 3], q[:4].contiguous(), [kn[0][:, :1].contiguous(), kn[1][:, :3].contiguous()],
+                           [kn[0][:, :1].contiguous(), kn[1][:, :3].contiguous()], reserve=True)   # still works afterwards
+    torch.cuda.synchronize()
+    assert pool.block_table(900)[1] == 33 and pool.block_table(901)[1] == 19 and np.all(np.isfinite(bits_to_f64(bits_of(out))))
+
+
+def test_varlen_step_fp8_pool_equals_ingest_then_attention():
+    """FP8 pool: the fused call quantises the new rows exactly as kv_ingest does (same bytes over the whole pool) and
+    returns the bits of paged_varlen_attention."""
+    import paper_2511_20982_b200 as kv
+    L, Hq, Hkv, d = 2, 32, 8, 128
+    prefix, q_lens = [300, 0, 17], [1, 90, 40]
+    w = W.Workload("varq_step_fp8", L, Hq, Hkv, d, 3, None, 31, max_len=512)
+    pools = []
+    for _ in range(2):
+        cfg = kv.PoolConfig(num_layers=L, num_q_heads=Hq, num_kv_heads=Hkv, head_dim=d, num_blocks=40, max_requests=8,
+                            max_blocks_per_request=32, alloc_seed=21, kv_dtype=B.KV_DTYPE_FP8_E4M3)
+        p = kv.KVPool(cfg, device=DEV)
+        p.slab[: p.kv_bytes].fill_(0xFF)
+        pools.append(p)
+    ids = [5, 6, 7]
+    have = [(u, n) for u, n in zip(ids, prefix) if n > 0]
+    srcs = [kv_src(w, u, 0, n, DEV) for u, n in have]
+    for p in pools:
+        p.ingest([u for u, _ in have], [s[0] for s in srcs], [s[1] for s in srcs])
+    new = [kv_src(w, u, n, n + ql, DEV) for u, n, ql in zip(ids, prefix, q_lens)]
+    for layer in range(L):
+        q = W.q_values(w.seed, 0, layer, sum(q_lens), Hq, d, DEV)
+        kl = [k[layer].contiguous() for k, _ in new]
+        vl = [v[layer].contiguous() for _, v in new]
+        out_a = pools[0].varlen_step(layer, ids, q_lens, q, kl, vl, reserve=(layer == 0))
+        B.kv_ingest(pools[1].handle, ids, q_lens, kl, vl, layer, 1)
+        out_b = pools[1].varlen_attention(layer, ids, q_lens, q)
+        torch.cuda.synchronize()
+        assert torch.equal(out_a.view(torch.int16), out_b.view(torch.int16))
+        assert np.all(np.isfinite(bits_to_f64(bits_of(out_a))))
+    assert torch.equal(pools[0].slab[: pools[0].kv_bytes], pools[1].slab[: pools[1].kv_bytes])
